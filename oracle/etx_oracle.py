@@ -1,0 +1,186 @@
+"""TEST INFRASTRUCTURE — Python (ctypes) face of the CPU oracle ``etx_oracle.cpp``.
+
+Only tests/, ``__graft_entry__.smoke()`` and bench.py's ``cpu_baseline`` / ``--impl reference`` legs
+may import this.  It imports nothing from the CUDA package; inputs are plain numpy arrays.
+Every function cites the passage of the thesis (P:line of PAPER.md) its C++ body follows.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import Dict, List, Optional, Sequence, Tuple
+
+import numpy as np
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_DIR, "etx_oracle.cpp")
+_LIB = os.path.join(_DIR, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -ffp-contract=off (the radius predicate must not be FMA-contracted) -fopenmp."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fopenmp", "-fPIC",
+                               "-shared", "-o", _LIB, _SRC])
+    return _LIB
+
+
+def _p(a: Optional[np.ndarray], t):
+    return None if a is None else a.ctypes.data_as(C.POINTER(t))
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_build_graph.restype = C.c_int64
+        _lib.orc_candidate_d2.restype = C.c_int64
+    return _lib
+
+
+def n_threads() -> int:
+    return int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def features(batch: Dict[str, np.ndarray], center: Sequence[float], scale: Sequence[float]):
+    """a0: returns f_emb [N,3] (r,phi,z) and f_node [N,3] (x,y,z)."""
+    n = len(batch["r"])
+    fe = np.empty((n, 3), np.float32)
+    fn = np.empty((n, 3), np.float32)
+    c, s = _f32(center), _f32(scale)
+    arrs = [_f32(batch[k]) for k in ("r", "phi", "z", "x", "y")]
+    lib().orc_features(C.c_int64(n), *[_p(a, C.c_float) for a in arrs], _p(c, C.c_float),
+                       _p(s, C.c_float), _p(fe, C.c_float), _p(fn, C.c_float))
+    return fe, fn
+
+
+def mlp(x: np.ndarray, dims: Sequence[int], blob: np.ndarray, offset: int) -> np.ndarray:
+    """Eqs. 4.24-4.27: ReLU hidden layers, linear output, weights at blob[offset:]."""
+    x = _f32(x)
+    n = x.shape[0]
+    d = np.asarray(dims, dtype=np.int32)
+    assert x.shape[1] == d[0]
+    out = np.empty((n, int(d[-1])), np.float32)
+    w = blob[offset:]
+    lib().orc_mlp(C.c_int64(n), C.c_int32(len(d) - 1), _p(d, C.c_int32), _p(w, C.c_float),
+                  _p(x, C.c_float), _p(out, C.c_float))
+    return out
+
+
+def build_graph(event_ptr, plane, emb, r2_max: float, gap: int, n_planes: int = 26,
+                band: float = 0.0, want_border: bool = False):
+    """a2 (Eq. 8.1): edges (src, dst) in (src asc, dst asc) order.
+    With want_border also the (i, j) pairs with |d - r| <= band, d evaluated in double (Q17)."""
+    event_ptr = np.ascontiguousarray(event_ptr, np.int32)
+    plane = np.ascontiguousarray(plane, np.uint8)
+    emb = _f32(emb)
+    n_ev = len(event_ptr) - 1
+    d = emb.shape[1]
+    nb = C.c_int64(0)
+    cap = 1 << 16
+    while True:
+        src = np.empty(cap, np.int32)
+        dst = np.empty(cap, np.int32)
+        bp = np.empty((cap, 2), np.int32) if want_border else None
+        E = lib().orc_build_graph(C.c_int32(n_ev), _p(event_ptr, C.c_int32), _p(plane, C.c_uint8),
+                                  C.c_int32(n_planes), _p(emb, C.c_float), C.c_int32(d),
+                                  C.c_float(r2_max), C.c_int32(gap), _p(src, C.c_int32),
+                                  _p(dst, C.c_int32), C.c_int64(cap), C.c_double(band),
+                                  _p(bp, C.c_int32), C.c_int64(cap), C.byref(nb))
+        if E <= cap and nb.value <= cap:
+            break
+        cap = max(int(E), int(nb.value)) + 16
+    if want_border:
+        return src[:E].copy(), dst[:E].copy(), bp[:nb.value].copy()
+    return src[:E].copy(), dst[:E].copy()
+
+
+def candidate_d2(event_ptr, plane, emb, gap: int, n_planes: int = 26) -> np.ndarray:
+    """All candidate pairs' d^2 in double (for the Q4 radius calibration)."""
+    event_ptr = np.ascontiguousarray(event_ptr, np.int32)
+    plane = np.ascontiguousarray(plane, np.uint8)
+    emb = _f32(emb)
+    args = (C.c_int32(len(event_ptr) - 1), _p(event_ptr, C.c_int32), _p(plane, C.c_uint8),
+            C.c_int32(n_planes), _p(emb, C.c_float), C.c_int32(emb.shape[1]), C.c_int32(gap))
+    n = lib().orc_candidate_d2(*args, None, C.c_int64(0))
+    out = np.empty(n, np.float64)
+    lib().orc_candidate_d2(*args, _p(out, C.c_double), C.c_int64(n))
+    return out
+
+
+def scatter(n_nodes: int, src, dst, e) -> np.ndarray:
+    """a4, Eq. 8.5: m [n_nodes, 2H] = [sum of outgoing, sum of incoming]."""
+    e = _f32(e)
+    src = np.ascontiguousarray(src, np.int32)
+    dst = np.ascontiguousarray(dst, np.int32)
+    H = e.shape[1]
+    m = np.empty((n_nodes, 2 * H), np.float32)
+    lib().orc_scatter(C.c_int64(n_nodes), C.c_int64(len(src)), _p(src, C.c_int32), _p(dst, C.c_int32),
+                      _p(e, C.c_float), C.c_int32(H), _p(m, C.c_float))
+    return m
+
+
+def gnn_forward(f_node, src, dst, H: int, n_layers: int, n_iter: int, blob: np.ndarray,
+                off_node_enc: int, off_edge_enc: int, off_node_net: Sequence[int],
+                off_edge_net: Sequence[int]) -> Tuple[np.ndarray, np.ndarray]:
+    """a3-a6: returns h^n [N,H], e^n [E,H]."""
+    f_node = _f32(f_node)
+    src = np.ascontiguousarray(src, np.int32)
+    dst = np.ascontiguousarray(dst, np.int32)
+    n, E = f_node.shape[0], len(src)
+    h = np.empty((n, H), np.float32)
+    e = np.empty((E, H), np.float32)
+    base = blob.ctypes.data
+    PP = C.POINTER(C.c_float)
+    nn = (PP * max(n_iter, 1))(*[C.cast(base + 4 * o, PP) for o in off_node_net])
+    en = (PP * max(n_iter, 1))(*[C.cast(base + 4 * o, PP) for o in off_edge_net])
+    lib().orc_gnn_forward(C.c_int64(n), C.c_int64(E), _p(src, C.c_int32), _p(dst, C.c_int32),
+                          _p(f_node, C.c_float), C.c_int32(H), C.c_int32(n_layers), C.c_int32(n_iter),
+                          C.cast(base + 4 * off_node_enc, PP), C.cast(base + 4 * off_edge_enc, PP),
+                          nn, en, _p(h, C.c_float), _p(e, C.c_float))
+    return h, e
+
+
+def edge_scores(e, H: int, n_layers: int, blob: np.ndarray, off_cls: int, want_logits=False):
+    """a7 (sigma P:1309): scores [E] fp32."""
+    e = _f32(e)
+    E = e.shape[0]
+    s = np.empty(E, np.float32)
+    lg = np.empty(E, np.float32)
+    lib().orc_edge_scores(C.c_int64(E), _p(e, C.c_float), C.c_int32(H), C.c_int32(n_layers),
+                          _p(blob[off_cls:], C.c_float), _p(s, C.c_float), _p(lg, C.c_float))
+    return (s, lg) if want_logits else s
+
+
+def run_path(batch: Dict[str, np.ndarray], blob: np.ndarray, layout: Dict[str, Tuple[Tuple[int, ...], int]],
+             H: int, n_iter: int, r2_max: float, gap: int, center, scale, n_planes: int = 26,
+             graph: Optional[Tuple[np.ndarray, np.ndarray]] = None) -> Dict[str, np.ndarray]:
+    """Whole hot path hits -> edge scores, steps a0..a7 in the thesis' order.
+
+    ``layout`` maps MLP name -> (dims, float offset in blob): "emb", "node_enc", "edge_enc",
+    "node_net_k", "edge_net_k", "cls".  ``graph`` overrides the built graph (for Q16-style tests)."""
+    blob = _f32(blob)
+    fe, fn = features(batch, center, scale)
+    emb = mlp(fe, *_lo(layout, "emb", blob))
+    if graph is None:
+        src, dst = build_graph(batch["event_ptr"], batch["plane"], emb, r2_max, gap, n_planes)
+    else:
+        src, dst = graph
+    n_layers = len(layout["node_enc"][0]) - 1
+    h, e = gnn_forward(fn, src, dst, H, n_layers, n_iter, blob, layout["node_enc"][1],
+                       layout["edge_enc"][1], [layout[f"node_net_{k}"][1] for k in range(n_iter)],
+                       [layout[f"edge_net_{k}"][1] for k in range(n_iter)])
+    s, lg = edge_scores(e, H, n_layers, blob, layout["cls"][1], want_logits=True)
+    return {"f_emb": fe, "f_node": fn, "emb": emb, "src": src, "dst": dst, "h": h, "e": e,
+            "scores": s, "logits": lg}
+
+
+def _lo(layout, name, blob):
+    dims, off = layout[name]
+    return dims, blob, off

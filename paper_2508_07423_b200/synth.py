@@ -1,0 +1,343 @@
+"""Seeded synthetic inputs: VELO-like events, Xavier weights, and the five BASELINE.json configs.
+
+This module is the ONLY code shared by the CPU oracle's tests and the CUDA path's tests/bench. It
+holds none of the method's arithmetic (no MLP, no distance, no scatter): it draws random numbers
+from a counter-based generator and lays them out in the input format both sides read.
+
+Recipe (BASELINE.json configs; thesis passages cited as P:line of PAPER.md):
+  * 26 planes at z_k = -275 + 40 k mm (26 planes: P:2680), sensitive annulus 5.1 <= r <= 42 mm
+    (5.1 mm: P:1819).
+  * straight tracks (no field in the VELO) from a vertex x,y ~ N(0, 0.05 mm), z ~ N(0, 50 mm)
+    (thesis: ~30 um, ~45 mm), eta ~ U[2,5], theta = 2 atan(exp(-eta)) (Eq. 3.2),
+    phi ~ U[0, 2 pi).  A hit on plane k iff z_k > z_vtx and true r in [5.1, 42]; x,y smeared by
+    N(0, 0.012 mm) (thesis 12.5 um); each hit dropped with probability 0.02.
+  * noise: round(frac * n_true_hits) extra hits per event, plane uniform in 0..25, uniform by area in
+    the annulus.
+  * hits of an event sorted by plane, then generation order (tracks ascending, noise last) (Q13).
+  * features r, phi = atan2(y, x), z, x, y computed here in double and stored fp32, so neither the
+    oracle nor the GPU path calls trig (Q6).
+  * weights: Xavier-uniform, bound sqrt(6/(fan_in+fan_out)); biases U(-0.05, 0.05); one gain g on the
+    last layer of every node/edge network (Q14) so that activations stay bounded and scores do not
+    saturate.
+
+Random numbers: SplitMix64 in counter mode.  value(key, i) = mix(key + (i+1) * GOLDEN); every event
+has its own keys, so an event generated alone is bit-identical to the same event inside a batch.
+"""
+from __future__ import annotations
+
+import dataclasses
+import json
+import os
+from typing import Dict, List, Optional, Sequence, Tuple
+
+import numpy as np
+
+MASTER_SEED = 250807423
+N_PLANES = 26
+PLANE_Z0 = -275.0
+PLANE_DZ = 40.0
+R_MIN = 5.1
+R_MAX = 42.0
+VTX_SIGMA_XY = 0.05
+VTX_SIGMA_Z = 50.0
+ETA_MIN, ETA_MAX = 2.0, 5.0
+HIT_SMEAR = 0.012
+HIT_INEFF = 0.02
+
+# normalisation constants: feature order r, phi, z, x, y ; f = (v - center) / scale
+NORM_CENTER = (0.0, 0.0, 225.0, 0.0, 0.0)
+NORM_SCALE = (42.0, float(np.pi), 500.0, 42.0, 42.0)
+
+PREC_FP32 = 0      # exact fp32 FFMA path
+PREC_TF32X3 = 1    # tensor cores, error-compensated 3xTF32 (fp32-equivalent)
+PREC_BF16 = 2      # tensor cores, bf16 operands, fp32 accumulate
+
+_U64 = np.uint64
+_GOLDEN = _U64(0x9E3779B97F4A7C15)
+_M1 = _U64(0xBF58476D1CE4E5B9)
+_M2 = _U64(0x94D049BB133111EB)
+
+
+def _mix(z: np.ndarray) -> np.ndarray:
+    """SplitMix64 output function on uint64 arrays (wrapping arithmetic)."""
+    z = np.asarray(z, dtype=_U64)
+    with np.errstate(over="ignore"):
+        z = (z ^ (z >> _U64(30))) * _M1
+        z = (z ^ (z >> _U64(27))) * _M2
+        z = z ^ (z >> _U64(31))
+    return z
+
+
+def make_key(*parts: int) -> np.uint64:
+    """Derive a stream key from integers (seed, config, purpose, ...)."""
+    k = _U64(0x243F6A8885A308D3)
+    with np.errstate(over="ignore"):
+        for p in parts:
+            k = _mix(np.asarray(k ^ _U64(int(p) & 0xFFFFFFFFFFFFFFFF)) + _GOLDEN)
+    return _U64(k)
+
+
+def _keys(base: np.uint64, idx: np.ndarray) -> np.ndarray:
+    """Per-index sub-keys (e.g. one per event)."""
+    with np.errstate(over="ignore"):
+        return _mix((np.asarray(idx, dtype=_U64) + _U64(1)) * _GOLDEN ^ _U64(base))
+
+
+def _raw(keys: np.ndarray, counters: np.ndarray) -> np.ndarray:
+    with np.errstate(over="ignore"):
+        return _mix(np.asarray(keys, dtype=_U64) + (np.asarray(counters, dtype=_U64) + _U64(1)) * _GOLDEN)
+
+
+def uniform01(keys, counters) -> np.ndarray:
+    """U[0,1) doubles, 53 bits."""
+    return (_raw(keys, counters) >> _U64(11)).astype(np.float64) * (1.0 / 9007199254740992.0)
+
+
+def normal01(keys, counters) -> np.ndarray:
+    """Standard normals by Box-Muller on counters 2i, 2i+1."""
+    c = np.asarray(counters, dtype=_U64)
+    u1 = ((_raw(keys, c * _U64(2)) >> _U64(11)).astype(np.float64) + 1.0) * (1.0 / 9007199254740992.0)
+    u2 = uniform01(keys, c * _U64(2) + _U64(1))
+    return np.sqrt(-2.0 * np.log(u1)) * np.cos(2.0 * np.pi * u2)
+
+
+# ----------------------------------------------------------------------------------------------
+# configs
+# ----------------------------------------------------------------------------------------------
+@dataclasses.dataclass(frozen=True)
+class Config:
+    name: str
+    seed_id: int                 # stream id for events and weights (C3 shares C2's)
+    n_events: int
+    tracks_mean: float
+    tracks_poisson: bool
+    noise_frac: float
+    emb_widths: Tuple[int, ...]  # e.g. (3, 128, 128, 128, 4)
+    gnn_hidden: int              # H = n_h = n_e
+    gnn_mlp_hidden_layers: int   # 2 -> three weight matrices per MLP
+    n_iter: int
+    target_degree: float
+    max_plane_gap: int = 3       # G (BASELINE.json C0 "plane gaps 1..3")
+    precision: int = PREC_FP32
+    gain: float = 0.5            # Q14 gain on the last layer of every node/edge network
+    calib_events: int = 16       # Q4: events used to calibrate r^2
+
+    @property
+    def emb_dim(self) -> int:
+        return self.emb_widths[-1]
+
+
+CONFIGS: Dict[str, Config] = {
+    # gains (Q14) chosen with the oracle so that scores spread over ~0.3..0.8 without saturating and
+    # bf16-operand error stays ~2.5x inside BASELINE.json's 2e-2
+    "c0": Config("c0", 0, 1, 20, False, 0.05, (3, 64, 64, 4), 64, 2, 4, 6.0, gain=0.8, calib_events=1),
+    "c1": Config("c1", 1, 1, 150, False, 0.05, (3, 128, 128, 128, 4), 128, 2, 6, 6.0, gain=0.5,
+                 calib_events=1),
+    "c2": Config("c2", 2, 1000, 150, True, 0.05, (3, 128, 128, 128, 4), 128, 2, 6, 6.0, gain=0.5),
+    "c3": Config("c3", 2, 1000, 150, True, 0.05, (3, 128, 128, 128, 4), 128, 2, 6, 6.0, gain=0.5,
+                 precision=PREC_BF16),
+    "c4": Config("c4", 4, 1000, 300, True, 0.10, (3, 128, 128, 128, 4), 128, 2, 8, 10.0, gain=0.3),
+}
+
+_P_EVENTS, _P_WEIGHTS = 1, 2
+(_S_NT, _S_VX, _S_VY, _S_VZ, _S_ETA, _S_PHI, _S_SMX, _S_SMY, _S_INEFF,
+ _S_NPLANE, _S_NR, _S_NPHI) = range(12)
+
+
+def plane_z() -> np.ndarray:
+    return PLANE_Z0 + PLANE_DZ * np.arange(N_PLANES, dtype=np.float64)
+
+
+def _n_tracks(cfg: Config, ev_ids: np.ndarray) -> np.ndarray:
+    if not cfg.tracks_poisson:
+        return np.full(len(ev_ids), int(cfg.tracks_mean), dtype=np.int64)
+    # Poisson(mean) = number of unit-rate exponential arrivals before `mean`
+    base = make_key(MASTER_SEED, cfg.seed_id, _P_EVENTS, _S_NT)
+    keys = _keys(base, ev_ids)[:, None]
+    m = int(2 * cfg.tracks_mean + 64)
+    u = uniform01(keys, np.arange(m)[None, :])
+    t = np.cumsum(-np.log1p(-u), axis=1)
+    return (t <= cfg.tracks_mean).sum(axis=1).astype(np.int64)
+
+
+def _gen_chunk(cfg: Config, ev_ids: np.ndarray):
+    """Hits of a few events -> per-hit arrays (event-local order not yet applied)."""
+    ne = len(ev_ids)
+    nt = _n_tracks(cfg, ev_ids)
+    mt = int(nt.max()) if ne else 0
+    zk = plane_z()
+
+    def ek(stream):
+        return _keys(make_key(MASTER_SEED, cfg.seed_id, _P_EVENTS, stream), ev_ids)
+
+    t_idx = np.arange(mt)[None, :]
+    vx = VTX_SIGMA_XY * normal01(ek(_S_VX)[:, None], t_idx)
+    vy = VTX_SIGMA_XY * normal01(ek(_S_VY)[:, None], t_idx)
+    vz = VTX_SIGMA_Z * normal01(ek(_S_VZ)[:, None], t_idx)
+    eta = ETA_MIN + (ETA_MAX - ETA_MIN) * uniform01(ek(_S_ETA)[:, None], t_idx)
+    phi = 2.0 * np.pi * uniform01(ek(_S_PHI)[:, None], t_idx)
+    slope = np.tan(2.0 * np.arctan(np.exp(-eta)))
+    valid_t = t_idx < nt[:, None]
+
+    dz = zk[None, None, :] - vz[:, :, None]                       # [ne, mt, 26]
+    xt = vx[:, :, None] + dz * (slope * np.cos(phi))[:, :, None]
+    yt = vy[:, :, None] + dz * (slope * np.sin(phi))[:, :, None]
+    rt = np.hypot(xt, yt)
+    tk = (t_idx[:, :, None] * N_PLANES + np.arange(N_PLANES)[None, None, :])
+    keep = uniform01(ek(_S_INEFF)[:, None, None], tk) >= HIT_INEFF
+    hit = valid_t[:, :, None] & (dz > 0.0) & (rt >= R_MIN) & (rt <= R_MAX) & keep
+    xs = xt + HIT_SMEAR * normal01(ek(_S_SMX)[:, None, None], tk)
+    ys = yt + HIT_SMEAR * normal01(ek(_S_SMY)[:, None, None], tk)
+
+    e_i, t_i, p_i = np.nonzero(hit)                                # row-major: event, track, plane
+    x_true, y_true = xs[e_i, t_i, p_i], ys[e_i, t_i, p_i]
+    n_true = np.bincount(e_i, minlength=ne)
+
+    # noise hits
+    n_noise = np.floor(cfg.noise_frac * n_true + 0.5).astype(np.int64)
+    mn = int(n_noise.max()) if ne else 0
+    n_idx = np.arange(mn)[None, :]
+    npl = np.minimum((uniform01(ek(_S_NPLANE)[:, None], n_idx) * N_PLANES).astype(np.int64), N_PLANES - 1)
+    nr = np.sqrt(R_MIN ** 2 + (R_MAX ** 2 - R_MIN ** 2) * uniform01(ek(_S_NR)[:, None], n_idx))
+    nphi = 2.0 * np.pi * uniform01(ek(_S_NPHI)[:, None], n_idx)
+    ne_i, nn_i = np.nonzero(n_idx < n_noise[:, None])
+
+    ev = np.concatenate([e_i, ne_i])
+    plane = np.concatenate([p_i, npl[ne_i, nn_i]])
+    order = np.concatenate([t_i * N_PLANES + p_i, mt * N_PLANES + nn_i])   # tracks first, noise last
+    x = np.concatenate([x_true, nr[ne_i, nn_i] * np.cos(nphi[ne_i, nn_i])])
+    y = np.concatenate([y_true, nr[ne_i, nn_i] * np.sin(nphi[ne_i, nn_i])])
+    track = np.concatenate([t_i, np.full(len(ne_i), -1, dtype=np.int64)])
+
+    perm = np.lexsort((order, plane, ev))
+    ev, plane, x, y, track = ev[perm], plane[perm], x[perm], y[perm], track[perm]
+    counts = np.bincount(ev, minlength=ne)
+    return counts, plane, x, y, track, nt
+
+
+def generate_events(cfg: Config, event_ids: Optional[Sequence[int]] = None, chunk: int = 64) -> Dict[str, np.ndarray]:
+    """CSR batch of events.  ``event_ids`` selects events of the config's stream (default: all).
+
+    Returns event_ptr int32 [n_ev+1], plane uint8 [N], r/phi/z/x/y float32 [N] (raw mm / rad),
+    track int32 [N] (generator track id, -1 noise), n_tracks int32 [n_ev].
+    """
+    ids = np.arange(cfg.n_events) if event_ids is None else np.asarray(event_ids, dtype=np.int64)
+    counts, planes, xs, ys, tracks, nts = [], [], [], [], [], []
+    for s in range(0, len(ids), chunk):
+        c, p, x, y, t, nt = _gen_chunk(cfg, ids[s:s + chunk])
+        counts.append(c); planes.append(p); xs.append(x); ys.append(y); tracks.append(t); nts.append(nt)
+    counts = np.concatenate(counts) if counts else np.zeros(0, np.int64)
+    plane = np.concatenate(planes) if planes else np.zeros(0, np.int64)
+    x = np.concatenate(xs) if xs else np.zeros(0)
+    y = np.concatenate(ys) if ys else np.zeros(0)
+    z = plane_z()[plane] if len(plane) else np.zeros(0)
+    event_ptr = np.zeros(len(ids) + 1, dtype=np.int64)
+    np.cumsum(counts, out=event_ptr[1:])
+    return {
+        "event_ptr": event_ptr.astype(np.int32),
+        "plane": plane.astype(np.uint8),
+        "r": np.hypot(x, y).astype(np.float32),
+        "phi": np.arctan2(y, x).astype(np.float32),
+        "z": z.astype(np.float32),
+        "x": x.astype(np.float32),
+        "y": y.astype(np.float32),
+        "track": (np.concatenate(tracks) if tracks else np.zeros(0, np.int64)).astype(np.int32),
+        "n_tracks": (np.concatenate(nts) if nts else np.zeros(0, np.int64)).astype(np.int32),
+    }
+
+
+def select_events(batch: Dict[str, np.ndarray], ev: Sequence[int]) -> Dict[str, np.ndarray]:
+    """Sub-batch holding the listed events of ``batch`` (copy)."""
+    ep = batch["event_ptr"].astype(np.int64)
+    idx = np.concatenate([np.arange(ep[e], ep[e + 1]) for e in ev]) if len(ev) else np.zeros(0, np.int64)
+    out = {k: batch[k][idx] for k in ("plane", "r", "phi", "z", "x", "y", "track")}
+    ptr = np.zeros(len(ev) + 1, dtype=np.int64)
+    np.cumsum([ep[e + 1] - ep[e] for e in ev], out=ptr[1:])
+    out["event_ptr"] = ptr.astype(np.int32)
+    out["n_tracks"] = batch["n_tracks"][np.asarray(ev, dtype=np.int64)]
+    return out
+
+
+# ----------------------------------------------------------------------------------------------
+# weights
+# ----------------------------------------------------------------------------------------------
+@dataclasses.dataclass(frozen=True)
+class MlpSpec:
+    name: str
+    dims: Tuple[int, ...]        # (in, hidden..., out)
+    offset: int                  # float offset of the first layer's W in the blob
+    gain: float = 1.0            # applied to the last layer's W and b
+
+    @property
+    def n_floats(self) -> int:
+        return sum(self.dims[i] * self.dims[i + 1] + self.dims[i + 1] for i in range(len(self.dims) - 1))
+
+    def layer_offsets(self) -> List[Tuple[int, int, int, int]]:
+        """[(w_offset, b_offset, fan_in, fan_out)] per layer; W is [out][in] row-major."""
+        res, o = [], self.offset
+        for i in range(len(self.dims) - 1):
+            fi, fo = self.dims[i], self.dims[i + 1]
+            res.append((o, o + fi * fo, fi, fo))
+            o += fi * fo + fo
+        return res
+
+
+def model_layout(cfg: Config) -> List[MlpSpec]:
+    """Blob order: embedding, node encoder, edge encoder, (node net k, edge net k) for k < n_iter,
+    classifier.  Every GNN MLP has ``gnn_mlp_hidden_layers`` hidden layers of width H."""
+    H, hl = cfg.gnn_hidden, cfg.gnn_mlp_hidden_layers
+    specs, off = [], 0
+
+    def add(name, dims, gain=1.0):
+        nonlocal off
+        s = MlpSpec(name, tuple(dims), off, gain)
+        specs.append(s)
+        off += s.n_floats
+
+    add("emb", cfg.emb_widths)
+    add("node_enc", (3,) + (H,) * hl + (H,))
+    add("edge_enc", (2 * H,) + (H,) * hl + (H,))
+    for k in range(cfg.n_iter):
+        add(f"node_net_{k}", (3 * H,) + (H,) * hl + (H,), cfg.gain)
+        add(f"edge_net_{k}", (3 * H,) + (H,) * hl + (H,), cfg.gain)
+    add("cls", (H,) + (H,) * hl + (1,))
+    return specs
+
+
+def n_weight_floats(cfg: Config) -> int:
+    s = model_layout(cfg)[-1]
+    return s.offset + s.n_floats
+
+
+def generate_weights(cfg: Config) -> np.ndarray:
+    """Flat fp32 blob in ``model_layout`` order (Xavier-uniform W, U(-0.05,0.05) b, Q14 gain)."""
+    blob = np.zeros(n_weight_floats(cfg), dtype=np.float32)
+    for mi, spec in enumerate(model_layout(cfg)):
+        layers = spec.layer_offsets()
+        for li, (wo, bo, fi, fo) in enumerate(layers):
+            g = spec.gain if li == len(layers) - 1 else 1.0
+            bound = np.sqrt(6.0 / (fi + fo))
+            kw = make_key(MASTER_SEED, cfg.seed_id, _P_WEIGHTS, mi, li, 0)
+            kb = make_key(MASTER_SEED, cfg.seed_id, _P_WEIGHTS, mi, li, 1)
+            w = (2.0 * uniform01(kw, np.arange(fi * fo)) - 1.0) * bound * g
+            b = (2.0 * uniform01(kb, np.arange(fo)) - 1.0) * 0.05 * g
+            blob[wo:wo + fi * fo] = w.astype(np.float32)
+            blob[bo:bo + fo] = b.astype(np.float32)
+    return blob
+
+
+# ----------------------------------------------------------------------------------------------
+# stored constants (radius per config), written by oracle/calibrate_radius.py (oracle-only script)
+# ----------------------------------------------------------------------------------------------
+_CONST_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "config_constants.json")
+
+
+def load_constants() -> Dict[str, dict]:
+    with open(_CONST_PATH) as f:
+        return json.load(f)
+
+
+def r2_max(cfg: Config) -> float:
+    """Stored fp32 r^2 for the config; both paths read this constant."""
+    key = {"c3": "c2"}.get(cfg.name, cfg.name)
+    return float(np.float32(load_constants()[key]["r2_max"]))
