@@ -1,0 +1,163 @@
+/* etx.h — C ABI of libetx: the hits -> edge-scores hot path of the ETX4VELO GNN tracking pipeline
+ * (F. Giasemis, arXiv 2508.07423; "P:n" = line n of PAPER.md), written for one NVIDIA B200 (sm_100a).
+ *
+ * The path (thesis §8.3; GPU pipeline steps P:2585-2593):
+ *   a0 features   recentre + rescale hit coordinates
+ *   a1 embed      embedding MLP, ReLU hidden layers, linear output (Eqs. 4.24-4.27)
+ *   a2 graph      hit i on plane p -> hits j of the same event on planes p+1..p+G with
+ *                 d^2(i,j) = |emb_i - emb_j|^2 < r2_max (Eq. 8.1)
+ *   a3 encoders   h0 = MLP_n(x,y,z) ; e0_ij = MLP_e([h0_i, h0_j])
+ *   a4-a6         n_iter x { m_l = [sum_{l->j} e_lj, sum_{i->l} e_il] (Eq. 8.5);
+ *                            h_l += phi_k([h_l, m_l]) ; e_ij += psi_k([h_i, h_j, e_ij]) }
+ *   a7 scores     s_ij = sigmoid(MLP_c(e_ij))
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE pointers owned by the caller (e.g. torch tensors); h_* are HOST
+ *     pointers.  The library never frees or reallocates caller memory.  `stream` is a cudaStream_t
+ *     passed as void* (NULL = default stream).  All work is enqueued on that stream.
+ *   - Every call returns an etx_status; no exceptions or aborts cross the ABI.  After a failure
+ *     etx_last_error(ctx) holds a message.  There is NO CPU fallback: without a CUDA device every
+ *     compute call returns ETX_ERR_CUDA.
+ *   - Events are independent; a batch is a CSR list of events: SoA fp32 hit arrays (P:2620,
+ *     P:2630) plus prefix-sum offsets.  Hits of an event must be sorted by plane.
+ *   - Weights: one flat fp32 host blob, MLPs in the order  embedding, node encoder, edge encoder,
+ *     (node network k, edge network k) for k = 0..n_iter-1, classifier; inside an MLP the layers are
+ *     consecutive, each W[out][in] row-major followed by b[out].  GNN MLPs have gnn_n_layers
+ *     matrices: in -> H -> ... -> H -> out with in = 3 (node enc), 2H (edge enc, [h_src, h_dst]),
+ *     3H (node net, [h, m_out, m_in]), 3H (edge net, [h_src, h_dst, e]), H (classifier, out = 1).
+ */
+#ifndef ETX_H_
+#define ETX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ETX_MAX_MLP_LAYERS 8
+
+typedef enum {
+  ETX_OK = 0,
+  ETX_ERR_INVALID = -1,   /* bad argument, unsupported shape, malformed batch                     */
+  ETX_ERR_CAPACITY = -2,  /* graph has more edges than edge_capacity (n_edges holds the need)     */
+  ETX_ERR_CUDA = -3,      /* CUDA runtime error or no device                                      */
+  ETX_ERR_UNSORTED = -4,  /* hits of an event are not sorted by plane                             */
+  ETX_ERR_NOMEM = -5      /* workspace missing or too small                                       */
+} etx_status;
+
+typedef enum {
+  ETX_PREC_FP32 = 0,    /* fp32 operands, FFMA on the CUDA cores, fp32 accumulate                 */
+  ETX_PREC_TF32X3 = 1,  /* tcgen05 tensor cores, error-compensated 3xTF32 split (fp32-equivalent) */
+  ETX_PREC_BF16 = 2     /* tcgen05 tensor cores, bf16 operands, fp32 accumulate, fp32 state       */
+} etx_precision;
+
+typedef struct {
+  int32_t emb_n_layers;                       /* weight matrices in the embedding MLP             */
+  int32_t emb_dims[ETX_MAX_MLP_LAYERS + 1];   /* e.g. {3,128,128,128,4}                           */
+  int32_t gnn_hidden;                         /* H = n_h = n_e; 64 or 128                */
+  int32_t gnn_n_layers;                       /* weight matrices per GNN MLP (hidden layers + 1)  */
+  int32_t n_iter;                             /* message-passing steps, distinct weights */
+  int32_t precision;                          /* etx_precision of the GNN / embedding MLPs        */
+  int32_t n_planes;                           /* 26                                      */
+  float norm_center[5];                       /* r, phi, z, x, y : f = (v - center) / scale       */
+  float norm_scale[5];
+} etx_model_desc;
+
+typedef struct {                /* CSR batch of events, device resident                           */
+  int32_t n_events, n_hits;
+  const int32_t* d_event_ptr;   /* [n_events+1] hit offsets, d_event_ptr[0] = 0                   */
+  const uint8_t* d_plane;       /* [n_hits] plane id < n_planes, ascending inside an event        */
+  const float *d_r, *d_phi, *d_z, *d_x, *d_y; /* [n_hits] raw mm / rad                            */
+} etx_batch;
+
+typedef struct {                /* same batch in HOST memory (for etx_infer_host)                 */
+  int32_t n_events, n_hits;
+  const int32_t* h_event_ptr;
+  const uint8_t* h_plane;
+  const float *h_r, *h_phi, *h_z, *h_x, *h_y;
+} etx_batch_host;
+
+typedef struct {                /* rough hit graph, arrays caller-allocated with capacity         */
+  int64_t edge_capacity;        /* in: entries available in d_src, d_dst, d_in_perm               */
+  int64_t n_edges;              /* out of etx_build_graph: E (also on ETX_ERR_CAPACITY)           */
+  int32_t* d_row_ptr;           /* [n_hits+1] CSR by source: edges of hit i are row_ptr[i]..      */
+  int32_t* d_src;               /* [cap] source hit of edge e; edges ordered (src asc, dst asc)   */
+  int32_t* d_dst;               /* [cap] destination hit of edge e                                */
+  int32_t* d_in_ptr;            /* [n_hits+1] CSR by destination                                  */
+  int32_t* d_in_perm;           /* [cap] edge ids entering hit j, in_ptr[j].., ascending edge id  */
+} etx_graph;
+
+typedef struct etx_ctx etx_ctx;
+
+/* Number of floats the weight blob must hold for `desc` (layout above); 0 if desc is invalid.     */
+size_t etx_weight_count(const etx_model_desc* desc);
+
+/* Create a context on CUDA device `device`: validates desc, copies the weights to the device and
+ * pre-arranges them for the kernels.  h_weights: host fp32 blob of n_weights floats.              */
+etx_status etx_create(etx_ctx** ctx, const etx_model_desc* desc, const float* h_weights,
+                      size_t n_weights, int device);
+etx_status etx_destroy(etx_ctx* ctx);
+const char* etx_last_error(const etx_ctx* ctx);   /* ctx may be NULL: last create error            */
+
+/* Device scratch the calls need for batches up to these sizes.  with_host_path adds the staging
+ * buffers etx_infer_host carves (device copies of the batch, embeddings, graph, encodings).       */
+size_t etx_workspace_bytes(const etx_ctx* ctx, int32_t n_events, int32_t n_hits,
+                           int64_t edge_capacity, int with_host_path);
+/* Hand the context a caller-owned device buffer (256-byte aligned); it stays caller-owned.        */
+etx_status etx_set_workspace(etx_ctx* ctx, void* d_workspace, size_t bytes);
+
+/* a0+a1: d_emb[n_hits, emb_dim] fp32 row-major = embedding MLP of ((r,phi,z) - center) / scale.   */
+etx_status etx_embed(etx_ctx* ctx, const etx_batch* batch, float* d_emb, void* stream);
+
+/* a2: fixed-radius search in embedding space.  Edge (i -> j) iff same event,
+ * 1 <= plane(j) - plane(i) <= max_plane_gap, and d^2 < r2_max with d^2 evaluated in fp32 as
+ * ((e0-f0)^2 + (e1-f1)^2) + ... left to right, each operation rounded (no FMA).  Output is the
+ * unique ordered CSR (src asc, dst asc) plus the by-destination lists.  k_max must be 0 (the k_max
+ * cap of P:2290 is not on this path).  Validates the batch (ETX_ERR_INVALID / ETX_ERR_UNSORTED).
+ * Synchronises the stream once to return g->n_edges; if E > edge_capacity returns ETX_ERR_CAPACITY
+ * with n_edges = E and d_src/d_dst/d_in_perm untouched.                                           */
+etx_status etx_build_graph(etx_ctx* ctx, const etx_batch* batch, const float* d_emb, float r2_max,
+                           int32_t max_plane_gap, int32_t k_max, etx_graph* g, void* stream);
+
+/* a3-a6: encoders + n_iter message-passing steps.  d_edge_enc [n_edges, H] fp32 receives e^n;
+ * d_hit_enc [n_hits, H] fp32 receives h^n if not NULL.                                            */
+etx_status etx_gnn_forward(etx_ctx* ctx, const etx_batch* batch, const etx_graph* g,
+                           float* d_edge_enc, float* d_hit_enc, void* stream);
+
+/* a7: d_scores[n_edges] fp32 = sigmoid(classifier(e)).                                            */
+etx_status etx_edge_scores(etx_ctx* ctx, const etx_graph* g, const float* d_edge_enc,
+                           float* d_scores, void* stream);
+
+/* Whole path with HOST buffers: copies the batch host->device, runs a0..a7, copies src/dst/scores
+ * back (h_src, h_dst may be NULL).  Needs a workspace sized with with_host_path = 1.  Host buffers
+ * should be pinned for the copies to be asynchronous.  Synchronises the stream before returning.  */
+etx_status etx_infer_host(etx_ctx* ctx, const etx_batch_host* batch, float r2_max,
+                          int32_t max_plane_gap, int64_t edge_capacity, int64_t* n_edges,
+                          int32_t* h_src, int32_t* h_dst, float* h_scores, void* stream);
+
+/* Number of kernels the library has launched on this context since creation (for accounting).     */
+int64_t etx_launch_count(const etx_ctx* ctx);
+
+/* Per-stage device timing.  While enabled, every group of launches of one class is bracketed by CUDA
+ * events on the call's stream.  etx_profile_read synchronises those events, returns the accumulated
+ * milliseconds and launch counts per class since the last read (arrays of ETX_K_COUNT), and resets.  */
+typedef enum {
+  ETX_K_EMBED = 0,      /* a0+a1 embedding MLP                                */
+  ETX_K_GRAPH = 1,      /* a2 plane index, search count/fill, scans           */
+  ETX_K_NODE_ENC = 2,   /* a3 node encoder                                    */
+  ETX_K_EDGE_ENC = 3,   /* a3 edge encoder                                    */
+  ETX_K_SCATTER = 4,    /* a4 message aggregation                             */
+  ETX_K_NODE_NET = 5,   /* a5 node network                                    */
+  ETX_K_EDGE_NET = 6,   /* a6 edge network (the dominant kernel)              */
+  ETX_K_CLS = 7,        /* a7 classifier + sigmoid                            */
+  ETX_K_COUNT = 8
+} etx_kernel_class;
+etx_status etx_profile_enable(etx_ctx* ctx, int on);
+etx_status etx_profile_read(etx_ctx* ctx, double* ms /*[ETX_K_COUNT]*/, int64_t* launches /*[ETX_K_COUNT]*/);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ETX_H_ */

@@ -1,0 +1,279 @@
+"""ctypes binding of libetx (include/etx.h): same names, argument marshalling only.
+
+PyTorch supplies device memory (tensors) and the stream; every step of the path runs in the library's
+kernels.  There is no fallback: if ``libetx.so`` is missing or fails to load, importing the symbols
+raises, and every failed call raises ``EtxError`` with the library's message.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Optional
+
+import numpy as np
+import torch
+
+from . import synth
+
+_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libetx.so")
+ETX_MAX_MLP_LAYERS = 8
+ETX_OK, ETX_ERR_INVALID, ETX_ERR_CAPACITY, ETX_ERR_CUDA, ETX_ERR_UNSORTED, ETX_ERR_NOMEM = 0, -1, -2, -3, -4, -5
+
+EXPORTS = ["etx_weight_count", "etx_create", "etx_destroy", "etx_last_error", "etx_workspace_bytes",
+           "etx_set_workspace", "etx_embed", "etx_build_graph", "etx_gnn_forward", "etx_edge_scores",
+           "etx_infer_host", "etx_launch_count", "etx_profile_enable", "etx_profile_read"]
+KERNEL_CLASSES = ["embed", "graph", "node_enc", "edge_enc", "scatter", "node_net", "edge_net", "cls"]
+
+
+class EtxError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"libetx status {status}: {msg}")
+        self.status = status
+
+
+class ModelDesc(C.Structure):
+    _fields_ = [("emb_n_layers", C.c_int32), ("emb_dims", C.c_int32 * (ETX_MAX_MLP_LAYERS + 1)),
+                ("gnn_hidden", C.c_int32), ("gnn_n_layers", C.c_int32), ("n_iter", C.c_int32),
+                ("precision", C.c_int32), ("n_planes", C.c_int32),
+                ("norm_center", C.c_float * 5), ("norm_scale", C.c_float * 5)]
+
+
+class Batch(C.Structure):
+    _fields_ = [("n_events", C.c_int32), ("n_hits", C.c_int32), ("d_event_ptr", C.c_void_p),
+                ("d_plane", C.c_void_p), ("d_r", C.c_void_p), ("d_phi", C.c_void_p), ("d_z", C.c_void_p),
+                ("d_x", C.c_void_p), ("d_y", C.c_void_p)]
+
+
+class BatchHost(C.Structure):
+    _fields_ = [("n_events", C.c_int32), ("n_hits", C.c_int32), ("h_event_ptr", C.c_void_p),
+                ("h_plane", C.c_void_p), ("h_r", C.c_void_p), ("h_phi", C.c_void_p), ("h_z", C.c_void_p),
+                ("h_x", C.c_void_p), ("h_y", C.c_void_p)]
+
+
+class Graph(C.Structure):
+    _fields_ = [("edge_capacity", C.c_int64), ("n_edges", C.c_int64), ("d_row_ptr", C.c_void_p),
+                ("d_src", C.c_void_p), ("d_dst", C.c_void_p), ("d_in_ptr", C.c_void_p),
+                ("d_in_perm", C.c_void_p)]
+
+
+_lib = None
+
+
+def load_library():
+    """Load libetx.so (in-tree).  Raises if it is missing — the product has no other path."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise FileNotFoundError(f"{_LIB_PATH} not built: run `python -m paper_2508_07423_b200.build` "
+                                    "(there is no CPU or PyTorch fallback)")
+        lib = C.CDLL(_LIB_PATH)
+        lib.etx_weight_count.restype = C.c_size_t
+        lib.etx_weight_count.argtypes = [C.POINTER(ModelDesc)]
+        lib.etx_create.restype = C.c_int
+        lib.etx_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(ModelDesc), C.c_void_p, C.c_size_t, C.c_int]
+        lib.etx_destroy.restype = C.c_int
+        lib.etx_destroy.argtypes = [C.c_void_p]
+        lib.etx_last_error.restype = C.c_char_p
+        lib.etx_last_error.argtypes = [C.c_void_p]
+        lib.etx_workspace_bytes.restype = C.c_size_t
+        lib.etx_workspace_bytes.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_int]
+        lib.etx_set_workspace.restype = C.c_int
+        lib.etx_set_workspace.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
+        lib.etx_embed.restype = C.c_int
+        lib.etx_embed.argtypes = [C.c_void_p, C.POINTER(Batch), C.c_void_p, C.c_void_p]
+        lib.etx_build_graph.restype = C.c_int
+        lib.etx_build_graph.argtypes = [C.c_void_p, C.POINTER(Batch), C.c_void_p, C.c_float, C.c_int32,
+                                        C.c_int32, C.POINTER(Graph), C.c_void_p]
+        lib.etx_gnn_forward.restype = C.c_int
+        lib.etx_gnn_forward.argtypes = [C.c_void_p, C.POINTER(Batch), C.POINTER(Graph), C.c_void_p,
+                                        C.c_void_p, C.c_void_p]
+        lib.etx_edge_scores.restype = C.c_int
+        lib.etx_edge_scores.argtypes = [C.c_void_p, C.POINTER(Graph), C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.etx_infer_host.restype = C.c_int
+        lib.etx_infer_host.argtypes = [C.c_void_p, C.POINTER(BatchHost), C.c_float, C.c_int32, C.c_int64,
+                                       C.POINTER(C.c_int64), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.etx_launch_count.restype = C.c_int64
+        lib.etx_launch_count.argtypes = [C.c_void_p]
+        lib.etx_profile_enable.restype = C.c_int
+        lib.etx_profile_enable.argtypes = [C.c_void_p, C.c_int]
+        lib.etx_profile_read.restype = C.c_int
+        lib.etx_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        _lib = lib
+    return _lib
+
+
+def make_desc(cfg: synth.Config, precision: Optional[int] = None) -> ModelDesc:
+    d = ModelDesc()
+    d.emb_n_layers = len(cfg.emb_widths) - 1
+    for i, w in enumerate(cfg.emb_widths):
+        d.emb_dims[i] = w
+    d.gnn_hidden = cfg.gnn_hidden
+    d.gnn_n_layers = cfg.gnn_mlp_hidden_layers + 1
+    d.n_iter = cfg.n_iter
+    d.precision = cfg.precision if precision is None else precision
+    d.n_planes = synth.N_PLANES
+    for i in range(5):
+        d.norm_center[i] = synth.NORM_CENTER[i]
+        d.norm_scale[i] = synth.NORM_SCALE[i]
+    return d
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+class DeviceBatch:
+    """Device-resident CSR batch (torch tensors) + the etx_batch struct that points at them."""
+
+    def __init__(self, batch: Dict[str, np.ndarray], device: torch.device):
+        self.n_events = len(batch["event_ptr"]) - 1
+        self.n_hits = len(batch["r"])
+        self.t = {k: torch.from_numpy(np.ascontiguousarray(batch[k])).to(device)
+                  for k in ("event_ptr", "plane", "r", "phi", "z", "x", "y")}
+        self.c = Batch(self.n_events, self.n_hits, *[_ptr(self.t[k]) for k in
+                                                     ("event_ptr", "plane", "r", "phi", "z", "x", "y")])
+
+
+class DeviceGraph:
+    def __init__(self, n_hits: int, capacity: int, device: torch.device):
+        i32 = dict(dtype=torch.int32, device=device)
+        self.row_ptr = torch.empty(n_hits + 1, **i32)
+        self.in_ptr = torch.empty(n_hits + 1, **i32)
+        self.src = torch.empty(max(capacity, 1), **i32)
+        self.dst = torch.empty(max(capacity, 1), **i32)
+        self.in_perm = torch.empty(max(capacity, 1), **i32)
+        self.c = Graph(capacity, 0, _ptr(self.row_ptr), _ptr(self.src), _ptr(self.dst), _ptr(self.in_ptr),
+                       _ptr(self.in_perm))
+
+    @property
+    def n_edges(self) -> int:
+        return int(self.c.n_edges)
+
+
+class Etx:
+    """One libetx context.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, desc: ModelDesc, weights: np.ndarray, device: int = 0):
+        self.lib = load_library()
+        self.desc = desc
+        self.device = torch.device("cuda", device)
+        w = np.ascontiguousarray(weights, dtype=np.float32)
+        self.handle = C.c_void_p()
+        st = self.lib.etx_create(C.byref(self.handle), C.byref(desc), w.ctypes.data_as(C.c_void_p), w.size, device)
+        if st != ETX_OK:
+            raise EtxError(st, self.lib.etx_last_error(None).decode())
+        self._ws = None
+
+    def close(self):
+        if getattr(self, "handle", None):
+            self.lib.etx_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st: int):
+        if st != ETX_OK:
+            raise EtxError(st, self.lib.etx_last_error(self.handle).decode())
+
+    @property
+    def emb_dim(self) -> int:
+        return int(self.desc.emb_dims[self.desc.emb_n_layers])
+
+    @staticmethod
+    def _stream() -> C.c_void_p:
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+    # ---- workspace
+    def workspace_bytes(self, n_events: int, n_hits: int, edge_capacity: int, with_host_path: bool = False) -> int:
+        return int(self.lib.etx_workspace_bytes(self.handle, n_events, n_hits, edge_capacity, int(with_host_path)))
+
+    def ensure_workspace(self, n_events: int, n_hits: int, edge_capacity: int, with_host_path: bool = False):
+        need = self.workspace_bytes(n_events, n_hits, edge_capacity, with_host_path)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+            off = (-self._ws.data_ptr()) % 256
+            self._check(self.lib.etx_set_workspace(self.handle, C.c_void_p(self._ws.data_ptr() + off), need))
+
+    def launch_count(self) -> int:
+        return int(self.lib.etx_launch_count(self.handle))
+
+    def profile_enable(self, on: bool = True):
+        self._check(self.lib.etx_profile_enable(self.handle, int(on)))
+
+    def profile_read(self):
+        """{class: (ms, launches)} accumulated since the last read."""
+        n = len(KERNEL_CLASSES)
+        ms = (C.c_double * n)()
+        ln = (C.c_int64 * n)()
+        self._check(self.lib.etx_profile_read(self.handle, ms, ln))
+        return {k: (float(ms[i]), int(ln[i])) for i, k in enumerate(KERNEL_CLASSES)}
+
+    # ---- the four path calls
+    def etx_embed(self, batch: DeviceBatch, emb: Optional[torch.Tensor] = None) -> torch.Tensor:
+        if emb is None:
+            emb = torch.empty(batch.n_hits, self.emb_dim, dtype=torch.float32, device=self.device)
+        self._check(self.lib.etx_embed(self.handle, C.byref(batch.c), _ptr(emb), self._stream()))
+        return emb
+
+    def etx_build_graph(self, batch: DeviceBatch, emb: torch.Tensor, r2_max: float, max_plane_gap: int,
+                        graph: DeviceGraph, k_max: int = 0) -> int:
+        self._check(self.lib.etx_build_graph(self.handle, C.byref(batch.c), _ptr(emb), r2_max, max_plane_gap,
+                                             k_max, C.byref(graph.c), self._stream()))
+        return graph.n_edges
+
+    def etx_gnn_forward(self, batch: DeviceBatch, graph: DeviceGraph, edge_enc: torch.Tensor,
+                        hit_enc: Optional[torch.Tensor] = None) -> torch.Tensor:
+        self._check(self.lib.etx_gnn_forward(self.handle, C.byref(batch.c), C.byref(graph.c), _ptr(edge_enc),
+                                             _ptr(hit_enc), self._stream()))
+        return edge_enc
+
+    def etx_edge_scores(self, graph: DeviceGraph, edge_enc: torch.Tensor, scores: torch.Tensor) -> torch.Tensor:
+        self._check(self.lib.etx_edge_scores(self.handle, C.byref(graph.c), _ptr(edge_enc), _ptr(scores),
+                                             self._stream()))
+        return scores
+
+    # ---- whole path with host buffers (pinned torch tensors or numpy arrays)
+    def etx_infer_host(self, host: Dict[str, torch.Tensor], r2_max: float, max_plane_gap: int,
+                       edge_capacity: int, out_src: Optional[torch.Tensor], out_dst: Optional[torch.Tensor],
+                       out_scores: torch.Tensor) -> int:
+        hb = BatchHost(len(host["event_ptr"]) - 1, len(host["r"]),
+                       *[C.c_void_p(host[k].data_ptr()) for k in ("event_ptr", "plane", "r", "phi", "z", "x", "y")])
+        n = C.c_int64(0)
+        st = self.lib.etx_infer_host(self.handle, C.byref(hb), r2_max, max_plane_gap, edge_capacity, C.byref(n),
+                                     None if out_src is None else C.c_void_p(out_src.data_ptr()),
+                                     None if out_dst is None else C.c_void_p(out_dst.data_ptr()),
+                                     C.c_void_p(out_scores.data_ptr()), self._stream())
+        self._check(st)
+        return int(n.value)
+
+
+def pinned_host_batch(batch: Dict[str, np.ndarray]) -> Dict[str, torch.Tensor]:
+    return {k: torch.from_numpy(np.ascontiguousarray(batch[k])).pin_memory()
+            for k in ("event_ptr", "plane", "r", "phi", "z", "x", "y")}
+
+
+def run_path(etx: Etx, batch: Dict[str, np.ndarray], r2_max: float, max_plane_gap: int,
+             edge_capacity: Optional[int] = None, graph_override=None) -> Dict[str, np.ndarray]:
+    """Convenience for tests: the four calls in order on device-resident inputs, results to numpy."""
+    dev = etx.device
+    db = DeviceBatch(batch, dev)
+    cap = edge_capacity if edge_capacity is not None else max(64 * db.n_hits, 1024)
+    etx.ensure_workspace(db.n_events, db.n_hits, cap)
+    emb = etx.etx_embed(db)
+    g = DeviceGraph(db.n_hits, cap, dev)
+    E = etx.etx_build_graph(db, emb, r2_max, max_plane_gap, g)
+    H = int(etx.desc.gnn_hidden)
+    e = torch.empty(max(E, 1), H, dtype=torch.float32, device=dev)
+    h = torch.empty(max(db.n_hits, 1), H, dtype=torch.float32, device=dev)
+    s = torch.empty(max(E, 1), dtype=torch.float32, device=dev)
+    etx.etx_gnn_forward(db, g, e, h)
+    etx.etx_edge_scores(g, e, s)
+    torch.cuda.synchronize()
+    return {"emb": emb.cpu().numpy(), "src": g.src[:E].cpu().numpy(), "dst": g.dst[:E].cpu().numpy(),
+            "row_ptr": g.row_ptr.cpu().numpy(), "in_ptr": g.in_ptr.cpu().numpy(),
+            "in_perm": g.in_perm[:E].cpu().numpy(), "h": h[:db.n_hits].cpu().numpy(), "e": e[:E].cpu().numpy(),
+            "scores": s[:E].cpu().numpy()}

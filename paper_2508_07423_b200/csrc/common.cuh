@@ -1,0 +1,101 @@
+// Internal declarations shared by the translation units of libetx (sm_100a).  Not part of the ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/etx.h"
+
+namespace etx {
+
+constexpr int kMaxLayers = ETX_MAX_MLP_LAYERS;
+
+// One MLP on the device.  Wt[l] is the layer's weight TRANSPOSED to [in][out] row-major (k-major, so
+// a K-chunk of it is a contiguous slab), b[l] its bias, both fp32.
+struct DevMlp {
+  int n_layers = 0;
+  int dims[kMaxLayers + 1] = {0};
+  const float* Wt[kMaxLayers] = {nullptr};
+  const float* b[kMaxLayers] = {nullptr};
+};
+
+struct Workspace {            // carved from the caller's buffer by carve_workspace()
+  int32_t* plane_ptr = nullptr;   // [n_events * (n_planes+1)]
+  int32_t* hit_event = nullptr;   // [n_hits]
+  int32_t* scan_tmp = nullptr;    // block sums for the device scan
+  int32_t* flags = nullptr;       // [8] validation flags / counters
+  float* h = nullptr;             // [n_hits, H]
+  float* m = nullptr;             // [n_hits, 2H]
+  // host-path staging
+  int32_t* s_event_ptr = nullptr; uint8_t* s_plane = nullptr;
+  float *s_r = nullptr, *s_phi = nullptr, *s_z = nullptr, *s_x = nullptr, *s_y = nullptr;
+  float* s_emb = nullptr;
+  int32_t *s_row_ptr = nullptr, *s_src = nullptr, *s_dst = nullptr, *s_in_ptr = nullptr, *s_in_perm = nullptr;
+  float* s_edge_enc = nullptr; float* s_scores = nullptr;
+  size_t total = 0;
+};
+
+}  // namespace etx
+
+struct etx_ctx {
+  etx_model_desc desc;
+  int device = 0;
+  int sm_count = 148;
+  float* d_weights = nullptr;      // transposed weights + biases, one allocation
+  size_t d_weights_floats = 0;
+  etx::DevMlp emb, node_enc, edge_enc, cls;
+  std::vector<etx::DevMlp> node_net, edge_net;
+  void* ws = nullptr;
+  size_t ws_bytes = 0;
+  int64_t launches = 0;
+  std::string err;
+  // per-stage profiling (etx_profile_enable / etx_profile_read)
+  bool prof_on = false;
+  struct ProfRec { int cls; int n; cudaEvent_t a, b; };
+  std::vector<ProfRec> prof_pending;
+  std::vector<cudaEvent_t> prof_pool;
+  double prof_ms[ETX_K_COUNT] = {0};
+  int64_t prof_n[ETX_K_COUNT] = {0};
+};
+
+namespace etx {
+
+// ---- graph.cu
+struct GraphArgs {
+  int n_events, n_hits, n_planes, d, gap;
+  float r2_max;
+  const int32_t* event_ptr; const uint8_t* plane; const float* emb;
+};
+// each returns the number of kernels launched; errors are reported through cudaGetLastError
+int launch_plane_index(const GraphArgs& a, int32_t* plane_ptr, int32_t* hit_event, int32_t* flags, cudaStream_t s);
+int launch_search_count(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
+                        const int32_t* flags, int32_t* out_deg, int32_t* in_deg, cudaStream_t s);
+int launch_exclusive_scan(int32_t* data /*[n+1], in place, data[n] = total*/, int n, int32_t* tmp, cudaStream_t s);
+int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
+                       const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst,
+                       const int32_t* in_ptr, int32_t* in_perm, cudaStream_t s);
+size_t scan_tmp_ints(int n);
+
+// ---- mlp_simt.cu
+struct Segment {              // input row r, column k (k < width): base[(idx ? idx[r] : r) * ld + k]
+  const float* base = nullptr; const int32_t* idx = nullptr; int width = 0; int ld = 0;
+};
+struct MlpArgs {
+  int n_rows = 0;
+  // first-layer input: either up to 3 gathered segments, or 3 features computed from SoA arrays
+  int n_seg = 0; Segment seg[3];
+  const float* feat[3] = {nullptr, nullptr, nullptr}; float fc[3] = {0, 0, 0}; float fs[3] = {1, 1, 1};
+  DevMlp mlp;
+  // output: mode 0 store, 1 residual add (out = res + y; res may alias out), 2 small-N linear,
+  // 3 small-N sigmoid
+  int out_mode = 0; float* out = nullptr; const float* res = nullptr; int out_ld = 0;
+};
+int launch_mlp_simt(const MlpArgs& a, cudaStream_t s);
+
+// ---- scatter.cu
+int launch_scatter(int n_nodes, int H, const int32_t* row_ptr, const int32_t* in_ptr,
+                   const int32_t* in_perm, const float* e, float* m, cudaStream_t s);
+
+}  // namespace etx

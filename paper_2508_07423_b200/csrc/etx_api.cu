@@ -1,0 +1,474 @@
+// C ABI of libetx (include/etx.h): context, weight staging, workspace carving, and the launch
+// sequences of the four path calls.  No arithmetic of the method happens on the host.
+#include <cstring>
+
+#include "common.cuh"
+
+namespace etx {
+namespace {
+
+std::string g_create_error;
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+bool valid_width(int h) { return h == 64 || h == 128; }
+
+const char* check_desc(const etx_model_desc* d) {
+  if (!d) return "desc is NULL";
+  if (d->emb_n_layers < 2 || d->emb_n_layers > kMaxLayers) return "emb_n_layers must be 2..8";
+  if (d->emb_dims[0] != 3) return "embedding input must be the 3 features (r, phi, z)";
+  for (int l = 1; l < d->emb_n_layers; ++l)
+    if (!valid_width(d->emb_dims[l]) || d->emb_dims[l] != d->emb_dims[1])
+      return "embedding hidden widths must all be 64 or all be 128";
+  if (d->emb_dims[d->emb_n_layers] < 1 || d->emb_dims[d->emb_n_layers] > 8) return "embedding dim must be 1..8";
+  if (!valid_width(d->gnn_hidden)) return "gnn_hidden must be 64 or 128";
+  if (d->gnn_n_layers < 2 || d->gnn_n_layers > kMaxLayers) return "gnn_n_layers must be 2..8";
+  if (d->n_iter < 0 || d->n_iter > 64) return "n_iter must be 0..64";
+  if (d->n_planes < 2 || d->n_planes > 255) return "n_planes must be 2..255";
+  if (d->precision < ETX_PREC_FP32 || d->precision > ETX_PREC_BF16) return "unknown precision";
+  for (int i = 0; i < 5; ++i)
+    if (!(d->norm_scale[i] != 0.0f)) return "norm_scale entries must be non-zero";
+  return nullptr;
+}
+
+struct HostMlp { int n_layers; int dims[kMaxLayers + 1]; };
+
+std::vector<HostMlp> mlp_list(const etx_model_desc& d) {
+  std::vector<HostMlp> v;
+  auto gnn = [&](int in, int out) {
+    HostMlp m; m.n_layers = d.gnn_n_layers; m.dims[0] = in;
+    for (int l = 1; l < d.gnn_n_layers; ++l) m.dims[l] = d.gnn_hidden;
+    m.dims[d.gnn_n_layers] = out;
+    return m;
+  };
+  HostMlp e; e.n_layers = d.emb_n_layers;
+  for (int l = 0; l <= d.emb_n_layers; ++l) e.dims[l] = d.emb_dims[l];
+  v.push_back(e);
+  const int H = d.gnn_hidden;
+  v.push_back(gnn(3, H));
+  v.push_back(gnn(2 * H, H));
+  for (int k = 0; k < d.n_iter; ++k) { v.push_back(gnn(3 * H, H)); v.push_back(gnn(3 * H, H)); }
+  v.push_back(gnn(H, 1));
+  return v;
+}
+
+size_t mlp_floats(const HostMlp& m) {
+  size_t n = 0;
+  for (int l = 0; l < m.n_layers; ++l) n += (size_t)m.dims[l] * m.dims[l + 1] + m.dims[l + 1];
+  return n;
+}
+
+Workspace carve(const etx_ctx* c, int32_t n_events, int32_t n_hits, int64_t cap, bool host_path, char* base) {
+  Workspace w;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { char* p = base ? base + off : nullptr; off += align_up(bytes ? bytes : 1, 256); return p; };
+  const int L = c->desc.n_planes, H = c->desc.gnn_hidden, d = c->desc.emb_dims[c->desc.emb_n_layers];
+  w.plane_ptr = (int32_t*)take(sizeof(int32_t) * (size_t)n_events * (L + 1));
+  w.hit_event = (int32_t*)take(sizeof(int32_t) * (size_t)n_hits);
+  w.scan_tmp = (int32_t*)take(sizeof(int32_t) * scan_tmp_ints(n_hits + 1));
+  w.flags = (int32_t*)take(sizeof(int32_t) * 8);
+  w.h = (float*)take(sizeof(float) * (size_t)n_hits * H);
+  w.m = (float*)take(sizeof(float) * (size_t)n_hits * 2 * H);
+  if (host_path) {
+    w.s_event_ptr = (int32_t*)take(sizeof(int32_t) * ((size_t)n_events + 1));
+    w.s_plane = (uint8_t*)take((size_t)n_hits);
+    w.s_r = (float*)take(sizeof(float) * (size_t)n_hits);
+    w.s_phi = (float*)take(sizeof(float) * (size_t)n_hits);
+    w.s_z = (float*)take(sizeof(float) * (size_t)n_hits);
+    w.s_x = (float*)take(sizeof(float) * (size_t)n_hits);
+    w.s_y = (float*)take(sizeof(float) * (size_t)n_hits);
+    w.s_emb = (float*)take(sizeof(float) * (size_t)n_hits * d);
+    w.s_row_ptr = (int32_t*)take(sizeof(int32_t) * ((size_t)n_hits + 1));
+    w.s_in_ptr = (int32_t*)take(sizeof(int32_t) * ((size_t)n_hits + 1));
+    w.s_src = (int32_t*)take(sizeof(int32_t) * (size_t)cap);
+    w.s_dst = (int32_t*)take(sizeof(int32_t) * (size_t)cap);
+    w.s_in_perm = (int32_t*)take(sizeof(int32_t) * (size_t)cap);
+    w.s_edge_enc = (float*)take(sizeof(float) * (size_t)cap * H);
+    w.s_scores = (float*)take(sizeof(float) * (size_t)cap);
+  }
+  w.total = off;
+  return w;
+}
+
+etx_status fail(etx_ctx* c, etx_status st, const std::string& msg) {
+  if (c) c->err = msg; else g_create_error = msg;
+  return st;
+}
+
+etx_status check_cuda(etx_ctx* c, const char* where) {
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(c, ETX_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+  return ETX_OK;
+}
+
+etx_status need_ws(etx_ctx* c, const Workspace& probe) {
+  if (!c->ws) return fail(c, ETX_ERR_NOMEM, "no workspace set (etx_set_workspace)");
+  if (probe.total > c->ws_bytes)
+    return fail(c, ETX_ERR_NOMEM, "workspace too small: need " + std::to_string(probe.total) + " bytes, have " +
+                                      std::to_string(c->ws_bytes));
+  return ETX_OK;
+}
+
+etx_status check_batch(etx_ctx* c, const etx_batch* b) {
+  if (!b) return fail(c, ETX_ERR_INVALID, "batch is NULL");
+  if (b->n_events < 0 || b->n_hits < 0) return fail(c, ETX_ERR_INVALID, "negative batch sizes");
+  if (!b->d_event_ptr) return fail(c, ETX_ERR_INVALID, "d_event_ptr is NULL");
+  if (b->n_hits > 0 && (!b->d_plane || !b->d_r || !b->d_phi || !b->d_z || !b->d_x || !b->d_y))
+    return fail(c, ETX_ERR_INVALID, "batch array is NULL");
+  return ETX_OK;
+}
+
+// Brackets a group of launches of one class with CUDA events when profiling is on.
+struct ProfScope {
+  etx_ctx* c; int cls; cudaStream_t s; int64_t l0; cudaEvent_t a = nullptr, b = nullptr;
+  ProfScope(etx_ctx* c_, int cls_, cudaStream_t s_) : c(c_), cls(cls_), s(s_), l0(c_->launches) {
+    if (!c->prof_on) return;
+    a = take(); b = take();
+    cudaEventRecord(a, s);
+  }
+  cudaEvent_t take() {
+    if (!c->prof_pool.empty()) { cudaEvent_t e = c->prof_pool.back(); c->prof_pool.pop_back(); return e; }
+    cudaEvent_t e; cudaEventCreate(&e); return e;
+  }
+  ~ProfScope() {
+    if (!a) return;
+    cudaEventRecord(b, s);
+    c->prof_pending.push_back(etx_ctx::ProfRec{cls, (int)(c->launches - l0), a, b});
+  }
+};
+
+int run_mlp(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
+  // precision dispatch: the tensor-core paths replace this call for the wide layers
+  return launch_mlp_simt(a, s);
+}
+
+}  // namespace
+}  // namespace etx
+
+using namespace etx;
+
+extern "C" {
+
+size_t etx_weight_count(const etx_model_desc* desc) {
+  if (check_desc(desc)) return 0;
+  size_t n = 0;
+  for (const HostMlp& m : mlp_list(*desc)) n += mlp_floats(m);
+  return n;
+}
+
+etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_weights,
+                      size_t n_weights, int device) {
+  if (!out) return fail(nullptr, ETX_ERR_INVALID, "ctx out pointer is NULL");
+  *out = nullptr;
+  if (const char* why = check_desc(desc)) return fail(nullptr, ETX_ERR_INVALID, why);
+  if (desc->precision != ETX_PREC_FP32)
+    return fail(nullptr, ETX_ERR_INVALID, "precision not available in this build");
+  if (!h_weights || n_weights != etx_weight_count(desc))
+    return fail(nullptr, ETX_ERR_INVALID, "weight blob size does not match desc (see etx_weight_count)");
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || device < 0 || device >= n_dev) {
+    cudaGetLastError();
+    return fail(nullptr, ETX_ERR_CUDA, "no such CUDA device (libetx has no CPU fallback)");
+  }
+  if (cudaSetDevice(device) != cudaSuccess) return fail(nullptr, ETX_ERR_CUDA, "cudaSetDevice failed");
+  etx_ctx* c = new etx_ctx();
+  c->desc = *desc;
+  c->device = device;
+  cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+
+  // stage weights: per layer W^T [in][out] (k-major) then b, every array 256-byte aligned
+  const std::vector<HostMlp> mlps = mlp_list(*desc);
+  std::vector<float> staged;
+  std::vector<DevMlp> dev(mlps.size());
+  std::vector<std::vector<size_t>> offW(mlps.size()), offB(mlps.size());
+  size_t src = 0;
+  for (size_t i = 0; i < mlps.size(); ++i) {
+    const HostMlp& m = mlps[i];
+    dev[i].n_layers = m.n_layers;
+    for (int l = 0; l <= m.n_layers; ++l) dev[i].dims[l] = m.dims[l];
+    for (int l = 0; l < m.n_layers; ++l) {
+      const int fi = m.dims[l], fo = m.dims[l + 1];
+      staged.resize(align_up(staged.size(), 64));
+      offW[i].push_back(staged.size());
+      staged.resize(staged.size() + (size_t)fi * fo);
+      float* Wt = staged.data() + offW[i].back();
+      const float* W = h_weights + src;                  // [out][in]
+      for (int o = 0; o < fo; ++o)
+        for (int k = 0; k < fi; ++k) Wt[(size_t)k * fo + o] = W[(size_t)o * fi + k];
+      src += (size_t)fi * fo;
+      staged.resize(align_up(staged.size(), 64));
+      offB[i].push_back(staged.size());
+      staged.insert(staged.end(), h_weights + src, h_weights + src + fo);
+      src += fo;
+    }
+  }
+  c->d_weights_floats = staged.size();
+  if (cudaMalloc(&c->d_weights, staged.size() * sizeof(float)) != cudaSuccess ||
+      cudaMemcpy(c->d_weights, staged.data(), staged.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) {
+    const std::string msg = std::string("weight upload failed: ") + cudaGetErrorString(cudaGetLastError());
+    if (c->d_weights) cudaFree(c->d_weights);
+    delete c;
+    return fail(nullptr, ETX_ERR_CUDA, msg);
+  }
+  for (size_t i = 0; i < mlps.size(); ++i)
+    for (int l = 0; l < mlps[i].n_layers; ++l) {
+      dev[i].Wt[l] = c->d_weights + offW[i][l];
+      dev[i].b[l] = c->d_weights + offB[i][l];
+    }
+  c->emb = dev[0];
+  c->node_enc = dev[1];
+  c->edge_enc = dev[2];
+  for (int k = 0; k < desc->n_iter; ++k) { c->node_net.push_back(dev[3 + 2 * k]); c->edge_net.push_back(dev[4 + 2 * k]); }
+  c->cls = dev.back();
+  *out = c;
+  return ETX_OK;
+}
+
+etx_status etx_destroy(etx_ctx* c) {
+  if (!c) return ETX_OK;
+  cudaSetDevice(c->device);
+  if (c->d_weights) cudaFree(c->d_weights);
+  for (const etx_ctx::ProfRec& r : c->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+  for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
+  delete c;
+  return ETX_OK;
+}
+
+const char* etx_last_error(const etx_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+size_t etx_workspace_bytes(const etx_ctx* c, int32_t n_events, int32_t n_hits, int64_t edge_capacity,
+                           int with_host_path) {
+  if (!c || n_events < 0 || n_hits < 0 || edge_capacity < 0) return 0;
+  return carve(c, n_events, n_hits, edge_capacity, with_host_path != 0, nullptr).total;
+}
+
+etx_status etx_set_workspace(etx_ctx* c, void* d_workspace, size_t bytes) {
+  if (!c) return ETX_ERR_INVALID;
+  if (((uintptr_t)d_workspace & 255) != 0) return fail(c, ETX_ERR_INVALID, "workspace must be 256-byte aligned");
+  c->ws = d_workspace;
+  c->ws_bytes = d_workspace ? bytes : 0;
+  return ETX_OK;
+}
+
+int64_t etx_launch_count(const etx_ctx* c) { return c ? c->launches : 0; }
+
+etx_status etx_profile_enable(etx_ctx* c, int on) {
+  if (!c) return ETX_ERR_INVALID;
+  c->prof_on = on != 0;
+  return ETX_OK;
+}
+
+etx_status etx_profile_read(etx_ctx* c, double* ms, int64_t* launches) {
+  if (!c) return ETX_ERR_INVALID;
+  cudaSetDevice(c->device);
+  for (const etx_ctx::ProfRec& r : c->prof_pending) {
+    float t = 0.f;
+    if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&t, r.a, r.b) != cudaSuccess)
+      return check_cuda(c, "etx_profile_read");
+    c->prof_ms[r.cls] += t;
+    c->prof_n[r.cls] += r.n;
+    c->prof_pool.push_back(r.a);
+    c->prof_pool.push_back(r.b);
+  }
+  c->prof_pending.clear();
+  for (int i = 0; i < ETX_K_COUNT; ++i) {
+    if (ms) ms[i] = c->prof_ms[i];
+    if (launches) launches[i] = c->prof_n[i];
+    c->prof_ms[i] = 0; c->prof_n[i] = 0;
+  }
+  return ETX_OK;
+}
+
+etx_status etx_embed(etx_ctx* c, const etx_batch* b, float* d_emb, void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (etx_status st = check_batch(c, b)) return st;
+  if (b->n_hits > 0 && !d_emb) return fail(c, ETX_ERR_INVALID, "d_emb is NULL");
+  cudaSetDevice(c->device);
+  MlpArgs a;
+  a.n_rows = b->n_hits;
+  a.n_seg = 0;
+  a.feat[0] = b->d_r; a.feat[1] = b->d_phi; a.feat[2] = b->d_z;
+  for (int i = 0; i < 3; ++i) { a.fc[i] = c->desc.norm_center[i]; a.fs[i] = c->desc.norm_scale[i]; }
+  a.mlp = c->emb;
+  a.out_mode = 2;
+  a.out = d_emb;
+  a.out_ld = c->emb.dims[c->emb.n_layers];
+  {
+    ProfScope ps(c, ETX_K_EMBED, (cudaStream_t)stream);
+    c->launches += run_mlp(c, a, (cudaStream_t)stream);
+  }
+  return check_cuda(c, "etx_embed");
+}
+
+etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, float r2_max,
+                           int32_t max_plane_gap, int32_t k_max, etx_graph* g, void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (etx_status st = check_batch(c, b)) return st;
+  if (!g || !g->d_row_ptr || !g->d_in_ptr) return fail(c, ETX_ERR_INVALID, "graph or its offset arrays are NULL");
+  if (k_max != 0) return fail(c, ETX_ERR_INVALID, "k_max cap is not on this path (must be 0)");
+  if (max_plane_gap < 1) return fail(c, ETX_ERR_INVALID, "max_plane_gap must be >= 1");
+  if (b->n_hits > 0 && !d_emb) return fail(c, ETX_ERR_INVALID, "d_emb is NULL");
+  if (g->edge_capacity < 0 || (g->edge_capacity > 0 && (!g->d_src || !g->d_dst || !g->d_in_perm)))
+    return fail(c, ETX_ERR_INVALID, "edge arrays are NULL");
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  if (etx_status st = need_ws(c, carve(c, b->n_events, b->n_hits, 0, false, nullptr))) return st;
+  const Workspace w = carve(c, b->n_events, b->n_hits, 0, false, (char*)c->ws);
+  GraphArgs a;
+  a.n_events = b->n_events; a.n_hits = b->n_hits; a.n_planes = c->desc.n_planes;
+  a.d = c->emb.dims[c->emb.n_layers]; a.gap = max_plane_gap; a.r2_max = r2_max;
+  a.event_ptr = b->d_event_ptr; a.plane = b->d_plane; a.emb = d_emb;
+
+  {
+    ProfScope ps(c, ETX_K_GRAPH, s);
+    c->launches += launch_plane_index(a, w.plane_ptr, w.hit_event, w.flags, s);
+    c->launches += launch_search_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_in_ptr, s);
+    c->launches += launch_exclusive_scan(g->d_row_ptr, b->n_hits + 1, w.scan_tmp, s);
+    c->launches += launch_exclusive_scan(g->d_in_ptr, b->n_hits + 1, w.scan_tmp, s);
+  }
+  int32_t host[2] = {0, 0};
+  cudaMemcpyAsync(&host[0], w.flags, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+  cudaMemcpyAsync(&host[1], g->d_row_ptr + b->n_hits, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+  if (cudaStreamSynchronize(s) != cudaSuccess) return check_cuda(c, "etx_build_graph (count)");
+  if (etx_status st = check_cuda(c, "etx_build_graph (count)")) return st;
+  if (host[0] & 1) return fail(c, ETX_ERR_INVALID, "malformed batch: event_ptr not monotone / plane id >= n_planes");
+  if (host[0] & 2) return fail(c, ETX_ERR_UNSORTED, "hits of an event are not sorted by plane");
+  g->n_edges = host[1];
+  if (g->n_edges > g->edge_capacity)
+    return fail(c, ETX_ERR_CAPACITY, "graph needs " + std::to_string(g->n_edges) + " edges, capacity " +
+                                         std::to_string(g->edge_capacity));
+  if (g->n_edges > 0) {
+    ProfScope ps(c, ETX_K_GRAPH, s);
+    c->launches += launch_search_fill(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_src, g->d_dst,
+                                      g->d_in_ptr, g->d_in_perm, s);
+  }
+  return check_cuda(c, "etx_build_graph (fill)");
+}
+
+etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, float* d_edge_enc,
+                           float* d_hit_enc, void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (etx_status st = check_batch(c, b)) return st;
+  if (!g || g->n_edges < 0 || g->n_edges > g->edge_capacity) return fail(c, ETX_ERR_INVALID, "graph is NULL or not built");
+  if (g->n_edges > 0 && !d_edge_enc) return fail(c, ETX_ERR_INVALID, "d_edge_enc is NULL");
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  if (etx_status st = need_ws(c, carve(c, b->n_events, b->n_hits, 0, false, nullptr))) return st;
+  const Workspace w = carve(c, b->n_events, b->n_hits, 0, false, (char*)c->ws);
+  const int H = c->desc.gnn_hidden, N = b->n_hits;
+  const int E = (int)g->n_edges;
+
+  {  // a3: h0 = MLP_n((x,y,z) normalised)
+    MlpArgs a;
+    a.n_rows = N; a.n_seg = 0;
+    a.feat[0] = b->d_x; a.feat[1] = b->d_y; a.feat[2] = b->d_z;
+    const int id[3] = {3, 4, 2};
+    for (int i = 0; i < 3; ++i) { a.fc[i] = c->desc.norm_center[id[i]]; a.fs[i] = c->desc.norm_scale[id[i]]; }
+    a.mlp = c->node_enc; a.out_mode = 0; a.out = w.h; a.out_ld = H;
+    ProfScope ps(c, ETX_K_NODE_ENC, s);
+    c->launches += run_mlp(c, a, s);
+  }
+  {  // a3: e0 = MLP_e([h0_src, h0_dst])
+    MlpArgs a;
+    a.n_rows = E; a.n_seg = 2;
+    a.seg[0] = Segment{w.h, g->d_src, H, H};
+    a.seg[1] = Segment{w.h, g->d_dst, H, H};
+    a.mlp = c->edge_enc; a.out_mode = 0; a.out = d_edge_enc; a.out_ld = H;
+    ProfScope ps(c, ETX_K_EDGE_ENC, s);
+    c->launches += run_mlp(c, a, s);
+  }
+  for (int k = 0; k < c->desc.n_iter; ++k) {
+    // a4: m = [sum out, sum in] of e^k
+    {
+      ProfScope ps(c, ETX_K_SCATTER, s);
+      c->launches += launch_scatter(N, H, g->d_row_ptr, g->d_in_ptr, g->d_in_perm, d_edge_enc, w.m, s);
+    }
+    {  // a5: h += phi_k([h, m])
+      MlpArgs a;
+      a.n_rows = N; a.n_seg = 2;
+      a.seg[0] = Segment{w.h, nullptr, H, H};
+      a.seg[1] = Segment{w.m, nullptr, 2 * H, 2 * H};
+      a.mlp = c->node_net[k]; a.out_mode = 1; a.out = w.h; a.res = w.h; a.out_ld = H;
+      ProfScope ps(c, ETX_K_NODE_NET, s);
+      c->launches += run_mlp(c, a, s);
+    }
+    {  // a6: e += psi_k([h_src, h_dst, e]) with the UPDATED h
+      MlpArgs a;
+      a.n_rows = E; a.n_seg = 3;
+      a.seg[0] = Segment{w.h, g->d_src, H, H};
+      a.seg[1] = Segment{w.h, g->d_dst, H, H};
+      a.seg[2] = Segment{d_edge_enc, nullptr, H, H};
+      a.mlp = c->edge_net[k]; a.out_mode = 1; a.out = d_edge_enc; a.res = d_edge_enc; a.out_ld = H;
+      ProfScope ps(c, ETX_K_EDGE_NET, s);
+      c->launches += run_mlp(c, a, s);
+    }
+  }
+  if (d_hit_enc && N > 0)
+    cudaMemcpyAsync(d_hit_enc, w.h, sizeof(float) * (size_t)N * H, cudaMemcpyDeviceToDevice, s);
+  return check_cuda(c, "etx_gnn_forward");
+}
+
+etx_status etx_edge_scores(etx_ctx* c, const etx_graph* g, const float* d_edge_enc, float* d_scores,
+                           void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (!g || g->n_edges < 0) return fail(c, ETX_ERR_INVALID, "graph is NULL or not built");
+  if (g->n_edges > 0 && (!d_edge_enc || !d_scores)) return fail(c, ETX_ERR_INVALID, "d_edge_enc / d_scores is NULL");
+  cudaSetDevice(c->device);
+  const int H = c->desc.gnn_hidden;
+  MlpArgs a;
+  a.n_rows = (int)g->n_edges; a.n_seg = 1;
+  a.seg[0] = Segment{d_edge_enc, nullptr, H, H};
+  a.mlp = c->cls; a.out_mode = 3; a.out = d_scores; a.out_ld = 1;
+  {
+    ProfScope ps(c, ETX_K_CLS, (cudaStream_t)stream);
+    c->launches += run_mlp(c, a, (cudaStream_t)stream);
+  }
+  return check_cuda(c, "etx_edge_scores");
+}
+
+etx_status etx_infer_host(etx_ctx* c, const etx_batch_host* hb, float r2_max, int32_t max_plane_gap,
+                          int64_t edge_capacity, int64_t* n_edges, int32_t* h_src, int32_t* h_dst,
+                          float* h_scores, void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (!hb || hb->n_events < 0 || hb->n_hits < 0 || !hb->h_event_ptr || edge_capacity < 0)
+    return fail(c, ETX_ERR_INVALID, "host batch is NULL or malformed");
+  if (hb->n_hits > 0 && (!hb->h_plane || !hb->h_r || !hb->h_phi || !hb->h_z || !hb->h_x || !hb->h_y))
+    return fail(c, ETX_ERR_INVALID, "host batch array is NULL");
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  if (etx_status st = need_ws(c, carve(c, hb->n_events, hb->n_hits, edge_capacity, true, nullptr))) return st;
+  const Workspace w = carve(c, hb->n_events, hb->n_hits, edge_capacity, true, (char*)c->ws);
+  const size_t nh = (size_t)hb->n_hits;
+  cudaMemcpyAsync(w.s_event_ptr, hb->h_event_ptr, sizeof(int32_t) * ((size_t)hb->n_events + 1), cudaMemcpyHostToDevice, s);
+  if (nh) {
+    cudaMemcpyAsync(w.s_plane, hb->h_plane, nh, cudaMemcpyHostToDevice, s);
+    cudaMemcpyAsync(w.s_r, hb->h_r, nh * 4, cudaMemcpyHostToDevice, s);
+    cudaMemcpyAsync(w.s_phi, hb->h_phi, nh * 4, cudaMemcpyHostToDevice, s);
+    cudaMemcpyAsync(w.s_z, hb->h_z, nh * 4, cudaMemcpyHostToDevice, s);
+    cudaMemcpyAsync(w.s_x, hb->h_x, nh * 4, cudaMemcpyHostToDevice, s);
+    cudaMemcpyAsync(w.s_y, hb->h_y, nh * 4, cudaMemcpyHostToDevice, s);
+  }
+  etx_batch b;
+  b.n_events = hb->n_events; b.n_hits = hb->n_hits;
+  b.d_event_ptr = w.s_event_ptr; b.d_plane = w.s_plane;
+  b.d_r = w.s_r; b.d_phi = w.s_phi; b.d_z = w.s_z; b.d_x = w.s_x; b.d_y = w.s_y;
+  etx_graph g;
+  g.edge_capacity = edge_capacity; g.n_edges = 0;
+  g.d_row_ptr = w.s_row_ptr; g.d_src = w.s_src; g.d_dst = w.s_dst; g.d_in_ptr = w.s_in_ptr; g.d_in_perm = w.s_in_perm;
+  if (etx_status st = etx_embed(c, &b, w.s_emb, stream)) return st;
+  etx_status st = etx_build_graph(c, &b, w.s_emb, r2_max, max_plane_gap, 0, &g, stream);
+  if (n_edges) *n_edges = g.n_edges;
+  if (st) return st;
+  if ((st = etx_gnn_forward(c, &b, &g, w.s_edge_enc, nullptr, stream))) return st;
+  if ((st = etx_edge_scores(c, &g, w.s_edge_enc, w.s_scores, stream))) return st;
+  const size_t ne = (size_t)g.n_edges;
+  if (ne) {
+    if (h_src) cudaMemcpyAsync(h_src, w.s_src, ne * 4, cudaMemcpyDeviceToHost, s);
+    if (h_dst) cudaMemcpyAsync(h_dst, w.s_dst, ne * 4, cudaMemcpyDeviceToHost, s);
+    if (h_scores) cudaMemcpyAsync(h_scores, w.s_scores, ne * 4, cudaMemcpyDeviceToHost, s);
+  }
+  if (cudaStreamSynchronize(s) != cudaSuccess) return check_cuda(c, "etx_infer_host");
+  return check_cuda(c, "etx_infer_host");
+}
+
+}  // extern "C"

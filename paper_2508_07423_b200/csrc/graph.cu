@@ -1,0 +1,278 @@
+// a2 — rough graph construction by fixed-radius search in embedding space (Eq. 8.1; P:2290;
+// sequential reference loop P:2674).  The thesis' kernel ran one thread per source hit looping over
+// the candidates ("lacks parallelization over neighbors").  Here one WARP owns a hit and its
+// 32 lanes test 32 candidates at a time; the candidates of a hit on plane p are the contiguous index
+// range of planes p+1..p+G of the same event (hits are plane-sorted, per-(event, plane) offsets are
+// the buckets), so loads are coalesced float4 reads that stay in L1/L2 (an event's embeddings are
+// ~25 KB).  A count pass, a device scan and a fill pass with ballot / popc compaction give the unique
+// ordered CSR (src asc, dst asc) with no atomics; the by-destination lists are produced the same way
+// by searching backwards (planes p-G..p-1) and locating the edge id by binary search in the
+// source's sorted neighbour list.
+//
+// d^2 is evaluated exactly as the ABI states: fp32, left to right, __fsub_rn/__fmul_rn/__fadd_rn so
+// that ptxas cannot contract to FMA — graph edges must match the oracle bit for bit.
+#include "common.cuh"
+
+namespace etx {
+namespace {
+
+constexpr int kWarpsPerBlock = 8;
+constexpr unsigned kFull = 0xffffffffu;
+
+__global__ void plane_index_kernel(GraphArgs a, int32_t* __restrict__ plane_ptr,
+                                   int32_t* __restrict__ hit_event, int32_t* __restrict__ flags) {
+  const int L = a.n_planes;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    if (a.event_ptr[0] != 0 || a.event_ptr[a.n_events] != a.n_hits) atomicOr(&flags[0], 1);
+  }
+  for (int ev = blockIdx.x; ev < a.n_events; ev += gridDim.x) {
+    const int lo = a.event_ptr[ev], hi = a.event_ptr[ev + 1];
+    if (lo < 0 || hi < lo || hi > a.n_hits) {
+      if (threadIdx.x == 0) atomicOr(&flags[0], 1);
+      continue;
+    }
+    int32_t* pp = plane_ptr + (size_t)ev * (L + 1);
+    for (int i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+      const int cur = a.plane[i];
+      const int prev = (i == lo) ? -1 : (int)a.plane[i - 1];
+      hit_event[i] = ev;
+      if (cur >= L) { atomicOr(&flags[0], 1); continue; }
+      if (cur < prev) { atomicOr(&flags[0], 2); continue; }
+      for (int p = prev + 1; p <= cur; ++p) pp[p] = i;     // first hit of planes prev+1..cur
+    }
+    if (threadIdx.x == 0) {
+      const int last = (hi > lo) ? (int)a.plane[hi - 1] : -1;
+      for (int p = last + 1; p <= L; ++p) pp[p] = hi;
+    }
+  }
+}
+
+template <int D>
+__device__ __forceinline__ void load_emb(const float* __restrict__ emb, int i, int d, float (&v)[8]) {
+  if (D == 4) {
+    const float4 t = __ldg(reinterpret_cast<const float4*>(emb) + i);
+    v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+  } else {
+#pragma unroll
+    for (int c = 0; c < 8; ++c) v[c] = (c < d) ? __ldg(emb + (size_t)i * d + c) : 0.0f;
+  }
+}
+
+template <int D>
+__device__ __forceinline__ float dist2(const float (&a)[8], const float (&b)[8], int d) {
+  float s = 0.0f;
+  const int n = (D == 4) ? 4 : d;
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    if (c < n) {
+      const float diff = __fsub_rn(a[c], b[c]);
+      const float sq = __fmul_rn(diff, diff);
+      s = (c == 0) ? sq : __fadd_rn(s, sq);
+    }
+  }
+  return s;
+}
+
+// MODE 0: count out- and in-degree.  MODE 1: fill out-edges.  MODE 2: fill in-edge permutation.
+template <int D, int MODE>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+search_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t* __restrict__ hit_event,
+              const int32_t* __restrict__ flags, int32_t* __restrict__ out_deg,
+              int32_t* __restrict__ in_deg, const int32_t* __restrict__ row_ptr,
+              int32_t* __restrict__ src, int32_t* __restrict__ dst,
+              const int32_t* __restrict__ in_ptr, int32_t* __restrict__ in_perm) {
+  if (flags[0] != 0) return;                       // malformed batch: plane_ptr is not trustworthy
+  const int lane = threadIdx.x & 31;
+  const int warp = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+  const int n_warps = gridDim.x * kWarpsPerBlock;
+  const unsigned lt = (1u << lane) - 1u;
+  const int L = a.n_planes;
+  for (int i = warp; i < a.n_hits; i += n_warps) {
+    const int ev = hit_event[i];
+    const int p = a.plane[i];
+    const int32_t* pp = plane_ptr + (size_t)ev * (L + 1);
+    float me[8], other[8];
+    load_emb<D>(a.emb, i, a.d, me);
+    if (MODE == 0 || MODE == 1) {                  // forward: i is the source
+      int cnt = 0;
+      if (p <= L - 2) {
+        const int j0 = pp[p + 1];
+        const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
+        const int j1 = pp[top + 1];
+        const int base_out = (MODE == 1) ? row_ptr[i] : 0;
+        for (int base = j0; base < j1; base += 32) {
+          const int j = base + lane;
+          bool ok = false;
+          if (j < j1) {
+            load_emb<D>(a.emb, j, a.d, other);
+            ok = dist2<D>(me, other, a.d) < a.r2_max;
+          }
+          const unsigned b = __ballot_sync(kFull, ok);
+          if (MODE == 1 && ok) {
+            const int pos = base_out + cnt + __popc(b & lt);
+            src[pos] = i;
+            dst[pos] = j;
+          }
+          cnt += __popc(b);
+        }
+      }
+      if (MODE == 0 && lane == 0) out_deg[i] = cnt;
+    }
+    if (MODE == 0 || MODE == 2) {                  // backward: i is the destination
+      int cnt = 0;
+      if (p >= 1) {
+        const int bot = (p - a.gap > 0) ? p - a.gap : 0;
+        const int s0 = pp[bot], s1 = pp[p];
+        const int base_in = (MODE == 2) ? in_ptr[i] : 0;
+        for (int base = s0; base < s1; base += 32) {
+          const int sidx = base + lane;
+          bool ok = false;
+          if (sidx < s1) {
+            load_emb<D>(a.emb, sidx, a.d, other);
+            ok = dist2<D>(other, me, a.d) < a.r2_max;     // source first, as in the forward pass
+          }
+          const unsigned b = __ballot_sync(kFull, ok);
+          if (MODE == 2 && ok) {
+            int lo = row_ptr[sidx], hi = row_ptr[sidx + 1];   // find i in the source's sorted list
+            while (lo < hi) {
+              const int mid = (lo + hi) >> 1;
+              if (dst[mid] < i) lo = mid + 1; else hi = mid;
+            }
+            in_perm[base_in + cnt + __popc(b & lt)] = lo;
+          }
+          cnt += __popc(b);
+        }
+      }
+      if (MODE == 0 && lane == 0) in_deg[i] = cnt;
+    }
+  }
+  if (MODE == 0 && blockIdx.x == 0 && threadIdx.x == 0) { out_deg[a.n_hits] = 0; in_deg[a.n_hits] = 0; }
+}
+
+// ------------------------------------------------------------------ device-wide exclusive scan
+constexpr int kScanThreads = 256;
+constexpr int kScanPerThread = 8;
+constexpr int kScanTile = kScanThreads * kScanPerThread;
+
+__device__ __forceinline__ int block_exclusive_scan(int v, int* total) {
+  __shared__ int warp_sums[kScanThreads / 32];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int t = __shfl_up_sync(kFull, inc, o);
+    if (lane >= o) inc += t;
+  }
+  if (lane == 31) warp_sums[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    int s = (lane < kScanThreads / 32) ? warp_sums[lane] : 0;
+#pragma unroll
+    for (int o = 1; o < kScanThreads / 32; o <<= 1) {
+      const int t = __shfl_up_sync(kFull, s, o);
+      if (lane >= o) s += t;
+    }
+    if (lane < kScanThreads / 32) warp_sums[lane] = s;
+  }
+  __syncthreads();
+  const int before = (w == 0) ? 0 : warp_sums[w - 1];
+  *total = warp_sums[kScanThreads / 32 - 1];
+  __syncthreads();
+  return before + inc - v;
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_block_sums(const int32_t* __restrict__ data, int n,
+                                                                int32_t* __restrict__ tmp) {
+  const int base = blockIdx.x * kScanTile + threadIdx.x * kScanPerThread;
+  int s = 0;
+#pragma unroll
+  for (int k = 0; k < kScanPerThread; ++k) s += (base + k < n) ? data[base + k] : 0;
+  int total;
+  block_exclusive_scan(s, &total);
+  if (threadIdx.x == 0) tmp[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_tmp_kernel(int32_t* __restrict__ tmp, int nb) {
+  int carry = 0;
+  for (int base = 0; base < nb; base += kScanThreads) {
+    const int i = base + threadIdx.x;
+    const int v = (i < nb) ? tmp[i] : 0;
+    int total;
+    const int ex = block_exclusive_scan(v, &total);
+    if (i < nb) tmp[i] = carry + ex;
+    carry += total;
+  }
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_apply(int32_t* __restrict__ data, int n,
+                                                           const int32_t* __restrict__ tmp) {
+  const int base = blockIdx.x * kScanTile + threadIdx.x * kScanPerThread;
+  int v[kScanPerThread];
+  int s = 0;
+#pragma unroll
+  for (int k = 0; k < kScanPerThread; ++k) { v[k] = (base + k < n) ? data[base + k] : 0; s += v[k]; }
+  int total;
+  int run = block_exclusive_scan(s, &total) + tmp[blockIdx.x];
+#pragma unroll
+  for (int k = 0; k < kScanPerThread; ++k) {
+    if (base + k < n) data[base + k] = run;
+    run += v[k];
+  }
+}
+
+inline int search_grid(int n_hits) {
+  const int need = (n_hits + kWarpsPerBlock - 1) / kWarpsPerBlock;
+  const int cap = 148 * 8;                         // 8 resident CTAs of 256 threads per SM
+  return need < 1 ? 1 : (need < cap ? need : cap);
+}
+
+}  // namespace
+
+size_t scan_tmp_ints(int n) { return (size_t)((n + kScanTile - 1) / kScanTile) + 1; }
+
+int launch_plane_index(const GraphArgs& a, int32_t* plane_ptr, int32_t* hit_event, int32_t* flags,
+                       cudaStream_t s) {
+  cudaMemsetAsync(flags, 0, 8 * sizeof(int32_t), s);
+  const int grid = a.n_events < 1 ? 1 : (a.n_events < 148 * 16 ? a.n_events : 148 * 16);
+  plane_index_kernel<<<grid, 128, 0, s>>>(a, plane_ptr, hit_event, flags);
+  return 1;
+}
+
+template <int MODE>
+static void launch_search(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
+                          const int32_t* flags, int32_t* out_deg, int32_t* in_deg,
+                          const int32_t* row_ptr, int32_t* src, int32_t* dst, const int32_t* in_ptr,
+                          int32_t* in_perm, cudaStream_t s) {
+  const int grid = search_grid(a.n_hits);
+  if (a.d == 4)
+    search_kernel<4, MODE><<<grid, kWarpsPerBlock * 32, 0, s>>>(a, plane_ptr, hit_event, flags, out_deg,
+                                                               in_deg, row_ptr, src, dst, in_ptr, in_perm);
+  else
+    search_kernel<0, MODE><<<grid, kWarpsPerBlock * 32, 0, s>>>(a, plane_ptr, hit_event, flags, out_deg,
+                                                               in_deg, row_ptr, src, dst, in_ptr, in_perm);
+}
+
+int launch_search_count(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
+                        const int32_t* flags, int32_t* out_deg, int32_t* in_deg, cudaStream_t s) {
+  launch_search<0>(a, plane_ptr, hit_event, flags, out_deg, in_deg, nullptr, nullptr, nullptr, nullptr,
+                   nullptr, s);
+  return 1;
+}
+
+int launch_exclusive_scan(int32_t* data, int n, int32_t* tmp, cudaStream_t s) {
+  const int nb = (n + kScanTile - 1) / kScanTile;
+  scan_block_sums<<<nb, kScanThreads, 0, s>>>(data, n, tmp);
+  scan_tmp_kernel<<<1, kScanThreads, 0, s>>>(tmp, nb);
+  scan_apply<<<nb, kScanThreads, 0, s>>>(data, n, tmp);
+  return 3;
+}
+
+int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
+                       const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst,
+                       const int32_t* in_ptr, int32_t* in_perm, cudaStream_t s) {
+  launch_search<1>(a, plane_ptr, hit_event, flags, nullptr, nullptr, row_ptr, src, dst, nullptr, nullptr, s);
+  launch_search<2>(a, plane_ptr, hit_event, flags, nullptr, nullptr, row_ptr, src, dst, in_ptr, in_perm, s);
+  return 2;
+}
+
+}  // namespace etx

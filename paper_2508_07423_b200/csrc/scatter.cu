@@ -1,0 +1,79 @@
+// a4 — message aggregation, Eq. 8.5: m_l = [ sum_{l->j} e_lj , sum_{i->l} e_il ].
+// The thesis' pipeline did this with a scatter_add operator / TensorRT plugin, i.e.
+// atomics.  Here both halves are SEGMENTED REDUCTIONS with a fixed summation order (deterministic):
+// edges are source-sorted, so the outgoing sum of hit l is a contiguous run of rows of e; the incoming
+// sum walks the by-destination list in_perm (ascending edge id).  One warp owns a hit; a lane owns
+// H/32 consecutive features, so every row read is one fully coalesced 512-byte (H=128) request, and
+// four rows are kept in flight per lane.  fp32 accumulation always (BASELINE.json C3).
+// Roofline: HBM — reads 2 x E x H x 4 B (+ 4 B per edge of in_perm), writes N x 2H x 4 B.
+#include "common.cuh"
+
+namespace etx {
+namespace {
+
+template <int V> struct Vec;
+template <> struct Vec<4> { using T = float4; };
+template <> struct Vec<2> { using T = float2; };
+
+__device__ __forceinline__ void add(float4& a, const float4& b) { a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w; }
+__device__ __forceinline__ void add(float2& a, const float2& b) { a.x += b.x; a.y += b.y; }
+__device__ __forceinline__ void zero(float4& a) { a = make_float4(0.f, 0.f, 0.f, 0.f); }
+__device__ __forceinline__ void zero(float2& a) { a = make_float2(0.f, 0.f); }
+
+template <int H>
+__global__ void __launch_bounds__(256) scatter_kernel(int n_nodes, const int32_t* __restrict__ row_ptr,
+                                                      const int32_t* __restrict__ in_ptr,
+                                                      const int32_t* __restrict__ in_perm,
+                                                      const float* __restrict__ e, float* __restrict__ m) {
+  using T = typename Vec<H / 32>::T;
+  const int lane = threadIdx.x & 31;
+  const int warp = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int n_warps = gridDim.x * (blockDim.x >> 5);
+  const T* __restrict__ ev = reinterpret_cast<const T*>(e);
+  T* __restrict__ mv = reinterpret_cast<T*>(m);
+  constexpr int RV = H / (H / 32);                 // vectors per row of e  (= 32)
+  for (int l = warp; l < n_nodes; l += n_warps) {
+    T acc_out, acc_in;
+    zero(acc_out); zero(acc_in);
+    {                                              // outgoing: contiguous rows row_ptr[l] .. row_ptr[l+1]
+      const int k0 = __ldg(row_ptr + l), k1 = __ldg(row_ptr + l + 1);
+      int k = k0;
+      for (; k + 4 <= k1; k += 4) {
+        const T a = __ldg(ev + (size_t)(k + 0) * RV + lane), b = __ldg(ev + (size_t)(k + 1) * RV + lane);
+        const T c = __ldg(ev + (size_t)(k + 2) * RV + lane), d = __ldg(ev + (size_t)(k + 3) * RV + lane);
+        add(acc_out, a); add(acc_out, b); add(acc_out, c); add(acc_out, d);
+      }
+      for (; k < k1; ++k) add(acc_out, __ldg(ev + (size_t)k * RV + lane));
+    }
+    {                                              // incoming: gathered rows in_perm[in_ptr[l] ..]
+      const int k0 = __ldg(in_ptr + l), k1 = __ldg(in_ptr + l + 1);
+      int k = k0;
+      for (; k + 4 <= k1; k += 4) {
+        const int i0 = __ldg(in_perm + k), i1 = __ldg(in_perm + k + 1);
+        const int i2 = __ldg(in_perm + k + 2), i3 = __ldg(in_perm + k + 3);
+        const T a = __ldg(ev + (size_t)i0 * RV + lane), b = __ldg(ev + (size_t)i1 * RV + lane);
+        const T c = __ldg(ev + (size_t)i2 * RV + lane), d = __ldg(ev + (size_t)i3 * RV + lane);
+        add(acc_in, a); add(acc_in, b); add(acc_in, c); add(acc_in, d);
+      }
+      for (; k < k1; ++k) add(acc_in, __ldg(ev + (size_t)__ldg(in_perm + k) * RV + lane));
+    }
+    mv[(size_t)l * 2 * RV + lane] = acc_out;       // outgoing first (Eq. 8.5)
+    mv[(size_t)l * 2 * RV + RV + lane] = acc_in;
+  }
+}
+
+}  // namespace
+
+int launch_scatter(int n_nodes, int H, const int32_t* row_ptr, const int32_t* in_ptr,
+                   const int32_t* in_perm, const float* e, float* m, cudaStream_t s) {
+  if (n_nodes <= 0) return 0;
+  const int need = (n_nodes + 7) / 8;
+  const int cap = 148 * 8;                         // 8 resident CTAs of 256 threads per SM
+  const int grid = need < cap ? need : cap;
+  if (H == 128) scatter_kernel<128><<<grid, 256, 0, s>>>(n_nodes, row_ptr, in_ptr, in_perm, e, m);
+  else if (H == 64) scatter_kernel<64><<<grid, 256, 0, s>>>(n_nodes, row_ptr, in_ptr, in_perm, e, m);
+  else return -1;
+  return 1;
+}
+
+}  // namespace etx

@@ -1,0 +1,72 @@
+"""Host-side checks that need no GPU: the C-ABI library builds, loads and exports every symbol that
+include/etx.h declares; argument validation that happens before any CUDA call."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2508_07423_b200 import binding, build, synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load_library()
+
+
+def test_exports_match_header(lib):
+    header = open(os.path.join(ROOT, "include", "etx.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(etx_[a-z_]+)\s*\(", header))
+    assert declared == set(binding.EXPORTS)
+    for name in declared:
+        assert getattr(lib, name) is not None          # raises AttributeError if not exported
+
+
+def test_weight_count_matches_generator_layout(lib):
+    for name, cfg in synth.CONFIGS.items():
+        d = binding.make_desc(cfg, precision=0)
+        assert lib.etx_weight_count(C.byref(d)) == synth.n_weight_floats(cfg), name
+    bad = binding.make_desc(synth.CONFIGS["c0"], precision=0)
+    bad.gnn_hidden = 96
+    assert lib.etx_weight_count(C.byref(bad)) == 0
+
+
+def test_struct_layouts_match_header():
+    # sizes implied by include/etx.h on LP64
+    assert C.sizeof(binding.ModelDesc) == 4 * (1 + 9 + 5) + 4 * 10
+    assert C.sizeof(binding.Batch) == 8 + 7 * 8
+    assert C.sizeof(binding.Graph) == 16 + 5 * 8
+
+
+def test_create_rejects_bad_arguments_and_has_no_cpu_fallback(lib):
+    import torch
+    cfg = synth.CONFIGS["c0"]
+    d = binding.make_desc(cfg, precision=0)
+    w = synth.generate_weights(cfg)
+    h = C.c_void_p()
+    st = lib.etx_create(C.byref(h), C.byref(d), w.ctypes.data_as(C.c_void_p), w.size - 1, 0)
+    assert st == binding.ETX_ERR_INVALID and b"weight blob" in lib.etx_last_error(None)
+    if not torch.cuda.is_available():
+        st = lib.etx_create(C.byref(h), C.byref(d), w.ctypes.data_as(C.c_void_p), w.size, 0)
+        assert st == binding.ETX_ERR_CUDA and h.value is None
+        assert b"no CPU fallback" in lib.etx_last_error(None)
+        with pytest.raises(binding.EtxError):
+            binding.Etx(d, w)
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2508_07423_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "etx_oracle" not in text and "import oracle" not in text and "from oracle" not in text, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp")) and f != "calibrate_radius.py":
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "binding" not in text and "libetx" not in text and "csrc" not in text.replace("paper_2508_07423_b200/csrc)", ""), f

@@ -1,0 +1,226 @@
+"""CUDA path (through the C ABI) vs the CPU oracle, element by element, on the same seeded inputs.
+
+Bars (BASELINE.json north_star; tolerances derived in DESIGN.md "Tolerances"):
+  * graph edges: bit-exact arrays when both paths start from the ORACLE's fp32 embeddings;
+  * embeddings / encodings: fp32 summation-order noise only;
+  * edge scores: |delta| <= 1e-4 absolute (fp32 path), 2e-2 (bf16 MLPs, on the oracle's graph).
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+from conftest import layout_dict, oracle_path
+from oracle import etx_oracle as orc
+from paper_2508_07423_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_SCORE_FP32 = 1e-4
+TOL_SCORE_BF16 = 2e-2
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2508_07423_b200 import binding, build
+    build.build()
+    return binding
+
+
+def make_etx(B, cfg, blob, precision=0):
+    return B.Etx(B.make_desc(cfg, precision=precision), blob)
+
+
+def gpu_from_oracle_graph(B, etx, batch, ora, r2, gap):
+    """GNN + scores on the graph the GPU builds from the ORACLE's embeddings (must equal the oracle's)."""
+    dev = etx.device
+    db = B.DeviceBatch(batch, dev)
+    cap = max(len(ora["src"]) + 7, 16)
+    etx.ensure_workspace(db.n_events, db.n_hits, cap)
+    g = B.DeviceGraph(db.n_hits, cap, dev)
+    emb = torch.from_numpy(ora["emb"]).to(dev)
+    E = etx.etx_build_graph(db, emb, r2, gap, g)
+    H = int(etx.desc.gnn_hidden)
+    e = torch.empty(max(E, 1), H, device=dev)
+    h = torch.empty(max(db.n_hits, 1), H, device=dev)
+    s = torch.empty(max(E, 1), device=dev)
+    etx.etx_gnn_forward(db, g, e, h)
+    etx.etx_edge_scores(g, e, s)
+    torch.cuda.synchronize()
+    return {"src": g.src[:E].cpu().numpy(), "dst": g.dst[:E].cpu().numpy(), "row_ptr": g.row_ptr.cpu().numpy(),
+            "in_ptr": g.in_ptr.cpu().numpy(), "in_perm": g.in_perm[:E].cpu().numpy(),
+            "h": h[:db.n_hits].cpu().numpy(), "e": e[:E].cpu().numpy(), "scores": s[:E].cpu().numpy()}
+
+
+def check_graph_arrays(out, ora, n_hits):
+    np.testing.assert_array_equal(out["src"], ora["src"])           # bit-exact, same order
+    np.testing.assert_array_equal(out["dst"], ora["dst"])
+    E = len(ora["src"])
+    rp = np.zeros(n_hits + 1, np.int64); np.cumsum(np.bincount(ora["src"], minlength=n_hits), out=rp[1:])
+    ip = np.zeros(n_hits + 1, np.int64); np.cumsum(np.bincount(ora["dst"], minlength=n_hits), out=ip[1:])
+    np.testing.assert_array_equal(out["row_ptr"], rp)
+    np.testing.assert_array_equal(out["in_ptr"], ip)
+    # by-destination lists: a permutation, grouped by destination, ascending edge id inside a group
+    want = np.lexsort((np.arange(E), ora["dst"]))
+    np.testing.assert_array_equal(out["in_perm"], want)
+
+
+def rel_close(a, b, tol):
+    scale = max(1.0, float(np.abs(b).max()))
+    return float(np.abs(a.astype(np.float64) - b).max()) <= tol * scale
+
+
+@pytest.mark.parametrize("name", ["c0", "c1"])
+def test_single_event_configs(B, name, request):
+    cfg, batch, blob = request.getfixturevalue(name)
+    ora = request.getfixturevalue(name + "_oracle")
+    etx = make_etx(B, cfg, blob)
+    r2, gap = synth.r2_max(cfg), cfg.max_plane_gap
+    # a1: embedding
+    full = B.run_path(etx, batch, r2, gap)
+    assert np.abs(full["emb"] - ora["emb"]).max() <= 2e-6
+    # a2: graph from the oracle's embeddings, bit-exact; a3-a7 on it
+    out = gpu_from_oracle_graph(B, etx, batch, ora, r2, gap)
+    check_graph_arrays(out, ora, len(batch["r"]))
+    assert rel_close(out["h"], ora["h"], 2e-5)
+    assert rel_close(out["e"], ora["e"], 2e-5)
+    err = np.abs(out["scores"].astype(np.float64) - ora["scores"])
+    assert err.max() <= TOL_SCORE_FP32, err.max()
+    # end to end (GPU embeddings -> GPU graph): edges may differ only inside the 1e-5 band around r
+    _, _, border = orc.build_graph(batch["event_ptr"], batch["plane"], ora["emb"], r2, gap, band=1e-5, want_border=True)
+    band = set(map(tuple, border.tolist()))
+    got = set(zip(full["src"].tolist(), full["dst"].tolist()))
+    want = set(zip(ora["src"].tolist(), ora["dst"].tolist()))
+    assert (got ^ want) <= band, sorted(got ^ want)[:10]
+    if got == want:
+        assert np.abs(full["scores"].astype(np.float64) - ora["scores"]).max() <= TOL_SCORE_FP32
+
+
+def test_multi_event_batch_and_ragged_tiles(B):
+    # 5 events of the throughput config: E and N are not multiples of the 128-row tile
+    cfg = synth.CONFIGS["c2"]
+    batch = synth.generate_events(cfg, [3, 11, 200, 512, 999])
+    blob = synth.generate_weights(cfg)
+    ora = oracle_path(cfg, batch, blob)
+    etx = make_etx(B, cfg, blob)
+    out = gpu_from_oracle_graph(B, etx, batch, ora, synth.r2_max(cfg), cfg.max_plane_gap)
+    check_graph_arrays(out, ora, len(batch["r"]))
+    assert len(ora["src"]) % 128 != 0 and len(batch["r"]) % 128 != 0
+    assert np.abs(out["scores"].astype(np.float64) - ora["scores"]).max() <= TOL_SCORE_FP32
+
+
+def test_stress_config_events(B):
+    cfg = synth.CONFIGS["c4"]
+    batch = synth.generate_events(cfg, [0, 1])
+    blob = synth.generate_weights(cfg)
+    ora = oracle_path(cfg, batch, blob)
+    etx = make_etx(B, cfg, blob)
+    out = gpu_from_oracle_graph(B, etx, batch, ora, synth.r2_max(cfg), cfg.max_plane_gap)
+    check_graph_arrays(out, ora, len(batch["r"]))
+    assert abs(len(ora["src"]) / len(batch["r"]) - 10.0) < 1.0
+    assert np.abs(out["scores"].astype(np.float64) - ora["scores"]).max() <= TOL_SCORE_FP32
+
+
+def test_thesis_settings_gap2_dim3(B):
+    # the thesis' own search setting: planes p+1, p+2 and a 3-dimensional embedding
+    cfg = dataclasses.replace(synth.CONFIGS["c0"], emb_widths=(3, 64, 64, 3), max_plane_gap=2)
+    batch = synth.generate_events(cfg, [0, 1, 2])
+    blob = synth.generate_weights(cfg)
+    ora = oracle_path(cfg, batch, blob, r2=2.5e-3, gap=2)
+    assert len(ora["src"]) > 100
+    etx = make_etx(B, cfg, blob)
+    out = gpu_from_oracle_graph(B, etx, batch, ora, 2.5e-3, 2)
+    check_graph_arrays(out, ora, len(batch["r"]))
+    assert np.abs(out["scores"].astype(np.float64) - ora["scores"]).max() <= TOL_SCORE_FP32
+
+
+def test_radius_extremes_and_empty_inputs(B, c0, c0_oracle):
+    cfg, batch, blob = c0
+    etx = make_etx(B, cfg, blob)
+    n = len(batch["r"])
+    # r = 0: no edges at all; the GNN and the head must accept E = 0
+    out = B.run_path(etx, batch, 0.0, cfg.max_plane_gap)
+    assert len(out["src"]) == 0 and np.all(out["row_ptr"] == 0) and np.all(out["in_ptr"] == 0)
+    lo = layout_dict(cfg)
+    h = orc.mlp(c0_oracle["f_node"], lo["node_enc"][0], blob, lo["node_enc"][1])
+    for k in range(cfg.n_iter):                                   # isolated hits: m = 0
+        x = np.concatenate([h, np.zeros((n, 2 * cfg.gnn_hidden), np.float32)], 1)
+        h = h + orc.mlp(x, lo[f"node_net_{k}"][0], blob, lo[f"node_net_{k}"][1])
+    assert rel_close(out["h"], h, 2e-5)
+    # r = inf: every allowed plane pair (closed form count)
+    cnt = np.bincount(batch["plane"], minlength=26)
+    want = sum(int(cnt[p]) * int(cnt[p + 1:p + 1 + cfg.max_plane_gap].sum()) for p in range(26))
+    out = B.run_path(etx, batch, float("inf"), cfg.max_plane_gap, edge_capacity=want)
+    assert len(out["src"]) == want
+    s, d = orc.build_graph(batch["event_ptr"], batch["plane"], out["emb"], np.inf, cfg.max_plane_gap)
+    np.testing.assert_array_equal(out["src"], s)
+    np.testing.assert_array_equal(out["dst"], d)
+    # empty batch, and a batch whose events are empty or hold one hit
+    empty = {k: v[:0] for k, v in batch.items() if k != "event_ptr"}
+    empty["event_ptr"] = np.zeros(1, np.int32)
+    out = B.run_path(etx, empty, 1.0, 3)
+    assert len(out["src"]) == 0 and len(out["scores"]) == 0
+    one = synth.select_events(batch, [0])
+    keep = np.array([0, n - 1])
+    tiny = {k: one[k][keep] for k in ("plane", "r", "phi", "z", "x", "y", "track")}
+    tiny["event_ptr"] = np.array([0, 0, 1, 1, 2], np.int32)       # events: empty, 1 hit, empty, 1 hit
+    out = B.run_path(etx, tiny, float("inf"), 3)
+    assert len(out["src"]) == 0 and out["h"].shape == (2, cfg.gnn_hidden)
+
+
+def test_error_paths(B, c0):
+    cfg, batch, blob = c0
+    etx = make_etx(B, cfg, blob)
+    with pytest.raises(B.EtxError) as ei:                         # capacity: nothing written, E reported
+        B.run_path(etx, batch, float("inf"), 3, edge_capacity=10)
+    assert ei.value.status == B.ETX_ERR_CAPACITY
+    bad = dict(batch)
+    bad["plane"] = batch["plane"][::-1].copy()
+    with pytest.raises(B.EtxError) as ei:
+        B.run_path(etx, bad, 1e-3, 3)
+    assert ei.value.status == B.ETX_ERR_UNSORTED
+    bad["plane"] = np.full_like(batch["plane"], 26)
+    with pytest.raises(B.EtxError) as ei:
+        B.run_path(etx, bad, 1e-3, 3)
+    assert ei.value.status == B.ETX_ERR_INVALID
+    db = B.DeviceBatch(batch, etx.device)
+    g = B.DeviceGraph(db.n_hits, 100000, etx.device)
+    emb = etx.etx_embed(db)
+    with pytest.raises(B.EtxError) as ei:                         # k_max cap is not on this path
+        etx.etx_build_graph(db, emb, 1e-3, 3, g, k_max=50)
+    assert ei.value.status == B.ETX_ERR_INVALID
+    fresh = make_etx(B, cfg, blob)
+    with pytest.raises(B.EtxError) as ei:                         # no workspace handed over
+        fresh.etx_build_graph(db, emb, 1e-3, 3, g)
+    assert ei.value.status == B.ETX_ERR_NOMEM
+
+
+def test_host_buffer_entry_point_equals_device_path(B, c1, c1_oracle):
+    cfg, batch, blob = c1
+    etx = make_etx(B, cfg, blob)
+    r2, gap = synth.r2_max(cfg), cfg.max_plane_gap
+    ref = B.run_path(etx, batch, r2, gap)
+    cap = len(ref["src"]) + 100
+    host = B.pinned_host_batch(batch)
+    etx.ensure_workspace(1, len(batch["r"]), cap, with_host_path=True)
+    src = torch.empty(cap, dtype=torch.int32).pin_memory()
+    dst = torch.empty(cap, dtype=torch.int32).pin_memory()
+    sc = torch.empty(cap, dtype=torch.float32).pin_memory()
+    E = etx.etx_infer_host(host, r2, gap, cap, src, dst, sc)
+    assert E == len(ref["src"])
+    np.testing.assert_array_equal(src[:E].numpy(), ref["src"])
+    np.testing.assert_array_equal(dst[:E].numpy(), ref["dst"])
+    np.testing.assert_array_equal(sc[:E].numpy(), ref["scores"])   # same kernels, same order: bitwise
+    assert etx.launch_count() > 0
+
+
+def test_deterministic_repeat(B, c1):
+    cfg, batch, blob = c1
+    etx = make_etx(B, cfg, blob)
+    a = B.run_path(etx, batch, synth.r2_max(cfg), cfg.max_plane_gap)
+    b = B.run_path(etx, batch, synth.r2_max(cfg), cfg.max_plane_gap)
+    for k in ("src", "dst", "in_perm", "scores", "e"):
+        np.testing.assert_array_equal(a[k], b[k])                  # no atomics anywhere on the path
