@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""Benchmark of the hits -> edge-scores hot path (BASELINE.json metric: events/s per B200).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config c2]
+
+A step is one pass of the whole path (etx_embed, etx_build_graph, etx_gnn_forward, etx_edge_scores)
+over one batch of synthetic events.  `value` is measured with the inputs resident in HBM; `e2e` is
+the same metric through etx_infer_host with pinned HOST buffers (H2D of the hits and D2H of the edge
+list and scores inside the timed region).  Rank 0 prints ONE JSON line.
+
+Multi-GPU (torchrun): events are independent, so every rank runs its own batch of the same
+config (rank r takes event ids r*n .. (r+1)*n-1): weak scaling, no data-path collective; only the
+timing is reduced (max over ranks).
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2508_07423_b200 import synth  # noqa: E402
+
+METRIC = "events/s per B200 (GNN graph build + message passing); % of tensor/HBM roofline"
+NAMES = {"c2": "c2: 1000 independent events, Poisson(150) tracks, 5% noise, fp32, emb 3-128-128-128-4, "
+               "GNN H=128, 6 iterations, G=3, mean out-degree 6",
+         "c3": "c3: c2 inputs with bf16 MLP operands, fp32 accumulate and state",
+         "c4": "c4: 1000 events, Poisson(300) tracks, 10% noise, out-degree 10, H=128, 8 iterations, fp32",
+         "c1": "c1: single Run-3-occupancy event", "c0": "c0: tiny single event"}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_tflops": d["bf16_tflops"],
+                "bf16_tflops_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                "sm_max_mhz": d.get("sm_max_mhz", 1965.0), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0,
+            "source": "fallback"}
+
+
+def flops_mlp(dims):
+    return sum(2 * dims[i] * dims[i + 1] for i in range(len(dims) - 1))
+
+
+def path_flops(cfg, N, E):
+    """Algorithmic FLOP of one step by kernel class."""
+    H, L = cfg.gnn_hidden, cfg.gnn_mlp_hidden_layers
+    hid = (H,) * L
+    return {"embed": N * flops_mlp(cfg.emb_widths),
+            "node_enc": N * flops_mlp((3,) + hid + (H,)),
+            "edge_enc": E * flops_mlp((2 * H,) + hid + (H,)),
+            "node_net": cfg.n_iter * N * flops_mlp((3 * H,) + hid + (H,)),
+            "edge_net": cfg.n_iter * E * flops_mlp((3 * H,) + hid + (H,)),
+            "cls": E * flops_mlp((H,) + hid + (1,)),
+            "scatter": cfg.n_iter * 2 * E * H}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+            self.thread.join(timeout=2)
+
+    def summary(self):
+        mhz, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                mhz.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not mhz:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(mhz)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "samples": len(mhz)}
+
+
+# --------------------------------------------------------------------------------------------------
+# reference arm: the oracle as it stands, on the host cores
+# --------------------------------------------------------------------------------------------------
+def oracle_events_per_s(cfg, event_ids):
+    from oracle import etx_oracle as orc
+    batch = synth.generate_events(cfg, event_ids)
+    blob = synth.generate_weights(cfg)
+    layout = {s.name: (s.dims, s.offset) for s in synth.model_layout(cfg)}
+    t = time.perf_counter()
+    out = orc.run_path(batch, blob, layout, cfg.gnn_hidden, cfg.n_iter, synth.r2_max(cfg), cfg.max_plane_gap,
+                       synth.NORM_CENTER, synth.NORM_SCALE)
+    dt = time.perf_counter() - t
+    return len(event_ids) / dt, dt, len(batch["r"]), len(out["src"])
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import etx_oracle as orc
+    cfg = synth.CONFIGS[args.config]
+    per_step = 2
+    for w in range(args.warmup):
+        oracle_events_per_s(cfg, [w * per_step + i for i in range(per_step)])
+    t_tot, n_ev = 0.0, 0
+    for k in range(args.steps):
+        _, dt, _, _ = oracle_events_per_s(cfg, [(args.warmup + k) * per_step + i for i in range(per_step)])
+        t_tot += dt
+        n_ev += per_step
+    v = n_ev / t_tot
+    sample = f"{per_step} events of {args.config} per step ({n_ev} timed), oracle/etx_oracle.cpp, OpenMP over rows"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": "events/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": NAMES[args.config], "sample": sample},
+        "cpu_baseline": {"value": v, "unit": "events/s", "cores": orc.n_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+# --------------------------------------------------------------------------------------------------
+# our arm
+# --------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2508_07423_b200 import binding, build
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    build.build()
+
+    cfg = synth.CONFIGS[args.config]
+    n_ev = args.events or cfg.n_events
+    batch = synth.generate_events(cfg, range(rank * n_ev, (rank + 1) * n_ev))
+    blob = synth.generate_weights(cfg)
+    etx = binding.Etx(binding.make_desc(cfg, precision=args.precision if args.precision is not None else cfg.precision),
+                      blob, device=local)
+    r2, gap, H = synth.r2_max(cfg), cfg.max_plane_gap, cfg.gnn_hidden
+    N = len(batch["r"])
+    cap = int(N * (cfg.target_degree * 1.25 + 2))
+    db = binding.DeviceBatch(batch, dev)
+    etx.ensure_workspace(db.n_events, N, cap, with_host_path=True)
+    g = binding.DeviceGraph(N, cap, dev)
+    emb = torch.empty(N, etx.emb_dim, device=dev)
+    enc = torch.empty(cap, H, device=dev)
+    scores = torch.empty(cap, device=dev)
+
+    def step():
+        etx.etx_embed(db, emb)
+        E = etx.etx_build_graph(db, emb, r2, gap, g)
+        etx.etx_gnn_forward(db, g, enc)
+        etx.etx_edge_scores(g, enc, scores)
+        return E
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        E = step()
+    barrier()
+    etx.profile_enable(True)
+    etx.profile_read()
+    l0 = etx.launch_count()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        barrier()
+        t0.record()
+        for _ in range(args.steps):
+            E = step()
+        t1.record()
+        barrier()
+    ms = t0.elapsed_time(t1)
+    launches = etx.launch_count() - l0
+    prof = etx.profile_read()
+    etx.profile_enable(False)
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_step = ms / args.steps
+    value = world * n_ev / (ms_step * 1e-3)
+
+    # ---- end to end through the host-buffer entry point
+    host = binding.pinned_host_batch(batch)
+    o_src = torch.empty(cap, dtype=torch.int32).pin_memory()
+    o_dst = torch.empty(cap, dtype=torch.int32).pin_memory()
+    o_sc = torch.empty(cap, dtype=torch.float32).pin_memory()
+    etx.etx_infer_host(host, r2, gap, cap, o_src, o_dst, o_sc)
+    barrier()
+    e2e_steps = max(2, min(args.steps, 5))
+    w0 = time.perf_counter()
+    t0.record()
+    for _ in range(e2e_steps):
+        E2 = etx.etx_infer_host(host, r2, gap, cap, o_src, o_dst, o_sc)
+    t1.record()
+    barrier()
+    e2e_ms = max(t0.elapsed_time(t1), 1e3 * (time.perf_counter() - w0)) / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    h2d = sum(host[k].numel() * host[k].element_size() for k in host)
+    d2h = E2 * 12
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    pk = peaks()
+    fl = path_flops(cfg, N, E)
+    stages = {}
+    for k, (kms, kn) in prof.items():
+        per = kms / args.steps
+        stages[k] = {"ms": per, "launches": kn // max(args.steps, 1),
+                     "events_per_s": (n_ev / (per * 1e-3)) if per > 0 else None}
+        if k in fl and per > 0:
+            stages[k]["tflops"] = fl[k] / (per * 1e-3) / 1e12
+    # scatter-sum algorithmic bytes: 2 reads of e + in_perm + write of m, per iteration
+    sc_bytes = cfg.n_iter * (2 * E * H * 4 + 4 * E + N * 2 * H * 4 + 8 * (N + 1))
+    if stages["scatter"]["ms"] > 0:
+        stages["scatter"]["gbs"] = sc_bytes / (stages["scatter"]["ms"] * 1e-3) / 1e9
+        stages["scatter"]["hbm_frac"] = stages["scatter"]["gbs"] / pk["hbm_gbs"]
+    gnn_ms = sum(stages[k]["ms"] for k in ("node_enc", "edge_enc", "scatter", "node_net", "edge_net"))
+    stages["message_passing_total"] = {"ms": gnn_ms, "events_per_s": n_ev / (gnn_ms * 1e-3) if gnn_ms else None}
+
+    # ---- roofline of the dominant kernel: the edge network (a6)
+    en = prof["edge_net"]
+    per_launch_ms = en[0] / max(en[1], 1)
+    per_launch_flop = fl["edge_net"] / cfg.n_iter
+    achieved = per_launch_flop / (per_launch_ms * 1e-3) / 1e12 if per_launch_ms > 0 else 0.0
+    prec = int(etx.desc.precision)
+    if prec == synth.PREC_FP32:
+        # FFMA: 148 SMs x 128 fp32 lanes x 2 FLOP x max SM clock (B200_PROFILING.md unit counts)
+        peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+        roof = {"bound": "alu", "unit": "TFLOP/s", "peak": peak,
+                "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x %.0f MHz" % pk["sm_max_mhz"]}
+        dtype = "f32"
+    elif prec == synth.PREC_TF32X3:
+        peak = pk["bf16_tflops_sustained"] * 0.5
+        roof = {"bound": "tensor", "unit": "TFLOP/s", "peak": peak,
+                "peak_source": f"{pk['source']} bf16 sustained x 0.5 (tf32 nominal ratio); achieved counts the 3 tf32 "
+                               "MMAs per algorithmic FLOP"}
+        achieved *= 3.0
+        dtype = "tf32x3"
+    else:
+        peak = pk["bf16_tflops_sustained"]
+        roof = {"bound": "tensor", "unit": "TFLOP/s", "peak": peak, "peak_source": f"{pk['source']} bf16 sustained"}
+        dtype = "bf16"
+    roof.update({"kernel": "edge network (a6)", "achieved": achieved, "frac": achieved / peak,
+                 "ms_per_launch": per_launch_ms, "traffic": read_traffic()})
+
+    # ---- CPU baseline: the oracle on a bounded sample, rank 0, N=1 only
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import etx_oracle as orc
+        _, dt1, _, _ = oracle_events_per_s(cfg, [0])
+        n_s = int(min(32, max(2, round(15.0 / max(dt1, 1e-3)))))
+        v, dt, nh, ne = oracle_events_per_s(cfg, list(range(n_s)))
+        cpu = {"value": v, "unit": "events/s", "cores": orc.n_threads(), "kind": "oracle",
+               "sample": f"first {n_s} events of {args.config} ({nh} hits, {ne} edges) in {dt:.1f} s"}
+
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": dtype, "data": "synthetic",
+        "config": {"workload": NAMES[args.config], "n_events_per_gpu": n_ev, "n_hits": N, "n_edges": int(E),
+                   "mean_out_degree": E / max(N, 1), "r2_max": r2, "hits_per_s": world * N / (ms_step * 1e-3),
+                   "l2": "state larger than L2 (edge encodings %.1f GB), no flush needed" % (E * H * 4 / 1e9),
+                   "parallelism": "events sharded across GPUs, no collective" if world > 1 else "single GPU"},
+        "roofline": roof, "cpu_baseline": cpu,
+        "e2e": {"value": world * n_ev / (e2e_ms * 1e-3), "unit": "events/s", "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms},
+        "gpu_launches": int(launches), "clocks": clk.summary(), "stages": stages}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def read_traffic():
+    """DRAM bytes per launch of the dominant kernel from the committed ncu summary (or null)."""
+    p = os.path.join(ROOT, "profiles", "edge_net_traffic.txt")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        if line.startswith("dram_bytes_per_launch"):
+            try:
+                return float(line.split("=")[1])
+            except ValueError:
+                return None
+    return None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c2", choices=sorted(synth.CONFIGS))
+    ap.add_argument("--events", type=int, default=0, help="events per GPU (default: the config's)")
+    ap.add_argument("--precision", type=int, default=None, help="override etx_precision (0 fp32, 1 tf32x3, 2 bf16)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
