@@ -19,6 +19,7 @@ struct DevMlp {
   int dims[kMaxLayers + 1] = {0};
   const float* Wt[kMaxLayers] = {nullptr};
   const float* b[kMaxLayers] = {nullptr};
+  const unsigned char* wimg = nullptr;   // tensor-core weight image (mlp_tc.cu), or null
 };
 
 struct Workspace {            // carved from the caller's buffer by carve_workspace()
@@ -45,6 +46,7 @@ struct etx_ctx {
   int sm_count = 148;
   float* d_weights = nullptr;      // transposed weights + biases, one allocation
   size_t d_weights_floats = 0;
+  unsigned char* d_wimg = nullptr; // tensor-core weight images, one allocation
   etx::DevMlp emb, node_enc, edge_enc, cls;
   std::vector<etx::DevMlp> node_net, edge_net;
   void* ws = nullptr;
@@ -93,6 +95,19 @@ struct MlpArgs {
   int out_mode = 0; float* out = nullptr; const float* res = nullptr; int out_ld = 0;
 };
 int launch_mlp_simt(const MlpArgs& a, cudaStream_t s);
+
+// ---- mlp_tc.cu (tcgen05 tensor-core path)
+struct TcArgs {
+  int n_rows = 0;
+  int n_seg = 0; Segment seg[3]; int K0 = 0;      // first-layer input: gathered segments, K0 = sum of widths
+  int n_layers = 0;
+  const unsigned char* wimg = nullptr;            // weight image: swizzled 16 KB tiles in consumption order
+  const float* bias[kMaxLayers] = {nullptr};
+  const float* w_last = nullptr;                  // classifier: fp32 weights of the 1-unit output layer
+  int out_mode = 0; float* out = nullptr; const float* res = nullptr; int out_ld = 0;
+};
+int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s);
+int tc_chunk_k(int mode);
 
 // ---- scatter.cu
 int launch_scatter(int n_nodes, int H, const int32_t* row_ptr, const int32_t* in_ptr,

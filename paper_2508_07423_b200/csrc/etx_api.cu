@@ -58,6 +58,48 @@ size_t mlp_floats(const HostMlp& m) {
   return n;
 }
 
+// Tensor-core weight image of the first n_gemm layers of an MLP (mlp_tc.cu): for every layer, for every
+// K-chunk of one 128-byte swizzle atom (32 tf32 / 64 bf16 values), one 16 KB tile per piece laid out
+// exactly as the canonical K-major SWIZZLE_128B shared-memory operand: row n (output neuron) at
+// n*128 bytes, its 16-byte groups XOR-ed with (n & 7).  TF32X3 stores two pieces (hi, lo) per chunk.
+uint16_t bf16_rne(float f) {
+  uint32_t u; std::memcpy(&u, &f, 4);
+  if ((u & 0x7fffffffu) > 0x7f800000u) return (uint16_t)((u >> 16) | 0x40);
+  u += 0x7fffu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+
+void append_wimg(std::vector<unsigned char>& img, const HostMlp& m, const float* w, int n_gemm, int mode) {
+  const int KA = tc_chunk_k(mode);
+  const int pieces = mode == ETX_PREC_TF32X3 ? 2 : 1;
+  const float* W = w;
+  for (int l = 0; l < n_gemm; ++l) {
+    const int fi = m.dims[l], fo = m.dims[l + 1];           // fo == 128
+    for (int k0 = 0; k0 < fi; k0 += KA) {
+      const size_t base = img.size();
+      img.resize(base + (size_t)pieces * 128 * 128, 0);
+      for (int n = 0; n < fo; ++n)
+        for (int kk = 0; kk < KA; ++kk) {
+          const float v = W[(size_t)n * fi + k0 + kk];
+          if (mode == ETX_PREC_TF32X3) {
+            uint32_t u; std::memcpy(&u, &v, 4);
+            const uint32_t hi_u = u & 0xffffe000u;
+            float hi; std::memcpy(&hi, &hi_u, 4);
+            const float lo = v - hi;
+            const size_t off = (size_t)n * 128 + (size_t)(((kk / 4) ^ (n & 7)) * 16) + (kk % 4) * 4;
+            std::memcpy(&img[base + off], &hi, 4);
+            std::memcpy(&img[base + 128 * 128 + off], &lo, 4);
+          } else {
+            const uint16_t b = bf16_rne(v);
+            const size_t off = (size_t)n * 128 + (size_t)(((kk / 8) ^ (n & 7)) * 16) + (kk % 8) * 2;
+            std::memcpy(&img[base + off], &b, 2);
+          }
+        }
+    }
+    W += (size_t)fi * fo + fo;
+  }
+}
+
 Workspace carve(const etx_ctx* c, int32_t n_events, int32_t n_hits, int64_t cap, bool host_path, char* base) {
   Workspace w;
   size_t off = 0;
@@ -137,9 +179,19 @@ struct ProfScope {
   }
 };
 
+// Precision dispatch.  MLPs with a tensor-core weight image run on tcgen05 (mlp_tc.cu); the two MLPs
+// fed by 3 raw features (embedding, node encoder) always run the fp32 FFMA kernel.
 int run_mlp(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
-  // precision dispatch: the tensor-core paths replace this call for the wide layers
-  return launch_mlp_simt(a, s);
+  if (c->desc.precision == ETX_PREC_FP32 || !a.mlp.wimg) return launch_mlp_simt(a, s);
+  TcArgs t;
+  t.n_rows = a.n_rows; t.n_seg = a.n_seg; t.K0 = a.mlp.dims[0];
+  for (int i = 0; i < 3; ++i) t.seg[i] = a.seg[i];
+  t.n_layers = a.mlp.n_layers;
+  t.wimg = a.mlp.wimg;
+  for (int l = 0; l < a.mlp.n_layers; ++l) t.bias[l] = a.mlp.b[l];
+  t.w_last = a.mlp.Wt[a.mlp.n_layers - 1];         // [H][1] == [H]
+  t.out_mode = a.out_mode; t.out = a.out; t.res = a.res; t.out_ld = a.out_ld;
+  return launch_mlp_tc(t, c->desc.precision, c->sm_count, s);
 }
 
 }  // namespace
@@ -161,8 +213,8 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
   if (!out) return fail(nullptr, ETX_ERR_INVALID, "ctx out pointer is NULL");
   *out = nullptr;
   if (const char* why = check_desc(desc)) return fail(nullptr, ETX_ERR_INVALID, why);
-  if (desc->precision != ETX_PREC_FP32)
-    return fail(nullptr, ETX_ERR_INVALID, "precision not available in this build");
+  if (desc->precision != ETX_PREC_FP32 && desc->gnn_hidden != 128)
+    return fail(nullptr, ETX_ERR_INVALID, "tensor-core precisions need gnn_hidden == 128");
   if (!h_weights || n_weights != etx_weight_count(desc))
     return fail(nullptr, ETX_ERR_INVALID, "weight blob size does not match desc (see etx_weight_count)");
   int n_dev = 0;
@@ -220,6 +272,33 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
   c->edge_enc = dev[2];
   for (int k = 0; k < desc->n_iter; ++k) { c->node_net.push_back(dev[3 + 2 * k]); c->edge_net.push_back(dev[4 + 2 * k]); }
   c->cls = dev.back();
+  if (desc->precision != ETX_PREC_FP32) {
+    // tensor-core weight images for every MLP whose first-layer input is a multiple of the chunk
+    // (edge encoder, node/edge networks, classifier); embedding and node encoder (3 inputs) stay SIMT
+    std::vector<unsigned char> img;
+    std::vector<size_t> img_off(mlps.size(), (size_t)-1);
+    size_t wsrc = 0;
+    for (size_t i = 0; i < mlps.size(); ++i) {
+      if (i >= 2) {
+        const bool is_cls = (i + 1 == mlps.size());
+        img_off[i] = img.size();
+        append_wimg(img, mlps[i], h_weights + wsrc, is_cls ? mlps[i].n_layers - 1 : mlps[i].n_layers, desc->precision);
+      }
+      wsrc += mlp_floats(mlps[i]);
+    }
+    if (cudaMalloc(&c->d_wimg, img.size()) != cudaSuccess ||
+        cudaMemcpy(c->d_wimg, img.data(), img.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+      const std::string msg = std::string("weight image upload failed: ") + cudaGetErrorString(cudaGetLastError());
+      etx_destroy(c);
+      return fail(nullptr, ETX_ERR_CUDA, msg);
+    }
+    c->edge_enc.wimg = c->d_wimg + img_off[2];
+    for (int k = 0; k < desc->n_iter; ++k) {
+      c->node_net[k].wimg = c->d_wimg + img_off[3 + 2 * k];
+      c->edge_net[k].wimg = c->d_wimg + img_off[4 + 2 * k];
+    }
+    c->cls.wimg = c->d_wimg + img_off[mlps.size() - 1];
+  }
   *out = c;
   return ETX_OK;
 }
@@ -228,6 +307,7 @@ etx_status etx_destroy(etx_ctx* c) {
   if (!c) return ETX_OK;
   cudaSetDevice(c->device);
   if (c->d_weights) cudaFree(c->d_weights);
+  if (c->d_wimg) cudaFree(c->d_wimg);
   for (const etx_ctx::ProfRec& r : c->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
   delete c;

@@ -224,3 +224,85 @@ def test_deterministic_repeat(B, c1):
     b = B.run_path(etx, batch, synth.r2_max(cfg), cfg.max_plane_gap)
     for k in ("src", "dst", "in_perm", "scores", "e"):
         np.testing.assert_array_equal(a[k], b[k])                  # no atomics anywhere on the path
+
+
+# ------------------------------------------------------------------------------------------------
+# tensor-core precisions (tcgen05): ETX_PREC_TF32X3 (fp32-equivalent) and ETX_PREC_BF16
+# ------------------------------------------------------------------------------------------------
+PREC = {"tf32x3": 1, "bf16": 2}
+REL_ENC = {"tf32x3": 2e-5, "bf16": 3e-2}          # relative to max |value| of the tensor
+TOL_SCORE = {"tf32x3": TOL_SCORE_FP32, "bf16": TOL_SCORE_BF16}
+
+
+@pytest.mark.parametrize("prec", ["tf32x3", "bf16"])
+def test_tc_edge_encoder_alone(B, c1, c1_oracle, prec):
+    """n_iter = 0: gnn_forward = node encoder (fp32 FFMA) + edge encoder (tcgen05, 2 gathered segments,
+    3 layers, plain store) — the smallest check of descriptors, swizzle and the TMEM operand path."""
+    cfg, batch, blob = c1
+    cfg0 = dataclasses.replace(cfg, n_iter=0)
+    blob0 = synth.generate_weights(cfg0)
+    ora = oracle_path(cfg0, batch, blob0, graph=(c1_oracle["src"], c1_oracle["dst"]))
+    ora["emb"] = c1_oracle["emb"]
+    etx = make_etx(B, cfg0, blob0, precision=PREC[prec])
+    out = gpu_from_oracle_graph(B, etx, batch, ora, synth.r2_max(cfg), cfg.max_plane_gap)
+    np.testing.assert_array_equal(out["src"], ora["src"])
+    assert rel_close(out["h"], ora["h"], 2e-5)                     # node encoder is always fp32
+    assert rel_close(out["e"], ora["e"], REL_ENC[prec]), np.abs(out["e"] - ora["e"]).max()
+    assert np.abs(out["scores"].astype(np.float64) - ora["scores"]).max() <= TOL_SCORE[prec]
+
+
+@pytest.mark.parametrize("prec", ["tf32x3", "bf16"])
+def test_tc_permutation_weights_reveal_layout(B, c1, c1_oracle, prec):
+    """Edge-encoder weights = signed permutation-like sparse matrices: any swapped k / n index in the
+    swizzled weight image or the TMEM operand layout moves values to the wrong column."""
+    cfg, batch, blob = c1
+    cfg0 = dataclasses.replace(cfg, n_iter=0)
+    blob0 = synth.generate_weights(cfg0).copy()
+    spec = [s for s in synth.model_layout(cfg0) if s.name == "edge_enc"][0]
+    rng = np.random.default_rng(11)
+    for (wo, bo, fi, fo) in spec.layer_offsets():
+        W = np.zeros((fo, fi), np.float32)
+        cols = rng.permutation(fi)[:fo]
+        W[np.arange(fo), cols] = rng.choice([-1.0, 1.0, 0.5, 2.0], size=fo)
+        blob0[wo:wo + fi * fo] = W.ravel()
+        blob0[bo:bo + fo] = rng.uniform(0.0, 0.25, fo).astype(np.float32)
+    ora = oracle_path(cfg0, batch, blob0, graph=(c1_oracle["src"], c1_oracle["dst"]))
+    ora["emb"] = c1_oracle["emb"]
+    etx = make_etx(B, cfg0, blob0, precision=PREC[prec])
+    out = gpu_from_oracle_graph(B, etx, batch, ora, synth.r2_max(cfg), cfg.max_plane_gap)
+    assert np.abs(ora["e"]).max() > 0.05
+    assert rel_close(out["e"], ora["e"], REL_ENC[prec]), np.abs(out["e"] - ora["e"]).max()
+
+
+@pytest.mark.parametrize("prec", ["tf32x3", "bf16"])
+def test_tc_single_event_full_path(B, c1, c1_oracle, prec):
+    cfg, batch, blob = c1
+    etx = make_etx(B, cfg, blob, precision=PREC[prec])
+    out = gpu_from_oracle_graph(B, etx, batch, c1_oracle, synth.r2_max(cfg), cfg.max_plane_gap)
+    check_graph_arrays(out, c1_oracle, len(batch["r"]))
+    err = np.abs(out["scores"].astype(np.float64) - c1_oracle["scores"])
+    assert err.max() <= TOL_SCORE[prec], err.max()
+    if prec == "tf32x3":
+        assert rel_close(out["e"], c1_oracle["e"], 5e-5)
+        assert rel_close(out["h"], c1_oracle["h"], 5e-5)
+
+
+@pytest.mark.parametrize("prec,name", [("tf32x3", "c2"), ("bf16", "c3"), ("tf32x3", "c4")])
+def test_tc_multi_event_batches(B, prec, name):
+    cfg = synth.CONFIGS[name]
+    ids = [3, 11, 200, 512, 999] if name != "c4" else [0, 1]
+    batch = synth.generate_events(cfg, ids)
+    blob = synth.generate_weights(cfg)
+    ora = oracle_path(cfg, batch, blob)
+    etx = make_etx(B, cfg, blob, precision=PREC[prec])
+    out = gpu_from_oracle_graph(B, etx, batch, ora, synth.r2_max(cfg), cfg.max_plane_gap)
+    check_graph_arrays(out, ora, len(batch["r"]))
+    err = np.abs(out["scores"].astype(np.float64) - ora["scores"])
+    assert err.max() <= TOL_SCORE[prec], err.max()
+
+
+def test_tc_rejects_unsupported_width(B, c0):
+    cfg, batch, blob = c0
+    with pytest.raises(B.EtxError) as ei:
+        make_etx(B, cfg, blob, precision=1)                          # H = 64: tensor-core path needs H = 128
+    assert ei.value.status == B.ETX_ERR_INVALID
