@@ -2,23 +2,26 @@
 //
 // Computes, for a tile of 128 rows (edges or hits), the whole chain of Eq. 4.27 layers of one
 // GNN MLP — edge encoder, node/edge network or classifier — without any
-// intermediate leaving the SM:
+// intermediate leaving the SM.  One persistent CTA per SM, ten warps:
 //
-//   * one persistent CTA per SM, six warps:
-//       warps 0-3  "row workers": thread r owns tile row r = TMEM lane r.  They gather the first
-//                  layer's input rows ([h_src | h_dst | e], [h | m], ...) straight from global memory,
-//                  convert them to the MMA operand type and write them into a TMEM operand ring with
-//                  tcgen05.st; after each layer they read the accumulator with tcgen05.ld, apply
-//                  bias + ReLU and write the next layer's A operand back into TMEM; after the last
-//                  layer they add the residual and store (or apply the 1-unit head + sigmoid).
-//       warp 4     weight loader: streams pre-swizzled weight tiles (16 KB, canonical K-major
-//                  SWIZZLE_128B images prepared once at etx_create) from L2 into a shared-memory ring
-//                  with cp.async.bulk (TMA bulk copy) completing on mbarriers.
-//       warp 5     MMA issuer: one thread issues tcgen05.mma with A from TMEM and B from shared
-//                  memory, accumulating in TMEM; tcgen05.commit releases ring slots and hands the
-//                  accumulator to the workers.
-//   * hidden activations never touch shared or global memory: accumulator -> registers -> TMEM.
-//   * TMEM map (512 columns): [0,128) accumulator | hidden A operand | first-layer A operand ring.
+//   warps 0-3  gather:   coalesced 16-byte loads of the first layer's input rows ([h_src | h_dst | e],
+//                        [h | m], ...) straight from the node / edge arrays (8 or 16 lanes per row, one
+//                        K-chunk prefetched in registers), conversion to the MMA operand type and
+//                        st.shared into a ring of canonical K-major SWIZZLE_128B operand tiles.
+//   warps 4-7  epilogue: thread r owns tile row r = TMEM lane r.  After a hidden layer: tcgen05.ld the
+//                        accumulator 32 columns at a time, bias + ReLU, convert, tcgen05.st the next
+//                        layer's A operand back into TMEM and release that K-chunk to the MMA warp at
+//                        once, so the next layer's MMAs start while the rest of the epilogue runs.
+//                        After the last layer: bias (+ residual) through a swizzled staging tile so
+//                        the global read-modify-write is coalesced, or the 1-unit head + sigmoid.
+//   warp 8     loader:   streams pre-swizzled weight tiles (prepared once at etx_create) from L2 into a
+//                        shared-memory ring with cp.async.bulk (TMA bulk copy) completing on mbarriers.
+//   warp 9     MMA:      one thread issues tcgen05.mma — SS form (A, B in shared memory) for the first
+//                        layer, TS form (A in TMEM) for the others — into one of two 128-column TMEM
+//                        accumulators (ping-pong), and tcgen05.commit-s ring slots / accumulators.
+//
+// TMEM map (512 columns): acc0 [0,128) | acc1 [128,256) | hidden A operand [256, ...).
+// Hidden activations never touch shared or global memory.
 //
 // Precision modes:
 //   ETX_PREC_TF32X3: x = hi + lo with hi = x & 0xffffe000 (top 11 significand bits), lo = x - hi;
@@ -32,27 +35,27 @@ namespace etx {
 namespace {
 
 constexpr int TM = 128;
-constexpr int kThreads = 192;
+constexpr int kThreads = 320;
 constexpr int HW = 128;                       // hidden width handled by this kernel
+constexpr int kAtomBytes = 128 * 128;         // one operand tile: 128 rows x 128 bytes (one swizzle atom wide)
 
 template <int MODE> struct Cfg;
 template <> struct Cfg<ETX_PREC_TF32X3> {
   static constexpr int KA = 32;               // K elements per 128-byte swizzle atom
   static constexpr int PIECES = 2;            // hi, lo
-  static constexpr int NSTAGE = 6;            // weight ring stages
-  static constexpr int NSLOT = 2;             // first-layer A operand ring slots (TMEM)
-  static constexpr int A_COLS = 32;           // TMEM columns per piece per chunk
+  static constexpr int NSTAGE_W = 4;          // weight ring stages (32 KB each)
+  static constexpr int NSTAGE_A = 2;          // first-layer A operand ring stages (32 KB each)
+  static constexpr int HID_COLS = 128;        // TMEM columns per piece of a hidden operand
   static constexpr uint32_t IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);
 };
 template <> struct Cfg<ETX_PREC_BF16> {
   static constexpr int KA = 64;
   static constexpr int PIECES = 1;
-  static constexpr int NSTAGE = 8;
-  static constexpr int NSLOT = 4;
-  static constexpr int A_COLS = 32;           // 64 bf16 = 32 columns
+  static constexpr int NSTAGE_W = 8;          // 16 KB each
+  static constexpr int NSTAGE_A = 4;          // 16 KB each
+  static constexpr int HID_COLS = 64;         // 128 bf16 = 64 columns
   static constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);
 };
-constexpr int kAtomBytes = 128 * 128;         // one weight tile: 128 rows (n) x 128 bytes (k)
 
 // ------------------------------------------------------------------------------------------------
 // PTX wrappers
@@ -81,6 +84,7 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
@@ -88,7 +92,20 @@ __device__ __forceinline__ void tc_wait_st() { asm volatile("tcgen05.wait::st.sy
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
-// D[tmem] (+)= A[tmem] * B[smem]^T     (TS form: A operand in tensor memory)
+__device__ __forceinline__ void epi_bar_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }   // epilogue warps only
+
+// D[tmem] (+)= A * B^T with B in shared memory; A in shared memory (SS) or tensor memory (TS)
+template <int MODE>
+__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t accumulate) {
+  if constexpr (MODE == ETX_PREC_TF32X3)
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
+  else
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
+}
 template <int MODE>
 __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t accumulate) {
   if constexpr (MODE == ETX_PREC_TF32X3)
@@ -134,60 +151,64 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {   // lo ->
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
   return d;
 }
-__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
-
-// Writes one chunk (KA k-values of this thread's row) of an A operand into TMEM at column `col`.
-// TF32X3: hi piece at col, lo piece at col + lo_off.  BF16: packed pairs at col.
-template <int MODE>
-__device__ __forceinline__ void store_operand_chunk(uint32_t lane_addr, uint32_t col, uint32_t lo_off,
-                                                    const float (&x)[Cfg<MODE>::KA]) {
-  uint32_t v[32];
-  if constexpr (MODE == ETX_PREC_TF32X3) {
-#pragma unroll
-    for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(x[i]) & 0xffffe000u;
-    tmem_st32(lane_addr + col, v);
-#pragma unroll
-    for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(x[i] - __uint_as_float(v[i]));
-    tmem_st32(lane_addr + col + lo_off, v);
-  } else {
-#pragma unroll
-    for (int i = 0; i < 32; ++i) v[i] = pack_bf16x2(x[2 * i], x[2 * i + 1]);
-    tmem_st32(lane_addr + col, v);
-  }
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ void st_shared_v2(uint32_t addr, uint32_t a, uint32_t b) {
+  asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(addr), "r"(a), "r"(b) : "memory");
+}
+__device__ __forceinline__ float4 ld_shared_v4(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  return v;
 }
 
 struct Bars {                                   // mbarriers (8 bytes each) + TMEM base
-  uint64_t w_full[8], w_empty[8], a_full[4], a_empty[4], acc_full, work_done;
+  uint64_t w_full[8], w_empty[8], a_full[4], a_empty[4], acc_full[2], acc_free[2], hid_ready[4];
   uint32_t tmem_base;
 };
 
 template <int MODE>
 __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   using C = Cfg<MODE>;
-  constexpr int KA = C::KA, P = C::PIECES, NSTAGE = C::NSTAGE, NSLOT = C::NSLOT, AC = C::A_COLS;
+  constexpr int KA = C::KA, P = C::PIECES, NSW = C::NSTAGE_W, NSA = C::NSTAGE_A, HID_COLS = C::HID_COLS;
   constexpr uint32_t kStageBytes = P * kAtomBytes;
-  constexpr int HID_COLS = HW * (MODE == ETX_PREC_TF32X3 ? 4 : 2) / 4;   // columns per piece of a hidden operand
-  constexpr uint32_t COL_ACC = 0, COL_HID = 128, COL_A = COL_HID + P * HID_COLS;
-  constexpr int HCH = HW / KA;                  // chunks per hidden layer
+  constexpr uint32_t COL_ACC = 0, COL_HID = 256;
+  constexpr int HCH = HW / KA;                  // K-chunks per hidden layer (4 / 2)
+  constexpr int LPR = KA * 4 / 16;              // gather lanes per row: 16-byte pieces of a chunk row (8 / 16)
+  constexpr int RPP = 128 / LPR;                // rows covered by one pass of the 128 gather threads (16 / 8)
+  constexpr int NPASS = TM / RPP;               // passes per chunk (8 / 16)
 
   extern __shared__ unsigned char smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
-  const uint32_t wring = (raw + 1023u) & ~1023u;                         // SWIZZLE_128B needs 1024-byte alignment
-  Bars* bars = reinterpret_cast<Bars*>(smem_raw + (wring - raw) + NSTAGE * kStageBytes);
+  const uint32_t base = (raw + 1023u) & ~1023u;                          // SWIZZLE_128B needs 1024-byte alignment
+  const uint32_t wring = base;
+  const uint32_t aring = wring + NSW * kStageBytes;
+  const uint32_t stage_out = aring + NSA * kStageBytes;                  // 16 KB swizzled staging tile
+  unsigned char* gen = smem_raw + (base - raw);
+  float* bias_s = reinterpret_cast<float*>(gen + (NSW + NSA) * kStageBytes + kAtomBytes);   // [kMaxLayers][128]
+  float* wlast_s = bias_s + kMaxLayers * HW;                                                  // [128]
+  Bars* bars = reinterpret_cast<Bars*>(wlast_s + HW);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_tiles = (a.n_rows + TM - 1) / TM;
   const int n_gemm = (a.out_mode == 3) ? a.n_layers - 1 : a.n_layers;
   const int nc1 = a.K0 / KA;
 
+  for (int i = threadIdx.x; i < a.n_layers * HW; i += kThreads) {
+    const int l = i / HW, j = i % HW;
+    bias_s[i] = (l < n_gemm) ? __ldg(a.bias[l] + j) : 0.f;
+  }
+  if (a.out_mode == 3)
+    for (int i = threadIdx.x; i < HW; i += kThreads) wlast_s[i] = __ldg(a.w_last + i);
   if (threadIdx.x == 0) {
-    for (int i = 0; i < NSTAGE; ++i) { mbar_init(smem_u32(&bars->w_full[i]), 1); mbar_init(smem_u32(&bars->w_empty[i]), 1); }
-    for (int i = 0; i < NSLOT; ++i) { mbar_init(smem_u32(&bars->a_full[i]), 128); mbar_init(smem_u32(&bars->a_empty[i]), 1); }
-    mbar_init(smem_u32(&bars->acc_full), 1);
-    mbar_init(smem_u32(&bars->work_done), 128);
+    for (int i = 0; i < NSW; ++i) { mbar_init(smem_u32(&bars->w_full[i]), 1); mbar_init(smem_u32(&bars->w_empty[i]), 1); }
+    for (int i = 0; i < NSA; ++i) { mbar_init(smem_u32(&bars->a_full[i]), 128); mbar_init(smem_u32(&bars->a_empty[i]), 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&bars->acc_full[i]), 1); mbar_init(smem_u32(&bars->acc_free[i]), 128); }
+    for (int i = 0; i < 4; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), 128);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 5) {                               // TMEM: all 512 columns of this SM (1 CTA per SM)
+  if (warp == 9) {                               // TMEM: all 512 columns of this SM (1 CTA per SM)
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&bars->tmem_base)) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
@@ -197,127 +218,169 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   const uint32_t tmem = bars->tmem_base;
 
   if (warp < 4) {
-    // =========================== row workers ===========================
-    const int r = threadIdx.x;
-    const uint32_t lane_addr = tmem + ((uint32_t)(warp * 32) << 16);
-    uint32_t a_cnt = 0, layer_cnt = 0;
+    // =========================== gather warps ===========================
+    const int t = threadIdx.x;                   // 0..127
+    const int jl = t % LPR;                      // 16-byte piece of the chunk row this thread moves
+    const int r0 = t / LPR;                      // first of its rows; then r0 + RPP, r0 + 2 RPP, ...
+    const int total_chunks = ((n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x) * nc1;
+    float4 cur[NPASS], nxt[NPASS];
+
+    // loads chunk number `ci` (counted over this CTA's tiles) into registers
+    auto load_chunk = [&](int ci, float4 (&dst)[NPASS]) {
+      const int tile = blockIdx.x + (ci / nc1) * gridDim.x;
+      const int k0 = (ci % nc1) * KA;
+      int s = 0, start = 0;
+      while (s < a.n_seg - 1 && k0 >= start + a.seg[s].width) { start += a.seg[s].width; ++s; }
+      const Segment sg = a.seg[s];
+      const int koff = k0 - start + jl * 4;
+#pragma unroll
+      for (int p = 0; p < NPASS; ++p) {
+        const int row = tile * TM + r0 + p * RPP;
+        const int grow = row < a.n_rows ? row : a.n_rows - 1;
+        const int idx = sg.idx ? __ldg(sg.idx + grow) : grow;
+        dst[p] = __ldg(reinterpret_cast<const float4*>(sg.base + (size_t)idx * sg.ld + koff));
+      }
+    };
+
+    if (total_chunks > 0) load_chunk(0, cur);
+    for (int ci = 0; ci < total_chunks; ++ci) {
+      if (ci + 1 < total_chunks) load_chunk(ci + 1, nxt);
+      const uint32_t slot = ci % NSA, n = ci / NSA;
+      mbar_wait(smem_u32(&bars->a_empty[slot]), (n & 1) ^ 1);
+      const uint32_t tile_hi = aring + slot * kStageBytes;
+#pragma unroll
+      for (int p = 0; p < NPASS; ++p) {
+        const int r = r0 + p * RPP;
+        const float4 v = cur[p];
+        if constexpr (MODE == ETX_PREC_TF32X3) {
+          const uint32_t off = r * 128 + ((jl ^ (r & 7)) << 4);
+          const uint32_t hx = __float_as_uint(v.x) & 0xffffe000u, hy = __float_as_uint(v.y) & 0xffffe000u;
+          const uint32_t hz = __float_as_uint(v.z) & 0xffffe000u, hw = __float_as_uint(v.w) & 0xffffe000u;
+          st_shared_v4(tile_hi + off, hx, hy, hz, hw);
+          st_shared_v4(tile_hi + kAtomBytes + off,
+                       __float_as_uint(v.x - __uint_as_float(hx)), __float_as_uint(v.y - __uint_as_float(hy)),
+                       __float_as_uint(v.z - __uint_as_float(hz)), __float_as_uint(v.w - __uint_as_float(hw)));
+        } else {                                 // 4 floats -> 4 bf16 = 8 bytes at k-byte offset 8*jl
+          const uint32_t off = r * 128 + (((jl >> 1) ^ (r & 7)) << 4) + ((jl & 1) << 3);
+          st_shared_v2(tile_hi + off, pack_bf16x2(v.x, v.y), pack_bf16x2(v.z, v.w));
+        }
+      }
+      fence_async_smem();                        // generic-proxy writes -> visible to the tensor core (async proxy)
+      mbar_arrive(smem_u32(&bars->a_full[slot]));
+#pragma unroll
+      for (int p = 0; p < NPASS; ++p) cur[p] = nxt[p];
+    }
+  } else if (warp < 8) {
+    // =========================== epilogue warps ===========================
+    const int et = threadIdx.x - 128;            // 0..127 = tile row = TMEM lane
+    const int q4 = warp & 3;                     // TMEM lane quarter this warp may access
+    const uint32_t lane_addr = tmem + ((uint32_t)(q4 * 32) << 16);
+    uint32_t g = 0, hcount = 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-      const int row = tile * TM + r;
-      const int grow = row < a.n_rows ? row : a.n_rows - 1;
-      const float* segp[3];
-#pragma unroll
-      for (int s = 0; s < 3; ++s) {
-        segp[s] = nullptr;
-        if (s < a.n_seg) {
-          const int idx = a.seg[s].idx ? __ldg(a.seg[s].idx + grow) : grow;
-          segp[s] = a.seg[s].base + (size_t)idx * a.seg[s].ld;
-        }
-      }
-      // ---- first layer: gather chunks into the TMEM operand ring
-      for (int c = 0; c < nc1; ++c, ++a_cnt) {
-        const uint32_t slot = a_cnt % NSLOT, n = a_cnt / NSLOT;
-        const int k0 = c * KA;
-        int s = 0, start = 0;
-        while (s < a.n_seg - 1 && k0 >= start + a.seg[s].width) { start += a.seg[s].width; ++s; }
-        const float4* src = reinterpret_cast<const float4*>((s == 0 ? segp[0] : (s == 1 ? segp[1] : segp[2])) + (k0 - start));
-        float x[KA];
-#pragma unroll
-        for (int i = 0; i < KA / 4; ++i) {
-          const float4 t = __ldg(src + i);
-          x[4 * i] = t.x; x[4 * i + 1] = t.y; x[4 * i + 2] = t.z; x[4 * i + 3] = t.w;
-        }
-        mbar_wait(smem_u32(&bars->a_empty[slot]), (n & 1) ^ 1);
+      for (int l = 0; l < n_gemm; ++l, ++g) {
+        const uint32_t b = g & 1;
+        const float* bias = bias_s + l * HW;
+        mbar_wait(smem_u32(&bars->acc_full[b]), (g >> 1) & 1);
         tc_fence_after();
-        store_operand_chunk<MODE>(lane_addr, COL_A + slot * P * AC, AC, x);
-        tc_wait_st();
-        tc_fence_before();
-        mbar_arrive(smem_u32(&bars->a_full[slot]));
-      }
-      // ---- epilogues
-      for (int l = 0; l < n_gemm; ++l, ++layer_cnt) {
-        const float* __restrict__ bias = a.bias[l];
-        mbar_wait(smem_u32(&bars->acc_full), layer_cnt & 1);
-        tc_fence_after();
-        const bool last = (l == n_gemm - 1);
-        if (!last) {                             // hidden layer: ReLU(x + b) -> next A operand in TMEM
+        const uint32_t acc = lane_addr + COL_ACC + b * 128;
+        if (l < n_gemm - 1) {
+          // ---- hidden layer: ReLU(x + b) -> next A operand in TMEM, released chunk by chunk
 #pragma unroll 1
-          for (int q = 0; q < HW / 32; ++q) {
-            uint32_t v[32];
-            tmem_ld32(lane_addr + COL_ACC + q * 32, v);
-            tc_wait_ld();
+          for (int c = 0; c < HCH; ++c) {
             if constexpr (MODE == ETX_PREC_TF32X3) {
-              float x[32];
+              uint32_t v[32], w[32];
+              tmem_ld32(acc + c * 32, v);
+              tc_wait_ld();
 #pragma unroll
-              for (int i = 0; i < 32; ++i) x[i] = fmaxf(__uint_as_float(v[i]) + __ldg(bias + q * 32 + i), 0.f);
-              store_operand_chunk<MODE>(lane_addr, COL_HID + q * 32, HID_COLS, reinterpret_cast<const float(&)[KA]>(x));
-            } else {                             // 32 accumulator columns -> 16 packed bf16 columns
-              uint32_t w[16];
+              for (int i = 0; i < 32; ++i) {
+                const float x = fmaxf(__uint_as_float(v[i]) + bias[c * 32 + i], 0.f);
+                w[i] = __float_as_uint(x) & 0xffffe000u;
+                v[i] = __float_as_uint(x - __uint_as_float(w[i]));
+              }
+              tmem_st32(lane_addr + COL_HID + c * 32, w);
+              tmem_st32(lane_addr + COL_HID + HID_COLS + c * 32, v);
+            } else {
+              uint32_t v0[32], v1[32], w[32];
+              tmem_ld32(acc + c * 64, v0);
+              tmem_ld32(acc + c * 64 + 32, v1);
+              tc_wait_ld();
 #pragma unroll
               for (int i = 0; i < 16; ++i) {
-                const float x0 = fmaxf(__uint_as_float(v[2 * i]) + __ldg(bias + q * 32 + 2 * i), 0.f);
-                const float x1 = fmaxf(__uint_as_float(v[2 * i + 1]) + __ldg(bias + q * 32 + 2 * i + 1), 0.f);
-                w[i] = pack_bf16x2(x0, x1);
+                w[i] = pack_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 2 * i], 0.f),
+                                   fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 2 * i + 1], 0.f));
+                w[16 + i] = pack_bf16x2(fmaxf(__uint_as_float(v1[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
+                                        fmaxf(__uint_as_float(v1[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f));
               }
-              asm volatile(
-                  "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
-                  "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
-                  ::"r"(lane_addr + COL_HID + q * 16),
-                    "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7]),
-                    "r"(w[8]), "r"(w[9]), "r"(w[10]), "r"(w[11]), "r"(w[12]), "r"(w[13]), "r"(w[14]), "r"(w[15])
-                  : "memory");
+              tmem_st32(lane_addr + COL_HID + c * 32, w);
             }
+            tc_wait_st();
+            tc_fence_before();
+            mbar_arrive(smem_u32(&bars->hid_ready[c]));
           }
-          tc_wait_st();
-        } else if (a.out_mode == 3) {            // classifier: last hidden layer, then 1 unit + sigmoid
+          mbar_arrive(smem_u32(&bars->acc_free[b]));
+          ++hcount;
+        } else if (a.out_mode == 3) {
+          // ---- classifier: last hidden layer, then 1 unit + sigmoid
           float logit = 0.f;
 #pragma unroll 1
           for (int q = 0; q < HW / 32; ++q) {
             uint32_t v[32];
-            tmem_ld32(lane_addr + COL_ACC + q * 32, v);
+            tmem_ld32(acc + q * 32, v);
             tc_wait_ld();
 #pragma unroll
-            for (int i = 0; i < 32; ++i) {
-              const float x = fmaxf(__uint_as_float(v[i]) + __ldg(bias + q * 32 + i), 0.f);
-              logit = fmaf(x, __ldg(a.w_last + q * 32 + i), logit);
-            }
+            for (int i = 0; i < 32; ++i)
+              logit = fmaf(fmaxf(__uint_as_float(v[i]) + bias[q * 32 + i], 0.f), wlast_s[q * 32 + i], logit);
           }
+          tc_fence_before();
+          mbar_arrive(smem_u32(&bars->acc_free[b]));
           logit += __ldg(a.bias[a.n_layers - 1]);
+          const int row = tile * TM + et;
           if (row < a.n_rows) a.out[row] = 1.0f / (1.0f + expf(-logit));
-        } else {                                 // linear output (+ residual) -> global
-          float* __restrict__ out = a.out + (size_t)grow * a.out_ld;
-          const float* __restrict__ res = a.res ? a.res + (size_t)grow * a.out_ld : nullptr;
+        } else {
+          // ---- linear output (+ residual): transpose through the swizzled staging tile, coalesced I/O
 #pragma unroll 1
           for (int q = 0; q < HW / 32; ++q) {
             uint32_t v[32];
-            tmem_ld32(lane_addr + COL_ACC + q * 32, v);
+            tmem_ld32(acc + q * 32, v);
             tc_wait_ld();
-            if (row < a.n_rows) {
+            if (q == HW / 32 - 1) { tc_fence_before(); mbar_arrive(smem_u32(&bars->acc_free[b])); }
+            epi_bar_sync();                      // previous round's readers are done with the staging tile
 #pragma unroll
-              for (int i = 0; i < 8; ++i) {
-                const float4 b = __ldg(reinterpret_cast<const float4*>(bias + q * 32) + i);
-                float4 y = make_float4(__uint_as_float(v[4 * i]) + b.x, __uint_as_float(v[4 * i + 1]) + b.y,
-                                       __uint_as_float(v[4 * i + 2]) + b.z, __uint_as_float(v[4 * i + 3]) + b.w);
+            for (int j = 0; j < 8; ++j) {
+              const float* bq = bias + q * 32 + 4 * j;
+              st_shared_v4(stage_out + et * 128 + ((j ^ (et & 7)) << 4),
+                           __float_as_uint(__uint_as_float(v[4 * j]) + bq[0]), __float_as_uint(__uint_as_float(v[4 * j + 1]) + bq[1]),
+                           __float_as_uint(__uint_as_float(v[4 * j + 2]) + bq[2]), __float_as_uint(__uint_as_float(v[4 * j + 3]) + bq[3]));
+            }
+            epi_bar_sync();
+            const int jl = et & 7, rr = et >> 3;
+#pragma unroll
+            for (int p = 0; p < 8; ++p) {
+              const int r = rr + p * 16;
+              const int row = tile * TM + r;
+              if (row < a.n_rows) {
+                float4 y = ld_shared_v4(stage_out + r * 128 + ((jl ^ (r & 7)) << 4));
+                const size_t off = (size_t)row * a.out_ld + q * 32 + jl * 4;
                 if (a.out_mode == 1) {
-                  const float4 t = *(reinterpret_cast<const float4*>(res + q * 32) + i);
-                  y.x += t.x; y.y += t.y; y.z += t.z; y.w += t.w;
+                  const float4 o = *reinterpret_cast<const float4*>(a.res + off);
+                  y.x += o.x; y.y += o.y; y.z += o.z; y.w += o.w;
                 }
-                *(reinterpret_cast<float4*>(out + q * 32) + i) = y;
+                *reinterpret_cast<float4*>(a.out + off) = y;
               }
             }
           }
         }
-        tc_fence_before();
-        mbar_arrive(smem_u32(&bars->work_done));
       }
     }
-  } else if (warp == 4) {
+    (void)hcount;
+  } else if (warp == 8) {
     // =========================== weight loader ===========================
     if (lane == 0) {
       const int chunks_per_tile = nc1 + (n_gemm - 1) * HCH;
       uint32_t w_cnt = 0;
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         for (int q = 0; q < chunks_per_tile; ++q, ++w_cnt) {
-          const uint32_t ws = w_cnt % NSTAGE, wn = w_cnt / NSTAGE;
+          const uint32_t ws = w_cnt % NSW, wn = w_cnt / NSW;
           mbar_wait(smem_u32(&bars->w_empty[ws]), (wn & 1) ^ 1);
           mbar_expect_tx(smem_u32(&bars->w_full[ws]), kStageBytes);
           bulk_g2s(wring + ws * kStageBytes, a.wimg + (size_t)q * kStageBytes, kStageBytes, smem_u32(&bars->w_full[ws]));
@@ -327,53 +390,68 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   } else {
     // =========================== MMA issuer ===========================
     if (lane == 0) {
-      uint32_t w_cnt = 0, a_cnt = 0, g = 0;
+      uint32_t w_cnt = 0, a_cnt = 0, g = 0, hcount = 0;
       for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         for (int l = 0; l < n_gemm; ++l, ++g) {
-          if (g > 0) {                           // previous epilogue done: accumulator free, hidden operand written
-            mbar_wait(smem_u32(&bars->work_done), (g - 1) & 1);
+          const uint32_t b = g & 1, u = g >> 1;
+          if (u >= 1) {                          // the epilogue that last read acc[b] has finished with it
+            mbar_wait(smem_u32(&bars->acc_free[b]), (u - 1) & 1);
             tc_fence_after();
           }
+          const uint32_t d_tmem = tmem + COL_ACC + b * 128;
           const int nch = (l == 0) ? nc1 : HCH;
           for (int c = 0; c < nch; ++c, ++w_cnt) {
-            const uint32_t ws = w_cnt % NSTAGE, wn = w_cnt / NSTAGE;
-            uint32_t a_col, lo_off, slot = 0;
+            const uint32_t ws = w_cnt % NSW, wn = w_cnt / NSW;
+            uint32_t slot = 0;
             if (l == 0) {
-              slot = a_cnt % NSLOT;
-              mbar_wait(smem_u32(&bars->a_full[slot]), (a_cnt / NSLOT) & 1);
-              a_col = COL_A + slot * P * AC; lo_off = AC;
+              slot = a_cnt % NSA;
+              mbar_wait(smem_u32(&bars->a_full[slot]), (a_cnt / NSA) & 1);
             } else {
-              a_col = COL_HID + c * AC; lo_off = HID_COLS;
+              mbar_wait(smem_u32(&bars->hid_ready[c]), hcount & 1);
             }
             mbar_wait(smem_u32(&bars->w_full[ws]), wn & 1);
             tc_fence_after();
             const uint32_t wb = wring + ws * kStageBytes;
+            const uint32_t ab = aring + slot * kStageBytes;
 #pragma unroll
             for (int ks = 0; ks < 4; ++ks) {       // 4 MMA k-steps of 32 bytes inside the 128-byte atom
-              const uint32_t acc = (c > 0 || ks > 0) ? 1u : 0u;
-              const uint32_t a_hi = tmem + a_col + ks * 8;
+              const uint32_t accum = (c > 0 || ks > 0) ? 1u : 0u;
               const uint64_t b_hi = smem_desc(wb + ks * 32);
-              if constexpr (MODE == ETX_PREC_TF32X3) {
-                const uint32_t a_lo = a_hi + lo_off;
-                const uint64_t b_lo = smem_desc(wb + kAtomBytes + ks * 32);
-                mma_ts<MODE>(tmem + COL_ACC, a_lo, b_hi, acc);       // small terms first
-                mma_ts<MODE>(tmem + COL_ACC, a_hi, b_lo, 1u);
-                mma_ts<MODE>(tmem + COL_ACC, a_hi, b_hi, 1u);
+              if (l == 0) {
+                const uint64_t a_hi = smem_desc(ab + ks * 32);
+                if constexpr (MODE == ETX_PREC_TF32X3) {
+                  const uint64_t a_lo = smem_desc(ab + kAtomBytes + ks * 32);
+                  const uint64_t b_lo = smem_desc(wb + kAtomBytes + ks * 32);
+                  mma_ss<MODE>(d_tmem, a_lo, b_hi, accum);             // small terms first
+                  mma_ss<MODE>(d_tmem, a_hi, b_lo, 1u);
+                  mma_ss<MODE>(d_tmem, a_hi, b_hi, 1u);
+                } else {
+                  mma_ss<MODE>(d_tmem, a_hi, b_hi, accum);
+                }
               } else {
-                mma_ts<MODE>(tmem + COL_ACC, a_hi, b_hi, acc);
+                const uint32_t a_hi = tmem + COL_HID + c * 32 + ks * 8;
+                if constexpr (MODE == ETX_PREC_TF32X3) {
+                  const uint64_t b_lo = smem_desc(wb + kAtomBytes + ks * 32);
+                  mma_ts<MODE>(d_tmem, a_hi + HID_COLS, b_hi, accum);
+                  mma_ts<MODE>(d_tmem, a_hi, b_lo, 1u);
+                  mma_ts<MODE>(d_tmem, a_hi, b_hi, 1u);
+                } else {
+                  mma_ts<MODE>(d_tmem, a_hi, b_hi, accum);
+                }
               }
             }
             tc_commit(smem_u32(&bars->w_empty[ws]));
             if (l == 0) { tc_commit(smem_u32(&bars->a_empty[slot])); ++a_cnt; }
           }
-          tc_commit(smem_u32(&bars->acc_full));
+          tc_commit(smem_u32(&bars->acc_full[b]));
+          if (l > 0) ++hcount;
         }
       }
     }
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 5) {
+  if (warp == 9) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
   }
@@ -383,7 +461,8 @@ template <int MODE>
 int launch_mode(const TcArgs& a, int sm_count, cudaStream_t s) {
   using C = Cfg<MODE>;
   static bool configured = false;
-  const size_t smem = 1024 + (size_t)C::NSTAGE * C::PIECES * kAtomBytes + sizeof(Bars) + 64;
+  const size_t smem = 1024 + (size_t)(C::NSTAGE_W + C::NSTAGE_A) * C::PIECES * kAtomBytes + kAtomBytes +
+                      (kMaxLayers + 1) * HW * sizeof(float) + sizeof(Bars) + 64;
   if (!configured) {
     cudaFuncSetAttribute(mlp_tc_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
