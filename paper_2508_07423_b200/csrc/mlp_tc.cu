@@ -2,21 +2,22 @@
 //
 // Computes, for a tile of 128 rows (edges or hits), the whole chain of Eq. 4.27 layers of one
 // GNN MLP — edge encoder, node/edge network or classifier — without any
-// intermediate leaving the SM.  One persistent CTA per SM, ten warps:
+// intermediate leaving the SM.  One persistent CTA per SM, fourteen warps:
 //
-//   warps 0-3  gather:   coalesced 16-byte loads of the first layer's input rows ([h_src | h_dst | e],
-//                        [h | m], ...) straight from the node / edge arrays (8 or 16 lanes per row, one
-//                        K-chunk prefetched in registers), conversion to the MMA operand type and
-//                        st.shared into a ring of canonical K-major SWIZZLE_128B operand tiles.
-//   warps 4-7  epilogue: thread r owns tile row r = TMEM lane r.  After a hidden layer: tcgen05.ld the
+//   warps 0-7  gather:   coalesced 16-byte loads of the first layer's input rows ([h_src | h_dst | e],
+//                        [h | m], ...) straight from the node / edge arrays (8 or 16 lanes per row, a
+//                        ring of K-chunks prefetched in registers: 64 KB in flight per SM), conversion
+//                        to the MMA operand type and st.shared into a ring of canonical K-major
+//                        SWIZZLE_128B operand tiles.
+//   warps 8-11 epilogue: thread r owns tile row r = TMEM lane r.  After a hidden layer: tcgen05.ld the
 //                        accumulator 32 columns at a time, bias + ReLU, convert, tcgen05.st the next
 //                        layer's A operand back into TMEM and release that K-chunk to the MMA warp at
 //                        once, so the next layer's MMAs start while the rest of the epilogue runs.
 //                        After the last layer: bias (+ residual) through a swizzled staging tile so
 //                        the global read-modify-write is coalesced, or the 1-unit head + sigmoid.
-//   warp 8     loader:   streams pre-swizzled weight tiles (prepared once at etx_create) from L2 into a
+//   warp 12    loader:   streams pre-swizzled weight tiles (prepared once at etx_create) from L2 into a
 //                        shared-memory ring with cp.async.bulk (TMA bulk copy) completing on mbarriers.
-//   warp 9     MMA:      one thread issues tcgen05.mma — SS form (A, B in shared memory) for the first
+//   warp 13    MMA:      one thread issues tcgen05.mma — SS form (A, B in shared memory) for the first
 //                        layer, TS form (A in TMEM) for the others — into one of two 128-column TMEM
 //                        accumulators (ping-pong), and tcgen05.commit-s ring slots / accumulators.
 //
@@ -35,7 +36,8 @@ namespace etx {
 namespace {
 
 constexpr int TM = 128;
-constexpr int kThreads = 320;
+constexpr int kGatherThreads = 256;      // warps 0-7
+constexpr int kThreads = kGatherThreads + 128 + 64;   // + epilogue warps 8-11, loader warp 12, MMA warp 13
 constexpr int HW = 128;                       // hidden width handled by this kernel
 constexpr int kAtomBytes = 128 * 128;         // one operand tile: 128 rows x 128 bytes (one swizzle atom wide)
 
@@ -45,6 +47,7 @@ template <> struct Cfg<ETX_PREC_TF32X3> {
   static constexpr int PIECES = 2;            // hi, lo
   static constexpr int NSTAGE_W = 4;          // weight ring stages (32 KB each)
   static constexpr int NSTAGE_A = 2;          // first-layer A operand ring stages (32 KB each)
+  static constexpr int PREFETCH = 4;          // K-chunks a gather thread keeps in flight in registers
   static constexpr int HID_COLS = 128;        // TMEM columns per piece of a hidden operand
   static constexpr uint32_t IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);
 };
@@ -53,6 +56,7 @@ template <> struct Cfg<ETX_PREC_BF16> {
   static constexpr int PIECES = 1;
   static constexpr int NSTAGE_W = 8;          // 16 KB each
   static constexpr int NSTAGE_A = 4;          // 16 KB each
+  static constexpr int PREFETCH = 2;
   static constexpr int HID_COLS = 64;         // 128 bf16 = 64 columns
   static constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);
 };
@@ -91,6 +95,21 @@ __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sy
 __device__ __forceinline__ void tc_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool elect_one() {      // one lane of a fully-active warp
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.b32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+// One lane polls the barrier, the rest of the warp follows through __syncwarp (256 threads polling
+// one shared-memory word, and 256 serialised arrivals on it, cost more than the work they guard).
+__device__ __forceinline__ void mbar_wait_warp(uint32_t bar, uint32_t parity, int lane) {
+  if (lane == 0) mbar_wait(bar, parity);
+  __syncwarp();
+}
+__device__ __forceinline__ void mbar_arrive_warp(uint32_t bar, int lane) {
+  __syncwarp();
+  if (lane == 0) mbar_arrive(bar);
 }
 __device__ __forceinline__ void epi_bar_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }   // epilogue warps only
 
@@ -141,11 +160,11 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32
         "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
       : "memory");
 }
-// K-major SWIZZLE_128B shared-memory matrix descriptor: 8-row groups 1024 B apart (SBO), version 1
-__device__ __forceinline__ uint64_t smem_desc(uint32_t addr) {
-  return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) |
-         ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
-}
+// K-major SWIZZLE_128B shared-memory matrix descriptor: 8-row groups 1024 B apart (SBO), version 1.
+// Shared addresses are < 256 KB, so (addr >> 4) never carries out of the 14-bit address field and a
+// descriptor for base + byte offset is desc(base) + (offset >> 4).
+constexpr uint64_t kDescHi = ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr) { return kDescHi | (uint64_t)(addr >> 4); }
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {   // lo -> bits [0,16)
   uint32_t d;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
@@ -176,8 +195,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   constexpr uint32_t COL_ACC = 0, COL_HID = 256;
   constexpr int HCH = HW / KA;                  // K-chunks per hidden layer (4 / 2)
   constexpr int LPR = KA * 4 / 16;              // gather lanes per row: 16-byte pieces of a chunk row (8 / 16)
-  constexpr int RPP = 128 / LPR;                // rows covered by one pass of the 128 gather threads (16 / 8)
-  constexpr int NPASS = TM / RPP;               // passes per chunk (8 / 16)
+  constexpr int RPP = kGatherThreads / LPR;     // rows covered by one pass of the gather threads (32 / 16)
+  constexpr int NPASS = TM / RPP;               // passes per chunk (4 / 8)
+  constexpr int D = C::PREFETCH;                // nc1 is a multiple of D for every MLP this kernel serves
 
   extern __shared__ unsigned char smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
@@ -203,12 +223,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
     for (int i = threadIdx.x; i < HW; i += kThreads) wlast_s[i] = __ldg(a.w_last + i);
   if (threadIdx.x == 0) {
     for (int i = 0; i < NSW; ++i) { mbar_init(smem_u32(&bars->w_full[i]), 1); mbar_init(smem_u32(&bars->w_empty[i]), 1); }
-    for (int i = 0; i < NSA; ++i) { mbar_init(smem_u32(&bars->a_full[i]), 128); mbar_init(smem_u32(&bars->a_empty[i]), 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&bars->acc_full[i]), 1); mbar_init(smem_u32(&bars->acc_free[i]), 128); }
-    for (int i = 0; i < 4; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), 128);
+    for (int i = 0; i < NSA; ++i) { mbar_init(smem_u32(&bars->a_full[i]), kGatherThreads / 32); mbar_init(smem_u32(&bars->a_empty[i]), 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&bars->acc_full[i]), 1); mbar_init(smem_u32(&bars->acc_free[i]), 4); }
+    for (int i = 0; i < 4; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), 4);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 9) {                               // TMEM: all 512 columns of this SM (1 CTA per SM)
+  if (warp == 13) {                              // TMEM: all 512 columns of this SM (1 CTA per SM)
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&bars->tmem_base)) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
@@ -217,13 +237,15 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
 
-  if (warp < 4) {
+  if (warp < 8) {
     // =========================== gather warps ===========================
-    const int t = threadIdx.x;                   // 0..127
+    const int t = threadIdx.x;                   // 0..255
     const int jl = t % LPR;                      // 16-byte piece of the chunk row this thread moves
     const int r0 = t / LPR;                      // first of its rows; then r0 + RPP, r0 + 2 RPP, ...
     const int total_chunks = ((n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x) * nc1;
-    float4 cur[NPASS], nxt[NPASS];
+    float4 buf[D][NPASS];
+    long long g_wait = 0;
+    const long long g_start = a.dbg ? clock64() : 0;
 
     // loads chunk number `ci` (counted over this CTA's tiles) into registers
     auto load_chunk = [&](int ci, float4 (&dst)[NPASS]) {
@@ -242,45 +264,61 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
       }
     };
 
-    if (total_chunks > 0) load_chunk(0, cur);
-    for (int ci = 0; ci < total_chunks; ++ci) {
-      if (ci + 1 < total_chunks) load_chunk(ci + 1, nxt);
-      const uint32_t slot = ci % NSA, n = ci / NSA;
-      mbar_wait(smem_u32(&bars->a_empty[slot]), (n & 1) ^ 1);
-      const uint32_t tile_hi = aring + slot * kStageBytes;
 #pragma unroll
-      for (int p = 0; p < NPASS; ++p) {
-        const int r = r0 + p * RPP;
-        const float4 v = cur[p];
-        if constexpr (MODE == ETX_PREC_TF32X3) {
-          const uint32_t off = r * 128 + ((jl ^ (r & 7)) << 4);
-          const uint32_t hx = __float_as_uint(v.x) & 0xffffe000u, hy = __float_as_uint(v.y) & 0xffffe000u;
-          const uint32_t hz = __float_as_uint(v.z) & 0xffffe000u, hw = __float_as_uint(v.w) & 0xffffe000u;
-          st_shared_v4(tile_hi + off, hx, hy, hz, hw);
-          st_shared_v4(tile_hi + kAtomBytes + off,
-                       __float_as_uint(v.x - __uint_as_float(hx)), __float_as_uint(v.y - __uint_as_float(hy)),
-                       __float_as_uint(v.z - __uint_as_float(hz)), __float_as_uint(v.w - __uint_as_float(hw)));
-        } else {                                 // 4 floats -> 4 bf16 = 8 bytes at k-byte offset 8*jl
-          const uint32_t off = r * 128 + (((jl >> 1) ^ (r & 7)) << 4) + ((jl & 1) << 3);
-          st_shared_v2(tile_hi + off, pack_bf16x2(v.x, v.y), pack_bf16x2(v.z, v.w));
+    for (int d = 0; d < D; ++d)
+      if (d < total_chunks) load_chunk(d, buf[d]);
+    for (int ci0 = 0; ci0 < total_chunks; ci0 += D) {
+#pragma unroll
+      for (int d = 0; d < D; ++d) {
+        const int ci = ci0 + d;
+        if (ci < total_chunks) {
+          const uint32_t slot = ci % NSA, n = ci / NSA;
+          long long tg0 = a.dbg ? clock64() : 0;
+          mbar_wait_warp(smem_u32(&bars->a_empty[slot]), (n & 1) ^ 1, lane);
+          if (a.dbg) g_wait += clock64() - tg0;
+          const uint32_t tile_hi = aring + slot * kStageBytes;
+#pragma unroll
+          for (int p = 0; p < NPASS; ++p) {
+            const int r = r0 + p * RPP;
+            const float4 v = buf[d][p];
+            if constexpr (MODE == ETX_PREC_TF32X3) {
+              const uint32_t off = r * 128 + ((jl ^ (r & 7)) << 4);
+              const uint32_t hx = __float_as_uint(v.x) & 0xffffe000u, hy = __float_as_uint(v.y) & 0xffffe000u;
+              const uint32_t hz = __float_as_uint(v.z) & 0xffffe000u, hw = __float_as_uint(v.w) & 0xffffe000u;
+              st_shared_v4(tile_hi + off, hx, hy, hz, hw);
+              st_shared_v4(tile_hi + kAtomBytes + off,
+                           __float_as_uint(v.x - __uint_as_float(hx)), __float_as_uint(v.y - __uint_as_float(hy)),
+                           __float_as_uint(v.z - __uint_as_float(hz)), __float_as_uint(v.w - __uint_as_float(hw)));
+            } else {                             // 4 floats -> 4 bf16 = 8 bytes at k-byte offset 8*jl
+              const uint32_t off = r * 128 + (((jl >> 1) ^ (r & 7)) << 4) + ((jl & 1) << 3);
+              st_shared_v2(tile_hi + off, pack_bf16x2(v.x, v.y), pack_bf16x2(v.z, v.w));
+            }
+          }
+          fence_async_smem();                    // generic-proxy writes -> visible to the tensor core (async proxy)
+          mbar_arrive_warp(smem_u32(&bars->a_full[slot]), lane);
+          if (ci + D < total_chunks) load_chunk(ci + D, buf[d]);
         }
       }
-      fence_async_smem();                        // generic-proxy writes -> visible to the tensor core (async proxy)
-      mbar_arrive(smem_u32(&bars->a_full[slot]));
-#pragma unroll
-      for (int p = 0; p < NPASS; ++p) cur[p] = nxt[p];
     }
-  } else if (warp < 8) {
+    if (a.dbg && t == 0) {
+      a.dbg[(size_t)blockIdx.x * 16 + 8] = (unsigned long long)g_wait;
+      a.dbg[(size_t)blockIdx.x * 16 + 9] = (unsigned long long)(clock64() - g_start);
+    }
+  } else if (warp < 12) {
     // =========================== epilogue warps ===========================
-    const int et = threadIdx.x - 128;            // 0..127 = tile row = TMEM lane
+    const int et = threadIdx.x - kGatherThreads; // 0..127 = tile row = TMEM lane
     const int q4 = warp & 3;                     // TMEM lane quarter this warp may access
     const uint32_t lane_addr = tmem + ((uint32_t)(q4 * 32) << 16);
     uint32_t g = 0, hcount = 0;
+    long long e_wait = 0;
+    const long long e_start = a.dbg ? clock64() : 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
       for (int l = 0; l < n_gemm; ++l, ++g) {
         const uint32_t b = g & 1;
         const float* bias = bias_s + l * HW;
-        mbar_wait(smem_u32(&bars->acc_full[b]), (g >> 1) & 1);
+        long long te0 = a.dbg ? clock64() : 0;
+        mbar_wait_warp(smem_u32(&bars->acc_full[b]), (g >> 1) & 1, lane);
+        if (a.dbg) e_wait += clock64() - te0;
         tc_fence_after();
         const uint32_t acc = lane_addr + COL_ACC + b * 128;
         if (l < n_gemm - 1) {
@@ -315,9 +353,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
             }
             tc_wait_st();
             tc_fence_before();
-            mbar_arrive(smem_u32(&bars->hid_ready[c]));
+            mbar_arrive_warp(smem_u32(&bars->hid_ready[c]), lane);
           }
-          mbar_arrive(smem_u32(&bars->acc_free[b]));
+          mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane);
           ++hcount;
         } else if (a.out_mode == 3) {
           // ---- classifier: last hidden layer, then 1 unit + sigmoid
@@ -332,40 +370,51 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
               logit = fmaf(fmaxf(__uint_as_float(v[i]) + bias[q * 32 + i], 0.f), wlast_s[q * 32 + i], logit);
           }
           tc_fence_before();
-          mbar_arrive(smem_u32(&bars->acc_free[b]));
+          mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane);
           logit += __ldg(a.bias[a.n_layers - 1]);
           const int row = tile * TM + et;
           if (row < a.n_rows) a.out[row] = 1.0f / (1.0f + expf(-logit));
         } else {
-          // ---- linear output (+ residual): transpose through the swizzled staging tile, coalesced I/O
-#pragma unroll 1
+          // ---- linear output (+ residual): transpose through the swizzled staging tile, coalesced I/O.
+          // The residual rows are prefetched one column group ahead (they come from HBM).
+          const int jl = et & 7, rr = et >> 3;
+          const bool has_res = (a.out_mode == 1);
+          float4 rbuf[2][8];
+          auto load_res = [&](int q, float4 (&dst)[8]) {
+#pragma unroll
+            for (int p = 0; p < 8; ++p) {
+              const int row = tile * TM + rr + p * 16;
+              const int grow = row < a.n_rows ? row : a.n_rows - 1;
+              dst[p] = has_res ? __ldg(reinterpret_cast<const float4*>(a.res + (size_t)grow * a.out_ld + q * 32 + jl * 4))
+                               : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+          };
+          load_res(0, rbuf[0]);
+#pragma unroll
           for (int q = 0; q < HW / 32; ++q) {
+            if (q + 1 < HW / 32) load_res(q + 1, rbuf[(q + 1) & 1]);
             uint32_t v[32];
             tmem_ld32(acc + q * 32, v);
             tc_wait_ld();
-            if (q == HW / 32 - 1) { tc_fence_before(); mbar_arrive(smem_u32(&bars->acc_free[b])); }
+            if (q == HW / 32 - 1) { tc_fence_before(); mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane); }
             epi_bar_sync();                      // previous round's readers are done with the staging tile
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-              const float* bq = bias + q * 32 + 4 * j;
+              const float4 bq = *reinterpret_cast<const float4*>(bias + q * 32 + 4 * j);
               st_shared_v4(stage_out + et * 128 + ((j ^ (et & 7)) << 4),
-                           __float_as_uint(__uint_as_float(v[4 * j]) + bq[0]), __float_as_uint(__uint_as_float(v[4 * j + 1]) + bq[1]),
-                           __float_as_uint(__uint_as_float(v[4 * j + 2]) + bq[2]), __float_as_uint(__uint_as_float(v[4 * j + 3]) + bq[3]));
+                           __float_as_uint(__uint_as_float(v[4 * j]) + bq.x), __float_as_uint(__uint_as_float(v[4 * j + 1]) + bq.y),
+                           __float_as_uint(__uint_as_float(v[4 * j + 2]) + bq.z), __float_as_uint(__uint_as_float(v[4 * j + 3]) + bq.w));
             }
             epi_bar_sync();
-            const int jl = et & 7, rr = et >> 3;
 #pragma unroll
             for (int p = 0; p < 8; ++p) {
               const int r = rr + p * 16;
               const int row = tile * TM + r;
               if (row < a.n_rows) {
                 float4 y = ld_shared_v4(stage_out + r * 128 + ((jl ^ (r & 7)) << 4));
-                const size_t off = (size_t)row * a.out_ld + q * 32 + jl * 4;
-                if (a.out_mode == 1) {
-                  const float4 o = *reinterpret_cast<const float4*>(a.res + off);
-                  y.x += o.x; y.y += o.y; y.z += o.z; y.w += o.w;
-                }
-                *reinterpret_cast<float4*>(a.out + off) = y;
+                const float4 o = rbuf[q & 1][p];
+                y.x += o.x; y.y += o.y; y.z += o.z; y.w += o.w;
+                *reinterpret_cast<float4*>(a.out + (size_t)row * a.out_ld + q * 32 + jl * 4) = y;
               }
             }
           }
@@ -373,7 +422,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
       }
     }
     (void)hcount;
-  } else if (warp == 8) {
+    if (a.dbg && et == 0) {
+      a.dbg[(size_t)blockIdx.x * 16 + 6] = (unsigned long long)e_wait;
+      a.dbg[(size_t)blockIdx.x * 16 + 7] = (unsigned long long)(clock64() - e_start);
+    }
+  } else if (warp == 12) {
     // =========================== weight loader ===========================
     if (lane == 0) {
       const int chunks_per_tile = nc1 + (n_gemm - 1) * HCH;
@@ -389,69 +442,90 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
     }
   } else {
     // =========================== MMA issuer ===========================
-    if (lane == 0) {
-      uint32_t w_cnt = 0, a_cnt = 0, g = 0, hcount = 0;
-      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        for (int l = 0; l < n_gemm; ++l, ++g) {
-          const uint32_t b = g & 1, u = g >> 1;
-          if (u >= 1) {                          // the epilogue that last read acc[b] has finished with it
-            mbar_wait(smem_u32(&bars->acc_free[b]), (u - 1) & 1);
-            tc_fence_after();
+    // Warp-uniform control flow: every lane waits on the barriers, one elected lane issues.  (Issuing
+    // from a divergent `if (lane == 0)` region makes ptxas wrap every UTCHMMA in an election loop,
+    // which left the tensor pipe idle half of the time.)
+    uint32_t w_cnt = 0, a_cnt = 0, g = 0, hcount = 0;
+    long long dt[6] = {0, 0, 0, 0, 0, 0};
+    const bool dbg = a.dbg != nullptr;
+    long long t_start = dbg ? clock64() : 0, t0 = 0;
+#define DBG_T0() if (dbg) t0 = clock64()
+#define DBG_ACC(i) if (dbg) dt[i] += clock64() - t0
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      for (int l = 0; l < n_gemm; ++l, ++g) {
+        const uint32_t b = g & 1, u = g >> 1;
+        DBG_T0();
+        if (u >= 1) mbar_wait(smem_u32(&bars->acc_free[b]), (u - 1) & 1);   // epilogue done with acc[b]
+        DBG_ACC(0);
+        const uint32_t d_tmem = tmem + COL_ACC + b * 128;
+        const int nch = (l == 0) ? nc1 : HCH;
+        for (int c = 0; c < nch; ++c, ++w_cnt) {
+          const uint32_t ws = w_cnt % NSW, wn = w_cnt / NSW;
+          uint32_t slot = 0;
+          DBG_T0();
+          if (l == 0) {
+            slot = a_cnt % NSA;
+            mbar_wait(smem_u32(&bars->a_full[slot]), (a_cnt / NSA) & 1);
+            DBG_ACC(1);
+          } else {
+            mbar_wait(smem_u32(&bars->hid_ready[c]), hcount & 1);
+            DBG_ACC(2);
           }
-          const uint32_t d_tmem = tmem + COL_ACC + b * 128;
-          const int nch = (l == 0) ? nc1 : HCH;
-          for (int c = 0; c < nch; ++c, ++w_cnt) {
-            const uint32_t ws = w_cnt % NSW, wn = w_cnt / NSW;
-            uint32_t slot = 0;
+          DBG_T0();
+          mbar_wait(smem_u32(&bars->w_full[ws]), wn & 1);
+          DBG_ACC(3);
+          tc_fence_after();
+          DBG_T0();
+          if (elect_one()) {
+            const uint64_t wd = smem_desc(wring + ws * kStageBytes);          // weight tile (hi piece)
+            const uint32_t accum0 = c > 0 ? 1u : 0u;
             if (l == 0) {
-              slot = a_cnt % NSA;
-              mbar_wait(smem_u32(&bars->a_full[slot]), (a_cnt / NSA) & 1);
-            } else {
-              mbar_wait(smem_u32(&bars->hid_ready[c]), hcount & 1);
-            }
-            mbar_wait(smem_u32(&bars->w_full[ws]), wn & 1);
-            tc_fence_after();
-            const uint32_t wb = wring + ws * kStageBytes;
-            const uint32_t ab = aring + slot * kStageBytes;
+              const uint64_t ad = smem_desc(aring + slot * kStageBytes);      // gathered operand tile (hi piece)
 #pragma unroll
-            for (int ks = 0; ks < 4; ++ks) {       // 4 MMA k-steps of 32 bytes inside the 128-byte atom
-              const uint32_t accum = (c > 0 || ks > 0) ? 1u : 0u;
-              const uint64_t b_hi = smem_desc(wb + ks * 32);
-              if (l == 0) {
-                const uint64_t a_hi = smem_desc(ab + ks * 32);
+              for (int ks = 0; ks < 4; ++ks) {     // 4 MMA k-steps of 32 bytes inside the 128-byte atom
+                const uint32_t accum = ks > 0 ? 1u : accum0;
                 if constexpr (MODE == ETX_PREC_TF32X3) {
-                  const uint64_t a_lo = smem_desc(ab + kAtomBytes + ks * 32);
-                  const uint64_t b_lo = smem_desc(wb + kAtomBytes + ks * 32);
-                  mma_ss<MODE>(d_tmem, a_lo, b_hi, accum);             // small terms first
-                  mma_ss<MODE>(d_tmem, a_hi, b_lo, 1u);
-                  mma_ss<MODE>(d_tmem, a_hi, b_hi, 1u);
+                  mma_ss<MODE>(d_tmem, ad + (kAtomBytes >> 4) + ks * 2, wd + ks * 2, accum);   // lo.hi  (small terms first)
+                  mma_ss<MODE>(d_tmem, ad + ks * 2, wd + (kAtomBytes >> 4) + ks * 2, 1u);      // hi.lo
+                  mma_ss<MODE>(d_tmem, ad + ks * 2, wd + ks * 2, 1u);                          // hi.hi
                 } else {
-                  mma_ss<MODE>(d_tmem, a_hi, b_hi, accum);
+                  mma_ss<MODE>(d_tmem, ad + ks * 2, wd + ks * 2, accum);
                 }
-              } else {
-                const uint32_t a_hi = tmem + COL_HID + c * 32 + ks * 8;
+              }
+            } else {
+              const uint32_t at = tmem + COL_HID + c * 32;
+#pragma unroll
+              for (int ks = 0; ks < 4; ++ks) {
+                const uint32_t accum = ks > 0 ? 1u : accum0;
                 if constexpr (MODE == ETX_PREC_TF32X3) {
-                  const uint64_t b_lo = smem_desc(wb + kAtomBytes + ks * 32);
-                  mma_ts<MODE>(d_tmem, a_hi + HID_COLS, b_hi, accum);
-                  mma_ts<MODE>(d_tmem, a_hi, b_lo, 1u);
-                  mma_ts<MODE>(d_tmem, a_hi, b_hi, 1u);
+                  mma_ts<MODE>(d_tmem, at + HID_COLS + ks * 8, wd + ks * 2, accum);
+                  mma_ts<MODE>(d_tmem, at + ks * 8, wd + (kAtomBytes >> 4) + ks * 2, 1u);
+                  mma_ts<MODE>(d_tmem, at + ks * 8, wd + ks * 2, 1u);
                 } else {
-                  mma_ts<MODE>(d_tmem, a_hi, b_hi, accum);
+                  mma_ts<MODE>(d_tmem, at + ks * 8, wd + ks * 2, accum);
                 }
               }
             }
             tc_commit(smem_u32(&bars->w_empty[ws]));
-            if (l == 0) { tc_commit(smem_u32(&bars->a_empty[slot])); ++a_cnt; }
+            if (l == 0) tc_commit(smem_u32(&bars->a_empty[slot]));
+            if (c == nch - 1) tc_commit(smem_u32(&bars->acc_full[b]));
           }
-          tc_commit(smem_u32(&bars->acc_full[b]));
-          if (l > 0) ++hcount;
+          __syncwarp();
+          DBG_ACC(4);
+          if (l == 0) ++a_cnt;
         }
+        if (l > 0) ++hcount;
       }
+    }
+    if (dbg && lane == 0) {
+      unsigned long long* o = a.dbg + (size_t)blockIdx.x * 16;
+      for (int i = 0; i < 5; ++i) o[i] = (unsigned long long)dt[i];
+      o[5] = (unsigned long long)(clock64() - t_start);
     }
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 9) {
+  if (warp == 13) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
   }
