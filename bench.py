@@ -51,6 +51,28 @@ def peaks():
             "source": "fallback"}
 
 
+def shard_event_ids(cfg, rank: int, n_ev: int):
+    """Events are independent: rank r takes event ids r*n_ev .. (r+1)*n_ev - 1 of the config's
+    stream (weak scaling, no data-path collective)."""
+    return range(rank * n_ev, (rank + 1) * n_ev)
+
+
+def reduce_max(value: float, device=None) -> float:
+    """Max over ranks of a per-rank time (the only collective of a multi-GPU run)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_events_per_s(world: int, n_ev_per_rank: int, ms_step_max: float) -> float:
+    """Whole-job throughput: all ranks' events over the slowest rank's step time."""
+    return world * n_ev_per_rank / (ms_step_max * 1e-3)
+
+
 def flops_mlp(dims):
     return sum(2 * dims[i] * dims[i + 1] for i in range(len(dims) - 1))
 
@@ -178,7 +200,7 @@ def run_ours(args):
 
     cfg = synth.CONFIGS[args.config]
     n_ev = args.events or cfg.n_events
-    batch = synth.generate_events(cfg, range(rank * n_ev, (rank + 1) * n_ev))
+    batch = synth.generate_events(cfg, shard_event_ids(cfg, rank, n_ev))
     blob = synth.generate_weights(cfg)
     etx = binding.Etx(binding.make_desc(cfg, precision=args.precision if args.precision is not None else cfg.precision),
                       blob, device=local)
@@ -222,12 +244,9 @@ def run_ours(args):
     launches = etx.launch_count() - l0
     prof = etx.profile_read()
     etx.profile_enable(False)
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = reduce_max(ms, dev)
     ms_step = ms / args.steps
-    value = world * n_ev / (ms_step * 1e-3)
+    value = aggregate_events_per_s(world, n_ev, ms_step)
 
     # ---- end to end through the host-buffer entry point
     host = binding.pinned_host_batch(batch)
@@ -244,10 +263,7 @@ def run_ours(args):
     t1.record()
     barrier()
     e2e_ms = max(t0.elapsed_time(t1), 1e3 * (time.perf_counter() - w0)) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = reduce_max(e2e_ms, dev)
     h2d = sum(host[k].numel() * host[k].element_size() for k in host)
     d2h = E2 * 12
 
@@ -292,6 +308,12 @@ def run_ours(args):
                                "MMAs per algorithmic FLOP"}
         achieved *= 3.0
         dtype = "tf32x3"
+    elif prec == synth.PREC_BF16X3:
+        peak = pk["bf16_tflops_sustained"]
+        roof = {"bound": "tensor", "unit": "TFLOP/s", "peak": peak,
+                "peak_source": f"{pk['source']} bf16 sustained; achieved counts the 3 bf16 MMAs per algorithmic FLOP"}
+        achieved *= 3.0
+        dtype = "bf16x3"
     else:
         peak = pk["bf16_tflops_sustained"]
         roof = {"bound": "tensor", "unit": "TFLOP/s", "peak": peak, "peak_source": f"{pk['source']} bf16 sustained"}
@@ -318,7 +340,7 @@ def run_ours(args):
                    "l2": "state larger than L2 (edge encodings %.1f GB), no flush needed" % (E * H * 4 / 1e9),
                    "parallelism": "events sharded across GPUs, no collective" if world > 1 else "single GPU"},
         "roofline": roof, "cpu_baseline": cpu,
-        "e2e": {"value": world * n_ev / (e2e_ms * 1e-3), "unit": "events/s", "h2d_bytes_per_step": int(h2d),
+        "e2e": {"value": aggregate_events_per_s(world, n_ev, e2e_ms), "unit": "events/s", "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms},
         "gpu_launches": int(launches), "clocks": clk.summary(), "stages": stages}))
     if world > 1:
@@ -347,7 +369,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c2", choices=sorted(synth.CONFIGS))
     ap.add_argument("--events", type=int, default=0, help="events per GPU (default: the config's)")
-    ap.add_argument("--precision", type=int, default=None, help="override etx_precision (0 fp32, 1 tf32x3, 2 bf16)")
+    ap.add_argument("--precision", type=int, default=None, help="override etx_precision (0 fp32, 1 tf32x3, 2 bf16, 3 bf16x3)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

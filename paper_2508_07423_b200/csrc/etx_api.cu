@@ -27,7 +27,7 @@ const char* check_desc(const etx_model_desc* d) {
   if (d->gnn_n_layers < 2 || d->gnn_n_layers > kMaxLayers) return "gnn_n_layers must be 2..8";
   if (d->n_iter < 0 || d->n_iter > 64) return "n_iter must be 0..64";
   if (d->n_planes < 2 || d->n_planes > 255) return "n_planes must be 2..255";
-  if (d->precision < ETX_PREC_FP32 || d->precision > ETX_PREC_BF16) return "unknown precision";
+  if (d->precision < ETX_PREC_FP32 || d->precision > ETX_PREC_BF16X3) return "unknown precision";
   for (int i = 0; i < 5; ++i)
     if (!(d->norm_scale[i] != 0.0f)) return "norm_scale entries must be non-zero";
   return nullptr;
@@ -63,7 +63,7 @@ size_t mlp_floats(const HostMlp& m) {
 // Tensor-core weight image of the first n_gemm layers of an MLP (mlp_tc.cu): for every layer, for every
 // K-chunk of one 128-byte swizzle atom (32 tf32 / 64 bf16 values), one 16 KB tile per piece laid out
 // exactly as the canonical K-major SWIZZLE_128B shared-memory operand: row n (output neuron) at
-// n*128 bytes, its 16-byte groups XOR-ed with (n & 7).  TF32X3 stores two pieces (hi, lo) per chunk.
+// n*128 bytes, its 16-byte groups XOR-ed with (n & 7).  TF32X3 / BF16X3 store two pieces (hi, lo) per chunk.
 uint16_t bf16_rne(float f) {
   uint32_t u; std::memcpy(&u, &f, 4);
   if ((u & 0x7fffffffu) > 0x7f800000u) return (uint16_t)((u >> 16) | 0x40);
@@ -73,7 +73,7 @@ uint16_t bf16_rne(float f) {
 
 void append_wimg(std::vector<unsigned char>& img, const HostMlp& m, const float* w, int n_gemm, int mode) {
   const int KA = tc_chunk_k(mode);
-  const int pieces = mode == ETX_PREC_TF32X3 ? 2 : 1;
+  const int pieces = mode == ETX_PREC_BF16 ? 1 : 2;
   const float* W = w;
   for (int l = 0; l < n_gemm; ++l) {
     const int fi = m.dims[l], fo = m.dims[l + 1];           // fo == 128
@@ -95,6 +95,12 @@ void append_wimg(std::vector<unsigned char>& img, const HostMlp& m, const float*
             const uint16_t b = bf16_rne(v);
             const size_t off = (size_t)n * 128 + (size_t)(((kk / 8) ^ (n & 7)) * 16) + (kk % 8) * 2;
             std::memcpy(&img[base + off], &b, 2);
+            if (pieces == 2) {                          // BF16X3: lo = bf16(w - hi)
+              const uint32_t hu = (uint32_t)b << 16;
+              float hf; std::memcpy(&hf, &hu, 4);
+              const uint16_t lo = bf16_rne(v - hf);
+              std::memcpy(&img[base + 128 * 128 + off], &lo, 2);
+            }
           }
         }
     }

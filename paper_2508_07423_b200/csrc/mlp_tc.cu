@@ -30,6 +30,10 @@
 //                    The dropped lo.w_lo term is ~2^-22 relative: fp32-equivalent.
 //   ETX_PREC_BF16:   operands rounded to bf16 (RNE), one kind::f16 MMA, fp32 accumulate; the state
 //                    (h, e, m) and the residual adds stay fp32.
+//   ETX_PREC_BF16X3: x = hi + lo with hi = bf16(x), lo = bf16(x - hi) (16 significand bits), three
+//                    kind::f16 MMAs lo.w_hi + hi.w_lo + hi.w_hi.  Half the MMA steps, shared-memory and
+//                    L2 bytes of TF32X3.  Measured score error is the same ~1e-5 as TF32X3, because both
+//                    are dominated by the tensor core's truncating fp32 accumulation.
 #include "common.cuh"
 
 namespace etx {
@@ -58,6 +62,15 @@ template <> struct Cfg<ETX_PREC_BF16> {
   static constexpr int NSTAGE_A = 4;          // 16 KB each
   static constexpr int PREFETCH = 2;
   static constexpr int HID_COLS = 64;         // 128 bf16 = 64 columns
+  static constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);
+};
+template <> struct Cfg<ETX_PREC_BF16X3> {
+  static constexpr int KA = 64;
+  static constexpr int PIECES = 2;            // hi, lo (bf16 each)
+  static constexpr int NSTAGE_W = 4;          // 32 KB each
+  static constexpr int NSTAGE_A = 2;          // 32 KB each
+  static constexpr int PREFETCH = 2;
+  static constexpr int HID_COLS = 64;
   static constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);
 };
 
@@ -169,6 +182,11 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {   // lo ->
   uint32_t d;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
   return d;
+}
+// (a, b) -> packed bf16 hi pair and the bf16 pair of the remainders a - hi(a), b - hi(b)
+__device__ __forceinline__ void split_bf16x2(float a, float b, uint32_t& hi, uint32_t& lo) {
+  hi = pack_bf16x2(a, b);
+  lo = pack_bf16x2(a - __uint_as_float(hi << 16), b - __uint_as_float(hi & 0xffff0000u));
 }
 __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
@@ -291,7 +309,15 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
                            __float_as_uint(v.z - __uint_as_float(hz)), __float_as_uint(v.w - __uint_as_float(hw)));
             } else {                             // 4 floats -> 4 bf16 = 8 bytes at k-byte offset 8*jl
               const uint32_t off = r * 128 + (((jl >> 1) ^ (r & 7)) << 4) + ((jl & 1) << 3);
-              st_shared_v2(tile_hi + off, pack_bf16x2(v.x, v.y), pack_bf16x2(v.z, v.w));
+              if constexpr (P == 2) {
+                uint32_t h0, l0, h1, l1;
+                split_bf16x2(v.x, v.y, h0, l0);
+                split_bf16x2(v.z, v.w, h1, l1);
+                st_shared_v2(tile_hi + off, h0, h1);
+                st_shared_v2(tile_hi + kAtomBytes + off, l0, l1);
+              } else {
+                st_shared_v2(tile_hi + off, pack_bf16x2(v.x, v.y), pack_bf16x2(v.z, v.w));
+              }
             }
           }
           fence_async_smem();                    // generic-proxy writes -> visible to the tensor core (async proxy)
@@ -337,6 +363,20 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
               }
               tmem_st32(lane_addr + COL_HID + c * 32, w);
               tmem_st32(lane_addr + COL_HID + HID_COLS + c * 32, v);
+            } else if constexpr (P == 2) {       // BF16X3: 64 accumulator columns -> 32 hi + 32 lo packed columns
+              uint32_t v0[32], v1[32], wh[32], wl[32];
+              tmem_ld32(acc + c * 64, v0);
+              tmem_ld32(acc + c * 64 + 32, v1);
+              tc_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 16; ++i) {
+                split_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 2 * i], 0.f),
+                             fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 2 * i + 1], 0.f), wh[i], wl[i]);
+                split_bf16x2(fmaxf(__uint_as_float(v1[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
+                             fmaxf(__uint_as_float(v1[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f), wh[16 + i], wl[16 + i]);
+              }
+              tmem_st32(lane_addr + COL_HID + c * 32, wh);
+              tmem_st32(lane_addr + COL_HID + HID_COLS + c * 32, wl);
             } else {
               uint32_t v0[32], v1[32], w[32];
               tmem_ld32(acc + c * 64, v0);
@@ -484,7 +524,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
 #pragma unroll
               for (int ks = 0; ks < 4; ++ks) {     // 4 MMA k-steps of 32 bytes inside the 128-byte atom
                 const uint32_t accum = ks > 0 ? 1u : accum0;
-                if constexpr (MODE == ETX_PREC_TF32X3) {
+                if constexpr (P == 2) {
                   mma_ss<MODE>(d_tmem, ad + (kAtomBytes >> 4) + ks * 2, wd + ks * 2, accum);   // lo.hi  (small terms first)
                   mma_ss<MODE>(d_tmem, ad + ks * 2, wd + (kAtomBytes >> 4) + ks * 2, 1u);      // hi.lo
                   mma_ss<MODE>(d_tmem, ad + ks * 2, wd + ks * 2, 1u);                          // hi.hi
@@ -497,7 +537,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
 #pragma unroll
               for (int ks = 0; ks < 4; ++ks) {
                 const uint32_t accum = ks > 0 ? 1u : accum0;
-                if constexpr (MODE == ETX_PREC_TF32X3) {
+                if constexpr (P == 2) {
                   mma_ts<MODE>(d_tmem, at + HID_COLS + ks * 8, wd + ks * 2, accum);
                   mma_ts<MODE>(d_tmem, at + ks * 8, wd + (kAtomBytes >> 4) + ks * 2, 1u);
                   mma_ts<MODE>(d_tmem, at + ks * 8, wd + ks * 2, 1u);
@@ -557,6 +597,7 @@ int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s) {
   if (a.n_rows <= 0) return 0;
   if (mode == ETX_PREC_TF32X3) return launch_mode<ETX_PREC_TF32X3>(a, sm_count, s);
   if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16>(a, sm_count, s);
+  if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3>(a, sm_count, s);
   return -1;
 }
 

@@ -1,0 +1,98 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times: the whole
+1000-event batch goes through the four C-ABI calls once; sampled events are then recomputed one by
+one by the CPU oracle and compared, and size-independent properties are checked on the whole batch."""
+import numpy as np
+import pytest
+import torch
+
+from conftest import oracle_path
+from oracle import etx_oracle as orc
+from paper_2508_07423_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL = {synth.PREC_FP32: 1e-4, synth.PREC_TF32X3: 1e-4, synth.PREC_BF16: 2e-2}
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2508_07423_b200 import binding, build
+    build.build()
+    return binding
+
+
+def run_full(B, cfg, batch, blob):
+    etx = B.Etx(B.make_desc(cfg), blob)                       # the config's bench precision
+    dev = etx.device
+    db = B.DeviceBatch(batch, dev)
+    N = db.n_hits
+    cap = int(N * (cfg.target_degree * 1.25 + 2))             # bench.py's capacity rule
+    etx.ensure_workspace(db.n_events, N, cap)
+    g = B.DeviceGraph(N, cap, dev)
+    emb = etx.etx_embed(db)
+    E = etx.etx_build_graph(db, emb, synth.r2_max(cfg), cfg.max_plane_gap, g)
+    enc = torch.empty(cap, cfg.gnn_hidden, device=dev)
+    sc = torch.empty(cap, device=dev)
+    etx.etx_gnn_forward(db, g, enc)
+    etx.etx_edge_scores(g, enc, sc)
+    torch.cuda.synchronize()
+    out = {"E": E, "src": g.src[:E].cpu().numpy(), "dst": g.dst[:E].cpu().numpy(),
+           "row_ptr": g.row_ptr.cpu().numpy(), "in_ptr": g.in_ptr.cpu().numpy(),
+           "in_perm": g.in_perm[:E].cpu().numpy(), "scores": sc[:E].cpu().numpy(), "emb": emb.cpu().numpy()}
+    del enc, sc, g, emb, db, etx
+    torch.cuda.empty_cache()
+    return out
+
+
+def check_properties(cfg, batch, out):
+    N, E = len(batch["r"]), out["E"]
+    src, dst = out["src"].astype(np.int64), out["dst"].astype(np.int64)
+    assert out["row_ptr"][0] == 0 and out["row_ptr"][-1] == E and np.all(np.diff(out["row_ptr"]) >= 0)
+    assert out["in_ptr"][0] == 0 and out["in_ptr"][-1] == E and np.all(np.diff(out["in_ptr"]) >= 0)
+    np.testing.assert_array_equal(np.bincount(src, minlength=N), np.diff(out["row_ptr"]))     # degree sums = E
+    np.testing.assert_array_equal(np.bincount(dst, minlength=N), np.diff(out["in_ptr"]))
+    key = src * N + dst
+    assert np.all(np.diff(key) > 0)                                 # ordered (src, dst): no duplicates
+    pl = batch["plane"].astype(np.int64)
+    dp = pl[dst] - pl[src]
+    assert dp.min() >= 1 and dp.max() <= cfg.max_plane_gap          # allowed plane pairs only
+    ev = np.repeat(np.arange(len(batch["event_ptr"]) - 1), np.diff(batch["event_ptr"]))
+    assert np.array_equal(ev[src], ev[dst])                         # never across events
+    perm = out["in_perm"].astype(np.int64)
+    assert np.array_equal(np.sort(perm), np.arange(E))              # a permutation of the edge ids
+    assert np.all(np.diff(dst[perm]) >= 0)                          # grouped by destination
+    same = np.diff(dst[perm]) == 0
+    assert np.all(np.diff(perm)[same] > 0)                          # ascending edge id inside a group
+    s = out["scores"]
+    assert np.all(np.isfinite(s)) and s.min() >= 0.0 and s.max() <= 1.0
+    assert s.std() > 0.01 and np.mean((s > 0.02) & (s < 0.98)) > 0.5    # not saturated (Q14)
+    return ev
+
+
+@pytest.mark.parametrize("name,sample", [("c2", [0, 137, 500, 999]), ("c3", [1, 998]), ("c4", [0, 999])])
+def test_full_batch_sampled_events(B, name, sample):
+    cfg = synth.CONFIGS[name]
+    batch = synth.generate_events(cfg)
+    blob = synth.generate_weights(cfg)
+    out = run_full(B, cfg, batch, blob)
+    ev = check_properties(cfg, batch, out)
+    assert abs(out["E"] / len(batch["r"]) - cfg.target_degree) < 0.08 * cfg.target_degree
+    ep = batch["event_ptr"].astype(np.int64)
+    worst = 0.0
+    for e in sample:
+        sub = synth.select_events(batch, [e])
+        ora = oracle_path(cfg, sub, blob)
+        sel = ev[out["src"]] == e
+        gs, gd = out["src"][sel] - ep[e], out["dst"][sel] - ep[e]
+        np.testing.assert_allclose(out["emb"][ep[e]:ep[e + 1]], ora["emb"], rtol=0, atol=2e-6)
+        _, _, border = orc.build_graph(sub["event_ptr"], sub["plane"], ora["emb"], synth.r2_max(cfg),
+                                       cfg.max_plane_gap, band=1e-5, want_border=True)
+        got, want = set(zip(gs.tolist(), gd.tolist())), set(zip(ora["src"].tolist(), ora["dst"].tolist()))
+        assert (got ^ want) <= set(map(tuple, border.tolist()))     # differences only inside the 1e-5 band
+        if got == want:
+            err = float(np.abs(out["scores"][sel].astype(np.float64) - ora["scores"]).max())
+            worst = max(worst, err)
+            assert err <= TOL[cfg.precision], (name, e, err)
+    print(f"{name}: N={len(batch['r'])} E={out['E']} worst sampled |score - oracle| = {worst:.3g}")
