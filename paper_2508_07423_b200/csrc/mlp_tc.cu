@@ -265,20 +265,38 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
     long long g_wait = 0;
     const long long g_start = a.dbg ? clock64() : 0;
 
-    // loads chunk number `ci` (counted over this CTA's tiles) into registers
+    // Row indices of this thread's NPASS rows for the (at most two) index-gathered segments, reloaded
+    // when the chunk stream enters a new tile (loads are issued strictly in chunk order, so one
+    // register set is enough).  This takes the dependent idx -> address -> data load chain off every
+    // chunk but the first of a tile.
+    int ridx[2][NPASS];
     auto load_chunk = [&](int ci, float4 (&dst)[NPASS]) {
       const int tile = blockIdx.x + (ci / nc1) * gridDim.x;
-      const int k0 = (ci % nc1) * KA;
-      int s = 0, start = 0;
-      while (s < a.n_seg - 1 && k0 >= start + a.seg[s].width) { start += a.seg[s].width; ++s; }
-      const Segment sg = a.seg[s];
-      const int koff = k0 - start + jl * 4;
+      const int c = ci % nc1;
+      if (c == 0) {
+#pragma unroll
+        for (int sgi = 0; sgi < 2; ++sgi) {
+          const int32_t* __restrict__ ip = sgi < a.n_seg ? a.seg[sgi].idx : nullptr;
+          if (ip) {
+#pragma unroll
+            for (int p = 0; p < NPASS; ++p) {
+              const int row = tile * TM + r0 + p * RPP;
+              ridx[sgi][p] = __ldg(ip + (row < a.n_rows ? row : a.n_rows - 1));
+            }
+          }
+        }
+      }
+      const int k0 = c * KA;
+      int sg = 0, start = 0;
+      while (sg < a.n_seg - 1 && k0 >= start + a.seg[sg].width) { start += a.seg[sg].width; ++sg; }
+      const float* __restrict__ base = a.seg[sg].base + (k0 - start + jl * 4);
+      const size_t ld = (size_t)a.seg[sg].ld;
+      const bool indexed = sg < 2 && a.seg[sg].idx != nullptr;     // only the first two segments may carry indices
 #pragma unroll
       for (int p = 0; p < NPASS; ++p) {
         const int row = tile * TM + r0 + p * RPP;
-        const int grow = row < a.n_rows ? row : a.n_rows - 1;
-        const int idx = sg.idx ? __ldg(sg.idx + grow) : grow;
-        dst[p] = __ldg(reinterpret_cast<const float4*>(sg.base + (size_t)idx * sg.ld + koff));
+        const int idx = indexed ? (sg == 0 ? ridx[0][p] : ridx[1][p]) : (row < a.n_rows ? row : a.n_rows - 1);
+        dst[p] = __ldg(reinterpret_cast<const float4*>(base + (size_t)idx * ld));
       }
     };
 
