@@ -351,10 +351,14 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   } else if (warp < 12) {
     // =========================== epilogue warps ===========================
     const int et = threadIdx.x - kGatherThreads; // 0..127 = tile row = TMEM lane
+    (void)et;
     const int q4 = warp & 3;                     // TMEM lane quarter this warp may access
     const uint32_t lane_addr = tmem + ((uint32_t)(q4 * 32) << 16);
     uint32_t g = 0, hcount = 0;
-    long long e_wait = 0;
+    long long e_wait = 0, ep[6] = {0, 0, 0, 0, 0, 0}, tp = 0;
+    const bool edbg = a.dbg != nullptr;
+#define EP_T0() if (edbg) tp = clock64()
+#define EP_ACC(i) if (edbg) { const long long tn = clock64(); ep[i] += tn - tp; tp = tn; }
     const long long e_start = a.dbg ? clock64() : 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
       for (int l = 0; l < n_gemm; ++l, ++g) {
@@ -369,10 +373,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
           // ---- hidden layer: ReLU(x + b) -> next A operand in TMEM, released chunk by chunk
 #pragma unroll 1
           for (int c = 0; c < HCH; ++c) {
+            EP_T0();
             if constexpr (MODE == ETX_PREC_TF32X3) {
               uint32_t v[32], w[32];
               tmem_ld32(acc + c * 32, v);
               tc_wait_ld();
+              EP_ACC(0);
 #pragma unroll
               for (int i = 0; i < 32; ++i) {
                 const float x = fmaxf(__uint_as_float(v[i]) + bias[c * 32 + i], 0.f);
@@ -386,6 +392,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
               tmem_ld32(acc + c * 64, v0);
               tmem_ld32(acc + c * 64 + 32, v1);
               tc_wait_ld();
+              EP_ACC(0);
 #pragma unroll
               for (int i = 0; i < 16; ++i) {
                 split_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 2 * i], 0.f),
@@ -400,6 +407,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
               tmem_ld32(acc + c * 64, v0);
               tmem_ld32(acc + c * 64 + 32, v1);
               tc_wait_ld();
+              EP_ACC(0);
 #pragma unroll
               for (int i = 0; i < 16; ++i) {
                 w[i] = pack_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 2 * i], 0.f),
@@ -409,9 +417,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
               }
               tmem_st32(lane_addr + COL_HID + c * 32, w);
             }
+            EP_ACC(1);
             tc_wait_st();
             tc_fence_before();
             mbar_arrive_warp(smem_u32(&bars->hid_ready[c]), lane);
+            EP_ACC(2);
           }
           mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane);
           ++hcount;
@@ -433,48 +443,46 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
           const int row = tile * TM + et;
           if (row < a.n_rows) a.out[row] = 1.0f / (1.0f + expf(-logit));
         } else {
-          // ---- linear output (+ residual): transpose through the swizzled staging tile, coalesced I/O.
-          // The residual rows are prefetched one column group ahead (they come from HBM).
-          const int jl = et & 7, rr = et >> 3;
-          const bool has_res = (a.out_mode == 1);
-          float4 rbuf[2][8];
-          auto load_res = [&](int q, float4 (&dst)[8]) {
-#pragma unroll
-            for (int p = 0; p < 8; ++p) {
-              const int row = tile * TM + rr + p * 16;
-              const int grow = row < a.n_rows ? row : a.n_rows - 1;
-              dst[p] = has_res ? __ldg(reinterpret_cast<const float4*>(a.res + (size_t)grow * a.out_ld + q * 32 + jl * 4))
-                               : make_float4(0.f, 0.f, 0.f, 0.f);
-            }
-          };
-          load_res(0, rbuf[0]);
-#pragma unroll
+          // ---- linear output (+ residual).  Each warp transposes its own 32 rows through a private 4 KB
+          // swizzled staging slice (thread = row on the TMEM side, 8 lanes per row on the global side),
+          // so only __syncwarp is needed.  The residual e += y is applied by a vector
+          // red.global.add on the in-place state: one IEEE fp32 add per element, performed at L2, no
+          // residual load, deterministic (each element is touched exactly once).
+          const uint32_t stg = stage_out + q4 * 4096;
+          const int jl = lane & 7, r8 = lane >> 3;
+          const bool in_place_add = (a.out_mode == 1);
+#pragma unroll 1
           for (int q = 0; q < HW / 32; ++q) {
-            if (q + 1 < HW / 32) load_res(q + 1, rbuf[(q + 1) & 1]);
+            EP_T0();
             uint32_t v[32];
             tmem_ld32(acc + q * 32, v);
             tc_wait_ld();
+            EP_ACC(3);
             if (q == HW / 32 - 1) { tc_fence_before(); mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane); }
-            epi_bar_sync();                      // previous round's readers are done with the staging tile
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
               const float4 bq = *reinterpret_cast<const float4*>(bias + q * 32 + 4 * j);
-              st_shared_v4(stage_out + et * 128 + ((j ^ (et & 7)) << 4),
+              st_shared_v4(stg + lane * 128 + ((j ^ (lane & 7)) << 4),
                            __float_as_uint(__uint_as_float(v[4 * j]) + bq.x), __float_as_uint(__uint_as_float(v[4 * j + 1]) + bq.y),
                            __float_as_uint(__uint_as_float(v[4 * j + 2]) + bq.z), __float_as_uint(__uint_as_float(v[4 * j + 3]) + bq.w));
             }
-            epi_bar_sync();
+            __syncwarp();
+            EP_ACC(4);
 #pragma unroll
-            for (int p = 0; p < 8; ++p) {
-              const int r = rr + p * 16;
-              const int row = tile * TM + r;
+            for (int it = 0; it < 8; ++it) {
+              const int r = r8 + 4 * it;
+              const int row = tile * TM + q4 * 32 + r;
               if (row < a.n_rows) {
-                float4 y = ld_shared_v4(stage_out + r * 128 + ((jl ^ (r & 7)) << 4));
-                const float4 o = rbuf[q & 1][p];
-                y.x += o.x; y.y += o.y; y.z += o.z; y.w += o.w;
-                *reinterpret_cast<float4*>(a.out + (size_t)row * a.out_ld + q * 32 + jl * 4) = y;
+                const float4 y = ld_shared_v4(stg + r * 128 + ((jl ^ (r & 7)) << 4));
+                float* dst = a.out + (size_t)row * a.out_ld + q * 32 + jl * 4;
+                if (in_place_add)
+                  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(y.x), "f"(y.y), "f"(y.z), "f"(y.w) : "memory");
+                else
+                  *reinterpret_cast<float4*>(dst) = y;
               }
             }
+            __syncwarp();
+            EP_ACC(5);
           }
         }
       }
@@ -483,6 +491,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
     if (a.dbg && et == 0) {
       a.dbg[(size_t)blockIdx.x * 16 + 6] = (unsigned long long)e_wait;
       a.dbg[(size_t)blockIdx.x * 16 + 7] = (unsigned long long)(clock64() - e_start);
+      for (int i = 0; i < 6; ++i) a.dbg[(size_t)blockIdx.x * 16 + 10 + i] = (unsigned long long)ep[i];
     }
   } else if (warp == 12) {
     // =========================== weight loader ===========================
