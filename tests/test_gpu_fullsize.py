@@ -11,7 +11,7 @@ from paper_2508_07423_b200 import synth
 
 pytestmark = pytest.mark.gpu
 
-TOL = {synth.PREC_FP32: 1e-4, synth.PREC_TF32X3: 1e-4, synth.PREC_BF16: 2e-2}
+TOL = {synth.PREC_FP32: 1e-4, synth.PREC_TF32X3: 1e-4, synth.PREC_BF16: 2e-2, synth.PREC_BF16X3: 1e-4}
 
 
 @pytest.fixture(scope="module")
@@ -23,8 +23,8 @@ def B():
     return binding
 
 
-def run_full(B, cfg, batch, blob):
-    etx = B.Etx(B.make_desc(cfg), blob)                       # the config's bench precision
+def run_full(B, cfg, batch, blob, precision=None):
+    etx = B.Etx(B.make_desc(cfg, precision=precision), blob)  # default: the config's bench precision
     dev = etx.device
     db = B.DeviceBatch(batch, dev)
     N = db.n_hits
@@ -71,12 +71,18 @@ def check_properties(cfg, batch, out):
     return ev
 
 
-@pytest.mark.parametrize("name,sample", [("c2", [0, 137, 500, 999]), ("c3", [1, 998]), ("c4", [0, 999])])
-def test_full_batch_sampled_events(B, name, sample):
+@pytest.mark.parametrize("name,sample,precision", [
+    ("c2", [0, 137, 500, 999], None), ("c3", [1, 998], None), ("c4", [0, 999], None),
+    ("c2", [0, 137, 500, 999], synth.PREC_TF32X3), ("c2", [0, 137, 500, 999], synth.PREC_BF16X3),
+    ("c2", [0, 999], synth.PREC_FP32), ("c4", [0, 999], synth.PREC_BF16X3)])
+def test_full_batch_sampled_events(B, name, sample, precision):
     cfg = synth.CONFIGS[name]
+    if precision is not None:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, precision=precision)
     batch = synth.generate_events(cfg)
     blob = synth.generate_weights(cfg)
-    out = run_full(B, cfg, batch, blob)
+    out = run_full(B, cfg, batch, blob, precision)
     ev = check_properties(cfg, batch, out)
     assert abs(out["E"] / len(batch["r"]) - cfg.target_degree) < 0.08 * cfg.target_degree
     ep = batch["event_ptr"].astype(np.int64)
@@ -95,4 +101,4 @@ def test_full_batch_sampled_events(B, name, sample):
             err = float(np.abs(out["scores"][sel].astype(np.float64) - ora["scores"]).max())
             worst = max(worst, err)
             assert err <= TOL[cfg.precision], (name, e, err)
-    print(f"{name}: N={len(batch['r'])} E={out['E']} worst sampled |score - oracle| = {worst:.3g}")
+    print(f"{name} precision={cfg.precision}: N={len(batch['r'])} E={out['E']} worst sampled |score - oracle| = {worst:.3g}")
