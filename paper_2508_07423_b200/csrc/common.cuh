@@ -106,6 +106,7 @@ struct TcArgs {
   const float* w_last = nullptr;                  // classifier: fp32 weights of the 1-unit output layer
   int out_mode = 0; float* out = nullptr; const float* res = nullptr; int out_ld = 0;
   unsigned long long* dbg = nullptr;              // optional [grid][16] cycle counters (ETX_TC_DEBUG)
+  int exp_flags = 0;                              // timing experiments only (ETX_TC_EXP): 1 skip gather stores, 2 skip weight copies
 };
 int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s);
 int tc_chunk_k(int mode);

@@ -199,24 +199,26 @@ int run_mlp(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   for (int l = 0; l < a.mlp.n_layers; ++l) t.bias[l] = a.mlp.b[l];
   t.w_last = a.mlp.Wt[a.mlp.n_layers - 1];         // [H][1] == [H]
   t.out_mode = a.out_mode; t.out = a.out; t.res = a.res; t.out_ld = a.out_ld;
+  static const char* expv = getenv("ETX_TC_EXP");                  // developer aid: timing experiments (wrong results)
+  t.exp_flags = expv ? atoi(expv) : 0;
   static const bool debug = getenv("ETX_TC_DEBUG") != nullptr;     // developer aid: per-role cycle counters
   if (!debug) return launch_mlp_tc(t, c->desc.precision, c->sm_count, s);
   static unsigned long long* d_dbg = nullptr;
-  if (!d_dbg) cudaMalloc(&d_dbg, sizeof(unsigned long long) * 16 * 256);
-  cudaMemsetAsync(d_dbg, 0, sizeof(unsigned long long) * 16 * 256, s);
+  if (!d_dbg) cudaMalloc(&d_dbg, sizeof(unsigned long long) * 32 * 256);
+  cudaMemsetAsync(d_dbg, 0, sizeof(unsigned long long) * 32 * 256, s);
   t.dbg = d_dbg;
   const int n = launch_mlp_tc(t, c->desc.precision, c->sm_count, s);
-  std::vector<unsigned long long> h(16 * 256);
+  std::vector<unsigned long long> h(32 * 256);
   cudaStreamSynchronize(s);
   cudaMemcpy(h.data(), d_dbg, h.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
   const int grid = std::min((a.n_rows + 127) / 128, c->sm_count);
-  double avg[16] = {0};
-  for (int b = 0; b < grid; ++b) for (int i = 0; i < 16; ++i) avg[i] += (double)h[b * 16 + i] / grid;
+  double avg[32] = {0};
+  for (int b = 0; b < grid; ++b) for (int i = 0; i < 32; ++i) avg[i] += (double)h[b * 32 + i] / grid;
   const double tiles = (double)((a.n_rows + 127) / 128) / grid;
   fprintf(stderr, "[tc dbg] rows=%d K0=%d tiles/cta=%.1f | per tile cycles: mma total %.0f = wait acc_free %.0f + a_full %.0f + "
-          "hid_ready %.0f + w_full %.0f + issue %.0f | epi: wait acc_full %.0f of %.0f [hid ld %.0f math %.0f st+arrive %.0f | fin ld %.0f bar+sts %.0f io %.0f] | gather: wait a_empty %.0f of %.0f\n",
+          "hid_ready %.0f + w_full %.0f + issue %.0f | epi: wait acc_full %.0f of %.0f [hid ld %.0f math %.0f st+arrive %.0f | fin ld %.0f bar+sts %.0f io %.0f] | gather: wait a_empty %.0f of %.0f [data wait %.0f cvt+sts %.0f fence+arrive %.0f issue loads %.0f]\n",
           a.n_rows, a.mlp.dims[0], tiles, avg[5] / tiles, avg[0] / tiles, avg[1] / tiles, avg[2] / tiles, avg[3] / tiles, avg[4] / tiles,
-          avg[6] / tiles, avg[7] / tiles, avg[10] / tiles, avg[11] / tiles, avg[12] / tiles, avg[13] / tiles, avg[14] / tiles, avg[15] / tiles, avg[8] / tiles, avg[9] / tiles);
+          avg[6] / tiles, avg[7] / tiles, avg[10] / tiles, avg[11] / tiles, avg[12] / tiles, avg[13] / tiles, avg[14] / tiles, avg[15] / tiles, avg[8] / tiles, avg[9] / tiles, avg[16] / tiles, avg[17] / tiles, avg[18] / tiles, avg[19] / tiles);
   return n;
 }
 

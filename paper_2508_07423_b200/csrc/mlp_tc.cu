@@ -262,47 +262,59 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
     const int r0 = t / LPR;                      // first of its rows; then r0 + RPP, r0 + 2 RPP, ...
     const int total_chunks = ((n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x) * nc1;
     float4 buf[D][NPASS];
-    long long g_wait = 0;
+    long long g_wait = 0, gp[4] = {0, 0, 0, 0}, tq = 0;
+    const bool gdbg = a.dbg != nullptr;
+#define GP_T0() if (gdbg) tq = clock64()
+#define GP_ACC(i) if (gdbg) { const long long tn = clock64(); gp[i] += tn - tq; tq = tn; }
     const long long g_start = a.dbg ? clock64() : 0;
 
-    // Row indices of this thread's NPASS rows for the (at most two) index-gathered segments, reloaded
-    // when the chunk stream enters a new tile (loads are issued strictly in chunk order, so one
-    // register set is enough).  This takes the dependent idx -> address -> data load chain off every
-    // chunk but the first of a tile.
-    int ridx[2][NPASS];
-    auto load_chunk = [&](int ci, float4 (&dst)[NPASS]) {
-      const int tile = blockIdx.x + (ci / nc1) * gridDim.x;
-      const int c = ci % nc1;
-      if (c == 0) {
+    // Producer cursor (tile, chunk, segment, k offset) advanced incrementally: no division, no dynamic
+    // indexing of kernel parameters, no segment search in the per-chunk path (these warps have almost
+    // no ILP, so every scalar instruction costs its full latency).  Row indices of this thread's NPASS
+    // rows for the (at most two) index-gathered segments are reloaded when the cursor enters a tile.
+    const char* sbase[3]; uint32_t sld[3]; int swidth[3]; const int32_t* sidx[2];
 #pragma unroll
-        for (int sgi = 0; sgi < 2; ++sgi) {
-          const int32_t* __restrict__ ip = sgi < a.n_seg ? a.seg[sgi].idx : nullptr;
-          if (ip) {
+    for (int i = 0; i < 3; ++i) {
+      sbase[i] = reinterpret_cast<const char*>(i < a.n_seg ? a.seg[i].base : nullptr) + jl * 16;
+      sld[i] = i < a.n_seg ? (uint32_t)a.seg[i].ld * 4u : 0u;
+      swidth[i] = i < a.n_seg ? a.seg[i].width : 0;
+    }
+    sidx[0] = a.n_seg > 0 ? a.seg[0].idx : nullptr;
+    sidx[1] = a.n_seg > 1 ? a.seg[1].idx : nullptr;
+    int ptile = blockIdx.x, pc = 0, pseg = 0, pk = 0;
+    int ridx[2][NPASS], rown[NPASS];
+    auto load_chunk = [&](float4 (&dst)[NPASS]) {
+      if (pc == 0) {
 #pragma unroll
-            for (int p = 0; p < NPASS; ++p) {
-              const int row = tile * TM + r0 + p * RPP;
-              ridx[sgi][p] = __ldg(ip + (row < a.n_rows ? row : a.n_rows - 1));
-            }
-          }
+        for (int p = 0; p < NPASS; ++p) {
+          const int row = ptile * TM + r0 + p * RPP;
+          rown[p] = row < a.n_rows ? row : a.n_rows - 1;
         }
+#pragma unroll
+        for (int sgi = 0; sgi < 2; ++sgi)
+          if (sidx[sgi]) {
+#pragma unroll
+            for (int p = 0; p < NPASS; ++p) ridx[sgi][p] = __ldg(sidx[sgi] + rown[p]);
+          }
       }
-      const int k0 = c * KA;
-      int sg = 0, start = 0;
-      while (sg < a.n_seg - 1 && k0 >= start + a.seg[sg].width) { start += a.seg[sg].width; ++sg; }
-      const float* __restrict__ base = a.seg[sg].base + (k0 - start + jl * 4);
-      const size_t ld = (size_t)a.seg[sg].ld;
-      const bool indexed = sg < 2 && a.seg[sg].idx != nullptr;     // only the first two segments may carry indices
+      const char* base = (pseg == 0 ? sbase[0] : (pseg == 1 ? sbase[1] : sbase[2])) + pk * 4;
+      const uint32_t ldb = pseg == 0 ? sld[0] : (pseg == 1 ? sld[1] : sld[2]);
+      const bool ix0 = pseg == 0 && sidx[0] != nullptr, ix1 = pseg == 1 && sidx[1] != nullptr;
 #pragma unroll
       for (int p = 0; p < NPASS; ++p) {
-        const int row = tile * TM + r0 + p * RPP;
-        const int idx = indexed ? (sg == 0 ? ridx[0][p] : ridx[1][p]) : (row < a.n_rows ? row : a.n_rows - 1);
-        dst[p] = __ldg(reinterpret_cast<const float4*>(base + (size_t)idx * ld));
+        const uint32_t idx = (uint32_t)(ix0 ? ridx[0][p] : (ix1 ? ridx[1][p] : rown[p]));
+        dst[p] = __ldg(reinterpret_cast<const float4*>(base + (size_t)idx * ldb));
       }
+      // advance the cursor
+      pk += KA;
+      const int w = pseg == 0 ? swidth[0] : (pseg == 1 ? swidth[1] : swidth[2]);
+      if (pk >= w) { pk = 0; ++pseg; }
+      if (++pc == nc1) { pc = 0; pseg = 0; pk = 0; ptile += gridDim.x; }
     };
 
 #pragma unroll
     for (int d = 0; d < D; ++d)
-      if (d < total_chunks) load_chunk(d, buf[d]);
+      if (d < total_chunks) load_chunk(buf[d]);
     for (int ci0 = 0; ci0 < total_chunks; ci0 += D) {
 #pragma unroll
       for (int d = 0; d < D; ++d) {
@@ -312,6 +324,14 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
           long long tg0 = a.dbg ? clock64() : 0;
           mbar_wait_warp(smem_u32(&bars->a_empty[slot]), (n & 1) ^ 1, lane);
           if (a.dbg) g_wait += clock64() - tg0;
+          GP_T0();
+          {   // timing aid: force the prefetched registers of this chunk to be resident before the store phase
+            float sdep = 0.f;
+#pragma unroll
+            for (int p = 0; p < NPASS; ++p) sdep += buf[d][p].x;
+            if (gdbg && sdep == 1.2345e30f) g_wait += 1;
+          }
+          GP_ACC(0);
           const uint32_t tile_hi = aring + slot * kStageBytes;
 #pragma unroll
           for (int p = 0; p < NPASS; ++p) {
@@ -338,15 +358,19 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
               }
             }
           }
+          GP_ACC(1);
           fence_async_smem();                    // generic-proxy writes -> visible to the tensor core (async proxy)
           mbar_arrive_warp(smem_u32(&bars->a_full[slot]), lane);
-          if (ci + D < total_chunks) load_chunk(ci + D, buf[d]);
+          GP_ACC(2);
+          if (ci + D < total_chunks) load_chunk(buf[d]);
+          GP_ACC(3);
         }
       }
     }
     if (a.dbg && t == 0) {
-      a.dbg[(size_t)blockIdx.x * 16 + 8] = (unsigned long long)g_wait;
-      a.dbg[(size_t)blockIdx.x * 16 + 9] = (unsigned long long)(clock64() - g_start);
+      a.dbg[(size_t)blockIdx.x * 32 + 8] = (unsigned long long)g_wait;
+      a.dbg[(size_t)blockIdx.x * 32 + 9] = (unsigned long long)(clock64() - g_start);
+      for (int i = 0; i < 4; ++i) a.dbg[(size_t)blockIdx.x * 32 + 16 + i] = (unsigned long long)gp[i];
     }
   } else if (warp < 12) {
     // =========================== epilogue warps ===========================
@@ -489,9 +513,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
     }
     (void)hcount;
     if (a.dbg && et == 0) {
-      a.dbg[(size_t)blockIdx.x * 16 + 6] = (unsigned long long)e_wait;
-      a.dbg[(size_t)blockIdx.x * 16 + 7] = (unsigned long long)(clock64() - e_start);
-      for (int i = 0; i < 6; ++i) a.dbg[(size_t)blockIdx.x * 16 + 10 + i] = (unsigned long long)ep[i];
+      a.dbg[(size_t)blockIdx.x * 32 + 6] = (unsigned long long)e_wait;
+      a.dbg[(size_t)blockIdx.x * 32 + 7] = (unsigned long long)(clock64() - e_start);
+      for (int i = 0; i < 6; ++i) a.dbg[(size_t)blockIdx.x * 32 + 10 + i] = (unsigned long long)ep[i];
     }
   } else if (warp == 12) {
     // =========================== weight loader ===========================
@@ -585,7 +609,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
       }
     }
     if (dbg && lane == 0) {
-      unsigned long long* o = a.dbg + (size_t)blockIdx.x * 16;
+      unsigned long long* o = a.dbg + (size_t)blockIdx.x * 32;
       for (int i = 0; i < 5; ++i) o[i] = (unsigned long long)dt[i];
       o[5] = (unsigned long long)(clock64() - t_start);
     }
