@@ -2,22 +2,23 @@
 //
 // Computes, for a tile of 128 rows (edges or hits), the whole chain of Eq. 4.27 layers of one
 // GNN MLP — edge encoder, node/edge network or classifier — without any
-// intermediate leaving the SM.  One persistent CTA per SM, fourteen warps:
+// intermediate leaving the SM.  One persistent CTA per SM, 28 warps in 7 warpgroups (register budgets
+// re-partitioned with setmaxnreg: gather 64, epilogue 104, loader/MMA 40):
 //
-//   warps 0-7  gather:   coalesced 16-byte loads of the first layer's input rows ([h_src | h_dst | e],
+//   warps 0-15 gather:   coalesced 16-byte loads of the first layer's input rows ([h_src | h_dst | e],
 //                        [h | m], ...) straight from the node / edge arrays (8 or 16 lanes per row, a
 //                        ring of K-chunks prefetched in registers: 64 KB in flight per SM), conversion
 //                        to the MMA operand type and st.shared into a ring of canonical K-major
 //                        SWIZZLE_128B operand tiles.
-//   warps 8-11 epilogue: thread r owns tile row r = TMEM lane r.  After a hidden layer: tcgen05.ld the
+//   warps 16-23 epilogue (lane quarter = warp & 3, column half = (warp-16) >> 2): thread r owns tile row r = TMEM lane r.  After a hidden layer: tcgen05.ld the
 //                        accumulator 32 columns at a time, bias + ReLU, convert, tcgen05.st the next
 //                        layer's A operand back into TMEM and release that K-chunk to the MMA warp at
 //                        once, so the next layer's MMAs start while the rest of the epilogue runs.
 //                        After the last layer: bias (+ residual) through a swizzled staging tile so
 //                        the global read-modify-write is coalesced, or the 1-unit head + sigmoid.
-//   warp 12    loader:   streams pre-swizzled weight tiles (prepared once at etx_create) from L2 into a
+//   warp 24    loader:   streams pre-swizzled weight tiles (prepared once at etx_create) from L2 into a
 //                        shared-memory ring with cp.async.bulk (TMA bulk copy) completing on mbarriers.
-//   warp 13    MMA:      one thread issues tcgen05.mma — SS form (A, B in shared memory) for the first
+//   warp 25    MMA:      one thread issues tcgen05.mma — SS form (A, B in shared memory) for the first
 //                        layer, TS form (A in TMEM) for the others — into one of two 128-column TMEM
 //                        accumulators (ping-pong), and tcgen05.commit-s ring slots / accumulators.
 //
@@ -36,12 +37,26 @@
 //                    are dominated by the tensor core's truncating fp32 accumulation.
 #include "common.cuh"
 
+// Per-role cycle counters (developer aid).  Compiled in only with -DETX_TC_COUNTERS (build.py:
+// ETX_TC_COUNTERS=1), because their 64-bit registers do not fit the 64-register gather budget.
+#ifdef ETX_TC_COUNTERS
+#define ETX_DBG(a) ((a).dbg != nullptr)
+#else
+#define ETX_DBG(a) false
+#endif
+
 namespace etx {
 namespace {
 
 constexpr int TM = 128;
-constexpr int kGatherThreads = 256;      // warps 0-7
-constexpr int kThreads = kGatherThreads + 128 + 64;   // + epilogue warps 8-11, loader warp 12, MMA warp 13
+constexpr int kGatherThreads = 512;      // warpgroups 0-3 (warps 0-15)
+constexpr int kEpiThreads = 256;         // warpgroups 4-5 (warps 16-23): lane quarter = warp & 3, column half = (warp - 16) >> 2
+constexpr int kThreads = kGatherThreads + kEpiThreads + 128;   // + warpgroup 6: loader warp 24, MMA warp 25, two idle warps
+constexpr int kWarpEpi0 = kGatherThreads / 32, kWarpLoader = kWarpEpi0 + kEpiThreads / 32, kWarpMma = kWarpLoader + 1;
+// Register re-partitioning (setmaxnreg, per warpgroup): the kernel launches at <= 72 registers per
+// thread (896 threads), then the gather warpgroups shrink to 64, loader/MMA to 40, and the epilogue
+// warpgroups grow to 104.  More, thinner warps: the SIMT roles are latency-bound, not issue-bound.
+constexpr int kRegGather = 64, kRegEpi = 104, kRegCtl = 40;
 constexpr int HW = 128;                       // hidden width handled by this kernel
 constexpr int kAtomBytes = 128 * 128;         // one operand tile: 128 rows x 128 bytes (one swizzle atom wide)
 
@@ -109,6 +124,8 @@ __device__ __forceinline__ void tc_wait_st() { asm volatile("tcgen05.wait::st.sy
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ bool elect_one() {      // one lane of a fully-active warp
   uint32_t pred;
   asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.b32 %0, 1, 0, P;\n\t}" : "=r"(pred));
@@ -242,11 +259,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   if (threadIdx.x == 0) {
     for (int i = 0; i < NSW; ++i) { mbar_init(smem_u32(&bars->w_full[i]), 1); mbar_init(smem_u32(&bars->w_empty[i]), 1); }
     for (int i = 0; i < NSA; ++i) { mbar_init(smem_u32(&bars->a_full[i]), kGatherThreads / 32); mbar_init(smem_u32(&bars->a_empty[i]), 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&bars->acc_full[i]), 1); mbar_init(smem_u32(&bars->acc_free[i]), 4); }
+    for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&bars->acc_full[i]), 1); mbar_init(smem_u32(&bars->acc_free[i]), kEpiThreads / 32); }
     for (int i = 0; i < 4; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), 4);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 13) {                              // TMEM: all 512 columns of this SM (1 CTA per SM)
+  if (warp == kWarpMma) {                        // TMEM: all 512 columns of this SM (1 CTA per SM)
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&bars->tmem_base)) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
@@ -255,18 +272,19 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
 
-  if (warp < 8) {
+  if (warp < kWarpEpi0) {
     // =========================== gather warps ===========================
-    const int t = threadIdx.x;                   // 0..255
+    reg_dec<kRegGather>();
+    const int t = threadIdx.x;                   // 0..511
     const int jl = t % LPR;                      // 16-byte piece of the chunk row this thread moves
     const int r0 = t / LPR;                      // first of its rows; then r0 + RPP, r0 + 2 RPP, ...
     const int total_chunks = ((n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x) * nc1;
     float4 buf[D][NPASS];
     long long g_wait = 0, gp[4] = {0, 0, 0, 0}, tq = 0;
-    const bool gdbg = a.dbg != nullptr;
+    const bool gdbg = ETX_DBG(a);
 #define GP_T0() if (gdbg) tq = clock64()
 #define GP_ACC(i) if (gdbg) { const long long tn = clock64(); gp[i] += tn - tq; tq = tn; }
-    const long long g_start = a.dbg ? clock64() : 0;
+    const long long g_start = gdbg ? clock64() : 0;
 
     // Producer cursor (tile, chunk, segment, k offset) advanced incrementally: no division, no dynamic
     // indexing of kernel parameters, no segment search in the per-chunk path (these warps have almost
@@ -289,12 +307,13 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
         for (int p = 0; p < NPASS; ++p) {
           const int row = ptile * TM + r0 + p * RPP;
           rown[p] = row < a.n_rows ? row : a.n_rows - 1;
+          if (a.exp_flags & 4) rown[p] = r0 + p * RPP;      // timing experiment: every tile reads the same rows
         }
 #pragma unroll
         for (int sgi = 0; sgi < 2; ++sgi)
           if (sidx[sgi]) {
 #pragma unroll
-            for (int p = 0; p < NPASS; ++p) ridx[sgi][p] = __ldg(sidx[sgi] + rown[p]);
+            for (int p = 0; p < NPASS; ++p) ridx[sgi][p] = (a.exp_flags & 4) ? rown[p] : __ldg(sidx[sgi] + rown[p]);
           }
       }
       const char* base = (pseg == 0 ? sbase[0] : (pseg == 1 ? sbase[1] : sbase[2])) + pk * 4;
@@ -321,9 +340,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
         const int ci = ci0 + d;
         if (ci < total_chunks) {
           const uint32_t slot = ci % NSA, n = ci / NSA;
-          long long tg0 = a.dbg ? clock64() : 0;
+          long long tg0 = gdbg ? clock64() : 0;
           mbar_wait_warp(smem_u32(&bars->a_empty[slot]), (n & 1) ^ 1, lane);
-          if (a.dbg) g_wait += clock64() - tg0;
+          if (gdbg) g_wait += clock64() - tg0;
           GP_T0();
           {   // timing aid: force the prefetched registers of this chunk to be resident before the store phase
             float sdep = 0.f;
@@ -367,36 +386,39 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
         }
       }
     }
-    if (a.dbg && t == 0) {
+    if (gdbg && t == 0) {
       a.dbg[(size_t)blockIdx.x * 32 + 8] = (unsigned long long)g_wait;
       a.dbg[(size_t)blockIdx.x * 32 + 9] = (unsigned long long)(clock64() - g_start);
       for (int i = 0; i < 4; ++i) a.dbg[(size_t)blockIdx.x * 32 + 16 + i] = (unsigned long long)gp[i];
     }
-  } else if (warp < 12) {
+  } else if (warp < kWarpLoader) {
     // =========================== epilogue warps ===========================
-    const int et = threadIdx.x - kGatherThreads; // 0..127 = tile row = TMEM lane
-    (void)et;
-    const int q4 = warp & 3;                     // TMEM lane quarter this warp may access
+    reg_inc<kRegEpi>();
+    const int ew = warp - kWarpEpi0;             // 0..7
+    const int q4 = ew & 3;                       // TMEM lane quarter this warp may access (= warp & 3)
+    const int hh = ew >> 2;                      // column half this warp owns
+    const int et = q4 * 32 + lane;               // tile row = TMEM lane
     const uint32_t lane_addr = tmem + ((uint32_t)(q4 * 32) << 16);
-    uint32_t g = 0, hcount = 0;
+    uint32_t g = 0;
     long long e_wait = 0, ep[6] = {0, 0, 0, 0, 0, 0}, tp = 0;
-    const bool edbg = a.dbg != nullptr;
+    const bool edbg = ETX_DBG(a);
 #define EP_T0() if (edbg) tp = clock64()
 #define EP_ACC(i) if (edbg) { const long long tn = clock64(); ep[i] += tn - tp; tp = tn; }
-    const long long e_start = a.dbg ? clock64() : 0;
+    const long long e_start = edbg ? clock64() : 0;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
       for (int l = 0; l < n_gemm; ++l, ++g) {
         const uint32_t b = g & 1;
         const float* bias = bias_s + l * HW;
-        long long te0 = a.dbg ? clock64() : 0;
+        long long te0 = edbg ? clock64() : 0;
         mbar_wait_warp(smem_u32(&bars->acc_full[b]), (g >> 1) & 1, lane);
-        if (a.dbg) e_wait += clock64() - te0;
+        if (edbg) e_wait += clock64() - te0;
         tc_fence_after();
         const uint32_t acc = lane_addr + COL_ACC + b * 128;
         if (l < n_gemm - 1) {
-          // ---- hidden layer: ReLU(x + b) -> next A operand in TMEM, released chunk by chunk
+          // ---- hidden layer: ReLU(x + b) -> next A operand in TMEM, released chunk by chunk.
+          // This warp's column half holds K-chunks hh*HCH/2 .. of the next layer.
 #pragma unroll 1
-          for (int c = 0; c < HCH; ++c) {
+          for (int c = hh * (HCH / 2); c < (hh + 1) * (HCH / 2); ++c) {
             EP_T0();
             if constexpr (MODE == ETX_PREC_TF32X3) {
               uint32_t v[32], w[32];
@@ -412,33 +434,37 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
               tmem_st32(lane_addr + COL_HID + c * 32, w);
               tmem_st32(lane_addr + COL_HID + HID_COLS + c * 32, v);
             } else if constexpr (P == 2) {       // BF16X3: 64 accumulator columns -> 32 hi + 32 lo packed columns
-              uint32_t v0[32], v1[32], wh[32], wl[32];
+              uint32_t v0[32], wh[32], wl[32];
               tmem_ld32(acc + c * 64, v0);
-              tmem_ld32(acc + c * 64 + 32, v1);
+              tc_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 16; ++i)
+                split_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 2 * i], 0.f),
+                             fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 2 * i + 1], 0.f), wh[i], wl[i]);
+              tmem_ld32(acc + c * 64 + 32, v0);
               tc_wait_ld();
               EP_ACC(0);
 #pragma unroll
-              for (int i = 0; i < 16; ++i) {
-                split_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 2 * i], 0.f),
-                             fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 2 * i + 1], 0.f), wh[i], wl[i]);
-                split_bf16x2(fmaxf(__uint_as_float(v1[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
-                             fmaxf(__uint_as_float(v1[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f), wh[16 + i], wl[16 + i]);
-              }
+              for (int i = 0; i < 16; ++i)
+                split_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
+                             fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f), wh[16 + i], wl[16 + i]);
               tmem_st32(lane_addr + COL_HID + c * 32, wh);
               tmem_st32(lane_addr + COL_HID + HID_COLS + c * 32, wl);
             } else {
-              uint32_t v0[32], v1[32], w[32];
+              uint32_t v0[32], w[32];
               tmem_ld32(acc + c * 64, v0);
-              tmem_ld32(acc + c * 64 + 32, v1);
+              tc_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 16; ++i)
+                w[i] = pack_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 2 * i], 0.f),
+                                   fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 2 * i + 1], 0.f));
+              tmem_ld32(acc + c * 64 + 32, v0);
               tc_wait_ld();
               EP_ACC(0);
 #pragma unroll
-              for (int i = 0; i < 16; ++i) {
-                w[i] = pack_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 2 * i], 0.f),
-                                   fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 2 * i + 1], 0.f));
-                w[16 + i] = pack_bf16x2(fmaxf(__uint_as_float(v1[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
-                                        fmaxf(__uint_as_float(v1[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f));
-              }
+              for (int i = 0; i < 16; ++i)
+                w[16 + i] = pack_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
+                                        fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f));
               tmem_st32(lane_addr + COL_HID + c * 32, w);
             }
             EP_ACC(1);
@@ -448,57 +474,67 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
             EP_ACC(2);
           }
           mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane);
-          ++hcount;
         } else if (a.out_mode == 3) {
-          // ---- classifier: last hidden layer, then 1 unit + sigmoid
-          float logit = 0.f;
+          // ---- classifier: last hidden layer, then 1 unit + sigmoid; column half 0
+          // warps do all 128 columns of their rows (a cross-warp sum is not worth it for 1 unit).
+          if (hh == 0) {
+            float logit = 0.f;
 #pragma unroll 1
-          for (int q = 0; q < HW / 32; ++q) {
-            uint32_t v[32];
-            tmem_ld32(acc + q * 32, v);
-            tc_wait_ld();
+            for (int q = 0; q < HW / 32; ++q) {
+              uint32_t v[32];
+              tmem_ld32(acc + q * 32, v);
+              tc_wait_ld();
 #pragma unroll
-            for (int i = 0; i < 32; ++i)
-              logit = fmaf(fmaxf(__uint_as_float(v[i]) + bias[q * 32 + i], 0.f), wlast_s[q * 32 + i], logit);
+              for (int i = 0; i < 32; ++i)
+                logit = fmaf(fmaxf(__uint_as_float(v[i]) + bias[q * 32 + i], 0.f), wlast_s[q * 32 + i], logit);
+            }
+            tc_fence_before();
+            mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane);
+            logit += __ldg(a.bias[a.n_layers - 1]);
+            const int row = tile * TM + et;
+            if (row < a.n_rows) a.out[row] = 1.0f / (1.0f + expf(-logit));
+          } else {
+            mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane);
           }
-          tc_fence_before();
-          mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane);
-          logit += __ldg(a.bias[a.n_layers - 1]);
-          const int row = tile * TM + et;
-          if (row < a.n_rows) a.out[row] = 1.0f / (1.0f + expf(-logit));
         } else {
-          // ---- linear output (+ residual).  Each warp transposes its own 32 rows through a private 4 KB
-          // swizzled staging slice (thread = row on the TMEM side, 8 lanes per row on the global side),
-          // so only __syncwarp is needed.  The residual e += y is applied by a vector
-          // red.global.add on the in-place state: one IEEE fp32 add per element, performed at L2, no
-          // residual load, deterministic (each element is touched exactly once).
-          const uint32_t stg = stage_out + q4 * 4096;
-          const int jl = lane & 7, r8 = lane >> 3;
+          // ---- linear output (+ residual).  Each warp transposes 16 columns of its own 32 rows at a
+          // time through a private 2 KB swizzled staging slice (thread = row on the TMEM side, 4 lanes
+          // per row on the global side), so only __syncwarp is needed.  The residual e += y is
+          // applied by a vector red.global.add on the in-place state: one IEEE fp32 add per element,
+          // performed at L2, no residual load, deterministic (each element is touched exactly once).
+          const uint32_t stg = stage_out + ew * 2048;
+          const int jl = lane & 3, r4 = lane >> 2;
           const bool in_place_add = (a.out_mode == 1);
 #pragma unroll 1
-          for (int q = 0; q < HW / 32; ++q) {
+          for (int q = 0; q < 4; ++q) {
+            const int col0 = hh * 64 + q * 16;
             EP_T0();
-            uint32_t v[32];
-            tmem_ld32(acc + q * 32, v);
+            uint32_t v[16];
+            asm volatile(
+                "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+                "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                  "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                : "r"(acc + col0) : "memory");
             tc_wait_ld();
             EP_ACC(3);
-            if (q == HW / 32 - 1) { tc_fence_before(); mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane); }
+            if (q == 3) { tc_fence_before(); mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane); }
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-              const float4 bq = *reinterpret_cast<const float4*>(bias + q * 32 + 4 * j);
-              st_shared_v4(stg + lane * 128 + ((j ^ (lane & 7)) << 4),
+            for (int j = 0; j < 4; ++j) {
+              const float4 bq = *reinterpret_cast<const float4*>(bias + col0 + 4 * j);
+              st_shared_v4(stg + lane * 64 + ((j ^ ((lane >> 1) & 3)) << 4),
                            __float_as_uint(__uint_as_float(v[4 * j]) + bq.x), __float_as_uint(__uint_as_float(v[4 * j + 1]) + bq.y),
                            __float_as_uint(__uint_as_float(v[4 * j + 2]) + bq.z), __float_as_uint(__uint_as_float(v[4 * j + 3]) + bq.w));
             }
             __syncwarp();
             EP_ACC(4);
 #pragma unroll
-            for (int it = 0; it < 8; ++it) {
-              const int r = r8 + 4 * it;
+            for (int it = 0; it < 4; ++it) {
+              const int r = r4 + 8 * it;
               const int row = tile * TM + q4 * 32 + r;
               if (row < a.n_rows) {
-                const float4 y = ld_shared_v4(stg + r * 128 + ((jl ^ (r & 7)) << 4));
-                float* dst = a.out + (size_t)row * a.out_ld + q * 32 + jl * 4;
+                const float4 y = ld_shared_v4(stg + r * 64 + ((jl ^ ((r >> 1) & 3)) << 4));
+                float* dst = a.out + (size_t)row * a.out_ld + col0 + jl * 4;
                 if (in_place_add)
                   asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(y.x), "f"(y.y), "f"(y.z), "f"(y.w) : "memory");
                 else
@@ -511,14 +547,14 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
         }
       }
     }
-    (void)hcount;
-    if (a.dbg && et == 0) {
+    if (edbg && ew == 0 && lane == 0) {
       a.dbg[(size_t)blockIdx.x * 32 + 6] = (unsigned long long)e_wait;
       a.dbg[(size_t)blockIdx.x * 32 + 7] = (unsigned long long)(clock64() - e_start);
       for (int i = 0; i < 6; ++i) a.dbg[(size_t)blockIdx.x * 32 + 10 + i] = (unsigned long long)ep[i];
     }
-  } else if (warp == 12) {
+  } else if (warp == kWarpLoader) {
     // =========================== weight loader ===========================
+    reg_dec<kRegCtl>();
     if (lane == 0) {
       const int chunks_per_tile = nc1 + (n_gemm - 1) * HCH;
       uint32_t w_cnt = 0;
@@ -526,19 +562,23 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
         for (int q = 0; q < chunks_per_tile; ++q, ++w_cnt) {
           const uint32_t ws = w_cnt % NSW, wn = w_cnt / NSW;
           mbar_wait(smem_u32(&bars->w_empty[ws]), (wn & 1) ^ 1);
+          if (a.exp_flags & 2) { mbar_arrive(smem_u32(&bars->w_full[ws])); continue; }
           mbar_expect_tx(smem_u32(&bars->w_full[ws]), kStageBytes);
           bulk_g2s(wring + ws * kStageBytes, a.wimg + (size_t)q * kStageBytes, kStageBytes, smem_u32(&bars->w_full[ws]));
         }
       }
     }
+  } else if (warp > kWarpMma) {
+    reg_dec<kRegCtl>();                          // idle warps that complete the control warpgroup
   } else {
     // =========================== MMA issuer ===========================
+    reg_dec<kRegCtl>();
     // Warp-uniform control flow: every lane waits on the barriers, one elected lane issues.  (Issuing
     // from a divergent `if (lane == 0)` region makes ptxas wrap every UTCHMMA in an election loop,
     // which left the tensor pipe idle half of the time.)
     uint32_t w_cnt = 0, a_cnt = 0, g = 0, hcount = 0;
     long long dt[6] = {0, 0, 0, 0, 0, 0};
-    const bool dbg = a.dbg != nullptr;
+    const bool dbg = ETX_DBG(a);
     long long t_start = dbg ? clock64() : 0, t0 = 0;
 #define DBG_T0() if (dbg) t0 = clock64()
 #define DBG_ACC(i) if (dbg) dt[i] += clock64() - t0
@@ -616,7 +656,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 13) {
+  if (warp == kWarpMma) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
   }
