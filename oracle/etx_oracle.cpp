@@ -12,6 +12,7 @@
 //
 // Pins (tests/test_oracle_*.py): brute-force N^2 search, dense incidence-matrix scatter, torch float64
 // linear layers, closed forms (r -> inf edge counts, zero/constant networks), invariants.
+// Track building (orc_wcc): scipy connected_components, hand-built graphs, partition invariants.
 // Whole path vs the thesis' TRAINED network: parity unpinned (no weights, data or printed outputs exist).
 #include <cmath>
 #include <cstdint>
@@ -219,6 +220,27 @@ void orc_edge_scores(int64_t n_edges, const float* e, int32_t H, int32_t n_layer
     scores[k] = (float)(1.0 / (1.0 + std::exp(-(double)lg[k])));
     if (logits) logits[k] = lg[k];
   }
+}
+
+// ---- NEXT-1: score cut + track building.  Purified hit graph = edges with
+//      score >= score_min; tracks = its weakly connected components.  Plain union-find over the kept
+//      edges (the textbook alternative to the DFS of Algs. 2-3, same result); the label of a hit is the
+//      smallest hit index of its component (a hit without kept edges keeps its own index).
+static int32_t uf_find(std::vector<int32_t>& parent, int32_t x) {
+  while (parent[x] != x) { parent[x] = parent[parent[x]]; x = parent[x]; }
+  return x;
+}
+
+void orc_wcc(int64_t n_hits, int64_t n_edges, const int32_t* src, const int32_t* dst, const float* scores,
+             float score_min, int32_t* labels) {
+  std::vector<int32_t> parent((size_t)n_hits);
+  for (int64_t i = 0; i < n_hits; ++i) parent[i] = (int32_t)i;
+  for (int64_t k = 0; k < n_edges; ++k) {
+    if (!(scores[k] >= score_min)) continue;              // edges below the minimum score are removed
+    const int32_t a = uf_find(parent, src[k]), b = uf_find(parent, dst[k]);
+    if (a != b) { if (a < b) parent[b] = a; else parent[a] = b; }   // root = smallest index of the set
+  }
+  for (int64_t i = 0; i < n_hits; ++i) labels[i] = uf_find(parent, (int32_t)i);
 }
 
 }  // extern "C"

@@ -158,6 +158,18 @@ def edge_scores(e, H: int, n_layers: int, blob: np.ndarray, off_cls: int, want_l
     return (s, lg) if want_logits else s
 
 
+def wcc(n_hits: int, src, dst, scores, score_min: float) -> np.ndarray:
+    """NEXT-1: labels [n_hits] = smallest hit index of the weakly connected
+    component of the purified graph (edges with score >= score_min)."""
+    src = np.ascontiguousarray(src, np.int32)
+    dst = np.ascontiguousarray(dst, np.int32)
+    scores = _f32(scores)
+    labels = np.empty(n_hits, np.int32)
+    lib().orc_wcc(C.c_int64(n_hits), C.c_int64(len(src)), _p(src, C.c_int32), _p(dst, C.c_int32),
+                  _p(scores, C.c_float), C.c_float(score_min), _p(labels, C.c_int32))
+    return labels
+
+
 def run_path(batch: Dict[str, np.ndarray], blob: np.ndarray, layout: Dict[str, Tuple[Tuple[int, ...], int]],
              H: int, n_iter: int, r2_max: float, gap: int, center, scale, n_planes: int = 26,
              graph: Optional[Tuple[np.ndarray, np.ndarray]] = None) -> Dict[str, np.ndarray]:
