@@ -248,6 +248,20 @@ def run_ours(args):
     ms_step = ms / args.steps
     value = aggregate_events_per_s(world, n_ev, ms_step)
 
+    # ---- next row beyond the step (reported separately, not part of `value`): score cut + WCC tracks
+    labels = torch.empty(max(N, 1), dtype=torch.int32, device=dev)
+    etx.etx_build_tracks(db, g, scores, 0.5, labels)
+    barrier()
+    t0.record()
+    for _ in range(3):
+        etx.etx_build_tracks(db, g, scores, 0.5, labels)
+    t1.record()
+    barrier()
+    wcc_ms = t0.elapsed_time(t1) / 3
+    sizes = torch.bincount(labels[:N].long(), minlength=1)
+    next_rows = {"wcc_tracks": {"ms": wcc_ms, "events_per_s": n_ev / (wcc_ms * 1e-3), "score_min": 0.5,
+                                "components_ge3_hits": int((sizes >= 3).sum().item())}}
+
     # ---- end to end through the host-buffer entry point
     host = binding.pinned_host_batch(batch)
     o_src = torch.empty(cap, dtype=torch.int32).pin_memory()
@@ -342,7 +356,7 @@ def run_ours(args):
         "roofline": roof, "cpu_baseline": cpu,
         "e2e": {"value": aggregate_events_per_s(world, n_ev, e2e_ms), "unit": "events/s", "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms},
-        "gpu_launches": int(launches), "clocks": clk.summary(), "stages": stages}))
+        "gpu_launches": int(launches), "clocks": clk.summary(), "stages": stages, "next_rows": next_rows}))
     if world > 1:
         dist.destroy_process_group()
 

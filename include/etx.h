@@ -133,6 +133,14 @@ etx_status etx_gnn_forward(etx_ctx* ctx, const etx_batch* batch, const etx_graph
 etx_status etx_edge_scores(etx_ctx* ctx, const etx_graph* g, const float* d_edge_enc,
                            float* d_scores, void* stream);
 
+/* Next row beyond the hits -> edge-scores path: score cut + track building.  The purified hit graph keeps
+ * the edges with score >= score_min; tracks are its weakly connected components
+ * (plane-sweep minimum-label propagation repeated until stable, so the result is the exact
+ * WCC).  d_labels[n_hits] receives for every hit the smallest hit index of its component (a hit without
+ * kept edges gets its own index).  Deterministic.                                                    */
+etx_status etx_build_tracks(etx_ctx* ctx, const etx_batch* batch, const etx_graph* g, const float* d_scores,
+                            float score_min, int32_t* d_labels, void* stream);
+
 /* Whole path with HOST buffers: copies the batch host->device, runs a0..a7, copies src/dst/scores
  * back (h_src, h_dst may be NULL).  Needs a workspace sized with with_host_path = 1.  Host buffers
  * should be pinned for the copies to be asynchronous.  Synchronises the stream before returning.  */
@@ -155,7 +163,8 @@ typedef enum {
   ETX_K_NODE_NET = 5,   /* a5 node network                                    */
   ETX_K_EDGE_NET = 6,   /* a6 edge network (the dominant kernel)              */
   ETX_K_CLS = 7,        /* a7 classifier + sigmoid                            */
-  ETX_K_COUNT = 8
+  ETX_K_TRACKS = 8,     /* next row: score cut + WCC track building             */
+  ETX_K_COUNT = 9
 } etx_kernel_class;
 etx_status etx_profile_enable(etx_ctx* ctx, int on);
 etx_status etx_profile_read(etx_ctx* ctx, double* ms /*[ETX_K_COUNT]*/, int64_t* launches /*[ETX_K_COUNT]*/);

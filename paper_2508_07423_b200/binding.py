@@ -21,8 +21,8 @@ ETX_OK, ETX_ERR_INVALID, ETX_ERR_CAPACITY, ETX_ERR_CUDA, ETX_ERR_UNSORTED, ETX_E
 
 EXPORTS = ["etx_weight_count", "etx_create", "etx_destroy", "etx_last_error", "etx_workspace_bytes",
            "etx_set_workspace", "etx_embed", "etx_build_graph", "etx_gnn_forward", "etx_edge_scores",
-           "etx_infer_host", "etx_launch_count", "etx_profile_enable", "etx_profile_read"]
-KERNEL_CLASSES = ["embed", "graph", "node_enc", "edge_enc", "scatter", "node_net", "edge_net", "cls"]
+           "etx_infer_host", "etx_launch_count", "etx_profile_enable", "etx_profile_read", "etx_build_tracks"]
+KERNEL_CLASSES = ["embed", "graph", "node_enc", "edge_enc", "scatter", "node_net", "edge_net", "cls", "tracks"]
 
 
 class EtxError(RuntimeError):
@@ -94,6 +94,9 @@ def load_library():
                                        C.POINTER(C.c_int64), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.etx_launch_count.restype = C.c_int64
         lib.etx_launch_count.argtypes = [C.c_void_p]
+        lib.etx_build_tracks.restype = C.c_int
+        lib.etx_build_tracks.argtypes = [C.c_void_p, C.POINTER(Batch), C.POINTER(Graph), C.c_void_p, C.c_float,
+                                         C.c_void_p, C.c_void_p]
         lib.etx_profile_enable.restype = C.c_int
         lib.etx_profile_enable.argtypes = [C.c_void_p, C.c_int]
         lib.etx_profile_read.restype = C.c_int
@@ -235,6 +238,14 @@ class Etx:
         self._check(self.lib.etx_edge_scores(self.handle, C.byref(graph.c), _ptr(edge_enc), _ptr(scores),
                                              self._stream()))
         return scores
+
+    def etx_build_tracks(self, batch: DeviceBatch, graph: DeviceGraph, scores: torch.Tensor, score_min: float,
+                         labels: Optional[torch.Tensor] = None) -> torch.Tensor:
+        if labels is None:
+            labels = torch.empty(max(batch.n_hits, 1), dtype=torch.int32, device=self.device)
+        self._check(self.lib.etx_build_tracks(self.handle, C.byref(batch.c), C.byref(graph.c), _ptr(scores),
+                                              score_min, _ptr(labels), self._stream()))
+        return labels
 
     # ---- whole path with host buffers (pinned torch tensors or numpy arrays)
     def etx_infer_host(self, host: Dict[str, torch.Tensor], r2_max: float, max_plane_gap: int,

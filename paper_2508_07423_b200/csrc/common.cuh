@@ -111,6 +111,10 @@ struct TcArgs {
 int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s);
 int tc_chunk_k(int mode);
 
+// ---- tracks.cu (next row: score cut + weakly connected components)
+int launch_wcc(int n_events, const int32_t* event_ptr, const int32_t* row_ptr, const int32_t* src,
+               const int32_t* dst, const float* scores, float score_min, int32_t* labels, cudaStream_t s);
+
 // ---- scatter.cu
 int launch_scatter(int n_nodes, int H, const int32_t* row_ptr, const int32_t* in_ptr,
                    const int32_t* in_perm, const float* e, float* m, cudaStream_t s);

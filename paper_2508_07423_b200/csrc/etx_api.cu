@@ -534,6 +534,22 @@ etx_status etx_edge_scores(etx_ctx* c, const etx_graph* g, const float* d_edge_e
   return check_cuda(c, "etx_edge_scores");
 }
 
+etx_status etx_build_tracks(etx_ctx* c, const etx_batch* b, const etx_graph* g, const float* d_scores,
+                            float score_min, int32_t* d_labels, void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (etx_status st = check_batch(c, b)) return st;
+  if (!g || g->n_edges < 0 || !g->d_row_ptr) return fail(c, ETX_ERR_INVALID, "graph is NULL or not built");
+  if (b->n_hits > 0 && !d_labels) return fail(c, ETX_ERR_INVALID, "d_labels is NULL");
+  if (g->n_edges > 0 && (!d_scores || !g->d_src || !g->d_dst)) return fail(c, ETX_ERR_INVALID, "scores / edge arrays are NULL");
+  cudaSetDevice(c->device);
+  {
+    ProfScope ps(c, ETX_K_TRACKS, (cudaStream_t)stream);
+    c->launches += launch_wcc(b->n_events, b->d_event_ptr, g->d_row_ptr, g->d_src, g->d_dst, d_scores, score_min,
+                              d_labels, (cudaStream_t)stream);
+  }
+  return check_cuda(c, "etx_build_tracks");
+}
+
 etx_status etx_infer_host(etx_ctx* c, const etx_batch_host* hb, float r2_max, int32_t max_plane_gap,
                           int64_t edge_capacity, int64_t* n_edges, int32_t* h_src, int32_t* h_dst,
                           float* h_scores, void* stream) {
