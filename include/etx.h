@@ -164,7 +164,8 @@ typedef enum {
   ETX_K_EDGE_NET = 6,   /* a6 edge network (the dominant kernel)              */
   ETX_K_CLS = 7,        /* a7 classifier + sigmoid                            */
   ETX_K_TRACKS = 8,     /* next row: score cut + WCC track building             */
-  ETX_K_COUNT = 9
+  ETX_K_EDGE_PROJ = 9,  /* a3/a6 per-hit first-layer projections [A h | B h] of the edge MLPs (tensor-core modes) */
+  ETX_K_COUNT = 10
 } etx_kernel_class;
 etx_status etx_profile_enable(etx_ctx* ctx, int on);
 etx_status etx_profile_read(etx_ctx* ctx, double* ms /*[ETX_K_COUNT]*/, int64_t* launches /*[ETX_K_COUNT]*/);

@@ -20,6 +20,11 @@ struct DevMlp {
   const float* Wt[kMaxLayers] = {nullptr};
   const float* b[kMaxLayers] = {nullptr};
   const unsigned char* wimg = nullptr;   // tensor-core weight image (mlp_tc.cu), or null
+  // First-layer factorisation (edge encoder / edge networks in tensor-core modes): the first layer's
+  // weight W1 = [A | B | C] over the inputs [h_src | h_dst | e] is split; wimg_a / wimg_b are the
+  // one-layer images of A and B (applied once per HIT), wimg then holds C (if any) and the other layers.
+  const unsigned char* wimg_a = nullptr;
+  const unsigned char* wimg_b = nullptr;
 };
 
 struct Workspace {            // carved from the caller's buffer by carve_workspace()
@@ -29,6 +34,7 @@ struct Workspace {            // carved from the caller's buffer by carve_worksp
   int32_t* flags = nullptr;       // [8] validation flags / counters
   float* h = nullptr;             // [n_hits, H]
   float* m = nullptr;             // [n_hits, 2H]
+  float* p = nullptr;             // [n_hits, 2H] per-hit first-layer projections [A h | B h] (tensor-core modes)
   // host-path staging
   int32_t* s_event_ptr = nullptr; uint8_t* s_plane = nullptr;
   float *s_r = nullptr, *s_phi = nullptr, *s_z = nullptr, *s_x = nullptr, *s_y = nullptr;
@@ -46,6 +52,7 @@ struct etx_ctx {
   int sm_count = 148;
   float* d_weights = nullptr;      // transposed weights + biases, one allocation
   size_t d_weights_floats = 0;
+  const float* d_zero_bias = nullptr;  // 128 zeros inside d_weights
   unsigned char* d_wimg = nullptr; // tensor-core weight images, one allocation
   etx::DevMlp emb, node_enc, edge_enc, cls;
   std::vector<etx::DevMlp> node_net, edge_net;
@@ -89,6 +96,9 @@ struct MlpArgs {
   // first-layer input: either up to 3 gathered segments, or 3 features computed from SoA arrays
   int n_seg = 0; Segment seg[3];
   const float* feat[3] = {nullptr, nullptr, nullptr}; float fc[3] = {0, 0, 0}; float fs[3] = {1, 1, 1};
+  // addend: the first layer's pre-activation starts from add[0][idx0[row]] + add[1][idx1[row]]
+  // (128 columns each) instead of zero (tensor-core path only; n_add is 0 or 2)
+  int n_add = 0; Segment add[2];
   DevMlp mlp;
   // output: mode 0 store, 1 residual add (out = res + y; res may alias out), 2 small-N linear,
   // 3 small-N sigmoid
@@ -99,7 +109,8 @@ int launch_mlp_simt(const MlpArgs& a, cudaStream_t s);
 // ---- mlp_tc.cu (tcgen05 tensor-core path)
 struct TcArgs {
   int n_rows = 0;
-  int n_seg = 0; Segment seg[3]; int K0 = 0;      // first-layer input: gathered segments, K0 = sum of widths
+  int n_seg = 0; Segment seg[3]; int K0 = 0;      // first-layer input: gathered segments, K0 = sum of widths (may be 0 with an addend)
+  int n_add = 0; Segment add[2];                  // 0 or 2 addend sources: layer-1 accumulator starts from their sum
   int n_layers = 0;
   const unsigned char* wimg = nullptr;            // weight image: swizzled 16 KB tiles in consumption order
   const float* bias[kMaxLayers] = {nullptr};

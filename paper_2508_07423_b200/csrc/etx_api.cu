@@ -71,39 +71,46 @@ uint16_t bf16_rne(float f) {
   return (uint16_t)(u >> 16);
 }
 
-void append_wimg(std::vector<unsigned char>& img, const HostMlp& m, const float* w, int n_gemm, int mode) {
+// Appends the image of input columns [k_begin, k_end) of one layer W [fo = 128][fi] (row-major, fp32).
+void append_wimg_slab(std::vector<unsigned char>& img, const float* W, int fi, int fo, int k_begin, int k_end, int mode) {
   const int KA = tc_chunk_k(mode);
   const int pieces = mode == ETX_PREC_BF16 ? 1 : 2;
+  for (int k0 = k_begin; k0 < k_end; k0 += KA) {
+    const size_t base = img.size();
+    img.resize(base + (size_t)pieces * 128 * 128, 0);
+    for (int n = 0; n < fo; ++n)
+      for (int kk = 0; kk < KA; ++kk) {
+        const float v = W[(size_t)n * fi + k0 + kk];
+        if (mode == ETX_PREC_TF32X3) {
+          uint32_t u; std::memcpy(&u, &v, 4);
+          const uint32_t hi_u = u & 0xffffe000u;
+          float hi; std::memcpy(&hi, &hi_u, 4);
+          const float lo = v - hi;
+          const size_t off = (size_t)n * 128 + (size_t)(((kk / 4) ^ (n & 7)) * 16) + (kk % 4) * 4;
+          std::memcpy(&img[base + off], &hi, 4);
+          std::memcpy(&img[base + 128 * 128 + off], &lo, 4);
+        } else {
+          const uint16_t b = bf16_rne(v);
+          const size_t off = (size_t)n * 128 + (size_t)(((kk / 8) ^ (n & 7)) * 16) + (kk % 8) * 2;
+          std::memcpy(&img[base + off], &b, 2);
+          if (pieces == 2) {                          // BF16X3: lo = bf16(w - hi)
+            const uint32_t hu = (uint32_t)b << 16;
+            float hf; std::memcpy(&hf, &hu, 4);
+            const uint16_t lo = bf16_rne(v - hf);
+            std::memcpy(&img[base + 128 * 128 + off], &lo, 2);
+          }
+        }
+      }
+  }
+}
+
+// Image of layers [l_begin, n_gemm) of an MLP; the first of them restricted to input columns >= k_first.
+void append_wimg(std::vector<unsigned char>& img, const HostMlp& m, const float* w, int l_begin, int k_first,
+                 int n_gemm, int mode) {
   const float* W = w;
   for (int l = 0; l < n_gemm; ++l) {
     const int fi = m.dims[l], fo = m.dims[l + 1];           // fo == 128
-    for (int k0 = 0; k0 < fi; k0 += KA) {
-      const size_t base = img.size();
-      img.resize(base + (size_t)pieces * 128 * 128, 0);
-      for (int n = 0; n < fo; ++n)
-        for (int kk = 0; kk < KA; ++kk) {
-          const float v = W[(size_t)n * fi + k0 + kk];
-          if (mode == ETX_PREC_TF32X3) {
-            uint32_t u; std::memcpy(&u, &v, 4);
-            const uint32_t hi_u = u & 0xffffe000u;
-            float hi; std::memcpy(&hi, &hi_u, 4);
-            const float lo = v - hi;
-            const size_t off = (size_t)n * 128 + (size_t)(((kk / 4) ^ (n & 7)) * 16) + (kk % 4) * 4;
-            std::memcpy(&img[base + off], &hi, 4);
-            std::memcpy(&img[base + 128 * 128 + off], &lo, 4);
-          } else {
-            const uint16_t b = bf16_rne(v);
-            const size_t off = (size_t)n * 128 + (size_t)(((kk / 8) ^ (n & 7)) * 16) + (kk % 8) * 2;
-            std::memcpy(&img[base + off], &b, 2);
-            if (pieces == 2) {                          // BF16X3: lo = bf16(w - hi)
-              const uint32_t hu = (uint32_t)b << 16;
-              float hf; std::memcpy(&hf, &hu, 4);
-              const uint16_t lo = bf16_rne(v - hf);
-              std::memcpy(&img[base + 128 * 128 + off], &lo, 2);
-            }
-          }
-        }
-    }
+    if (l >= l_begin) append_wimg_slab(img, W, fi, fo, l == l_begin ? k_first : 0, fi, mode);
     W += (size_t)fi * fo + fo;
   }
 }
@@ -119,6 +126,7 @@ Workspace carve(const etx_ctx* c, int32_t n_events, int32_t n_hits, int64_t cap,
   w.flags = (int32_t*)take(sizeof(int32_t) * 8);
   w.h = (float*)take(sizeof(float) * (size_t)n_hits * H);
   w.m = (float*)take(sizeof(float) * (size_t)n_hits * 2 * H);
+  if (c->desc.precision != ETX_PREC_FP32) w.p = (float*)take(sizeof(float) * (size_t)n_hits * 2 * H);
   if (host_path) {
     w.s_event_ptr = (int32_t*)take(sizeof(int32_t) * ((size_t)n_events + 1));
     w.s_plane = (uint8_t*)take((size_t)n_hits);
@@ -194,6 +202,7 @@ int run_mlp(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   TcArgs t;
   t.n_rows = a.n_rows; t.n_seg = a.n_seg; t.K0 = a.mlp.dims[0];
   for (int i = 0; i < 3; ++i) t.seg[i] = a.seg[i];
+  t.n_add = a.n_add; t.add[0] = a.add[0]; t.add[1] = a.add[1];
   t.n_layers = a.mlp.n_layers;
   t.wimg = a.mlp.wimg;
   for (int l = 0; l < a.mlp.n_layers; ++l) t.bias[l] = a.mlp.b[l];
@@ -282,6 +291,9 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
       src += fo;
     }
   }
+  staged.resize(align_up(staged.size(), 64));
+  const size_t off_zero = staged.size();               // 128 zeros: bias of the per-hit projection launches
+  staged.resize(staged.size() + 128, 0.0f);
   c->d_weights_floats = staged.size();
   if (cudaMalloc(&c->d_weights, staged.size() * sizeof(float)) != cudaSuccess ||
       cudaMemcpy(c->d_weights, staged.data(), staged.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) {
@@ -295,6 +307,7 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
       dev[i].Wt[l] = c->d_weights + offW[i][l];
       dev[i].b[l] = c->d_weights + offB[i][l];
     }
+  c->d_zero_bias = c->d_weights + off_zero;
   c->emb = dev[0];
   c->node_enc = dev[1];
   c->edge_enc = dev[2];
@@ -304,13 +317,27 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
     // tensor-core weight images for every MLP whose first-layer input is a multiple of the chunk
     // (edge encoder, node/edge networks, classifier); embedding and node encoder (3 inputs) stay SIMT
     std::vector<unsigned char> img;
-    std::vector<size_t> img_off(mlps.size(), (size_t)-1);
+    std::vector<size_t> img_off(mlps.size(), (size_t)-1), img_a(mlps.size(), (size_t)-1), img_b(mlps.size(), (size_t)-1);
+    const int H = desc->gnn_hidden, mode = desc->precision;
     size_t wsrc = 0;
     for (size_t i = 0; i < mlps.size(); ++i) {
+      const float* w = h_weights + wsrc;
       if (i >= 2) {
         const bool is_cls = (i + 1 == mlps.size());
-        img_off[i] = img.size();
-        append_wimg(img, mlps[i], h_weights + wsrc, is_cls ? mlps[i].n_layers - 1 : mlps[i].n_layers, desc->precision);
+        const bool is_node = !is_cls && i >= 3 && ((i - 3) % 2 == 0);
+        if (is_cls || is_node) {
+          img_off[i] = img.size();
+          append_wimg(img, mlps[i], w, 0, 0, is_cls ? mlps[i].n_layers - 1 : mlps[i].n_layers, mode);
+        } else {
+          // edge encoder ([h_src | h_dst]) and edge networks ([h_src | h_dst | e]): first layer factorised
+          // into the per-hit parts A (columns [0,H)), B ([H,2H)) and the per-edge part C ([2H,3H), networks only)
+          const int fi = mlps[i].dims[0];
+          img_a[i] = img.size(); append_wimg_slab(img, w, fi, H, 0, H, mode);
+          img_b[i] = img.size(); append_wimg_slab(img, w, fi, H, H, 2 * H, mode);
+          img_off[i] = img.size();
+          if (fi > 2 * H) append_wimg(img, mlps[i], w, 0, 2 * H, mlps[i].n_layers, mode);
+          else append_wimg(img, mlps[i], w, 1, 0, mlps[i].n_layers, mode);
+        }
       }
       wsrc += mlp_floats(mlps[i]);
     }
@@ -320,12 +347,13 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
       etx_destroy(c);
       return fail(nullptr, ETX_ERR_CUDA, msg);
     }
-    c->edge_enc.wimg = c->d_wimg + img_off[2];
-    for (int k = 0; k < desc->n_iter; ++k) {
-      c->node_net[k].wimg = c->d_wimg + img_off[3 + 2 * k];
-      c->edge_net[k].wimg = c->d_wimg + img_off[4 + 2 * k];
-    }
-    c->cls.wimg = c->d_wimg + img_off[mlps.size() - 1];
+    auto place = [&](DevMlp& m, size_t i) {
+      m.wimg = c->d_wimg + img_off[i];
+      if (img_a[i] != (size_t)-1) { m.wimg_a = c->d_wimg + img_a[i]; m.wimg_b = c->d_wimg + img_b[i]; }
+    };
+    place(c->edge_enc, 2);
+    for (int k = 0; k < desc->n_iter; ++k) { place(c->node_net[k], 3 + 2 * k); place(c->edge_net[k], 4 + 2 * k); }
+    place(c->cls, mlps.size() - 1);
   }
   *out = c;
   return ETX_OK;
@@ -476,12 +504,39 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
     ProfScope ps(c, ETX_K_NODE_ENC, s);
     c->launches += run_mlp(c, a, s);
   }
+  // Tensor-core modes factorise the first layer of the edge MLPs: with W1 = [A | B | C]
+  // over [h_src | h_dst | e],  W1 [h_i, h_j, e] = (A h_i) + (B h_j) + C e.  The per-hit projections
+  // p_l = [A h_l | B h_l] cost 4 H^2 flop per HIT instead of per EDGE; the edge kernel gathers the two
+  // 128-wide rows, adds them and starts its layer-1 accumulator from the sum.
+  const bool fact = c->desc.precision != ETX_PREC_FP32;
+  auto project = [&](const DevMlp& mlp) {              // p = [A h | B h], two one-layer launches over the hits
+    ProfScope ps(c, ETX_K_EDGE_PROJ, s);
+    for (int part = 0; part < 2; ++part) {
+      MlpArgs a;
+      a.n_rows = N; a.n_seg = 1;
+      a.seg[0] = Segment{w.h, nullptr, H, H};
+      a.mlp.n_layers = 1; a.mlp.dims[0] = H; a.mlp.dims[1] = H;
+      a.mlp.wimg = part == 0 ? mlp.wimg_a : mlp.wimg_b;
+      a.mlp.b[0] = c->d_zero_bias; a.mlp.Wt[0] = c->d_zero_bias;
+      a.out_mode = 0; a.out = w.p + part * H; a.out_ld = 2 * H;
+      c->launches += run_mlp(c, a, s);
+    }
+  };
   {  // a3: e0 = MLP_e([h0_src, h0_dst])
     MlpArgs a;
-    a.n_rows = E; a.n_seg = 2;
-    a.seg[0] = Segment{w.h, g->d_src, H, H};
-    a.seg[1] = Segment{w.h, g->d_dst, H, H};
+    a.n_rows = E;
     a.mlp = c->edge_enc; a.out_mode = 0; a.out = d_edge_enc; a.out_ld = H;
+    if (fact) {
+      if (E > 0) project(c->edge_enc);
+      a.n_seg = 0; a.n_add = 2;
+      a.add[0] = Segment{w.p, g->d_src, H, 2 * H};
+      a.add[1] = Segment{w.p + H, g->d_dst, H, 2 * H};
+      a.mlp.dims[0] = 0;                               // no per-edge operand in layer 1
+    } else {
+      a.n_seg = 2;
+      a.seg[0] = Segment{w.h, g->d_src, H, H};
+      a.seg[1] = Segment{w.h, g->d_dst, H, H};
+    }
     ProfScope ps(c, ETX_K_EDGE_ENC, s);
     c->launches += run_mlp(c, a, s);
   }
@@ -502,11 +557,21 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
     }
     {  // a6: e += psi_k([h_src, h_dst, e]) with the UPDATED h
       MlpArgs a;
-      a.n_rows = E; a.n_seg = 3;
-      a.seg[0] = Segment{w.h, g->d_src, H, H};
-      a.seg[1] = Segment{w.h, g->d_dst, H, H};
-      a.seg[2] = Segment{d_edge_enc, nullptr, H, H};
+      a.n_rows = E;
       a.mlp = c->edge_net[k]; a.out_mode = 1; a.out = d_edge_enc; a.res = d_edge_enc; a.out_ld = H;
+      if (fact) {
+        if (E > 0) project(c->edge_net[k]);
+        a.n_seg = 1; a.n_add = 2;
+        a.seg[0] = Segment{d_edge_enc, nullptr, H, H};
+        a.add[0] = Segment{w.p, g->d_src, H, 2 * H};
+        a.add[1] = Segment{w.p + H, g->d_dst, H, 2 * H};
+        a.mlp.dims[0] = H;                             // per-edge operand of layer 1: e only
+      } else {
+        a.n_seg = 3;
+        a.seg[0] = Segment{w.h, g->d_src, H, H};
+        a.seg[1] = Segment{w.h, g->d_dst, H, H};
+        a.seg[2] = Segment{d_edge_enc, nullptr, H, H};
+      }
       ProfScope ps(c, ETX_K_EDGE_NET, s);
       c->launches += run_mlp(c, a, s);
     }

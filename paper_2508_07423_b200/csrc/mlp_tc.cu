@@ -53,7 +53,8 @@ constexpr int TM = 128;
 constexpr int kGatherThreads = 512;      // warpgroups 0-3 (warps 0-15)
 constexpr int kEpiThreads = 256;         // warpgroups 4-5 (warps 16-23): lane quarter = warp & 3, column half = (warp - 16) >> 2
 constexpr int kThreads = kGatherThreads + kEpiThreads + 128;   // + warpgroup 6: loader warp 24, MMA warp 25, two idle warps
-constexpr int kWarpEpi0 = kGatherThreads / 32, kWarpLoader = kWarpEpi0 + kEpiThreads / 32, kWarpMma = kWarpLoader + 1;
+constexpr int kWarpEpi0 = kGatherThreads / 32, kWarpLoader = kWarpEpi0 + kEpiThreads / 32, kWarpMma = kWarpLoader + 1, kWarpCommit = kWarpMma + 1;
+constexpr uint32_t kBarEntry0 = 2;       // named barriers 2 .. 2 + NSTAGE_A - 1: one per operand-ring entry
 // Register re-partitioning (setmaxnreg, per warpgroup): the kernel launches at <= 72 registers per
 // thread (896 threads), then the gather warpgroups shrink to 64, loader/MMA to 40, and the epilogue
 // warpgroups grow to 104.  More, thinner warps: the SIMT roles are latency-bound, not issue-bound.
@@ -116,10 +117,26 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
                  ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
 }
 
-struct Bars {                                   // mbarriers (8 bytes each) + TMEM base
-  uint64_t w_full[8], w_empty[8], a_full[4], a_empty[4], acc_full[2], acc_free[2], hid_ready[4];
-  uint32_t tmem_base;
+struct Unit {                                   // one gather unit: KA columns of one source (16 bytes)
+  const char* base;                             // source base + column offset (bytes)
+  uint32_t ldb;                                 // row stride in bytes
+  int32_t sel;                                  // row index: 0 / 1 = first / second index array, -1 = the tile row itself
 };
+constexpr int kMaxUnits = 24;
+
+struct Bars {                                   // mbarriers (8 bytes each) + TMEM base + gather unit table
+  uint64_t w_full[8], w_empty[8], a_full[4], a_empty[4], acc_full[2], acc_free[2], hid_ready[8];
+  uint32_t tmem_base;
+  Unit utab[kMaxUnits];
+};
+
+// tcgen05.cp: 128 lanes x 256 bits (8 fp32 columns) from a K-major SWIZZLE_128B shared-memory tile into
+// tensor memory.  Reads exactly the slab a kind::tf32 MMA k-step reads as its A operand (measured:
+// [tmem + 8 ks] <- desc + 2 ks gives lane r, column c = tile element (r, c)); ordered with the
+// tcgen05.mma issued after it by the same thread, tracked by tcgen05.commit.
+__device__ __forceinline__ void tmem_cp_128x256b(uint32_t taddr, uint64_t desc) {
+  asm volatile("tcgen05.cp.cta_group::1.128x256b [%0], %1;" ::"r"(taddr), "l"(desc) : "memory");
+}
 
 template <int MODE>
 __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
@@ -127,6 +144,13 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   constexpr int KA = C::KA, P = C::PIECES, NSW = C::NSTAGE_W, NSA = C::NSTAGE_A, HID_COLS = C::HID_COLS;
   constexpr uint32_t kStageBytes = P * kAtomBytes;
   constexpr uint32_t COL_ACC = 0, COL_HID = 256;
+  // Tiles in flight per CTA.  The bf16 modes keep TWO 128-row tiles in flight (slot s: accumulator s,
+  // hidden operand region s): the MMA warp issues layer l of tile A, then of tile B, while the epilogue
+  // warps turn A's accumulator into its next operand; both tiles use each weight stage before it is
+  // released, so the weight ring moves half the bytes.  TF32X3 needs 256 columns per hidden operand
+  // and keeps one tile in flight with ping-pong accumulators.
+  constexpr int NSLOT = (MODE == ETX_PREC_TF32X3) ? 1 : 2;
+  constexpr uint32_t HIDW = P * HID_COLS;       // TMEM columns of one hidden operand region (256 / 128 / 64)
   constexpr int HCH = HW / KA;                  // K-chunks per hidden layer (4 / 2)
   constexpr int LPR = KA * 4 / 16;              // gather lanes per row: 16-byte pieces of a chunk row (8 / 16)
   constexpr int RPP = kGatherThreads / LPR;     // rows covered by one pass of the gather threads (32 / 16)
@@ -148,6 +172,39 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   const int n_tiles = (a.n_rows + TM - 1) / TM;
   const int n_gemm = (a.out_mode == 3) ? a.n_layers - 1 : a.n_layers;
   const int nc1 = a.K0 / KA;
+  const int my_tiles = (n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles blockIdx.x + i * gridDim.x
+  const int n_pairs = (my_tiles + NSLOT - 1) / NSLOT;
+  const bool share1 = nc1 * 2 <= NSW;           // first-layer weight stages shared by the tiles of a pair
+  // Addend (first-layer factorisation): the accumulator of layer 1 starts from
+  // add[0][idx0[row]] + add[1][idx1[row]] (128 fp32 columns) instead of zero.
+  const int n_addu = a.n_add ? 2 * HCH : 0;     // addend gather units per tile (two sources x 128 / KA column chunks)
+  const int n_addg = n_addu / D;                // = 2 groups of 64 columns
+  const int n_units = n_addu + nc1;
+  Unit* utab = bars->utab;
+  if ((int)threadIdx.x < n_units) {
+    const int u = threadIdx.x;
+    Unit un;
+    if (u < n_addu) {
+      const bool second = (u & 1) != 0;
+      const float* b = second ? a.add[1].base : a.add[0].base;
+      const int ld = second ? a.add[1].ld : a.add[0].ld;
+      const bool has_idx = (second ? a.add[1].idx : a.add[0].idx) != nullptr;
+      un.base = reinterpret_cast<const char*>(b + (u >> 1) * KA);
+      un.ldb = (uint32_t)ld * 4u;
+      un.sel = has_idx ? (u & 1) : -1;
+    } else {
+      int k = (u - n_addu) * KA, sg = 0;
+      if (a.n_seg > 1 && k >= a.seg[0].width) { k -= a.seg[0].width; sg = 1; }
+      if (sg == 1 && a.n_seg > 2 && k >= a.seg[1].width) { k -= a.seg[1].width; sg = 2; }
+      const float* b = sg == 0 ? a.seg[0].base : (sg == 1 ? a.seg[1].base : a.seg[2].base);
+      const int ld = sg == 0 ? a.seg[0].ld : (sg == 1 ? a.seg[1].ld : a.seg[2].ld);
+      const bool has_idx = (sg == 0 ? a.seg[0].idx : (sg == 1 ? a.seg[1].idx : nullptr)) != nullptr;
+      un.base = reinterpret_cast<const char*>(b + k);
+      un.ldb = (uint32_t)ld * 4u;
+      un.sel = (has_idx && !a.n_add) ? sg : -1;
+    }
+    utab[u] = un;
+  }
 
   for (int i = threadIdx.x; i < a.n_layers * HW; i += kThreads) {
     const int l = i / HW, j = i % HW;
@@ -157,9 +214,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
     for (int i = threadIdx.x; i < HW; i += kThreads) wlast_s[i] = __ldg(a.w_last + i);
   if (threadIdx.x == 0) {
     for (int i = 0; i < NSW; ++i) { mbar_init(smem_u32(&bars->w_full[i]), 1); mbar_init(smem_u32(&bars->w_empty[i]), 1); }
-    for (int i = 0; i < NSA; ++i) { mbar_init(smem_u32(&bars->a_full[i]), kGatherThreads / 32); mbar_init(smem_u32(&bars->a_empty[i]), 1); }
+    for (int i = 0; i < NSA; ++i) { mbar_init(smem_u32(&bars->a_full[i]), 1); mbar_init(smem_u32(&bars->a_empty[i]), 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&bars->acc_full[i]), 1); mbar_init(smem_u32(&bars->acc_free[i]), kEpiThreads / 32); }
-    for (int i = 0; i < 4; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), 4);
+    for (int i = 0; i < 8; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), 4);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == kWarpMma) {                        // TMEM: all 512 columns of this SM (1 CTA per SM)
@@ -177,7 +234,6 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
     const int t = threadIdx.x;                   // 0..511
     const int jl = t % LPR;                      // 16-byte piece of the chunk row this thread moves
     const int r0 = t / LPR;                      // first of its rows; then r0 + RPP, r0 + 2 RPP, ...
-    const int total_chunks = ((n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x) * nc1;
     float4 buf[D][NPASS];
     long long g_wait = 0, gp[4] = {0, 0, 0, 0}, tq = 0;
     const bool gdbg = ETX_DBG(a);
@@ -185,105 +241,139 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
 #define GP_ACC(i) if (gdbg) { const long long tn = clock64(); gp[i] += tn - tq; tq = tn; }
     const long long g_start = gdbg ? clock64() : 0;
 
-    // Producer cursor (tile, chunk, segment, k offset) advanced incrementally: no division, no dynamic
-    // indexing of kernel parameters, no segment search in the per-chunk path (these warps have almost
-    // no ILP, so every scalar instruction costs its full latency).  Row indices of this thread's NPASS
-    // rows for the (at most two) index-gathered segments are reloaded when the cursor enters a tile.
-    const char* sbase[3]; uint32_t sld[3]; int swidth[3]; const int32_t* sidx[2];
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      sbase[i] = reinterpret_cast<const char*>(i < a.n_seg ? a.seg[i].base : nullptr) + jl * 16;
-      sld[i] = i < a.n_seg ? (uint32_t)a.seg[i].ld * 4u : 0u;
-      swidth[i] = i < a.n_seg ? a.seg[i].width : 0;
-    }
-    sidx[0] = a.n_seg > 0 ? a.seg[0].idx : nullptr;
-    sidx[1] = a.n_seg > 1 ? a.seg[1].idx : nullptr;
-    int ptile = blockIdx.x, pc = 0, pseg = 0, pk = 0;
+    // Producer cursor (tile, unit).  A unit is KA consecutive columns of one source for the 128 rows of a
+    // tile; the per-unit source (base + column offset, row stride, which row-index array) sits in a
+    // small shared-memory table built once per launch, so the per-unit path has no segment search, no
+    // division and no dynamic indexing of kernel parameters (these warps have almost no ILP: every
+    // scalar instruction costs its full latency).  Units of a tile: first the addend units (source 0 /
+    // source 1 alternating, column chunk by column chunk), then the K-chunks of the MMA operand.
+    const int32_t* sidx0 = a.n_add ? a.add[0].idx : (a.n_seg > 0 ? a.seg[0].idx : nullptr);
+    const int32_t* sidx1 = a.n_add ? a.add[1].idx : (a.n_seg > 1 ? a.seg[1].idx : nullptr);
+    const int total_groups = my_tiles * (n_units / D);
+    int ptile = blockIdx.x, pu = 0;
     int ridx[2][NPASS], rown[NPASS];
-    auto load_chunk = [&](float4 (&dst)[NPASS]) {
-      if (pc == 0) {
+    auto load_unit = [&](float4 (&dst)[NPASS]) {
+      if (pu == 0) {
 #pragma unroll
         for (int p = 0; p < NPASS; ++p) {
           const int row = ptile * TM + r0 + p * RPP;
           rown[p] = row < a.n_rows ? row : a.n_rows - 1;
           if (a.exp_flags & 4) rown[p] = r0 + p * RPP;      // timing experiment: every tile reads the same rows
         }
+        if (sidx0) {
 #pragma unroll
-        for (int sgi = 0; sgi < 2; ++sgi)
-          if (sidx[sgi]) {
+          for (int p = 0; p < NPASS; ++p) ridx[0][p] = (a.exp_flags & 4) ? rown[p] : __ldg(sidx0 + rown[p]);
+        }
+        if (sidx1) {
 #pragma unroll
-            for (int p = 0; p < NPASS; ++p) ridx[sgi][p] = (a.exp_flags & 4) ? rown[p] : __ldg(sidx[sgi] + rown[p]);
-          }
+          for (int p = 0; p < NPASS; ++p) ridx[1][p] = (a.exp_flags & 4) ? rown[p] : __ldg(sidx1 + rown[p]);
+        }
       }
-      const char* base = (pseg == 0 ? sbase[0] : (pseg == 1 ? sbase[1] : sbase[2])) + pk * 4;
-      const uint32_t ldb = pseg == 0 ? sld[0] : (pseg == 1 ? sld[1] : sld[2]);
-      const bool ix0 = pseg == 0 && sidx[0] != nullptr, ix1 = pseg == 1 && sidx[1] != nullptr;
+      const Unit un = utab[pu];
+      const char* base = un.base + jl * 16;
 #pragma unroll
       for (int p = 0; p < NPASS; ++p) {
-        const uint32_t idx = (uint32_t)(ix0 ? ridx[0][p] : (ix1 ? ridx[1][p] : rown[p]));
-        dst[p] = __ldg(reinterpret_cast<const float4*>(base + (size_t)idx * ldb));
+        const uint32_t idx = (uint32_t)(un.sel == 0 ? ridx[0][p] : (un.sel == 1 ? ridx[1][p] : rown[p]));
+        dst[p] = __ldg(reinterpret_cast<const float4*>(base + (size_t)idx * un.ldb));
       }
-      // advance the cursor
-      pk += KA;
-      const int w = pseg == 0 ? swidth[0] : (pseg == 1 ? swidth[1] : swidth[2]);
-      if (pk >= w) { pk = 0; ++pseg; }
-      if (++pc == nc1) { pc = 0; pseg = 0; pk = 0; ptile += gridDim.x; }
+      if (++pu == n_units) { pu = 0; ptile += gridDim.x; }
+    };
+    // store one K-chunk of the MMA operand (converted / split) into ring entry `slot`
+    auto store_operand = [&](const float4 (&src)[NPASS], uint32_t slot) {
+      const uint32_t tile_hi = aring + slot * kStageBytes;
+#pragma unroll
+      for (int p = 0; p < NPASS; ++p) {
+        const int r = r0 + p * RPP;
+        const float4 v = src[p];
+        if constexpr (MODE == ETX_PREC_TF32X3) {
+          const uint32_t off = r * 128 + ((jl ^ (r & 7)) << 4);
+          const uint32_t hx = __float_as_uint(v.x) & 0xffffe000u, hy = __float_as_uint(v.y) & 0xffffe000u;
+          const uint32_t hz = __float_as_uint(v.z) & 0xffffe000u, hw = __float_as_uint(v.w) & 0xffffe000u;
+          st_shared_v4(tile_hi + off, hx, hy, hz, hw);
+          st_shared_v4(tile_hi + kAtomBytes + off,
+                       __float_as_uint(v.x - __uint_as_float(hx)), __float_as_uint(v.y - __uint_as_float(hy)),
+                       __float_as_uint(v.z - __uint_as_float(hz)), __float_as_uint(v.w - __uint_as_float(hw)));
+        } else {                             // 4 floats -> 4 bf16 = 8 bytes at k-byte offset 8*jl
+          const uint32_t off = r * 128 + (((jl >> 1) ^ (r & 7)) << 4) + ((jl & 1) << 3);
+          if constexpr (P == 2) {
+            uint32_t h0, l0, h1, l1;
+            split_bf16x2(v.x, v.y, h0, l0);
+            split_bf16x2(v.z, v.w, h1, l1);
+            st_shared_v2(tile_hi + off, h0, h1);
+            st_shared_v2(tile_hi + kAtomBytes + off, l0, l1);
+          } else {
+            st_shared_v2(tile_hi + off, pack_bf16x2(v.x, v.y), pack_bf16x2(v.z, v.w));
+          }
+        }
+      }
+    };
+    auto wait_entry = [&](uint32_t cnt) {
+      const long long tg0 = gdbg ? clock64() : 0;
+      mbar_wait_warp(smem_u32(&bars->a_empty[cnt % NSA]), ((cnt / NSA) & 1) ^ 1, lane);
+      if (gdbg) g_wait += clock64() - tg0;
     };
 
+    if (total_groups > 0) {
 #pragma unroll
-    for (int d = 0; d < D; ++d)
-      if (d < total_chunks) load_chunk(buf[d]);
-    for (int ci0 = 0; ci0 < total_chunks; ci0 += D) {
+      for (int d = 0; d < D; ++d) load_unit(buf[d]);
+    }
+    uint32_t ecnt = 0;                         // ring entries produced so far (the MMA warp counts the same)
+    int gi = 0;                                // group of D units inside the tile
+    for (int g = 0; g < total_groups; ++g) {
+      const bool more = g + 1 < total_groups;
+      if (gi < n_addg) {
+        // ---- addend group: 64 fp32 columns of add[0][idx0[row]] + add[1][idx1[row]] as two 16 KB tiles in
+        // the operand layout (tcgen05.cp moves them into the accumulator, see the MMA warp).  P == 2:
+        // both tiles in one ring entry; P == 1 (16 KB entries): two consecutive entries.
+        constexpr int ENT = (P == 2) ? 1 : 2;
+        wait_entry(ecnt);
+        if constexpr (ENT == 2) wait_entry(ecnt + 1);
+        GP_T0();
 #pragma unroll
-      for (int d = 0; d < D; ++d) {
-        const int ci = ci0 + d;
-        if (ci < total_chunks) {
-          const uint32_t slot = ci % NSA, n = ci / NSA;
-          long long tg0 = gdbg ? clock64() : 0;
-          mbar_wait_warp(smem_u32(&bars->a_empty[slot]), (n & 1) ^ 1, lane);
-          if (gdbg) g_wait += clock64() - tg0;
+        for (int p = 0; p < NPASS; ++p) {
+          const int r = r0 + p * RPP;
+          if constexpr (LPR == 8) {            // unit = 32 columns: (buf0 + buf1) -> tile 0, (buf2 + buf3) -> tile 1
+            const uint32_t dst0 = aring + (ecnt % NSA) * kStageBytes + r * 128 + ((jl ^ (r & 7)) << 4);
+            const float4 x = buf[0][p], y = buf[1][p], z = buf[D - 2][p], w = buf[D - 1][p];
+            st_shared_v4(dst0, __float_as_uint(x.x + y.x), __float_as_uint(x.y + y.y), __float_as_uint(x.z + y.z), __float_as_uint(x.w + y.w));
+            st_shared_v4(dst0 + kAtomBytes, __float_as_uint(z.x + w.x), __float_as_uint(z.y + w.y), __float_as_uint(z.z + w.z), __float_as_uint(z.w + w.w));
+          } else {                             // unit = 64 columns: lanes 0-7 of a row -> tile 0, lanes 8-15 -> tile 1
+            const uint32_t tsel = jl >> 3;
+            const uint32_t tbase = (P == 2) ? aring + (ecnt % NSA) * kStageBytes + tsel * kAtomBytes
+                                            : aring + ((ecnt + tsel) % NSA) * kStageBytes;
+            const float4 x = buf[0][p], y = buf[1][p];
+            st_shared_v4(tbase + r * 128 + (((jl & 7) ^ (r & 7)) << 4),
+                         __float_as_uint(x.x + y.x), __float_as_uint(x.y + y.y), __float_as_uint(x.z + y.z), __float_as_uint(x.w + y.w));
+          }
+        }
+        GP_ACC(1);
+        // Hand-off without a release arrive or a proxy fence in THESE warps (either would wait for their
+        // in-flight prefetch loads): bar.arrive on the entry's named barrier; the commit warp completes that
+        // barrier, fences and arrives on a_full (see below).
+        named_bar_arrive(kBarEntry0 + ecnt % NSA, kGatherThreads + 32);
+        if constexpr (ENT == 2) named_bar_arrive(kBarEntry0 + (ecnt + 1) % NSA, kGatherThreads + 32);
+        ecnt += ENT;
+        GP_ACC(2);
+        if (more) {
+#pragma unroll
+          for (int d = 0; d < D; ++d) load_unit(buf[d]);
+        }
+        GP_ACC(3);
+      } else {
+#pragma unroll
+        for (int d = 0; d < D; ++d) {
+          wait_entry(ecnt);
           GP_T0();
-          {   // timing aid: force the prefetched registers of this chunk to be resident before the store phase
-            float sdep = 0.f;
-#pragma unroll
-            for (int p = 0; p < NPASS; ++p) sdep += buf[d][p].x;
-            if (gdbg && sdep == 1.2345e30f) g_wait += 1;
-          }
-          GP_ACC(0);
-          const uint32_t tile_hi = aring + slot * kStageBytes;
-#pragma unroll
-          for (int p = 0; p < NPASS; ++p) {
-            const int r = r0 + p * RPP;
-            const float4 v = buf[d][p];
-            if constexpr (MODE == ETX_PREC_TF32X3) {
-              const uint32_t off = r * 128 + ((jl ^ (r & 7)) << 4);
-              const uint32_t hx = __float_as_uint(v.x) & 0xffffe000u, hy = __float_as_uint(v.y) & 0xffffe000u;
-              const uint32_t hz = __float_as_uint(v.z) & 0xffffe000u, hw = __float_as_uint(v.w) & 0xffffe000u;
-              st_shared_v4(tile_hi + off, hx, hy, hz, hw);
-              st_shared_v4(tile_hi + kAtomBytes + off,
-                           __float_as_uint(v.x - __uint_as_float(hx)), __float_as_uint(v.y - __uint_as_float(hy)),
-                           __float_as_uint(v.z - __uint_as_float(hz)), __float_as_uint(v.w - __uint_as_float(hw)));
-            } else {                             // 4 floats -> 4 bf16 = 8 bytes at k-byte offset 8*jl
-              const uint32_t off = r * 128 + (((jl >> 1) ^ (r & 7)) << 4) + ((jl & 1) << 3);
-              if constexpr (P == 2) {
-                uint32_t h0, l0, h1, l1;
-                split_bf16x2(v.x, v.y, h0, l0);
-                split_bf16x2(v.z, v.w, h1, l1);
-                st_shared_v2(tile_hi + off, h0, h1);
-                st_shared_v2(tile_hi + kAtomBytes + off, l0, l1);
-              } else {
-                st_shared_v2(tile_hi + off, pack_bf16x2(v.x, v.y), pack_bf16x2(v.z, v.w));
-              }
-            }
-          }
+          store_operand(buf[d], ecnt % NSA);
           GP_ACC(1);
-          fence_async_smem();                    // generic-proxy writes -> visible to the tensor core (async proxy)
-          mbar_arrive_warp(smem_u32(&bars->a_full[slot]), lane);
+          named_bar_arrive(kBarEntry0 + ecnt % NSA, kGatherThreads + 32);
+          ++ecnt;
           GP_ACC(2);
-          if (ci + D < total_chunks) load_chunk(buf[d]);
+          if (more) load_unit(buf[d]);
           GP_ACC(3);
         }
       }
+      if (++gi == n_units / D) gi = 0;
     }
     if (gdbg && t == 0) {
       a.dbg[(size_t)blockIdx.x * 32 + 8] = (unsigned long long)g_wait;
@@ -304,12 +394,19 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
 #define EP_T0() if (edbg) tp = clock64()
 #define EP_ACC(i) if (edbg) { const long long tn = clock64(); ep[i] += tn - tp; tp = tn; }
     const long long e_start = edbg ? clock64() : 0;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-      for (int l = 0; l < n_gemm; ++l, ++g) {
-        const uint32_t b = g & 1;
+    uint32_t uacc[2] = {0, 0};                   // jobs seen per accumulator (mbarrier phase)
+    for (int pi = 0; pi < n_pairs; ++pi) {
+      const int ns = (my_tiles - pi * NSLOT) < NSLOT ? (my_tiles - pi * NSLOT) : NSLOT;
+      for (int l = 0; l < n_gemm; ++l)
+      for (int sl = 0; sl < ns; ++sl, ++g) {
+        const uint32_t b = (NSLOT == 2) ? (uint32_t)sl : (g & 1);
+        const int tile = blockIdx.x + (pi * NSLOT + sl) * gridDim.x;
+        const uint32_t hid = lane_addr + COL_HID + (NSLOT == 2 ? sl * HIDW : 0);
+        uint64_t* hid_ready = bars->hid_ready + (NSLOT == 2 ? sl * 4 : 0);
         const float* bias = bias_s + l * HW;
         long long te0 = edbg ? clock64() : 0;
-        mbar_wait_warp(smem_u32(&bars->acc_full[b]), (g >> 1) & 1, lane);
+        mbar_wait_warp(smem_u32(&bars->acc_full[b]), uacc[b] & 1, lane);
+        ++uacc[b];
         if (edbg) e_wait += clock64() - te0;
         tc_fence_after();
         const uint32_t acc = lane_addr + COL_ACC + b * 128;
@@ -330,8 +427,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
                 w[i] = __float_as_uint(x) & 0xffffe000u;
                 v[i] = __float_as_uint(x - __uint_as_float(w[i]));
               }
-              tmem_st32(lane_addr + COL_HID + c * 32, w);
-              tmem_st32(lane_addr + COL_HID + HID_COLS + c * 32, v);
+              tmem_st32(hid + c * 32, w);
+              tmem_st32(hid + HID_COLS + c * 32, v);
             } else if constexpr (P == 2) {       // BF16X3: 64 accumulator columns -> 32 hi + 32 lo packed columns
               uint32_t v0[32], wh[32], wl[32];
               tmem_ld32(acc + c * 64, v0);
@@ -347,8 +444,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
               for (int i = 0; i < 16; ++i)
                 split_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
                              fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f), wh[16 + i], wl[16 + i]);
-              tmem_st32(lane_addr + COL_HID + c * 32, wh);
-              tmem_st32(lane_addr + COL_HID + HID_COLS + c * 32, wl);
+              tmem_st32(hid + c * 32, wh);
+              tmem_st32(hid + HID_COLS + c * 32, wl);
             } else {
               uint32_t v0[32], w[32];
               tmem_ld32(acc + c * 64, v0);
@@ -364,15 +461,16 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
               for (int i = 0; i < 16; ++i)
                 w[16 + i] = pack_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
                                         fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f));
-              tmem_st32(lane_addr + COL_HID + c * 32, w);
+              tmem_st32(hid + c * 32, w);
             }
             EP_ACC(1);
             tc_wait_st();
             tc_fence_before();
-            mbar_arrive_warp(smem_u32(&bars->hid_ready[c]), lane);
+            mbar_arrive_relaxed_warp(smem_u32(&hid_ready[c]), lane);
             EP_ACC(2);
           }
-          mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane);
+          tc_fence_before();
+          mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
         } else if (a.out_mode == 3) {
           // ---- classifier: last hidden layer, then 1 unit + sigmoid; column half 0
           // warps do all 128 columns of their rows (a cross-warp sum is not worth it for 1 unit).
@@ -388,12 +486,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
                 logit = fmaf(fmaxf(__uint_as_float(v[i]) + bias[q * 32 + i], 0.f), wlast_s[q * 32 + i], logit);
             }
             tc_fence_before();
-            mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane);
+            mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
             logit += __ldg(a.bias[a.n_layers - 1]);
             const int row = tile * TM + et;
             if (row < a.n_rows) a.out[row] = 1.0f / (1.0f + expf(-logit));
           } else {
-            mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane);
+            mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
           }
         } else {
           // ---- linear output (+ residual).  Each warp transposes 16 columns of its own 32 rows at a
@@ -417,7 +515,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
                 : "r"(acc + col0) : "memory");
             tc_wait_ld();
             EP_ACC(3);
-            if (q == 3) { tc_fence_before(); mbar_arrive_warp(smem_u32(&bars->acc_free[b]), lane); }
+            if (q == 3) { tc_fence_before(); mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane); }
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
               const float4 bq = *reinterpret_cast<const float4*>(bias + col0 + 4 * j);
@@ -457,8 +555,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
     if (lane == 0) {
       const int chunks_per_tile = nc1 + (n_gemm - 1) * HCH;
       uint32_t w_cnt = 0;
-      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        for (int q = 0; q < chunks_per_tile; ++q, ++w_cnt) {
+      for (int pi = 0; pi < n_pairs; ++pi) {        // per tile pair: a shared stage serves both tiles before its release
+        const int ns = (my_tiles - pi * NSLOT) < NSLOT ? (my_tiles - pi * NSLOT) : NSLOT;
+        const int rep1 = share1 ? 1 : ns;           // an unshared first layer is streamed once per tile
+        for (int qq = 0; qq < chunks_per_tile + (rep1 - 1) * nc1; ++qq, ++w_cnt) {
+          const int q = qq < rep1 * nc1 ? qq % (nc1 > 0 ? nc1 : 1) : qq - (rep1 - 1) * nc1;
           const uint32_t ws = w_cnt % NSW, wn = w_cnt / NSW;
           mbar_wait(smem_u32(&bars->w_empty[ws]), (wn & 1) ^ 1);
           if (a.exp_flags & 2) { mbar_arrive(smem_u32(&bars->w_full[ws])); continue; }
@@ -467,28 +568,76 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
         }
       }
     }
+  } else if (warp == kWarpCommit) {
+    // =========================== operand-ring commit warp ===========================
+    // Completes, entry by entry, the named barrier the 16 gather warps bar.arrive on after their
+    // st.shared, then makes those generic-proxy writes visible to the tensor core (fence.proxy.async)
+    // and arrives on the entry's a_full mbarrier.  This warp has no memory traffic of its own, so the
+    // release + fence cost nothing; in the gather warps they cost a global-load latency per entry.
+    reg_dec<kRegCtl>();
+    const int ent_per_tile = (a.n_add ? ((P == 2) ? 2 : 4) : 0) + nc1;
+    const uint32_t total = (uint32_t)my_tiles * (uint32_t)ent_per_tile;
+    for (uint32_t cnt = 0; cnt < total; ++cnt) {
+      named_bar_sync(kBarEntry0 + cnt % NSA, kGatherThreads + 32);
+      fence_async_smem();
+      if (lane == 0) mbar_arrive(smem_u32(&bars->a_full[cnt % NSA]));
+      __syncwarp();
+    }
   } else if (warp > kWarpMma) {
-    reg_dec<kRegCtl>();                          // idle warps that complete the control warpgroup
+    reg_dec<kRegCtl>();                          // idle warp that completes the control warpgroup
   } else {
     // =========================== MMA issuer ===========================
     reg_dec<kRegCtl>();
     // Warp-uniform control flow: every lane waits on the barriers, one elected lane issues.  (Issuing
     // from a divergent `if (lane == 0)` region makes ptxas wrap every UTCHMMA in an election loop,
     // which left the tensor pipe idle half of the time.)
-    uint32_t w_cnt = 0, a_cnt = 0, g = 0, hcount = 0;
+    uint32_t w_cnt = 0, a_cnt = 0, g = 0;
     long long dt[6] = {0, 0, 0, 0, 0, 0};
     const bool dbg = ETX_DBG(a);
     long long t_start = dbg ? clock64() : 0, t0 = 0;
 #define DBG_T0() if (dbg) t0 = clock64()
 #define DBG_ACC(i) if (dbg) dt[i] += clock64() - t0
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-      for (int l = 0; l < n_gemm; ++l, ++g) {
-        const uint32_t b = g & 1, u = g >> 1;
+    uint32_t uacc[2] = {0, 0}, uhid[2] = {0, 0};  // jobs issued per accumulator / per hidden region (mbarrier phases)
+    for (int pi = 0; pi < n_pairs; ++pi) {
+      const int ns = (my_tiles - pi * NSLOT) < NSLOT ? (my_tiles - pi * NSLOT) : NSLOT;
+      for (int l = 0; l < n_gemm; ++l) {
+       const int nch = (l == 0) ? nc1 : HCH;
+       // The tiles of a pair share the weight stages of a layer when the whole layer fits in half the
+       // ring (every hidden layer; a first layer of <= NSW/2 chunks); otherwise the loader streams the
+       // layer once per tile.
+       const bool shared_w = (l > 0) || share1;
+       const uint32_t w_cnt0 = w_cnt;              // first weight stage of this layer
+       for (int sl = 0; sl < ns; ++sl, ++g) {
+        const uint32_t b = (NSLOT == 2) ? (uint32_t)sl : (g & 1);
+        const uint32_t hs = (NSLOT == 2) ? (uint32_t)sl : 0u;
+        if (shared_w) w_cnt = w_cnt0;
         DBG_T0();
-        if (u >= 1) mbar_wait(smem_u32(&bars->acc_free[b]), (u - 1) & 1);   // epilogue done with acc[b]
+        if (uacc[b] >= 1) mbar_wait(smem_u32(&bars->acc_free[b]), (uacc[b] - 1) & 1);   // epilogue done with acc[b]
         DBG_ACC(0);
         const uint32_t d_tmem = tmem + COL_ACC + b * 128;
-        const int nch = (l == 0) ? nc1 : HCH;
+        if (l == 0 && a.n_add) {
+          // addend tiles -> accumulator (tcgen05.cp, ordered before the MMAs issued below)
+          constexpr int NENT = (P == 2) ? 2 : 4, TPE = (P == 2) ? 2 : 1;     // ring entries per tile, 16 KB tiles per entry
+          for (int en = 0; en < NENT; ++en, ++a_cnt) {
+            const uint32_t slot = a_cnt % NSA;
+            DBG_T0();
+            mbar_wait(smem_u32(&bars->a_full[slot]), (a_cnt / NSA) & 1);
+            DBG_ACC(1);
+            fence_async_smem();                  // gather warps' st.shared (generic proxy) -> tcgen05.cp (async proxy)
+            tc_fence_after();
+            if (elect_one()) {
+#pragma unroll
+              for (int t = 0; t < TPE; ++t) {
+                const uint64_t sd = smem_desc(aring + slot * kStageBytes + t * kAtomBytes);
+#pragma unroll
+                for (int ks = 0; ks < 4; ++ks) tmem_cp_128x256b(d_tmem + (en * TPE + t) * 32 + ks * 8, sd + ks * 2);
+              }
+              tc_commit(smem_u32(&bars->a_empty[slot]));
+              if (nch == 0 && en == NENT - 1) tc_commit(smem_u32(&bars->acc_full[b]));
+            }
+            __syncwarp();
+          }
+        }
         for (int c = 0; c < nch; ++c, ++w_cnt) {
           const uint32_t ws = w_cnt % NSW, wn = w_cnt / NSW;
           uint32_t slot = 0;
@@ -496,19 +645,25 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
           if (l == 0) {
             slot = a_cnt % NSA;
             mbar_wait(smem_u32(&bars->a_full[slot]), (a_cnt / NSA) & 1);
+            // The proxy fence that makes the gather warps' st.shared (generic proxy) visible to the
+            // tensor core (async proxy) sits HERE, on the consumer side of the mbarrier: the writes are
+            // ordered before it by the barrier's release/acquire, and it precedes the MMAs in program
+            // order.  Executed by the writers it would also wait for their in-flight prefetch loads
+            // (measured: ~1.2k cycles per K-chunk, the whole global-load latency, on every chunk).
+            fence_async_smem();
             DBG_ACC(1);
           } else {
-            mbar_wait(smem_u32(&bars->hid_ready[c]), hcount & 1);
+            mbar_wait(smem_u32(&bars->hid_ready[hs * 4 + c]), uhid[hs] & 1);
             DBG_ACC(2);
           }
           DBG_T0();
-          mbar_wait(smem_u32(&bars->w_full[ws]), wn & 1);
+          if (!shared_w || sl == 0) mbar_wait(smem_u32(&bars->w_full[ws]), wn & 1);   // shared: the pair's second tile finds it already there
           DBG_ACC(3);
           tc_fence_after();
           DBG_T0();
           if (elect_one()) {
             const uint64_t wd = smem_desc(wring + ws * kStageBytes);          // weight tile (hi piece)
-            const uint32_t accum0 = c > 0 ? 1u : 0u;
+            const uint32_t accum0 = (c > 0 || (l == 0 && a.n_add)) ? 1u : 0u;
             if (l == 0) {
               const uint64_t ad = smem_desc(aring + slot * kStageBytes);      // gathered operand tile (hi piece)
 #pragma unroll
@@ -523,7 +678,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
                 }
               }
             } else {
-              const uint32_t at = tmem + COL_HID + c * 32;
+              const uint32_t at = tmem + COL_HID + hs * HIDW + c * 32;
 #pragma unroll
               for (int ks = 0; ks < 4; ++ks) {
                 const uint32_t accum = ks > 0 ? 1u : accum0;
@@ -536,7 +691,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
                 }
               }
             }
-            tc_commit(smem_u32(&bars->w_empty[ws]));
+            if (!shared_w || sl == ns - 1) tc_commit(smem_u32(&bars->w_empty[ws]));
             if (l == 0) tc_commit(smem_u32(&bars->a_empty[slot]));
             if (c == nch - 1) tc_commit(smem_u32(&bars->acc_full[b]));
           }
@@ -544,7 +699,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
           DBG_ACC(4);
           if (l == 0) ++a_cnt;
         }
-        if (l > 0) ++hcount;
+        ++uacc[b];
+        if (l > 0) ++uhid[hs];
+       }
+       if (shared_w) w_cnt = w_cnt0 + nch;
       }
     }
     if (dbg && lane == 0) {

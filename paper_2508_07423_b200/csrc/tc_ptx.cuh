@@ -59,7 +59,25 @@ __device__ __forceinline__ void mbar_arrive_warp(uint32_t bar, int lane) {
   __syncwarp();
   if (lane == 0) mbar_arrive(bar);
 }
-__device__ __forceinline__ void epi_bar_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }   // epilogue warps only
+// Arrival WITHOUT release semantics.  A default (.release) arrive makes ptxas emit MEMBAR.ALL.CTA, which
+// waits for every outstanding memory operation of the warp -- the gather warps' in-flight prefetch loads,
+// the epilogue warps' fire-and-forget red.global.add -- i.e. a full global round trip per arrival.  Use
+// only where the hand-off does not go through generic-proxy memory: TMEM hand-offs are ordered by
+// tcgen05.wait::ld/st + tcgen05.fence::before_thread_sync.
+__device__ __forceinline__ void mbar_arrive_relaxed(uint32_t bar) {
+  asm volatile("mbarrier.arrive.relaxed.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_relaxed_warp(uint32_t bar, int lane) {
+  __syncwarp();
+  if (lane == 0) mbar_arrive_relaxed(bar);
+}
+// Named barriers (bar.arrive does not block and does not wait for the caller's outstanding global loads).
+__device__ __forceinline__ void named_bar_arrive(uint32_t id, uint32_t count) {
+  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t count) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
+}
 
 // 32 lanes x 32 consecutive columns: thread i of the warp owns lane (base + i)
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
