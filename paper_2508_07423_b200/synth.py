@@ -129,20 +129,22 @@ class Config:
 
 
 CONFIGS: Dict[str, Config] = {
-    # gains (Q14) chosen with the oracle so that scores spread over ~0.3..0.8 without saturating and
-    # bf16-operand error stays ~2.5x inside BASELINE.json's 2e-2
+    # gains (Q14) chosen so that scores do not saturate and the score tolerances of BASELINE.json hold for
+    # EVERY edge of the full 1000-event batches, not only on sampled events (DESIGN.md "Input recipe":
+    # at gain 0.5 the bf16 mode reached 4.7e-2 on the worst of C3's 9.6 M edges, at 0.4 it stays <= 1.3e-2)
     "c0": Config("c0", 0, 1, 20, False, 0.05, (3, 64, 64, 4), 64, 2, 4, 6.0, gain=0.8, calib_events=1),
-    # precision = the library mode bench.py uses for the config: BASELINE.json's "fp32" configs run the
-    # fp32-equivalent 3xTF32 tensor-core mode (tcgen05 has no fp32 MMA);
-    # the exact-FFMA mode (PREC_FP32) is tested on every config and is what C0 (H = 64) uses.
-    "c1": Config("c1", 1, 1, 150, False, 0.05, (3, 128, 128, 128, 4), 128, 2, 6, 6.0, gain=0.5,
-                 calib_events=1, precision=PREC_TF32X3),
-    "c2": Config("c2", 2, 1000, 150, True, 0.05, (3, 128, 128, 128, 4), 128, 2, 6, 6.0, gain=0.5,
-                 precision=PREC_TF32X3),
-    "c3": Config("c3", 2, 1000, 150, True, 0.05, (3, 128, 128, 128, 4), 128, 2, 6, 6.0, gain=0.5,
+    # precision = the library mode bench.py uses for the config: BASELINE.json's "fp32" configs run an
+    # fp32-equivalent split tensor-core mode (tcgen05 has no fp32 MMA):
+    # bf16 hi/lo split, three MMAs.  The exact-FFMA mode (PREC_FP32) is tested on every config and is what
+    # C0 (H = 64) uses; the 3xTF32 mode is tested on every H = 128 config as well.
+    "c1": Config("c1", 1, 1, 150, False, 0.05, (3, 128, 128, 128, 4), 128, 2, 6, 6.0, gain=0.4,
+                 calib_events=1, precision=PREC_BF16X3),
+    "c2": Config("c2", 2, 1000, 150, True, 0.05, (3, 128, 128, 128, 4), 128, 2, 6, 6.0, gain=0.4,
+                 precision=PREC_BF16X3),
+    "c3": Config("c3", 2, 1000, 150, True, 0.05, (3, 128, 128, 128, 4), 128, 2, 6, 6.0, gain=0.4,
                  precision=PREC_BF16),
-    "c4": Config("c4", 4, 1000, 300, True, 0.10, (3, 128, 128, 128, 4), 128, 2, 8, 10.0, gain=0.3,
-                 precision=PREC_TF32X3),
+    "c4": Config("c4", 4, 1000, 300, True, 0.10, (3, 128, 128, 128, 4), 128, 2, 8, 10.0, gain=0.25,
+                 precision=PREC_BF16X3),
 }
 
 _P_EVENTS, _P_WEIGHTS = 1, 2
