@@ -99,6 +99,7 @@ struct MlpArgs {
   // addend: the first layer's pre-activation starts from add[0][idx0[row]] + add[1][idx1[row]]
   // (128 columns each) instead of zero (tensor-core path only; n_add is 0 or 2)
   int n_add = 0; Segment add[2];
+  int wide = 0;               // tensor-core path: one layer with 256 outputs (weight image = two 128-output images back to back)
   DevMlp mlp;
   // output: mode 0 store, 1 residual add (out = res + y; res may alias out), 2 small-N linear,
   // 3 small-N sigmoid
@@ -112,6 +113,7 @@ struct TcArgs {
   int n_seg = 0; Segment seg[3]; int K0 = 0;      // first-layer input: gathered segments, K0 = sum of widths (may be 0 with an addend)
   int n_add = 0; Segment add[2];                  // 0 or 2 addend sources: layer-1 accumulator starts from their sum
   int n_layers = 0;
+  int wide = 0;                                   // one layer, two 128-column output halves per row tile (bf16 modes)
   const unsigned char* wimg = nullptr;            // weight image: swizzled 16 KB tiles in consumption order
   const float* bias[kMaxLayers] = {nullptr};
   const float* w_last = nullptr;                  // classifier: fp32 weights of the 1-unit output layer

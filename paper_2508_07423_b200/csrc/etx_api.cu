@@ -204,6 +204,7 @@ int run_mlp(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   for (int i = 0; i < 3; ++i) t.seg[i] = a.seg[i];
   t.n_add = a.n_add; t.add[0] = a.add[0]; t.add[1] = a.add[1];
   t.n_layers = a.mlp.n_layers;
+  t.wide = a.wide;
   t.wimg = a.mlp.wimg;
   for (int l = 0; l < a.mlp.n_layers; ++l) t.bias[l] = a.mlp.b[l];
   t.w_last = a.mlp.Wt[a.mlp.n_layers - 1];         // [H][1] == [H]
@@ -509,15 +510,19 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
   // p_l = [A h_l | B h_l] cost 4 H^2 flop per HIT instead of per EDGE; the edge kernel gathers the two
   // 128-wide rows, adds them and starts its layer-1 accumulator from the sum.
   const bool fact = c->desc.precision != ETX_PREC_FP32;
-  auto project = [&](const DevMlp& mlp) {              // p = [A h | B h], two one-layer launches over the hits
+  auto project = [&](const DevMlp& mlp) {              // p = [A h | B h] over the hits
     ProfScope ps(c, ETX_K_EDGE_PROJ, s);
-    for (int part = 0; part < 2; ++part) {
+    // bf16 modes: ONE launch, h read once, both 128-column halves (the images of A and B are adjacent);
+    // TF32X3 (one tile in flight, no second accumulator slot): one launch per half
+    const bool wide = c->desc.precision != ETX_PREC_TF32X3;
+    for (int part = 0; part < (wide ? 1 : 2); ++part) {
       MlpArgs a;
       a.n_rows = N; a.n_seg = 1;
       a.seg[0] = Segment{w.h, nullptr, H, H};
       a.mlp.n_layers = 1; a.mlp.dims[0] = H; a.mlp.dims[1] = H;
       a.mlp.wimg = part == 0 ? mlp.wimg_a : mlp.wimg_b;
       a.mlp.b[0] = c->d_zero_bias; a.mlp.Wt[0] = c->d_zero_bias;
+      a.wide = wide ? 1 : 0;
       a.out_mode = 0; a.out = w.p + part * H; a.out_ld = 2 * H;
       c->launches += run_mlp(c, a, s);
     }

@@ -35,6 +35,9 @@
 //                    kind::f16 MMAs lo.w_hi + hi.w_lo + hi.w_hi.  Half the MMA steps, shared-memory and
 //                    L2 bytes of TF32X3.  Measured score error is the same ~1e-5 as TF32X3, because both
 //                    are dominated by the tensor core's truncating fp32 accumulation.
+#include <cuda.h>
+#include <cstring>
+
 #include "common.cuh"
 #include "tc_ptx.cuh"
 
@@ -141,8 +144,8 @@ __device__ __forceinline__ void tmem_cp_128x256b(uint32_t taddr, uint64_t desc) 
   asm volatile("tcgen05.cp.cta_group::1.128x256b [%0], %1;" ::"r"(taddr), "l"(desc) : "memory");
 }
 
-template <int MODE>
-__global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
+template <int MODE, bool WIDE>
+__global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap tmap) {
   using C = Cfg<MODE>;
   constexpr int KA = C::KA, P = C::PIECES, NSW = C::NSTAGE_W, NSA = C::NSTAGE_A, HID_COLS = C::HID_COLS;
   constexpr uint32_t kStageBytes = P * kAtomBytes;
@@ -177,8 +180,15 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   const int n_gemm = (a.out_mode == 3) ? a.n_layers - 1 : a.n_layers;
   const int nc1 = a.K0 / KA;
   const int my_tiles = (n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles blockIdx.x + i * gridDim.x
-  const int n_pairs = (my_tiles + NSLOT - 1) / NSLOT;
-  const bool share1 = nc1 <= NSW;                         // first-layer weight stages shared by the tiles of a pair
+  // Wide mode (one layer, 256 outputs: the per-hit projections [A h | B h] of the factorised edge MLPs):
+  // the two slots of a "pair" are the two 128-column output halves of ONE row tile -- the operand entries
+  // are gathered once and serve both halves, each half has its own weight chunks and accumulator.
+  constexpr bool wide = WIDE;                   // (a compile-time switch: the regular kernels carry none of it)
+  static_assert(!WIDE || NSLOT == 2, "wide mode needs two accumulator slots");
+  const int n_pairs = wide ? my_tiles : (my_tiles + NSLOT - 1) / NSLOT;
+  auto slots_of = [&](int pi) { return wide ? 2 : ((my_tiles - pi * NSLOT) < NSLOT ? (my_tiles - pi * NSLOT) : NSLOT); };
+  auto tile_of = [&](int pi, int sl) { return (int)blockIdx.x + (wide ? pi : pi * NSLOT + sl) * (int)gridDim.x; };
+  const bool share1 = !wide && nc1 <= NSW;      // first-layer weight stages shared by the tiles of a pair
   // Addend (first-layer factorisation): the accumulator of layer 1 starts from
   // add[0][idx0[row]] + add[1][idx1[row]] (128 fp32 columns) instead of zero.
   const int n_addu = a.n_add ? 2 * HCH : 0;     // addend gather units per tile (two sources x 128 / KA column chunks)
@@ -400,11 +410,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
     const long long e_start = edbg ? clock64() : 0;
     uint32_t uacc[2] = {0, 0};                   // jobs seen per accumulator (mbarrier phase)
     for (int pi = 0; pi < n_pairs; ++pi) {
-      const int ns = (my_tiles - pi * NSLOT) < NSLOT ? (my_tiles - pi * NSLOT) : NSLOT;
+      const int ns = slots_of(pi);
       for (int l = 0; l < n_gemm; ++l)
       for (int sl = 0; sl < ns; ++sl, ++g) {
         const uint32_t b = (NSLOT == 2) ? (uint32_t)sl : (g & 1);
-        const int tile = blockIdx.x + (pi * NSLOT + sl) * gridDim.x;
+        const int tile = tile_of(pi, sl);
         const uint32_t hid = lane_addr + COL_HID + (NSLOT == 2 ? sl * HIDW : 0);
         uint64_t* hid_ready = bars->hid_ready + (NSLOT == 2 ? sl * 4 : 0);
         const float* bias = bias_s + l * HW;
@@ -498,14 +508,16 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
             mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
           }
         } else {
-          // ---- linear output (+ residual).  Each warp transposes 16 columns of its own 32 rows at a
-          // time through a private 2 KB swizzled staging slice (thread = row on the TMEM side, 4 lanes
-          // per row on the global side), so only __syncwarp is needed.  The residual e += y is
-          // applied by a vector red.global.add on the in-place state: one IEEE fp32 add per element,
-          // performed at L2, no residual load, deterministic (each element is touched exactly once).
+          // ---- linear output (+ residual).  Each warp moves 16 columns of its own 32 rows at a time:
+          // thread = row = TMEM lane writes its 64 bytes (+ bias) into a private 2 KB staging box laid out
+          // as the SWIZZLE_64B tensor-map box [32 rows x 16 columns], and one lane hands the box to the TMA
+          // unit -- a tensor store, or for the residual e += y a tensor REDUCE-ADD on the in-place
+          // state: one IEEE fp32 add per element, performed at L2, no residual load, deterministic (each
+          // element is touched exactly once).  No SIMT global traffic, no read-back of the staging tile,
+          // rows past n_rows are clipped by the tensor map.
           const uint32_t stg = stage_out + ew * 2048;
-          const int jl = lane & 3, r4 = lane >> 2;
           const bool in_place_add = (a.out_mode == 1);
+          const int row0 = tile * TM + q4 * 32;
 #pragma unroll 1
           for (int q = 0; q < 4; ++q) {
             const int col0 = hh * 64 + q * 16;
@@ -520,6 +532,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
             tc_wait_ld();
             EP_ACC(3);
             if (q == 3) { tc_fence_before(); mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane); }
+            if (lane == 0) bulk_wait_read0();      // the TMA unit has read the previous box out of the staging slice
+            __syncwarp();
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
               const float4 bq = *reinterpret_cast<const float4*>(bias + col0 + 4 * j);
@@ -527,27 +541,22 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
                            __float_as_uint(__uint_as_float(v[4 * j]) + bq.x), __float_as_uint(__uint_as_float(v[4 * j + 1]) + bq.y),
                            __float_as_uint(__uint_as_float(v[4 * j + 2]) + bq.z), __float_as_uint(__uint_as_float(v[4 * j + 3]) + bq.w));
             }
+            fence_async_smem();                    // generic-proxy writes -> async proxy (TMA)
             __syncwarp();
             EP_ACC(4);
-#pragma unroll
-            for (int it = 0; it < 4; ++it) {
-              const int r = r4 + 8 * it;
-              const int row = tile * TM + q4 * 32 + r;
-              if (row < a.n_rows) {
-                const float4 y = ld_shared_v4(stg + r * 64 + ((jl ^ ((r >> 1) & 3)) << 4));
-                float* dst = a.out + (size_t)row * a.out_ld + col0 + jl * 4;
-                if (in_place_add)
-                  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(y.x), "f"(y.y), "f"(y.z), "f"(y.w) : "memory");
-                else
-                  *reinterpret_cast<float4*>(dst) = y;
-              }
+            if (lane == 0) {
+              const int cg = (wide ? sl * HW : 0) + col0;
+              if (in_place_add) tma_reduce_add_2d(&tmap, stg, cg, row0);
+              else tma_store_2d(&tmap, stg, cg, row0);
+              bulk_commit();
             }
-            __syncwarp();
             EP_ACC(5);
           }
         }
       }
     }
+    if (lane == 0) bulk_wait_all();              // every output box has left the SM before the CTA retires
+    __syncwarp();
     if (edbg && ew == 0 && lane == 0) {
       a.dbg[(size_t)blockIdx.x * 32 + 6] = (unsigned long long)e_wait;
       a.dbg[(size_t)blockIdx.x * 32 + 7] = (unsigned long long)(clock64() - e_start);
@@ -560,10 +569,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
       const int chunks_per_tile = nc1 + (n_gemm - 1) * HCH;
       uint32_t w_cnt = 0;
       for (int pi = 0; pi < n_pairs; ++pi) {        // per tile pair: a shared stage serves both tiles before its release
-        const int ns = (my_tiles - pi * NSLOT) < NSLOT ? (my_tiles - pi * NSLOT) : NSLOT;
+        const int ns = slots_of(pi);
         const int rep1 = share1 ? 1 : ns;           // an unshared first layer is streamed once per tile
         for (int qq = 0; qq < chunks_per_tile + (rep1 - 1) * nc1; ++qq, ++w_cnt) {
-          const int q = qq < rep1 * nc1 ? qq % (nc1 > 0 ? nc1 : 1) : qq - (rep1 - 1) * nc1;
+          const int q = wide ? qq : (qq < rep1 * nc1 ? qq % (nc1 > 0 ? nc1 : 1) : qq - (rep1 - 1) * nc1);
           const uint32_t ws = w_cnt % NSW, wn = w_cnt / NSW;
           mbar_wait(smem_u32(&bars->w_empty[ws]), (wn & 1) ^ 1);
           if (a.exp_flags & 2) { mbar_arrive(smem_u32(&bars->w_full[ws])); continue; }
@@ -603,7 +612,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
 #define DBG_ACC(i) if (dbg) dt[i] += clock64() - t0
     uint32_t uacc[2] = {0, 0}, uhid[2] = {0, 0};  // jobs issued per accumulator / per hidden region (mbarrier phases)
     for (int pi = 0; pi < n_pairs; ++pi) {
-      const int ns = (my_tiles - pi * NSLOT) < NSLOT ? (my_tiles - pi * NSLOT) : NSLOT;
+      const int ns = slots_of(pi);
       for (int l = 0; l < n_gemm; ++l) {
        const int nch = (l == 0) ? nc1 : HCH;
        // The tiles of a pair share the weight stages of a layer when the whole layer fits in half the
@@ -615,6 +624,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
         const uint32_t b = (NSLOT == 2) ? (uint32_t)sl : (g & 1);
         const uint32_t hs = (NSLOT == 2) ? (uint32_t)sl : 0u;
         if (shared_w) w_cnt = w_cnt0;
+        if (wide && sl == 1) a_cnt -= nch;          // second output half: the same operand entries again
         DBG_T0();
         if (uacc[b] >= 1) mbar_wait(smem_u32(&bars->acc_free[b]), (uacc[b] - 1) & 1);   // epilogue done with acc[b]
         DBG_ACC(0);
@@ -696,7 +706,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
               }
             }
             if (!shared_w || sl == ns - 1) tc_commit(smem_u32(&bars->w_empty[ws]));
-            if (l == 0) tc_commit(smem_u32(&bars->a_empty[slot]));
+            if (l == 0 && (!wide || sl == 1)) tc_commit(smem_u32(&bars->a_empty[slot]));
             if (c == nch - 1) tc_commit(smem_u32(&bars->acc_full[b]));
           }
           __syncwarp();
@@ -723,19 +733,44 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a) {
   }
 }
 
-template <int MODE>
+// Tensor map of the output [n_rows][n_cols] fp32 (row stride out_ld floats) with the epilogue's box: 16 columns
+// (64 bytes, SWIZZLE_64B) x 32 rows.  cuTensorMapEncodeTiled is fetched through the runtime (no link-time
+// dependency on libcuda: the library must still load on a machine without a driver).
+bool encode_out_map(CUtensorMap* m, float* out, int n_rows, int n_cols, int out_ld) {
+  using Fn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                          const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                          CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static Fn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return reinterpret_cast<Fn>(p);
+  }();
+  if (!fn || (reinterpret_cast<uintptr_t>(out) & 15) || (out_ld & 3)) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)n_cols, (cuuint64_t)n_rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)out_ld * sizeof(float)};
+  const cuuint32_t box[2] = {16, 32}, estr[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, out, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int MODE, bool WIDE>
 int launch_mode(const TcArgs& a, int sm_count, cudaStream_t s) {
   using C = Cfg<MODE>;
   static bool configured = false;
   const size_t smem = 1024 + (size_t)(C::NSTAGE_W + C::NSTAGE_A) * C::PIECES * kAtomBytes + kAtomBytes +
                       (kMaxLayers + 1) * HW * sizeof(float) + sizeof(Bars) + 64;
   if (!configured) {
-    cudaFuncSetAttribute(mlp_tc_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(mlp_tc_kernel<MODE, WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
   const int n_tiles = (a.n_rows + TM - 1) / TM;
   const int grid = n_tiles < sm_count ? n_tiles : sm_count;
-  mlp_tc_kernel<MODE><<<grid, kThreads, smem, s>>>(a);
+  CUtensorMap tmap;
+  std::memset(&tmap, 0, sizeof(tmap));
+  if (a.out_mode != 3 && !encode_out_map(&tmap, a.out, a.n_rows, WIDE ? 2 * HW : HW, a.out_ld)) return -1;
+  mlp_tc_kernel<MODE, WIDE><<<grid, kThreads, smem, s>>>(a, tmap);
   return 1;
 }
 
@@ -747,9 +782,15 @@ int tc_chunk_k(int mode) { return mode == ETX_PREC_TF32X3 ? Cfg<ETX_PREC_TF32X3>
 // segment widths multiples of it; out_mode 0/1 needs dims[L] == 128; out_mode 3 needs dims[L] == 1.
 int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s) {
   if (a.n_rows <= 0) return 0;
-  if (mode == ETX_PREC_TF32X3) return launch_mode<ETX_PREC_TF32X3>(a, sm_count, s);
-  if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16>(a, sm_count, s);
-  if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3>(a, sm_count, s);
+  if (a.wide) {                                  // one layer, no addend, two output halves; bf16 modes only
+    if (a.n_layers != 1 || a.n_add != 0 || a.out_mode != 0) return -1;
+    if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, true>(a, sm_count, s);
+    if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, true>(a, sm_count, s);
+    return -1;
+  }
+  if (mode == ETX_PREC_TF32X3) return launch_mode<ETX_PREC_TF32X3, false>(a, sm_count, s);
+  if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, false>(a, sm_count, s);
+  if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, false>(a, sm_count, s);
   return -1;
 }
 
