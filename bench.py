@@ -299,8 +299,9 @@ def run_ours(args):
                      "events_per_s": (n_ev / (per * 1e-3)) if per > 0 else None}
         if k in fl and per > 0:
             stages[k]["tflops"] = fl[k] / (per * 1e-3) / 1e12
-    # scatter-sum algorithmic bytes: 2 reads of e + in_perm + write of m, per iteration
-    sc_bytes = cfg.n_iter * (2 * E * H * 4 + 4 * E + N * 2 * H * 4 + 8 * (N + 1))
+    # scatter-sum algorithmic bytes (e read once when both sums come from one pass -- the second
+    # use of a row is an L2 hit by construction, scatter.cu) + in_perm + write of m, per iteration
+    sc_bytes = cfg.n_iter * (E * H * 4 + 4 * E + N * 2 * H * 4 + 8 * (N + 1))
     if stages["scatter"]["ms"] > 0:
         stages["scatter"]["gbs"] = sc_bytes / (stages["scatter"]["ms"] * 1e-3) / 1e9
         stages["scatter"]["hbm_frac"] = stages["scatter"]["gbs"] / pk["hbm_gbs"]

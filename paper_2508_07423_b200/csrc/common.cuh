@@ -32,6 +32,7 @@ struct Workspace {            // carved from the caller's buffer by carve_worksp
   int32_t* hit_event = nullptr;   // [n_hits]
   int32_t* scan_tmp = nullptr;    // block sums for the device scan
   int32_t* flags = nullptr;       // [8] validation flags / counters
+  int32_t* sched = nullptr;       // [8] work counters of the dynamically scheduled kernels (scatter)
   float* h = nullptr;             // [n_hits, H]
   float* m = nullptr;             // [n_hits, 2H]
   float* p = nullptr;             // [n_hits, 2H] per-hit first-layer projections [A h | B h] (tensor-core modes)
@@ -130,6 +131,6 @@ int launch_wcc(int n_events, const int32_t* event_ptr, const int32_t* row_ptr, c
 
 // ---- scatter.cu
 int launch_scatter(int n_nodes, int H, const int32_t* row_ptr, const int32_t* in_ptr,
-                   const int32_t* in_perm, const float* e, float* m, cudaStream_t s);
+                   const int32_t* in_perm, const float* e, float* m, int32_t* counter /*device, 1 int*/, cudaStream_t s);
 
 }  // namespace etx

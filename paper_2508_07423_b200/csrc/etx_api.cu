@@ -124,6 +124,7 @@ Workspace carve(const etx_ctx* c, int32_t n_events, int32_t n_hits, int64_t cap,
   w.hit_event = (int32_t*)take(sizeof(int32_t) * (size_t)n_hits);
   w.scan_tmp = (int32_t*)take(sizeof(int32_t) * scan_tmp_ints(n_hits + 1));
   w.flags = (int32_t*)take(sizeof(int32_t) * 8);
+  w.sched = (int32_t*)take(sizeof(int32_t) * 8);
   w.h = (float*)take(sizeof(float) * (size_t)n_hits * H);
   w.m = (float*)take(sizeof(float) * (size_t)n_hits * 2 * H);
   if (c->desc.precision != ETX_PREC_FP32) w.p = (float*)take(sizeof(float) * (size_t)n_hits * 2 * H);
@@ -549,7 +550,7 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
     // a4: m = [sum out, sum in] of e^k
     {
       ProfScope ps(c, ETX_K_SCATTER, s);
-      c->launches += launch_scatter(N, H, g->d_row_ptr, g->d_in_ptr, g->d_in_perm, d_edge_enc, w.m, s);
+      c->launches += launch_scatter(N, H, g->d_row_ptr, g->d_in_ptr, g->d_in_perm, d_edge_enc, w.m, w.sched, s);
     }
     {  // a5: h += phi_k([h, m])
       MlpArgs a;
