@@ -14,9 +14,11 @@
 // linear layers, closed forms (r -> inf edge counts, zero/constant networks), invariants.
 // Track building (orc_wcc): scipy connected_components, hand-built graphs, partition invariants.
 // Whole path vs the thesis' TRAINED network: parity unpinned (no weights, data or printed outputs exist).
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
+#include <utility>
 #include <vector>
 
 extern "C" {
@@ -124,6 +126,50 @@ int64_t orc_build_graph(int32_t n_events, const int32_t* event_ptr, const uint8_
     }
   }
   if (n_border) *n_border = nb;
+  return E;
+}
+
+// ---- next row: k_max-capped rough graph, P:2290 ("a maximum of k_max edges per
+//      node is imposed ... a k_max-NN algorithm ... under a maximum squared distance") and Algorithm 1
+//      (P:2664-2672): list L of (j, d_j) over the candidates of source i, sort by d ascending, take the
+//      first k.  Candidates are the hits of planes p+1..p+G of the same event inside the radius
+//      (d^2 < r2_max, same fp32 predicate as orc_build_graph); the sort is STABLE on the fp32 d^2, so
+//      equal distances keep ascending j (reading Q2: order (d^2, then j)) -- this is also what
+//      the thesis' streaming "replace the farthest if the new hit is closer" loop retains.
+//      The kept neighbours are emitted in ascending j (edge order convention Q13).  k_max <= 0: no cap.
+int64_t orc_build_graph_kmax(int32_t n_events, const int32_t* event_ptr, const uint8_t* plane,
+                             int32_t n_planes, const float* emb, int32_t d, float r2_max, int32_t gap,
+                             int32_t k_max, int32_t* src, int32_t* dst, int64_t capacity) {
+  int64_t E = 0;
+  std::vector<std::pair<float, int32_t>> L;
+  std::vector<int32_t> keep;
+  for (int32_t ev = 0; ev < n_events; ++ev) {
+    const int32_t lo = event_ptr[ev], hi = event_ptr[ev + 1];
+    for (int32_t i = lo; i < hi; ++i) {
+      const int pi = plane[i];
+      if (pi > n_planes - 2) continue;
+      L.clear();
+      for (int32_t j = i + 1; j < hi; ++j) {
+        const int dp = (int)plane[j] - pi;
+        if (dp < 1) continue;
+        if (dp > gap) break;
+        const float d2 = d2_fp32(emb + (int64_t)i * d, emb + (int64_t)j * d, d);
+        if (d2 < r2_max) L.emplace_back(d2, j);
+      }
+      if (k_max > 0 && (int64_t)L.size() > k_max) {
+        std::stable_sort(L.begin(), L.end(),
+                         [](const std::pair<float, int32_t>& a, const std::pair<float, int32_t>& b) { return a.first < b.first; });
+        L.resize(k_max);
+      }
+      keep.clear();
+      for (const auto& q : L) keep.push_back(q.second);
+      std::sort(keep.begin(), keep.end());
+      for (int32_t j : keep) {
+        if (E < capacity) { src[E] = i; dst[E] = j; }
+        ++E;
+      }
+    }
+  }
   return E;
 }
 

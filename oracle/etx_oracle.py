@@ -37,6 +37,7 @@ def lib():
         _lib = C.CDLL(build())
         _lib.orc_build_graph.restype = C.c_int64
         _lib.orc_candidate_d2.restype = C.c_int64
+        _lib.orc_build_graph_kmax.restype = C.c_int64
     return _lib
 
 
@@ -98,6 +99,27 @@ def build_graph(event_ptr, plane, emb, r2_max: float, gap: int, n_planes: int = 
         cap = max(int(E), int(nb.value)) + 16
     if want_border:
         return src[:E].copy(), dst[:E].copy(), bp[:nb.value].copy()
+    return src[:E].copy(), dst[:E].copy()
+
+
+def build_graph_kmax(event_ptr, plane, emb, r2_max: float, gap: int, k_max: int, n_planes: int = 26):
+    """Next row (Algorithm 1): the radius graph with at most k_max out-edges per hit, the
+    k_max nearest by (d^2 fp32, then j); edges in (src asc, dst asc) order.  k_max <= 0: no cap."""
+    event_ptr = np.ascontiguousarray(event_ptr, np.int32)
+    plane = np.ascontiguousarray(plane, np.uint8)
+    emb = _f32(emb)
+    n_ev = len(event_ptr) - 1
+    cap = 1 << 16
+    while True:
+        src = np.empty(cap, np.int32)
+        dst = np.empty(cap, np.int32)
+        E = lib().orc_build_graph_kmax(C.c_int32(n_ev), _p(event_ptr, C.c_int32), _p(plane, C.c_uint8),
+                                       C.c_int32(n_planes), _p(emb, C.c_float), C.c_int32(emb.shape[1]),
+                                       C.c_float(r2_max), C.c_int32(gap), C.c_int32(k_max),
+                                       _p(src, C.c_int32), _p(dst, C.c_int32), C.c_int64(cap))
+        if E <= cap:
+            break
+        cap = int(E) + 16
     return src[:E].copy(), dst[:E].copy()
 
 
