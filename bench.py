@@ -266,6 +266,20 @@ def run_ours(args):
     next_rows = {"wcc_tracks": {"ms": wcc_ms, "events_per_s": n_ev / (wcc_ms * 1e-3), "score_min": 0.5,
                                 "components_ge3_hits": int((sizes >= 3).sum().item())}}
 
+    # next row NEXT-2: k_max-capped search (the thesis' k_max = 50, which rarely binds, and a cap that does)
+    g2 = binding.DeviceGraph(N, cap, dev)
+    for kk in (50, 4):
+        etx.etx_build_graph(db, emb, r2, gap, g2, k_max=kk)
+        barrier()
+        t0.record()
+        for _ in range(3):
+            Ek = etx.etx_build_graph(db, emb, r2, gap, g2, k_max=kk)
+        t1.record()
+        barrier()
+        kms = t0.elapsed_time(t1) / 3
+        next_rows[f"graph_kmax_{kk}"] = {"ms": kms, "events_per_s": n_ev / (kms * 1e-3), "n_edges": int(Ek)}
+    del g2
+
     # ---- end to end through the host-buffer entry point
     host = binding.pinned_host_batch(batch)
     o_src = torch.empty(cap, dtype=torch.int32).pin_memory()

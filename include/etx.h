@@ -117,8 +117,10 @@ etx_status etx_embed(etx_ctx* ctx, const etx_batch* batch, float* d_emb, void* s
 /* a2: fixed-radius search in embedding space.  Edge (i -> j) iff same event,
  * 1 <= plane(j) - plane(i) <= max_plane_gap, and d^2 < r2_max with d^2 evaluated in fp32 as
  * ((e0-f0)^2 + (e1-f1)^2) + ... left to right, each operation rounded (no FMA).  Output is the
- * unique ordered CSR (src asc, dst asc) plus the by-destination lists.  k_max must be 0 (the k_max
- * cap of P:2290 is not on this path).  Validates the batch (ETX_ERR_INVALID / ETX_ERR_UNSORTED).
+ * unique ordered CSR (src asc, dst asc) plus the by-destination lists.  k_max = 0: pure fixed
+ * radius (the hot path).  k_max > 0 (next row; Algorithm 1): at most k_max
+ * out-edges per hit, the k_max nearest by (d^2 as above, then hit index), still in ascending dst
+ * order; k_max < 0 is ETX_ERR_INVALID.  Validates the batch (ETX_ERR_INVALID / ETX_ERR_UNSORTED).
  * Synchronises the stream once to return g->n_edges; if E > edge_capacity returns ETX_ERR_CAPACITY
  * with n_edges = E and d_src/d_dst/d_in_perm untouched.                                           */
 etx_status etx_build_graph(etx_ctx* ctx, const etx_batch* batch, const float* d_emb, float r2_max,

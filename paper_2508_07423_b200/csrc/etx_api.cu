@@ -443,7 +443,7 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
   if (!c) return ETX_ERR_INVALID;
   if (etx_status st = check_batch(c, b)) return st;
   if (!g || !g->d_row_ptr || !g->d_in_ptr) return fail(c, ETX_ERR_INVALID, "graph or its offset arrays are NULL");
-  if (k_max != 0) return fail(c, ETX_ERR_INVALID, "k_max cap is not on this path (must be 0)");
+  if (k_max < 0) return fail(c, ETX_ERR_INVALID, "k_max must be >= 0 (0 = no cap)");
   if (max_plane_gap < 1) return fail(c, ETX_ERR_INVALID, "max_plane_gap must be >= 1");
   if (b->n_hits > 0 && !d_emb) return fail(c, ETX_ERR_INVALID, "d_emb is NULL");
   if (g->edge_capacity < 0 || (g->edge_capacity > 0 && (!g->d_src || !g->d_dst || !g->d_in_perm)))
@@ -460,9 +460,14 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
   {
     ProfScope ps(c, ETX_K_GRAPH, s);
     c->launches += launch_plane_index(a, w.plane_ptr, w.hit_event, w.flags, s);
-    c->launches += launch_search_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_in_ptr, s);
-    c->launches += launch_exclusive_scan(g->d_row_ptr, b->n_hits + 1, w.scan_tmp, s);
-    c->launches += launch_exclusive_scan(g->d_in_ptr, b->n_hits + 1, w.scan_tmp, s);
+    if (k_max == 0) {
+      c->launches += launch_search_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_in_ptr, s);
+      c->launches += launch_exclusive_scan(g->d_row_ptr, b->n_hits + 1, w.scan_tmp, s);
+      c->launches += launch_exclusive_scan(g->d_in_ptr, b->n_hits + 1, w.scan_tmp, s);
+    } else {                                       // next row: capped search (graph_kmax.cu)
+      c->launches += launch_kmax_count(a, k_max, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, s);
+      c->launches += launch_exclusive_scan(g->d_row_ptr, b->n_hits + 1, w.scan_tmp, s);
+    }
   }
   int32_t host[2] = {0, 0};
   cudaMemcpyAsync(&host[0], w.flags, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
@@ -475,7 +480,18 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
   if (g->n_edges > g->edge_capacity)
     return fail(c, ETX_ERR_CAPACITY, "graph needs " + std::to_string(g->n_edges) + " edges, capacity " +
                                          std::to_string(g->edge_capacity));
-  if (g->n_edges > 0) {
+  if (k_max > 0) {
+    // the by-destination lists depend on which edges survived the cap: forward fill first, then count,
+    // scan and fill the incoming side from the capped neighbour lists
+    ProfScope ps(c, ETX_K_GRAPH, s);
+    if (g->n_edges > 0)
+      c->launches += launch_kmax_fill(a, k_max, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_src, g->d_dst, s);
+    c->launches += launch_kmax_in_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_dst, g->d_in_ptr, s);
+    c->launches += launch_exclusive_scan(g->d_in_ptr, b->n_hits + 1, w.scan_tmp, s);
+    if (g->n_edges > 0)
+      c->launches += launch_kmax_in_fill(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_dst, g->d_in_ptr,
+                                         g->d_in_perm, s);
+  } else if (g->n_edges > 0) {
     ProfScope ps(c, ETX_K_GRAPH, s);
     c->launches += launch_search_fill(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_src, g->d_dst,
                                       g->d_in_ptr, g->d_in_perm, s);

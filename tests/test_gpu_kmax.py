@@ -1,0 +1,93 @@
+"""Next row: k_max-capped radius search on the GPU vs the oracle (Algorithm 1).
+Integer work from identical fp32 embeddings: every array must be bit-equal, in the same order."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import etx_oracle as orc
+from paper_2508_07423_b200 import synth
+from test_gpu_parity import check_graph_arrays
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2508_07423_b200 import binding, build
+    build.build()
+    return binding
+
+
+def gpu_graph(B, etx, batch, emb, r2, gap, k_max, cap):
+    dev = etx.device
+    db = B.DeviceBatch(batch, dev)
+    etx.ensure_workspace(db.n_events, db.n_hits, cap)
+    g = B.DeviceGraph(db.n_hits, cap, dev)
+    E = etx.etx_build_graph(db, torch.from_numpy(np.ascontiguousarray(emb, np.float32)).to(dev), r2, gap, g, k_max=k_max)
+    torch.cuda.synchronize()
+    return {"src": g.src[:E].cpu().numpy(), "dst": g.dst[:E].cpu().numpy(), "row_ptr": g.row_ptr.cpu().numpy(),
+            "in_ptr": g.in_ptr.cpu().numpy(), "in_perm": g.in_perm[:E].cpu().numpy()}
+
+
+def compare(B, etx, batch, emb, r2, gap, k_max):
+    s, d = orc.build_graph_kmax(batch["event_ptr"], batch["plane"], emb, r2, gap, k_max)
+    out = gpu_graph(B, etx, batch, emb, r2, gap, k_max, len(s) + 9)
+    check_graph_arrays(out, {"src": s, "dst": d}, len(batch["r"]))
+    return s
+
+
+def test_kmax_c1_oracle_embeddings(B, c1, c1_oracle):
+    cfg, batch, blob = c1
+    etx = B.Etx(B.make_desc(cfg, precision=0), blob)
+    emb, r2 = c1_oracle["emb"], synth.r2_max(cfg)
+    n = len(batch["r"])
+    # the calibrated radius (mean out-degree 6): caps 1..4 bind for many hits, 50 (the thesis' value) for none
+    for k in (1, 2, 4, 50):
+        s = compare(B, etx, batch, emb, r2, cfg.max_plane_gap, k)
+        assert np.bincount(s, minlength=n).max() == min(k, np.bincount(c1_oracle["src"], minlength=n).max())
+    # a radius that takes in every candidate: the thesis' k_max = 50 binds for most hits
+    s = compare(B, etx, batch, emb, 1e9, cfg.max_plane_gap, 50)
+    assert (np.bincount(s, minlength=n) == 50).mean() > 0.5
+    # cap not binding == the hot path's graph (k_max = 0), same arrays
+    out0 = gpu_graph(B, etx, batch, emb, r2, cfg.max_plane_gap, 0, len(c1_oracle["src"]) + 9)
+    outk = gpu_graph(B, etx, batch, emb, r2, cfg.max_plane_gap, 10 ** 6, len(c1_oracle["src"]) + 9)
+    for key in out0:
+        np.testing.assert_array_equal(out0[key], outk[key])
+
+
+def test_kmax_ties_multi_event_and_generic_dim(B):
+    cfg = synth.CONFIGS["c2"]
+    batch = synth.generate_events(cfg, range(100, 124))
+    blob = synth.generate_weights(cfg)
+    etx = B.Etx(B.make_desc(cfg, precision=0), blob)
+    rng = np.random.default_rng(17)
+    n = len(batch["r"])
+    # coarse lattice embeddings: many exactly equal distances -> the (d^2, then index) tie rule decides
+    emb4 = rng.integers(-3, 4, size=(n, 4)).astype(np.float32) * np.float32(0.25)
+    for gap, r2, k in ((3, 0.9, 5), (2, 0.3, 3), (3, 4.0, 50)):
+        compare(B, etx, batch, emb4, r2, gap, k)
+    # the thesis' setting: 3-d embedding, planes p+1 and p+2, d2_max = 0.9, k_max = 50 -- generic-d path
+    cfg3 = dataclasses.replace(synth.CONFIGS["c0"], emb_widths=(3, 64, 64, 3), max_plane_gap=2)
+    etx3 = B.Etx(B.make_desc(cfg3, precision=0), synth.generate_weights(cfg3))
+    emb3 = rng.normal(size=(n, 3)).astype(np.float32) * np.float32(0.5)
+    s = compare(B, etx3, batch, emb3, 0.9, 2, 50)
+    assert np.bincount(s, minlength=n).max() == 50
+
+
+def test_kmax_empty_and_capacity(B, c0):
+    cfg, batch, blob = c0
+    etx = B.Etx(B.make_desc(cfg, precision=0), blob)
+    n = len(batch["r"])
+    emb = np.random.default_rng(2).normal(size=(n, 4)).astype(np.float32)
+    out = gpu_graph(B, etx, batch, emb, 0.0, 3, 7, 16)                  # r = 0: no edges
+    assert len(out["src"]) == 0 and out["row_ptr"].max() == 0 and out["in_ptr"].max() == 0
+    s, _ = orc.build_graph_kmax(batch["event_ptr"], batch["plane"], emb, 1e9, 3, 3)
+    db = B.DeviceBatch(batch, etx.device)
+    g = B.DeviceGraph(n, len(s) - 1, etx.device)
+    with pytest.raises(B.EtxError) as ei:                              # one edge short: reported, nothing written past it
+        etx.etx_build_graph(db, torch.from_numpy(emb).to(etx.device), 1e9, 3, g, k_max=3)
+    assert ei.value.status == B.ETX_ERR_CAPACITY and g.n_edges == len(s)

@@ -189,8 +189,8 @@ def test_error_paths(B, c0):
     db = B.DeviceBatch(batch, etx.device)
     g = B.DeviceGraph(db.n_hits, 100000, etx.device)
     emb = etx.etx_embed(db)
-    with pytest.raises(B.EtxError) as ei:                         # k_max cap is not on this path
-        etx.etx_build_graph(db, emb, 1e-3, 3, g, k_max=50)
+    with pytest.raises(B.EtxError) as ei:                         # k_max: 0 = no cap, > 0 = cap (next row)
+        etx.etx_build_graph(db, emb, 1e-3, 3, g, k_max=-1)
     assert ei.value.status == B.ETX_ERR_INVALID
     fresh = make_etx(B, cfg, blob)
     with pytest.raises(B.EtxError) as ei:                         # no workspace handed over
