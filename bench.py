@@ -252,33 +252,32 @@ def run_ours(args):
     ms_step = ms / args.steps
     value = aggregate_events_per_s(world, n_ev, ms_step)
 
-    # ---- next row beyond the step (reported separately, not part of `value`): score cut + WCC tracks
-    labels = torch.empty(max(N, 1), dtype=torch.int32, device=dev)
-    etx.etx_build_tracks(db, g, scores, 0.5, labels)
-    barrier()
-    t0.record()
-    for _ in range(3):
-        etx.etx_build_tracks(db, g, scores, 0.5, labels)
-    t1.record()
-    barrier()
-    wcc_ms = t0.elapsed_time(t1) / 3
-    sizes = torch.bincount(labels[:N].long(), minlength=1)
-    next_rows = {"wcc_tracks": {"ms": wcc_ms, "events_per_s": n_ev / (wcc_ms * 1e-3), "score_min": 0.5,
-                                "components_ge3_hits": int((sizes >= 3).sum().item())}}
+    # ---- next rows beyond the step (reported separately, not part of `value`)
+    next_rows = {}
 
-    # next row NEXT-2: k_max-capped search (the thesis' k_max = 50, which rarely binds, and a cap that does)
-    g2 = binding.DeviceGraph(N, cap, dev)
-    for kk in (50, 4):
-        etx.etx_build_graph(db, emb, r2, gap, g2, k_max=kk)
+    def time3(fn):
+        fn()
         barrier()
         t0.record()
         for _ in range(3):
-            Ek = etx.etx_build_graph(db, emb, r2, gap, g2, k_max=kk)
+            r = fn()
         t1.record()
         barrier()
-        kms = t0.elapsed_time(t1) / 3
-        next_rows[f"graph_kmax_{kk}"] = {"ms": kms, "events_per_s": n_ev / (kms * 1e-3), "n_edges": int(Ek)}
-    del g2
+        return t0.elapsed_time(t1) / 3, r
+
+    if not args.no_next_rows:
+        # NEXT-1: score cut + WCC tracks
+        labels = torch.empty(max(N, 1), dtype=torch.int32, device=dev)
+        wcc_ms, _ = time3(lambda: etx.etx_build_tracks(db, g, scores, 0.5, labels))
+        sizes = torch.bincount(labels[:N].long(), minlength=1)
+        next_rows["wcc_tracks"] = {"ms": wcc_ms, "events_per_s": n_ev / (wcc_ms * 1e-3), "score_min": 0.5,
+                                   "components_ge3_hits": int((sizes >= 3).sum().item())}
+        # NEXT-2: k_max-capped search (the thesis' k_max = 50, which rarely binds, and a cap that does)
+        g2 = binding.DeviceGraph(N, cap, dev)
+        for kk in (50, 4):
+            kms, Ek = time3(lambda: etx.etx_build_graph(db, emb, r2, gap, g2, k_max=kk))
+            next_rows[f"graph_kmax_{kk}"] = {"ms": kms, "events_per_s": n_ev / (kms * 1e-3), "n_edges": int(Ek)}
+        del g2
 
     # ---- end to end through the host-buffer entry point
     host = binding.pinned_host_batch(batch)
@@ -412,6 +411,7 @@ def main():
     ap.add_argument("--events", type=int, default=0, help="events per GPU (default: the config's)")
     ap.add_argument("--precision", type=int, default=None, help="override etx_precision (0 fp32, 1 tf32x3, 2 bf16, 3 bf16x3)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-next-rows", action="store_true", help="skip the next-row timings (launch lists of the step only)")
     ap.add_argument("--tracks-mean", type=float, default=0.0,
                     help="override the config's mean tracks per event (occupancy sweep, cf. thesis Figs. 9.11-9.13)")
     args = ap.parse_args()
