@@ -123,6 +123,10 @@ struct TcArgs {
   int n_rows = 0;
   int n_seg = 0; Segment seg[3]; int K0 = 0;      // first-layer input: gathered segments, K0 = sum of widths (may be 0 with an addend)
   int n_add = 0; Segment add[2];                  // 0 or 2 addend sources: layer-1 accumulator starts from their sum
+  // feature mode (w1 != null): operand of the first tensor-core layer = ReLU(w1^T f + b1), f = (feat - fc) / fs
+  const float* feat[3] = {nullptr, nullptr, nullptr}; float fc[3] = {0, 0, 0}; float fs[3] = {1, 1, 1};
+  const float* w1 = nullptr;                      // [3][128] fp32 (k-major), the MLP's own first layer
+  const float* b1 = nullptr;                      // [128]
   int n_layers = 0;
   int wide = 0;                                   // one layer, two 128-column output halves per row tile (bf16 modes)
   const unsigned char* wimg = nullptr;            // weight image: swizzled 16 KB tiles in consumption order

@@ -196,8 +196,9 @@ struct ProfScope {
   }
 };
 
-// Precision dispatch.  MLPs with a tensor-core weight image run on tcgen05 (mlp_tc.cu); the two MLPs
-// fed by 3 raw features (embedding, node encoder) always run the fp32 FFMA kernel.
+// Precision dispatch.  MLPs with a tensor-core weight image run on tcgen05 (mlp_tc.cu).  The embedding MLP
+// always runs the exact fp32 FFMA kernel (the graph must match the oracle edge for edge); the node encoder,
+// also fed by 3 raw features, runs its first layer in the gather warps of the tensor-core kernel.
 int run_mlp(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   if (c->desc.precision == ETX_PREC_FP32 || !a.mlp.wimg) return launch_mlp_simt(a, s);
   TcArgs t;
@@ -208,6 +209,15 @@ int run_mlp(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   t.wide = a.wide;
   t.wimg = a.mlp.wimg;
   for (int l = 0; l < a.mlp.n_layers; ++l) t.bias[l] = a.mlp.b[l];
+  if (a.n_seg == 0 && a.n_add == 0) {
+    // 3 raw features in (node encoder): the MLP's first layer runs in the gather warps, the tensor-core
+    // chain is layers 2.. (the weight image starts at layer 2)
+    for (int i = 0; i < 3; ++i) { t.feat[i] = a.feat[i]; t.fc[i] = a.fc[i]; t.fs[i] = a.fs[i]; }
+    t.w1 = a.mlp.Wt[0]; t.b1 = a.mlp.b[0];
+    t.K0 = a.mlp.dims[1];
+    t.n_layers = a.mlp.n_layers - 1;
+    for (int l = 0; l + 1 < a.mlp.n_layers; ++l) t.bias[l] = a.mlp.b[l + 1];
+  }
   t.w_last = a.mlp.Wt[a.mlp.n_layers - 1];         // [H][1] == [H]
   t.out_mode = a.out_mode; t.out = a.out; t.res = a.res; t.out_ld = a.out_ld;
   static const char* expv = getenv("ETX_TC_EXP");                  // developer aid: timing experiments (wrong results)
@@ -324,6 +334,10 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
     size_t wsrc = 0;
     for (size_t i = 0; i < mlps.size(); ++i) {
       const float* w = h_weights + wsrc;
+      if (i == 1 && mlps[i].n_layers >= 2) {             // node encoder: layers 2.. (layer 1 runs in the gather warps)
+        img_off[i] = img.size();
+        append_wimg(img, mlps[i], w, 1, 0, mlps[i].n_layers, mode);
+      }
       if (i >= 2) {
         const bool is_cls = (i + 1 == mlps.size());
         const bool is_node = !is_cls && i >= 3 && ((i - 3) % 2 == 0);
@@ -353,6 +367,7 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
       m.wimg = c->d_wimg + img_off[i];
       if (img_a[i] != (size_t)-1) { m.wimg_a = c->d_wimg + img_a[i]; m.wimg_b = c->d_wimg + img_b[i]; }
     };
+    place(c->node_enc, 1);
     place(c->edge_enc, 2);
     for (int k = 0; k < desc->n_iter; ++k) { place(c->node_net[k], 3 + 2 * k); place(c->edge_net[k], 4 + 2 * k); }
     place(c->cls, mlps.size() - 1);

@@ -144,7 +144,8 @@ __device__ __forceinline__ void tmem_cp_128x256b(uint32_t taddr, uint64_t desc) 
   asm volatile("tcgen05.cp.cta_group::1.128x256b [%0], %1;" ::"r"(taddr), "l"(desc) : "memory");
 }
 
-template <int MODE, bool WIDE>
+// VAR: 0 regular, 1 wide (one layer, 256 outputs), 2 feat (first-layer operand computed from 3 raw features)
+template <int MODE, int VAR>
 __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap tmap) {
   using C = Cfg<MODE>;
   constexpr int KA = C::KA, P = C::PIECES, NSW = C::NSTAGE_W, NSA = C::NSTAGE_A, HID_COLS = C::HID_COLS;
@@ -183,8 +184,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   // Wide mode (one layer, 256 outputs: the per-hit projections [A h | B h] of the factorised edge MLPs):
   // the two slots of a "pair" are the two 128-column output halves of ONE row tile -- the operand entries
   // are gathered once and serve both halves, each half has its own weight chunks and accumulator.
-  constexpr bool wide = WIDE;                   // (a compile-time switch: the regular kernels carry none of it)
-  static_assert(!WIDE || NSLOT == 2, "wide mode needs two accumulator slots");
+  constexpr bool wide = (VAR == 1);             // (compile-time switches: the regular kernels carry none of it)
+  constexpr bool feat = (VAR == 2);
+  static_assert(!wide || NSLOT == 2, "wide mode needs two accumulator slots");
   const int n_pairs = wide ? my_tiles : (my_tiles + NSLOT - 1) / NSLOT;
   auto slots_of = [&](int pi) { return wide ? 2 : ((my_tiles - pi * NSLOT) < NSLOT ? (my_tiles - pi * NSLOT) : NSLOT); };
   auto tile_of = [&](int pi, int sl) { return (int)blockIdx.x + (wide ? pi : pi * NSLOT + sl) * (int)gridDim.x; };
@@ -267,6 +269,36 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
     int ptile = blockIdx.x, pu = 0;
     int ridx[2][NPASS], rown[NPASS];
     auto load_unit = [&](float4 (&dst)[NPASS]) {
+      if constexpr (feat) {
+        // Feature mode (node encoder): the operand of the first tensor-core layer is the output of the
+        // MLP's own first layer, ReLU(W1 f + b1) with f = the 3 normalised features of the row -- 3 FMAs per
+        // value, computed here instead of being loaded.  ridx[0..1] / rown hold the row's 3 features.
+        if (pu == 0) {
+#pragma unroll
+          for (int p = 0; p < NPASS; ++p) {
+            int row = ptile * TM + r0 + p * RPP;
+            row = row < a.n_rows ? row : a.n_rows - 1;
+            ridx[0][p] = __float_as_int(__fdiv_rn(__fsub_rn(__ldg(a.feat[0] + row), a.fc[0]), a.fs[0]));
+            ridx[1][p] = __float_as_int(__fdiv_rn(__fsub_rn(__ldg(a.feat[1] + row), a.fc[1]), a.fs[1]));
+            rown[p] = __float_as_int(__fdiv_rn(__fsub_rn(__ldg(a.feat[2] + row), a.fc[2]), a.fs[2]));
+          }
+        }
+        const int c0 = pu * KA + jl * 4;             // this thread's 4 columns of the layer-1 output
+        const float4 w0 = __ldg(reinterpret_cast<const float4*>(a.w1 + c0));
+        const float4 w1 = __ldg(reinterpret_cast<const float4*>(a.w1 + HW + c0));
+        const float4 w2 = __ldg(reinterpret_cast<const float4*>(a.w1 + 2 * HW + c0));
+        const float4 bb = __ldg(reinterpret_cast<const float4*>(a.b1 + c0));
+#pragma unroll
+        for (int p = 0; p < NPASS; ++p) {
+          const float fx = __int_as_float(ridx[0][p]), fy = __int_as_float(ridx[1][p]), fz = __int_as_float(rown[p]);
+          dst[p].x = fmaxf(fmaf(w2.x, fz, fmaf(w1.x, fy, fmaf(w0.x, fx, bb.x))), 0.f);
+          dst[p].y = fmaxf(fmaf(w2.y, fz, fmaf(w1.y, fy, fmaf(w0.y, fx, bb.y))), 0.f);
+          dst[p].z = fmaxf(fmaf(w2.z, fz, fmaf(w1.z, fy, fmaf(w0.z, fx, bb.z))), 0.f);
+          dst[p].w = fmaxf(fmaf(w2.w, fz, fmaf(w1.w, fy, fmaf(w0.w, fx, bb.w))), 0.f);
+        }
+        if (++pu == n_units) { pu = 0; ptile += gridDim.x; }
+        return;
+      }
       if (pu == 0) {
 #pragma unroll
         for (int p = 0; p < NPASS; ++p) {
@@ -755,22 +787,22 @@ bool encode_out_map(CUtensorMap* m, float* out, int n_rows, int n_cols, int out_
             CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int MODE, bool WIDE>
+template <int MODE, int VAR>
 int launch_mode(const TcArgs& a, int sm_count, cudaStream_t s) {
   using C = Cfg<MODE>;
   static bool configured = false;
   const size_t smem = 1024 + (size_t)(C::NSTAGE_W + C::NSTAGE_A) * C::PIECES * kAtomBytes + kAtomBytes +
                       (kMaxLayers + 1) * HW * sizeof(float) + sizeof(Bars) + 64;
   if (!configured) {
-    cudaFuncSetAttribute(mlp_tc_kernel<MODE, WIDE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(mlp_tc_kernel<MODE, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
   const int n_tiles = (a.n_rows + TM - 1) / TM;
   const int grid = n_tiles < sm_count ? n_tiles : sm_count;
   CUtensorMap tmap;
   std::memset(&tmap, 0, sizeof(tmap));
-  if (a.out_mode != 3 && !encode_out_map(&tmap, a.out, a.n_rows, WIDE ? 2 * HW : HW, a.out_ld)) return -1;
-  mlp_tc_kernel<MODE, WIDE><<<grid, kThreads, smem, s>>>(a, tmap);
+  if (a.out_mode != 3 && !encode_out_map(&tmap, a.out, a.n_rows, VAR == 1 ? 2 * HW : HW, a.out_ld)) return -1;
+  mlp_tc_kernel<MODE, VAR><<<grid, kThreads, smem, s>>>(a, tmap);
   return 1;
 }
 
@@ -784,13 +816,20 @@ int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s) {
   if (a.n_rows <= 0) return 0;
   if (a.wide) {                                  // one layer, no addend, two output halves; bf16 modes only
     if (a.n_layers != 1 || a.n_add != 0 || a.out_mode != 0) return -1;
-    if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, true>(a, sm_count, s);
-    if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, true>(a, sm_count, s);
+    if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, 1>(a, sm_count, s);
+    if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, 1>(a, sm_count, s);
     return -1;
   }
-  if (mode == ETX_PREC_TF32X3) return launch_mode<ETX_PREC_TF32X3, false>(a, sm_count, s);
-  if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, false>(a, sm_count, s);
-  if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, false>(a, sm_count, s);
+  if (a.w1) {                                    // first-layer operand computed from 3 features (node encoder)
+    if (a.n_add != 0 || a.n_seg != 0 || a.K0 != HW || !a.b1 || !a.feat[0] || !a.feat[1] || !a.feat[2]) return -1;
+    if (mode == ETX_PREC_TF32X3) return launch_mode<ETX_PREC_TF32X3, 2>(a, sm_count, s);
+    if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, 2>(a, sm_count, s);
+    if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, 2>(a, sm_count, s);
+    return -1;
+  }
+  if (mode == ETX_PREC_TF32X3) return launch_mode<ETX_PREC_TF32X3, 0>(a, sm_count, s);
+  if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, 0>(a, sm_count, s);
+  if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, 0>(a, sm_count, s);
   return -1;
 }
 
