@@ -30,6 +30,7 @@ struct DevMlp {
 struct Workspace {            // carved from the caller's buffer by carve_workspace()
   int32_t* plane_ptr = nullptr;   // [n_events * (n_planes+1)]
   int32_t* hit_event = nullptr;   // [n_hits]
+  int32_t* cursor = nullptr;      // [n_hits] per-destination fill cursors of the graph build
   int32_t* scan_tmp = nullptr;    // block sums for the device scan
   int32_t* flags = nullptr;       // [8] validation flags / counters
   int32_t* sched = nullptr;       // [8] work counters of the dynamically scheduled kernels (scatter)
@@ -85,7 +86,7 @@ int launch_search_count(const GraphArgs& a, const int32_t* plane_ptr, const int3
 int launch_exclusive_scan(int32_t* data /*[n+1], in place, data[n] = total*/, int n, int32_t* tmp, cudaStream_t s);
 int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
                        const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst,
-                       const int32_t* in_ptr, int32_t* in_perm, cudaStream_t s);
+                       const int32_t* in_ptr, int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/, cudaStream_t s);
 size_t scan_tmp_ints(int n);
 // ---- graph_kmax.cu (next row: k_max-capped search)
 int launch_kmax_count(const GraphArgs& a, int k_max, const int32_t* plane_ptr, const int32_t* hit_event,

@@ -122,6 +122,7 @@ Workspace carve(const etx_ctx* c, int32_t n_events, int32_t n_hits, int64_t cap,
   const int L = c->desc.n_planes, H = c->desc.gnn_hidden, d = c->desc.emb_dims[c->desc.emb_n_layers];
   w.plane_ptr = (int32_t*)take(sizeof(int32_t) * (size_t)n_events * (L + 1));
   w.hit_event = (int32_t*)take(sizeof(int32_t) * (size_t)n_hits);
+  w.cursor = (int32_t*)take(sizeof(int32_t) * (size_t)n_hits);
   w.scan_tmp = (int32_t*)take(sizeof(int32_t) * scan_tmp_ints(n_hits + 1));
   w.flags = (int32_t*)take(sizeof(int32_t) * 8);
   w.sched = (int32_t*)take(sizeof(int32_t) * 8);
@@ -509,7 +510,7 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
   } else if (g->n_edges > 0) {
     ProfScope ps(c, ETX_K_GRAPH, s);
     c->launches += launch_search_fill(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_src, g->d_dst,
-                                      g->d_in_ptr, g->d_in_perm, s);
+                                      g->d_in_ptr, g->d_in_perm, w.cursor, s);
   }
   return check_cuda(c, "etx_build_graph (fill)");
 }

@@ -5,9 +5,10 @@
 // range of planes p+1..p+G of the same event (hits are plane-sorted, per-(event, plane) offsets are
 // the buckets), so loads are coalesced float4 reads that stay in L1/L2 (an event's embeddings are
 // ~25 KB).  A count pass, a device scan and a fill pass with ballot / popc compaction give the unique
-// ordered CSR (src asc, dst asc) with no atomics; the by-destination lists are produced the same way
-// by searching backwards (planes p-G..p-1) and locating the edge id by binary search in the
-// source's sorted neighbour list.
+// ordered CSR (src asc, dst asc).  The by-destination lists need no second search: the count pass bumps
+// an integer in-degree counter per found edge, the fill pass drops each edge id into its destination's
+// segment through an integer cursor, and a last pass sorts every (short) segment ascending -- integer
+// atomics only, so the result is still one unique array.
 //
 // d^2 is evaluated exactly as the ABI states: fp32, left to right, __fsub_rn/__fmul_rn/__fadd_rn so
 // that ptxas cannot contract to FMA — graph edges must match the oracle bit for bit.
@@ -73,14 +74,15 @@ __device__ __forceinline__ float dist2(const float (&a)[8], const float (&b)[8],
   return s;
 }
 
-// MODE 0: count out- and in-degree.  MODE 1: fill out-edges.  MODE 2: fill in-edge permutation.
+// MODE 0: count out-degree (and in-degree, by integer atomics).  MODE 1: fill the edges and drop every edge
+// id into its destination's segment of in_perm (unordered; sort_in_lists_kernel orders it).
 template <int D, int MODE>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 search_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t* __restrict__ hit_event,
               const int32_t* __restrict__ flags, int32_t* __restrict__ out_deg,
               int32_t* __restrict__ in_deg, const int32_t* __restrict__ row_ptr,
               int32_t* __restrict__ src, int32_t* __restrict__ dst,
-              const int32_t* __restrict__ in_ptr, int32_t* __restrict__ in_perm) {
+              const int32_t* __restrict__ in_ptr, int32_t* __restrict__ in_perm, int32_t* __restrict__ cursor) {
   if (flags[0] != 0) return;                       // malformed batch: plane_ptr is not trustworthy
   const int lane = threadIdx.x & 31;
   const int warp = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
@@ -93,60 +95,51 @@ search_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t*
     const int32_t* pp = plane_ptr + (size_t)ev * (L + 1);
     float me[8], other[8];
     load_emb<D>(a.emb, i, a.d, me);
-    if (MODE == 0 || MODE == 1) {                  // forward: i is the source
-      int cnt = 0;
-      if (p <= L - 2) {
-        const int j0 = pp[p + 1];
-        const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
-        const int j1 = pp[top + 1];
-        const int base_out = (MODE == 1) ? row_ptr[i] : 0;
-        for (int base = j0; base < j1; base += 32) {
-          const int j = base + lane;
-          bool ok = false;
-          if (j < j1) {
-            load_emb<D>(a.emb, j, a.d, other);
-            ok = dist2<D>(me, other, a.d) < a.r2_max;
-          }
-          const unsigned b = __ballot_sync(kFull, ok);
-          if (MODE == 1 && ok) {
+    int cnt = 0;
+    if (p <= L - 2) {
+      const int j0 = pp[p + 1];
+      const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
+      const int j1 = pp[top + 1];
+      const int base_out = (MODE == 1) ? row_ptr[i] : 0;
+      for (int base = j0; base < j1; base += 32) {
+        const int j = base + lane;
+        bool ok = false;
+        if (j < j1) {
+          load_emb<D>(a.emb, j, a.d, other);
+          ok = dist2<D>(me, other, a.d) < a.r2_max;
+        }
+        const unsigned b = __ballot_sync(kFull, ok);
+        if (ok) {
+          if (MODE == 0) {
+            atomicAdd(&in_deg[j], 1);
+          } else {
             const int pos = base_out + cnt + __popc(b & lt);
             src[pos] = i;
             dst[pos] = j;
+            in_perm[in_ptr[j] + atomicAdd(&cursor[j], 1)] = pos;
           }
-          cnt += __popc(b);
         }
+        cnt += __popc(b);
       }
-      if (MODE == 0 && lane == 0) out_deg[i] = cnt;
     }
-    if (MODE == 0 || MODE == 2) {                  // backward: i is the destination
-      int cnt = 0;
-      if (p >= 1) {
-        const int bot = (p - a.gap > 0) ? p - a.gap : 0;
-        const int s0 = pp[bot], s1 = pp[p];
-        const int base_in = (MODE == 2) ? in_ptr[i] : 0;
-        for (int base = s0; base < s1; base += 32) {
-          const int sidx = base + lane;
-          bool ok = false;
-          if (sidx < s1) {
-            load_emb<D>(a.emb, sidx, a.d, other);
-            ok = dist2<D>(other, me, a.d) < a.r2_max;     // source first, as in the forward pass
-          }
-          const unsigned b = __ballot_sync(kFull, ok);
-          if (MODE == 2 && ok) {
-            int lo = row_ptr[sidx], hi = row_ptr[sidx + 1];   // find i in the source's sorted list
-            while (lo < hi) {
-              const int mid = (lo + hi) >> 1;
-              if (dst[mid] < i) lo = mid + 1; else hi = mid;
-            }
-            in_perm[base_in + cnt + __popc(b & lt)] = lo;
-          }
-          cnt += __popc(b);
-        }
-      }
-      if (MODE == 0 && lane == 0) in_deg[i] = cnt;
+    if (MODE == 0 && lane == 0) out_deg[i] = cnt;
+  }
+  if (MODE == 0 && blockIdx.x == 0 && threadIdx.x == 0) out_deg[a.n_hits] = 0;
+}
+
+// Orders every destination's list of edge ids ascending (in-degrees are ~6-10: insertion sort, one thread per hit).
+__global__ void __launch_bounds__(256) sort_in_lists_kernel(int n_hits, const int32_t* __restrict__ flags,
+                                                            const int32_t* __restrict__ in_ptr, int32_t* __restrict__ in_perm) {
+  if (flags[0] != 0) return;
+  for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n_hits; j += gridDim.x * blockDim.x) {
+    const int k0 = in_ptr[j], k1 = in_ptr[j + 1];
+    for (int k = k0 + 1; k < k1; ++k) {
+      const int v = in_perm[k];
+      int q = k - 1;
+      while (q >= k0 && in_perm[q] > v) { in_perm[q + 1] = in_perm[q]; --q; }
+      in_perm[q + 1] = v;
     }
   }
-  if (MODE == 0 && blockIdx.x == 0 && threadIdx.x == 0) { out_deg[a.n_hits] = 0; in_deg[a.n_hits] = 0; }
 }
 
 // ------------------------------------------------------------------ device-wide exclusive scan
@@ -242,20 +235,21 @@ template <int MODE>
 static void launch_search(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
                           const int32_t* flags, int32_t* out_deg, int32_t* in_deg,
                           const int32_t* row_ptr, int32_t* src, int32_t* dst, const int32_t* in_ptr,
-                          int32_t* in_perm, cudaStream_t s) {
+                          int32_t* in_perm, int32_t* cursor, cudaStream_t s) {
   const int grid = search_grid(a.n_hits);
   if (a.d == 4)
-    search_kernel<4, MODE><<<grid, kWarpsPerBlock * 32, 0, s>>>(a, plane_ptr, hit_event, flags, out_deg,
-                                                               in_deg, row_ptr, src, dst, in_ptr, in_perm);
+    search_kernel<4, MODE><<<grid, kWarpsPerBlock * 32, 0, s>>>(a, plane_ptr, hit_event, flags, out_deg, in_deg,
+                                                               row_ptr, src, dst, in_ptr, in_perm, cursor);
   else
-    search_kernel<0, MODE><<<grid, kWarpsPerBlock * 32, 0, s>>>(a, plane_ptr, hit_event, flags, out_deg,
-                                                               in_deg, row_ptr, src, dst, in_ptr, in_perm);
+    search_kernel<0, MODE><<<grid, kWarpsPerBlock * 32, 0, s>>>(a, plane_ptr, hit_event, flags, out_deg, in_deg,
+                                                               row_ptr, src, dst, in_ptr, in_perm, cursor);
 }
 
 int launch_search_count(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
                         const int32_t* flags, int32_t* out_deg, int32_t* in_deg, cudaStream_t s) {
+  cudaMemsetAsync(in_deg, 0, sizeof(int32_t) * ((size_t)a.n_hits + 1), s);
   launch_search<0>(a, plane_ptr, hit_event, flags, out_deg, in_deg, nullptr, nullptr, nullptr, nullptr,
-                   nullptr, s);
+                   nullptr, nullptr, s);
   return 1;
 }
 
@@ -269,9 +263,11 @@ int launch_exclusive_scan(int32_t* data, int n, int32_t* tmp, cudaStream_t s) {
 
 int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
                        const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst,
-                       const int32_t* in_ptr, int32_t* in_perm, cudaStream_t s) {
-  launch_search<1>(a, plane_ptr, hit_event, flags, nullptr, nullptr, row_ptr, src, dst, nullptr, nullptr, s);
-  launch_search<2>(a, plane_ptr, hit_event, flags, nullptr, nullptr, row_ptr, src, dst, in_ptr, in_perm, s);
+                       const int32_t* in_ptr, int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/, cudaStream_t s) {
+  cudaMemsetAsync(cursor, 0, sizeof(int32_t) * (size_t)a.n_hits, s);
+  launch_search<1>(a, plane_ptr, hit_event, flags, nullptr, nullptr, row_ptr, src, dst, in_ptr, in_perm, cursor, s);
+  const int need = (a.n_hits + 255) / 256;
+  sort_in_lists_kernel<<<need < 148 * 8 ? (need < 1 ? 1 : need) : 148 * 8, 256, 0, s>>>(a.n_hits, flags, in_ptr, in_perm);
   return 2;
 }
 
