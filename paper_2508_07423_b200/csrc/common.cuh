@@ -88,16 +88,15 @@ int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32
                        const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst,
                        const int32_t* in_ptr, int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/, cudaStream_t s);
 size_t scan_tmp_ints(int n);
+int launch_sort_in_lists(int n_hits, const int32_t* flags, const int32_t* in_ptr, int32_t* in_perm, cudaStream_t s);
 // ---- graph_kmax.cu (next row: k_max-capped search)
 int launch_kmax_count(const GraphArgs& a, int k_max, const int32_t* plane_ptr, const int32_t* hit_event,
                       const int32_t* flags, int32_t* out_deg, cudaStream_t s);
 int launch_kmax_fill(const GraphArgs& a, int k_max, const int32_t* plane_ptr, const int32_t* hit_event,
                      const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst, cudaStream_t s);
-int launch_kmax_in_count(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event, const int32_t* flags,
-                         const int32_t* row_ptr, const int32_t* dst, int32_t* in_deg, cudaStream_t s);
-int launch_kmax_in_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event, const int32_t* flags,
-                        const int32_t* row_ptr, const int32_t* dst, const int32_t* in_ptr, int32_t* in_perm,
-                        cudaStream_t s);
+int launch_kmax_in_count(const GraphArgs& a, int64_t n_edges, const int32_t* dst, int32_t* in_deg, cudaStream_t s);
+int launch_kmax_in_fill(const GraphArgs& a, int64_t n_edges, const int32_t* flags, const int32_t* dst, const int32_t* in_ptr,
+                        int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/, cudaStream_t s);
 
 // ---- mlp_simt.cu
 struct Segment {              // input row r, column k (k < width): base[(idx ? idx[r] : r) * ld + k]

@@ -497,16 +497,14 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
     return fail(c, ETX_ERR_CAPACITY, "graph needs " + std::to_string(g->n_edges) + " edges, capacity " +
                                          std::to_string(g->edge_capacity));
   if (k_max > 0) {
-    // the by-destination lists depend on which edges survived the cap: forward fill first, then count,
-    // scan and fill the incoming side from the capped neighbour lists
+    // the by-destination lists depend on which edges survived the cap: forward fill first, then in-degrees,
+    // scan, and the incoming side from the capped edge list
     ProfScope ps(c, ETX_K_GRAPH, s);
     if (g->n_edges > 0)
       c->launches += launch_kmax_fill(a, k_max, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_src, g->d_dst, s);
-    c->launches += launch_kmax_in_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_dst, g->d_in_ptr, s);
+    c->launches += launch_kmax_in_count(a, g->n_edges, g->d_dst, g->d_in_ptr, s);
     c->launches += launch_exclusive_scan(g->d_in_ptr, b->n_hits + 1, w.scan_tmp, s);
-    if (g->n_edges > 0)
-      c->launches += launch_kmax_in_fill(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_dst, g->d_in_ptr,
-                                         g->d_in_perm, s);
+    c->launches += launch_kmax_in_fill(a, g->n_edges, w.flags, g->d_dst, g->d_in_ptr, g->d_in_perm, w.cursor, s);
   } else if (g->n_edges > 0) {
     ProfScope ps(c, ETX_K_GRAPH, s);
     c->launches += launch_search_fill(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_src, g->d_dst,

@@ -266,9 +266,13 @@ int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32
                        const int32_t* in_ptr, int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/, cudaStream_t s) {
   cudaMemsetAsync(cursor, 0, sizeof(int32_t) * (size_t)a.n_hits, s);
   launch_search<1>(a, plane_ptr, hit_event, flags, nullptr, nullptr, row_ptr, src, dst, in_ptr, in_perm, cursor, s);
-  const int need = (a.n_hits + 255) / 256;
-  sort_in_lists_kernel<<<need < 148 * 8 ? (need < 1 ? 1 : need) : 148 * 8, 256, 0, s>>>(a.n_hits, flags, in_ptr, in_perm);
-  return 2;
+  return 1 + launch_sort_in_lists(a.n_hits, flags, in_ptr, in_perm, s);
+}
+
+int launch_sort_in_lists(int n_hits, const int32_t* flags, const int32_t* in_ptr, int32_t* in_perm, cudaStream_t s) {
+  const int need = (n_hits + 255) / 256;
+  sort_in_lists_kernel<<<need < 148 * 8 ? (need < 1 ? 1 : need) : 148 * 8, 256, 0, s>>>(n_hits, flags, in_ptr, in_perm);
+  return 1;
 }
 
 }  // namespace etx

@@ -6,12 +6,13 @@
 //
 // The thesis kept a k_max-slot list per thread and replaced its farthest entry.  Here one warp owns a source
 // hit, as in graph.cu: a count pass (degree = min(in-radius candidates, k_max)), a scan, and a fill pass.
-// A source over the cap (the thesis: < 0.1 % of hits) finds the k_max-th smallest key (d^2 bits : index) by
-// a bitwise bisection — 64 warp-wide counting sweeps over its candidate window, no list, no sort, no
-// shared memory — and then emits the candidates with key <= threshold in ascending index through the same
-// ballot / popc compaction, so the CSR is again the unique ordered array.  The by-destination lists need
-// the capped forward lists: a hit counts (and then locates, by binary search) itself in the neighbour
-// lists of its in-radius source candidates, sources ascending = edge ids ascending.
+// A source over the cap (the thesis: < 0.1 % of hits) with at most 128 candidates inside the radius compacts
+// their keys (d^2 bits : index) into a per-warp shared-memory list and every lane ranks its own keys against
+// the list (rank < k_max = kept); a longer list finds the k_max-th smallest key by a bitwise bisection (64
+// warp-wide counting sweeps over the candidate window, no list, no sort).  Either way the kept candidates
+// are emitted in ascending index through the same ballot / popc compaction, so the CSR is again the unique
+// ordered array.  The by-destination lists are built from the
+// capped edge list with integer counters, a cursor and graph.cu's per-segment sort (no second search).
 #include "common.cuh"
 
 namespace etx {
@@ -19,6 +20,7 @@ namespace {
 
 constexpr int kWarpsPerBlock = 8;
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kListMax = 128;                   // in-radius candidates ranked in shared memory (4 per lane)
 
 __device__ __forceinline__ float dist2(const float* __restrict__ emb, int i, int j, int d) {
   float s = 0.0f;
@@ -42,6 +44,7 @@ kmax_forward_kernel(GraphArgs a, int k_max, const int32_t* __restrict__ plane_pt
                     int32_t* __restrict__ out_deg, const int32_t* __restrict__ row_ptr,
                     int32_t* __restrict__ src, int32_t* __restrict__ dst) {
   if (flags[0] != 0) return;
+  __shared__ unsigned long long s_keys[FILL ? kWarpsPerBlock : 1][FILL ? kListMax : 1];
   const int lane = threadIdx.x & 31;
   const int warp = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
   const int n_warps = gridDim.x * kWarpsPerBlock;
@@ -75,6 +78,42 @@ kmax_forward_kernel(GraphArgs a, int k_max, const int32_t* __restrict__ plane_pt
         const int j = base + lane;
         const bool ok = j < j1 && dist2(a.emb, i, j, a.d) < a.r2_max;
         total += __popc(__ballot_sync(kFull, ok));
+      }
+      if (total > k_max && total <= kListMax) {
+        // short list: compact the keys (ascending index = ascending slot), rank, emit
+        unsigned long long* keys = s_keys[FILL ? (threadIdx.x >> 5) : 0];
+        int n = 0;
+        for (int base = j0; base < j1; base += 32) {
+          const int j = base + lane;
+          bool ok = false;
+          float d2 = 0.f;
+          if (j < j1) { d2 = dist2(a.emb, i, j, a.d); ok = d2 < a.r2_max; }
+          const unsigned b = __ballot_sync(kFull, ok);
+          if (ok) keys[n + __popc(b & lt)] = key_of(d2, j);
+          n += __popc(b);
+        }
+        __syncwarp();
+        int cnt = 0;
+        for (int t0 = 0; t0 < total; t0 += 32) {
+          const int slot = t0 + lane;
+          bool keep = false;
+          unsigned long long mine = 0ull;
+          if (slot < total) {
+            mine = keys[slot];
+            int rank = 0;
+            for (int m = 0; m < total; ++m) rank += keys[m] < mine;
+            keep = rank < k_max;
+          }
+          const unsigned b = __ballot_sync(kFull, keep);
+          if (keep) {
+            const int pos = begin + cnt + __popc(b & lt);
+            src[pos] = i;
+            dst[pos] = (int)(unsigned)(mine & 0xffffffffull);
+          }
+          cnt += __popc(b);
+        }
+        __syncwarp();
+        continue;
       }
       if (total > k_max) {
         thr = 0ull;                                // invariant: thr <= k-th smallest key
@@ -113,49 +152,21 @@ kmax_forward_kernel(GraphArgs a, int k_max, const int32_t* __restrict__ plane_pt
   }
 }
 
-// Destination side, after the forward lists exist.  FILL = false: in_deg[i]; FILL = true: in_perm.
-template <bool FILL>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-kmax_backward_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t* __restrict__ hit_event,
-                     const int32_t* __restrict__ flags, const int32_t* __restrict__ row_ptr,
-                     const int32_t* __restrict__ dst, int32_t* __restrict__ in_deg,
-                     const int32_t* __restrict__ in_ptr, int32_t* __restrict__ in_perm) {
-  if (flags[0] != 0) return;
-  const int lane = threadIdx.x & 31;
-  const int warp = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
-  const int n_warps = gridDim.x * kWarpsPerBlock;
-  const unsigned lt = (1u << lane) - 1u;
-  const int L = a.n_planes;
-  for (int i = warp; i < a.n_hits; i += n_warps) {
-    const int p = a.plane[i];
-    int cnt = 0;
-    if (p >= 1) {
-      const int32_t* pp = plane_ptr + (size_t)hit_event[i] * (L + 1);
-      const int bot = (p - a.gap > 0) ? p - a.gap : 0;
-      const int s0 = pp[bot], s1 = pp[p];
-      const int base_in = FILL ? in_ptr[i] : 0;
-      for (int base = s0; base < s1; base += 32) {
-        const int sidx = base + lane;
-        bool ok = false;
-        int lo = 0;
-        if (sidx < s1 && dist2(a.emb, sidx, i, a.d) < a.r2_max) {       // source first, as in the forward pass
-          int hi = row_ptr[sidx + 1];
-          lo = row_ptr[sidx];
-          const int end = hi;
-          while (lo < hi) {                                              // is i in the source's (capped) list?
-            const int mid = (lo + hi) >> 1;
-            if (dst[mid] < i) lo = mid + 1; else hi = mid;
-          }
-          ok = lo < end && dst[lo] == i;
-        }
-        const unsigned b = __ballot_sync(kFull, ok);
-        if (FILL && ok) in_perm[base_in + cnt + __popc(b & lt)] = lo;
-        cnt += __popc(b);
-      }
-    }
-    if (!FILL && lane == 0) in_deg[i] = cnt;
+// Destination side, after the capped forward lists exist: in-degrees by integer atomics over the edge list,
+// scan, every edge id dropped into its destination's segment through an integer cursor; graph.cu's segment
+// sort then orders each list ascending.
+__global__ void __launch_bounds__(256) kmax_in_degree_kernel(int64_t n_edges, const int32_t* __restrict__ dst,
+                                                             int32_t* __restrict__ in_deg) {
+  for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n_edges; e += (int64_t)gridDim.x * blockDim.x)
+    atomicAdd(&in_deg[dst[e]], 1);
+}
+__global__ void __launch_bounds__(256) kmax_in_scatter_kernel(int64_t n_edges, const int32_t* __restrict__ dst,
+                                                              const int32_t* __restrict__ in_ptr, int32_t* __restrict__ cursor,
+                                                              int32_t* __restrict__ in_perm) {
+  for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n_edges; e += (int64_t)gridDim.x * blockDim.x) {
+    const int j = dst[e];
+    in_perm[in_ptr[j] + atomicAdd(&cursor[j], 1)] = (int32_t)e;
   }
-  if (!FILL && blockIdx.x == 0 && threadIdx.x == 0) in_deg[a.n_hits] = 0;
 }
 
 inline int search_grid(int n_hits) {
@@ -181,19 +192,21 @@ int launch_kmax_fill(const GraphArgs& a, int k_max, const int32_t* plane_ptr, co
   return 1;
 }
 
-int launch_kmax_in_count(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event, const int32_t* flags,
-                         const int32_t* row_ptr, const int32_t* dst, int32_t* in_deg, cudaStream_t s) {
-  kmax_backward_kernel<false><<<search_grid(a.n_hits), kWarpsPerBlock * 32, 0, s>>>(a, plane_ptr, hit_event, flags, row_ptr,
-                                                                                    dst, in_deg, nullptr, nullptr);
+int launch_kmax_in_count(const GraphArgs& a, int64_t n_edges, const int32_t* dst, int32_t* in_deg, cudaStream_t s) {
+  cudaMemsetAsync(in_deg, 0, sizeof(int32_t) * ((size_t)a.n_hits + 1), s);
+  if (n_edges <= 0) return 0;
+  const int64_t need = (n_edges + 255) / 256;
+  kmax_in_degree_kernel<<<(int)(need < 148 * 16 ? need : 148 * 16), 256, 0, s>>>(n_edges, dst, in_deg);
   return 1;
 }
 
-int launch_kmax_in_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event, const int32_t* flags,
-                        const int32_t* row_ptr, const int32_t* dst, const int32_t* in_ptr, int32_t* in_perm,
-                        cudaStream_t s) {
-  kmax_backward_kernel<true><<<search_grid(a.n_hits), kWarpsPerBlock * 32, 0, s>>>(a, plane_ptr, hit_event, flags, row_ptr,
-                                                                                   dst, nullptr, in_ptr, in_perm);
-  return 1;
+int launch_kmax_in_fill(const GraphArgs& a, int64_t n_edges, const int32_t* flags, const int32_t* dst, const int32_t* in_ptr,
+                        int32_t* in_perm, int32_t* cursor, cudaStream_t s) {
+  if (n_edges <= 0) return 0;
+  cudaMemsetAsync(cursor, 0, sizeof(int32_t) * (size_t)a.n_hits, s);
+  const int64_t need = (n_edges + 255) / 256;
+  kmax_in_scatter_kernel<<<(int)(need < 148 * 16 ? need : 148 * 16), 256, 0, s>>>(n_edges, dst, in_ptr, cursor, in_perm);
+  return 1 + launch_sort_in_lists(a.n_hits, flags, in_ptr, in_perm, s);
 }
 
 }  // namespace etx
