@@ -127,17 +127,30 @@ search_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t*
   if (MODE == 0 && blockIdx.x == 0 && threadIdx.x == 0) out_deg[a.n_hits] = 0;
 }
 
-// Orders every destination's list of edge ids ascending (in-degrees are ~6-10: insertion sort, one thread per hit).
+// Orders every destination's list of edge ids ascending.  One warp per hit: a list of <= 32 ids (in-degrees are
+// ~6-10) sits one id per lane, each lane ranks its id with shuffles and writes it to its place (coalesced both
+// ways); a longer list is insertion-sorted by one lane.
 __global__ void __launch_bounds__(256) sort_in_lists_kernel(int n_hits, const int32_t* __restrict__ flags,
                                                             const int32_t* __restrict__ in_ptr, int32_t* __restrict__ in_perm) {
   if (flags[0] != 0) return;
-  for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n_hits; j += gridDim.x * blockDim.x) {
-    const int k0 = in_ptr[j], k1 = in_ptr[j + 1];
-    for (int k = k0 + 1; k < k1; ++k) {
-      const int v = in_perm[k];
-      int q = k - 1;
-      while (q >= k0 && in_perm[q] > v) { in_perm[q + 1] = in_perm[q]; --q; }
-      in_perm[q + 1] = v;
+  const int lane = threadIdx.x & 31;
+  const int n_warps = gridDim.x * (blockDim.x >> 5);
+  for (int j = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); j < n_hits; j += n_warps) {
+    const int k0 = in_ptr[j], n = in_ptr[j + 1] - k0;
+    if (n <= 1) continue;
+    if (n <= 32) {
+      const int v = lane < n ? in_perm[k0 + lane] : 0x7fffffff;
+      int rank = 0;
+      for (int m = 0; m < n; ++m) rank += __shfl_sync(kFull, v, m) < v;      // ids are distinct
+      __syncwarp();
+      if (lane < n) in_perm[k0 + rank] = v;
+    } else if (lane == 0) {
+      for (int k = k0 + 1; k < k0 + n; ++k) {
+        const int v = in_perm[k];
+        int q = k - 1;
+        while (q >= k0 && in_perm[q] > v) { in_perm[q + 1] = in_perm[q]; --q; }
+        in_perm[q + 1] = v;
+      }
     }
   }
 }
@@ -270,7 +283,7 @@ int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32
 }
 
 int launch_sort_in_lists(int n_hits, const int32_t* flags, const int32_t* in_ptr, int32_t* in_perm, cudaStream_t s) {
-  const int need = (n_hits + 255) / 256;
+  const int need = (n_hits + 7) / 8;
   sort_in_lists_kernel<<<need < 148 * 8 ? (need < 1 ? 1 : need) : 148 * 8, 256, 0, s>>>(n_hits, flags, in_ptr, in_perm);
   return 1;
 }
