@@ -62,6 +62,8 @@ struct etx_ctx {
   size_t ws_bytes = 0;
   int64_t launches = 0;
   std::string err;
+  cudaStream_t copy_stream = nullptr;   // etx_infer_host: edge-list copy-out underneath the message passing
+  cudaEvent_t copy_event = nullptr;
   // per-stage profiling (etx_profile_enable / etx_profile_read)
   bool prof_on = false;
   struct ProfRec { int cls; int n; cudaEvent_t a, b; };

@@ -384,6 +384,7 @@ etx_status etx_destroy(etx_ctx* c) {
   if (c->d_wimg) cudaFree(c->d_wimg);
   for (const etx_ctx::ProfRec& r : c->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
+  if (c->copy_stream) { cudaStreamDestroy(c->copy_stream); cudaEventDestroy(c->copy_event); }
   delete c;
   return ETX_OK;
 }
@@ -684,15 +685,25 @@ etx_status etx_infer_host(etx_ctx* c, const etx_batch_host* hb, float r2_max, in
   etx_status st = etx_build_graph(c, &b, w.s_emb, r2_max, max_plane_gap, 0, &g, stream);
   if (n_edges) *n_edges = g.n_edges;
   if (st) return st;
-  if ((st = etx_gnn_forward(c, &b, &g, w.s_edge_enc, nullptr, stream))) return st;
-  if ((st = etx_edge_scores(c, &g, w.s_edge_enc, w.s_scores, stream))) return st;
+  // the edge list is final once the graph is built: its device-to-host copy runs on the context's copy stream
+  // underneath the message passing; only the scores are copied after the last kernel
   const size_t ne = (size_t)g.n_edges;
-  if (ne) {
-    if (h_src) cudaMemcpyAsync(h_src, w.s_src, ne * 4, cudaMemcpyDeviceToHost, s);
-    if (h_dst) cudaMemcpyAsync(h_dst, w.s_dst, ne * 4, cudaMemcpyDeviceToHost, s);
-    if (h_scores) cudaMemcpyAsync(h_scores, w.s_scores, ne * 4, cudaMemcpyDeviceToHost, s);
+  if (!c->copy_stream) {
+    cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    cudaEventCreateWithFlags(&c->copy_event, cudaEventDisableTiming);
   }
-  if (cudaStreamSynchronize(s) != cudaSuccess) return check_cuda(c, "etx_infer_host");
+  if (ne && (h_src || h_dst)) {
+    cudaEventRecord(c->copy_event, s);
+    cudaStreamWaitEvent(c->copy_stream, c->copy_event, 0);
+    if (h_src) cudaMemcpyAsync(h_src, w.s_src, ne * 4, cudaMemcpyDeviceToHost, c->copy_stream);
+    if (h_dst) cudaMemcpyAsync(h_dst, w.s_dst, ne * 4, cudaMemcpyDeviceToHost, c->copy_stream);
+  }
+  if (!(st = etx_gnn_forward(c, &b, &g, w.s_edge_enc, nullptr, stream)))
+    st = etx_edge_scores(c, &g, w.s_edge_enc, w.s_scores, stream);
+  if (!st && ne && h_scores) cudaMemcpyAsync(h_scores, w.s_scores, ne * 4, cudaMemcpyDeviceToHost, s);
+  const cudaError_t e1 = cudaStreamSynchronize(c->copy_stream), e2 = cudaStreamSynchronize(s);
+  if (st) return st;
+  if (e1 != cudaSuccess || e2 != cudaSuccess) return check_cuda(c, "etx_infer_host");
   return check_cuda(c, "etx_infer_host");
 }
 
