@@ -42,8 +42,13 @@ def calibrate(name: str) -> dict:
 
 
 def main():
-    out = {name: calibrate(name) for name in ("c0", "c1", "c2", "c4")}
     path = os.path.join(os.path.dirname(os.path.abspath(synth.__file__)), "config_constants.json")
+    out = {}
+    if os.path.exists(path):                      # keep what other calibration scripts stored (oracle/calibrate_int8.py)
+        with open(path) as f:
+            out = json.load(f)
+    for name in ("c0", "c1", "c2", "c4"):
+        out.setdefault(name, {}).update(calibrate(name))
     with open(path, "w") as f:
         json.dump(out, f, indent=1, sort_keys=True)
         f.write("\n")

@@ -74,6 +74,79 @@ void orc_mlp(int64_t n, int32_t n_layers, const int32_t* dims, const float* w, c
   }
 }
 
+// ---- next row (embedding part): the embedding MLP in INT8 by static post-training
+//      quantisation, symmetric scheme of Eqs. 4.31-4.33:
+//        S = alpha / 127 (alpha mapped to the highest INT8 value),  x_q = clip(round(x / S), -127, 127).
+//      Per layer l (the Q -> quantised node -> DQ chain of P:2725): the layer's input is quantised with the
+//      per-tensor scale S_a[l] = alpha_a[l] / 127 (alpha_a = calibrated range of that activation, an INPUT of
+//      this function), its weight with S_w[l] = max|W_l| / 127 (the weight range is known), the
+//      products are summed exactly in integers and de-quantised:
+//        y_o = float(sum_k x_q[k] w_q[o][k]) * (S_a S_w) + b_o ;  ReLU on hidden layers (biases stay fp32).
+//      Every float step is a single fp32 operation (x / S, rint = round-half-even, S_a * S_w, * , +; compile
+//      with -ffp-contract=off), so the integer codes -- and with them the outputs -- are reproducible bit
+//      for bit (reading Q21).
+static inline int32_t quant_code(float x, float S) {
+  float q = std::nearbyintf(x / S);                 // default rounding mode: to nearest, ties to even
+  if (q > 127.0f) q = 127.0f;
+  if (q < -127.0f) q = -127.0f;
+  return (int32_t)q;
+}
+
+void orc_quantize(int64_t n, const float* x, float alpha, int8_t* codes, float* scale_out) {
+  const float S = alpha / 127.0f;
+  if (scale_out) *scale_out = S;
+  for (int64_t i = 0; i < n; ++i) codes[i] = (int8_t)quant_code(x[i], S);
+}
+
+void orc_mlp_int8(int64_t n, int32_t n_layers, const int32_t* dims, const float* w, const float* in,
+                  const float* act_alpha /*[n_layers]*/, float* out) {
+  int32_t maxw = 0;
+  for (int l = 0; l <= n_layers; ++l) maxw = dims[l] > maxw ? dims[l] : maxw;
+  // weight codes and scales, once
+  std::vector<std::vector<int32_t>> wq(n_layers);
+  std::vector<float> sw(n_layers);
+  {
+    const float* p = w;
+    for (int l = 0; l < n_layers; ++l) {
+      const int64_t cnt = (int64_t)dims[l] * dims[l + 1];
+      float m = 0.0f;
+      for (int64_t i = 0; i < cnt; ++i) m = std::fabs(p[i]) > m ? std::fabs(p[i]) : m;
+      sw[l] = m / 127.0f;
+      wq[l].resize(cnt);
+      for (int64_t i = 0; i < cnt; ++i) wq[l][i] = quant_code(p[i], sw[l]);
+      p += cnt + dims[l + 1];
+    }
+  }
+#pragma omp parallel
+  {
+    std::vector<float> a(maxw), b(maxw);
+    std::vector<int32_t> aq(maxw);
+#pragma omp for schedule(static)
+    for (int64_t row = 0; row < n; ++row) {
+      for (int i = 0; i < dims[0]; ++i) a[i] = in[row * dims[0] + i];
+      const float* p = w;
+      for (int l = 0; l < n_layers; ++l) {
+        const int fi = dims[l], fo = dims[l + 1];
+        const float* bias = p + (int64_t)fi * fo;
+        const float sa = act_alpha[l] / 127.0f;
+        const float sc = sa * sw[l];
+        for (int i = 0; i < fi; ++i) aq[i] = quant_code(a[i], sa);
+        for (int o = 0; o < fo; ++o) {
+          int64_t acc = 0;
+          for (int i = 0; i < fi; ++i) acc += (int64_t)aq[i] * wq[l][(int64_t)o * fi + i];
+          const float prod = (float)acc * sc;
+          float v = prod + bias[o];
+          if (l < n_layers - 1 && !(v > 0.0f)) v = 0.0f;
+          b[o] = v;
+        }
+        a.swap(b);
+        p = bias + fo;
+      }
+      for (int o = 0; o < dims[n_layers]; ++o) out[row * dims[n_layers] + o] = a[o];
+    }
+  }
+}
+
 // ---- a2 rough graph: hit i on plane p connects to hits j of the same event on planes
 //      p+1 .. min(p+G, L-1) iff d^2(i,j) < r2_max (Eq. 8.1; strict "<": P:2674).
 //      Sequential loop over candidates in ascending index, as P:2674 describes, so edges come out in

@@ -74,6 +74,41 @@ def mlp(x: np.ndarray, dims: Sequence[int], blob: np.ndarray, offset: int) -> np
     return out
 
 
+def quantize(x: np.ndarray, alpha: float):
+    """Eqs. 4.31-4.33 (P:1469-1481): S = alpha / 127, codes = clip(round(x / S), -127, 127).  Returns (codes, S)."""
+    x = _f32(x).ravel()
+    codes = np.empty(x.size, np.int8)
+    S = C.c_float(0.0)
+    lib().orc_quantize(C.c_int64(x.size), _p(x, C.c_float), C.c_float(alpha), _p(codes, C.c_int8), C.byref(S))
+    return codes, float(S.value)
+
+
+def mlp_int8(x: np.ndarray, dims: Sequence[int], blob: np.ndarray, offset: int, act_alpha: Sequence[float]) -> np.ndarray:
+    """Next row: the MLP chain with INT8 weights and activations (static PTQ, symmetric per-tensor
+    scales); act_alpha[l] = calibrated range of layer l's input."""
+    x = _f32(x)
+    d = np.ascontiguousarray(dims, np.int32)
+    al = _f32(np.asarray(act_alpha, np.float32))
+    assert len(al) == len(d) - 1
+    n = x.shape[0]
+    out = np.empty((n, int(d[-1])), np.float32)
+    w = blob[offset:]
+    lib().orc_mlp_int8(C.c_int64(n), C.c_int32(len(d) - 1), _p(d, C.c_int32), _p(w, C.c_float),
+                       _p(x, C.c_float), _p(al, C.c_float), _p(out, C.c_float))
+    return out
+
+
+def int8_calibration(x: np.ndarray, dims: Sequence[int], blob: np.ndarray, offset: int) -> np.ndarray:
+    """Static PTQ calibration with a max observer: range of every layer's INPUT over the sample x,
+    taken from the fp32 oracle MLP."""
+    x = _f32(x)
+    alphas = [float(np.abs(x).max())]
+    for l in range(1, len(dims) - 1):
+        z = mlp(x, list(dims[:l + 1]), blob, offset)          # linear output of layer l
+        alphas.append(float(np.maximum(z, 0.0).max()))        # its ReLU is the next layer's input
+    return np.asarray(alphas, np.float32)
+
+
 def build_graph(event_ptr, plane, emb, r2_max: float, gap: int, n_planes: int = 26,
                 band: float = 0.0, want_border: bool = False):
     """a2 (Eq. 8.1): edges (src, dst) in (src asc, dst asc) order.

@@ -345,6 +345,12 @@ def load_constants() -> Dict[str, dict]:
         return json.load(f)
 
 
+def int8_act_alpha(cfg: Config) -> np.ndarray:
+    """Stored calibrated activation ranges of the INT8 embedding (next row; oracle/calibrate_int8.py)."""
+    key = {"c3": "c2"}.get(cfg.name, cfg.name)
+    return np.asarray(load_constants()[key]["int8_act_alpha"], np.float32)
+
+
 def r2_max(cfg: Config) -> float:
     """Stored fp32 r^2 for the config; both paths read this constant."""
     key = {"c3": "c2"}.get(cfg.name, cfg.name)
