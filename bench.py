@@ -278,6 +278,15 @@ def run_ours(args):
             kms, Ek = time3(lambda: etx.etx_build_graph(db, emb, r2, gap, g2, k_max=kk))
             next_rows[f"graph_kmax_{kk}"] = {"ms": kms, "events_per_s": n_ev / (kms * 1e-3), "n_edges": int(Ek)}
         del g2
+        # NEXT-3 (embedding part): INT8 embedding MLP with the stored calibrated ranges, and the graph it gives
+        al = synth.int8_act_alpha(cfg)
+        emb8 = torch.empty_like(emb)
+        ims, _ = time3(lambda: etx.etx_embed_int8(db, al, emb8))
+        g3 = binding.DeviceGraph(N, int(cap * 1.5), dev)
+        E8 = etx.etx_build_graph(db, emb8, r2, gap, g3)
+        next_rows["embed_int8"] = {"ms": ims, "events_per_s": n_ev / (ims * 1e-3), "fp32_embed_ms": stages_embed_ms(prof, args.steps),
+                                   "n_edges": int(E8), "edges_vs_fp32": E8 / max(int(E), 1)}
+        del g3, emb8
 
     # ---- end to end through the host-buffer entry point
     host = binding.pinned_host_batch(batch)
@@ -385,6 +394,10 @@ def run_ours(args):
         "gpu_launches": int(launches), "clocks": clk.summary(), "stages": stages, "next_rows": next_rows}))
     if world > 1:
         dist.destroy_process_group()
+
+
+def stages_embed_ms(prof, steps):
+    return prof["embed"][0] / max(steps, 1)
 
 
 def read_traffic():

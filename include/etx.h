@@ -114,6 +114,15 @@ etx_status etx_set_workspace(etx_ctx* ctx, void* d_workspace, size_t bytes);
 /* a0+a1: d_emb[n_hits, emb_dim] fp32 row-major = embedding MLP of ((r,phi,z) - center) / scale.   */
 etx_status etx_embed(etx_ctx* ctx, const etx_batch* batch, float* d_emb, void* stream);
 
+/* Next row (embedding part): the embedding MLP of etx_embed with INT8 weights and
+ * activations, static post-training quantisation with the symmetric scheme of Eqs. 4.31-4.33:
+ * S = alpha / 127, x_q = clip(round(x / S), -127, 127) (round half to even, fp32 division).  Per layer the input
+ * is quantised with S_a = h_act_alpha[l] / 127 (HOST array of emb_n_layers calibrated ranges, > 0), the weight
+ * with S_w = max|W_l| / 127 (done once at etx_create); y = float(int32 sum) * (S_a * S_w) + b, ReLU on hidden
+ * layers, every float step one rounded fp32 operation.  d_emb[n_hits, emb_dim] fp32 as etx_embed.               */
+etx_status etx_embed_int8(etx_ctx* ctx, const etx_batch* batch, const float* h_act_alpha, int32_t n_alpha,
+                          float* d_emb, void* stream);
+
 /* a2: fixed-radius search in embedding space.  Edge (i -> j) iff same event,
  * 1 <= plane(j) - plane(i) <= max_plane_gap, and d^2 < r2_max with d^2 evaluated in fp32 as
  * ((e0-f0)^2 + (e1-f1)^2) + ... left to right, each operation rounded (no FMA).  Output is the

@@ -81,6 +81,8 @@ def load_library():
         lib.etx_set_workspace.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
         lib.etx_embed.restype = C.c_int
         lib.etx_embed.argtypes = [C.c_void_p, C.POINTER(Batch), C.c_void_p, C.c_void_p]
+        lib.etx_embed_int8.restype = C.c_int
+        lib.etx_embed_int8.argtypes = [C.c_void_p, C.POINTER(Batch), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
         lib.etx_build_graph.restype = C.c_int
         lib.etx_build_graph.argtypes = [C.c_void_p, C.POINTER(Batch), C.c_void_p, C.c_float, C.c_int32,
                                         C.c_int32, C.POINTER(Graph), C.c_void_p]
@@ -220,6 +222,14 @@ class Etx:
         if emb is None:
             emb = torch.empty(batch.n_hits, self.emb_dim, dtype=torch.float32, device=self.device)
         self._check(self.lib.etx_embed(self.handle, C.byref(batch.c), _ptr(emb), self._stream()))
+        return emb
+
+    def etx_embed_int8(self, batch: DeviceBatch, act_alpha, emb: Optional[torch.Tensor] = None) -> torch.Tensor:
+        if emb is None:
+            emb = torch.empty(batch.n_hits, self.emb_dim, dtype=torch.float32, device=self.device)
+        al = np.ascontiguousarray(act_alpha, dtype=np.float32)
+        self._check(self.lib.etx_embed_int8(self.handle, C.byref(batch.c), al.ctypes.data_as(C.c_void_p), len(al),
+                                            _ptr(emb), self._stream()))
         return emb
 
     def etx_build_graph(self, batch: DeviceBatch, emb: torch.Tensor, r2_max: float, max_plane_gap: int,

@@ -62,6 +62,9 @@ struct etx_ctx {
   size_t ws_bytes = 0;
   int64_t launches = 0;
   std::string err;
+  int* d_emb_wq = nullptr;              // INT8 codes of the embedding MLP's weights (next row), packed 4 per word
+  int emb_wq_off[etx::kMaxLayers] = {0};
+  float emb_sw[etx::kMaxLayers] = {0};  // their per-layer scales max|W| / 127
   cudaStream_t copy_stream = nullptr;   // etx_infer_host: edge-list copy-out underneath the message passing
   cudaEvent_t copy_event = nullptr;
   // per-stage profiling (etx_profile_enable / etx_profile_read)
@@ -144,6 +147,19 @@ int tc_chunk_k(int mode);
 // ---- tracks.cu (next row: score cut + weakly connected components)
 int launch_wcc(int n_events, const int32_t* event_ptr, const int32_t* row_ptr, const int32_t* src,
                const int32_t* dst, const float* scores, float score_min, int32_t* labels, cudaStream_t s);
+
+// ---- embed_int8.cu (next row: INT8 embedding MLP)
+struct Int8Args {
+  int n_rows = 0, n_layers = 0, n_out = 0;
+  const float* feat[3] = {nullptr, nullptr, nullptr}; float fc[3] = {0, 0, 0}; float fs[3] = {1, 1, 1};
+  const int* wq = nullptr;                 // packed int8 weight codes, per layer [out][ceil(in/4)] words
+  int w_off[kMaxLayers] = {0};             // word offset of every layer inside wq
+  const float* bias[kMaxLayers] = {nullptr};
+  float sa[kMaxLayers] = {0};              // activation scale of every layer's input (alpha / 127)
+  float sc[kMaxLayers] = {0};              // sa * weight scale
+  float* out = nullptr;                    // [n_rows, n_out] fp32
+};
+int launch_embed_int8(const Int8Args& a, int H, cudaStream_t s);
 
 // ---- scatter.cu
 int launch_scatter(int n_nodes, int H, const int32_t* row_ptr, const int32_t* in_ptr,

@@ -1,0 +1,114 @@
+// Next row (embedding part): the hit-embedding MLP in INT8 (static post-training
+// quantisation; symmetric scheme of Eqs. 4.31-4.33).  Per layer: the input is
+// quantised with a calibrated per-tensor scale S_a = alpha_a / 127, the weight (quantised once at etx_create)
+// with S_w = max|W| / 127; products are summed exactly in int32 (dp4a) and de-quantised in fp32,
+//   y = float(sum) * (S_a S_w) + b ,  ReLU on hidden layers,
+// every float step a single rounded fp32 operation, so the integer codes and the embedding match the oracle
+// bit for bit.  The thesis ran this on the INT8 tensor cores through TensorRT; this first version uses the
+// integer dot-product units (dp4a): a 64-row tile per CTA, activations and the layer's weights as packed
+// int8 words in shared memory, a 4 x (H/16) int32 register tile per thread.
+#include "common.cuh"
+
+namespace etx {
+namespace {
+
+constexpr int TM = 64;
+constexpr int NT = 256;
+
+__device__ __forceinline__ int quant_code(float x, float S) {
+  float q = rintf(__fdiv_rn(x, S));                 // round to nearest, ties to even
+  q = fminf(fmaxf(q, -127.0f), 127.0f);
+  return (int)q;
+}
+
+template <int H>
+__global__ void __launch_bounds__(NT) embed_int8_kernel(const Int8Args a) {
+  constexpr int KWH = H / 4;                         // packed words per row of an H-wide operand
+  constexpr int LD = KWH + 1;                        // padded: conflict-free for the strided weight rows
+  constexpr int NJ = H / 16;
+  __shared__ int Wq[H * LD];
+  __shared__ int Aq[2][TM * LD];
+  const int tid = threadIdx.x, rg = tid >> 4, og = tid & 15;
+  const int row0 = blockIdx.x * TM;
+  const int L = a.n_layers;
+
+  // layer-0 input: the 3 normalised features (a0: P:2285), quantised and packed into one word per row
+  if (tid < TM) {
+    const int gr = (row0 + tid < a.n_rows) ? row0 + tid : a.n_rows - 1;
+    unsigned word = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const float f = __fdiv_rn(__fsub_rn(__ldg(a.feat[k] + gr), a.fc[k]), a.fs[k]);
+      word |= ((unsigned)quant_code(f, a.sa[0]) & 0xffu) << (8 * k);
+    }
+    Aq[0][tid * LD] = (int)word;
+  }
+  int cur = 0;
+  for (int l = 0; l < L - 1; ++l) {                  // layers with H outputs
+    const int KW = (l == 0) ? 1 : KWH;
+    const int* __restrict__ gw = a.wq + a.w_off[l];
+    for (int i = tid; i < H * KW; i += NT) Wq[(i / KW) * LD + (i % KW)] = __ldg(gw + i);
+    __syncthreads();
+    int acc[4][NJ];
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) acc[r][j] = 0;
+    for (int kw = 0; kw < KW; ++kw) {
+      int av[4], wv[NJ];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) av[r] = Aq[cur][(rg * 4 + r) * LD + kw];
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) wv[j] = Wq[(og + 16 * j) * LD + kw];
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) acc[r][j] = __dp4a(av[r], wv[j], acc[r][j]);
+    }
+    // de-quantise, bias, ReLU, re-quantise for the next layer (Q -> node -> DQ chain)
+    const float sc = a.sc[l], sn = a.sa[l + 1];
+    const float* __restrict__ bias = a.bias[l];
+    signed char* nxt = reinterpret_cast<signed char*>(Aq[cur ^ 1]);
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      const int o = og + 16 * j;
+      const float b = __ldg(bias + o);
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        float y = __fadd_rn(__fmul_rn((float)acc[r][j], sc), b);
+        if (!(y > 0.0f)) y = 0.0f;
+        nxt[(rg * 4 + r) * (LD * 4) + o] = (signed char)quant_code(y, sn);
+      }
+    }
+    cur ^= 1;
+    __syncthreads();
+  }
+  // output layer: H -> d (d <= 8), linear, fp32 out
+  {
+    const int l = L - 1, d = a.n_out;
+    const int* __restrict__ gw = a.wq + a.w_off[l];
+    const float sc = a.sc[l];
+    const float* __restrict__ bias = a.bias[l];
+    for (int i = tid; i < TM * d; i += NT) {
+      const int r = i / d, o = i % d;
+      int acc = 0;
+      for (int kw = 0; kw < KWH; ++kw) acc = __dp4a(Aq[cur][r * LD + kw], __ldg(gw + o * KWH + kw), acc);
+      const int row = row0 + r;
+      if (row < a.n_rows) a.out[(size_t)row * d + o] = __fadd_rn(__fmul_rn((float)acc, sc), __ldg(bias + o));
+    }
+  }
+}
+
+}  // namespace
+
+// Requirements (checked by the caller): 3 inputs, hidden widths all H in {64, 128}, 2 <= n_layers <= 8, n_out <= 8.
+int launch_embed_int8(const Int8Args& a, int H, cudaStream_t s) {
+  if (a.n_rows <= 0) return 0;
+  const int grid = (a.n_rows + TM - 1) / TM;
+  if (H == 128) embed_int8_kernel<128><<<grid, NT, 0, s>>>(a);
+  else if (H == 64) embed_int8_kernel<64><<<grid, NT, 0, s>>>(a);
+  else return -1;
+  return 1;
+}
+
+}  // namespace etx

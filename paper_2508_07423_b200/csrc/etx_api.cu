@@ -1,6 +1,7 @@
 // C ABI of libetx (include/etx.h): context, weight staging, workspace carving, and the launch
 // sequences of the four path calls.  No arithmetic of the method happens on the host.
 #include <algorithm>
+#include <cmath>
 #include <cstdlib>
 #include <cstring>
 
@@ -326,6 +327,35 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
   c->edge_enc = dev[2];
   for (int k = 0; k < desc->n_iter; ++k) { c->node_net.push_back(dev[3 + 2 * k]); c->edge_net.push_back(dev[4 + 2 * k]); }
   c->cls = dev.back();
+  {
+    // next row: INT8 codes of the embedding MLP's weights (Eqs. 4.31-4.33): S_w = max|W| / 127,
+    // w_q = clip(round(W / S_w), -127, 127), packed 4 consecutive inputs per word, rows padded with zeros
+    const HostMlp& m = mlps[0];
+    std::vector<int> codes;
+    const float* W = h_weights;
+    for (int l = 0; l < m.n_layers; ++l) {
+      const int fi = m.dims[l], fo = m.dims[l + 1], kw = (fi + 3) / 4;
+      float mx = 0.0f;
+      for (size_t i = 0; i < (size_t)fi * fo; ++i) mx = std::max(mx, std::fabs(W[i]));
+      const float sw = mx / 127.0f;
+      c->emb_sw[l] = sw;
+      c->emb_wq_off[l] = (int)codes.size();
+      codes.resize(codes.size() + (size_t)fo * kw, 0);
+      for (int o = 0; o < fo; ++o)
+        for (int k = 0; k < fi; ++k) {
+          float q = std::nearbyintf(W[(size_t)o * fi + k] / sw);
+          q = std::min(std::max(q, -127.0f), 127.0f);
+          codes[c->emb_wq_off[l] + (size_t)o * kw + k / 4] |= (int)(((unsigned)(int)q & 0xffu) << (8 * (k % 4)));
+        }
+      W += (size_t)fi * fo + fo;
+    }
+    if (cudaMalloc(&c->d_emb_wq, codes.size() * sizeof(int)) != cudaSuccess ||
+        cudaMemcpy(c->d_emb_wq, codes.data(), codes.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
+      const std::string msg = std::string("int8 weight upload failed: ") + cudaGetErrorString(cudaGetLastError());
+      etx_destroy(c);
+      return fail(nullptr, ETX_ERR_CUDA, msg);
+    }
+  }
   if (desc->precision != ETX_PREC_FP32) {
     // tensor-core weight images for every MLP whose first-layer input is a multiple of the chunk
     // (edge encoder, node/edge networks, classifier); embedding and node encoder (3 inputs) stay SIMT
@@ -382,6 +412,7 @@ etx_status etx_destroy(etx_ctx* c) {
   cudaSetDevice(c->device);
   if (c->d_weights) cudaFree(c->d_weights);
   if (c->d_wimg) cudaFree(c->d_wimg);
+  if (c->d_emb_wq) cudaFree(c->d_emb_wq);
   for (const etx_ctx::ProfRec& r : c->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
   if (c->copy_stream) { cudaStreamDestroy(c->copy_stream); cudaEventDestroy(c->copy_event); }
@@ -453,6 +484,37 @@ etx_status etx_embed(etx_ctx* c, const etx_batch* b, float* d_emb, void* stream)
     c->launches += run_mlp(c, a, (cudaStream_t)stream);
   }
   return check_cuda(c, "etx_embed");
+}
+
+etx_status etx_embed_int8(etx_ctx* c, const etx_batch* b, const float* h_act_alpha, int32_t n_alpha, float* d_emb,
+                          void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (etx_status st = check_batch(c, b)) return st;
+  if (b->n_hits > 0 && !d_emb) return fail(c, ETX_ERR_INVALID, "d_emb is NULL");
+  const int L = c->emb.n_layers;
+  if (!h_act_alpha || n_alpha != L) return fail(c, ETX_ERR_INVALID, "act_alpha needs one calibrated range per embedding layer");
+  for (int l = 0; l < L; ++l)
+    if (!(h_act_alpha[l] > 0.0f)) return fail(c, ETX_ERR_INVALID, "activation ranges must be positive");
+  cudaSetDevice(c->device);
+  Int8Args a;
+  a.n_rows = b->n_hits; a.n_layers = L; a.n_out = c->emb.dims[L];
+  a.feat[0] = b->d_r; a.feat[1] = b->d_phi; a.feat[2] = b->d_z;
+  for (int i = 0; i < 3; ++i) { a.fc[i] = c->desc.norm_center[i]; a.fs[i] = c->desc.norm_scale[i]; }
+  a.wq = c->d_emb_wq;
+  for (int l = 0; l < L; ++l) {
+    a.w_off[l] = c->emb_wq_off[l];
+    a.bias[l] = c->emb.b[l];
+    a.sa[l] = h_act_alpha[l] / 127.0f;
+    a.sc[l] = a.sa[l] * c->emb_sw[l];
+  }
+  a.out = d_emb;
+  {
+    ProfScope ps(c, ETX_K_EMBED, (cudaStream_t)stream);
+    const int n = launch_embed_int8(a, c->emb.dims[1], (cudaStream_t)stream);
+    if (n < 0) return fail(c, ETX_ERR_INVALID, "unsupported embedding width for the INT8 path");
+    c->launches += n;
+  }
+  return check_cuda(c, "etx_embed_int8");
 }
 
 etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, float r2_max,
