@@ -136,7 +136,7 @@ etx_status etx_build_graph(etx_ctx* ctx, const etx_batch* batch, const float* d_
                            int32_t max_plane_gap, int32_t k_max, etx_graph* g, void* stream);
 
 /* a3-a6: encoders + n_iter message-passing steps.  d_edge_enc [n_edges, H] fp32 receives e^n;
- * d_hit_enc [n_hits, H] fp32 receives h^n if not NULL.                                            */
+ * d_hit_enc [n_hits, H] fp32 receives h^n if not NULL.  Both must be 16-byte aligned (ETX_ERR_INVALID).                                            */
 etx_status etx_gnn_forward(etx_ctx* ctx, const etx_batch* batch, const etx_graph* g,
                            float* d_edge_enc, float* d_hit_enc, void* stream);
 

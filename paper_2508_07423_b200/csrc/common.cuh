@@ -61,6 +61,7 @@ struct etx_ctx {
   void* ws = nullptr;
   size_t ws_bytes = 0;
   int64_t launches = 0;
+  bool launch_refused = false;          // a launcher returned < 0 during the current API call (see check_cuda)
   std::string err;
   int* d_emb_wq = nullptr;              // INT8 codes of the embedding MLP's weights (next row), packed 4 per word
   int emb_wq_off[etx::kMaxLayers] = {0};

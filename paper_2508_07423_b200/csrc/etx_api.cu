@@ -157,6 +157,11 @@ etx_status fail(etx_ctx* c, etx_status st, const std::string& msg) {
 }
 
 etx_status check_cuda(etx_ctx* c, const char* where) {
+  if (c && c->launch_refused) {
+    c->launch_refused = false;
+    return fail(c, ETX_ERR_INVALID, std::string(where) + ": a kernel launcher refused its arguments (unsupported layer "
+                                    "shape, or an output buffer that is not 16-byte aligned)");
+  }
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(c, ETX_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
   return ETX_OK;
@@ -201,7 +206,15 @@ struct ProfScope {
 // Precision dispatch.  MLPs with a tensor-core weight image run on tcgen05 (mlp_tc.cu).  The embedding MLP
 // always runs the exact fp32 FFMA kernel (the graph must match the oracle edge for edge); the node encoder,
 // also fed by 3 raw features, runs its first layer in the gather warps of the tensor-core kernel.
+int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s);
+// A launcher that refuses its arguments (unsupported shape, output not 16-byte aligned for the tensor map)
+// must not pass silently: the refusal is recorded and the API call that asked for it returns ETX_ERR_INVALID.
 int run_mlp(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
+  const int n = run_mlp_raw(c, a, s);
+  if (n < 0) { c->launch_refused = true; return 0; }
+  return n;
+}
+int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   if (c->desc.precision == ETX_PREC_FP32 || !a.mlp.wimg) return launch_mlp_simt(a, s);
   TcArgs t;
   t.n_rows = a.n_rows; t.n_seg = a.n_seg; t.K0 = a.mlp.dims[0];
@@ -582,6 +595,8 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
   if (etx_status st = check_batch(c, b)) return st;
   if (!g || g->n_edges < 0 || g->n_edges > g->edge_capacity) return fail(c, ETX_ERR_INVALID, "graph is NULL or not built");
   if (g->n_edges > 0 && !d_edge_enc) return fail(c, ETX_ERR_INVALID, "d_edge_enc is NULL");
+  if (((uintptr_t)d_edge_enc & 15) || ((uintptr_t)d_hit_enc & 15))
+    return fail(c, ETX_ERR_INVALID, "d_edge_enc / d_hit_enc must be 16-byte aligned (vector and TMA accesses)");
   cudaSetDevice(c->device);
   cudaStream_t s = (cudaStream_t)stream;
   if (etx_status st = need_ws(c, carve(c, b->n_events, b->n_hits, 0, false, nullptr))) return st;
@@ -685,6 +700,7 @@ etx_status etx_edge_scores(etx_ctx* c, const etx_graph* g, const float* d_edge_e
   if (!c) return ETX_ERR_INVALID;
   if (!g || g->n_edges < 0) return fail(c, ETX_ERR_INVALID, "graph is NULL or not built");
   if (g->n_edges > 0 && (!d_edge_enc || !d_scores)) return fail(c, ETX_ERR_INVALID, "d_edge_enc / d_scores is NULL");
+  if ((uintptr_t)d_edge_enc & 15) return fail(c, ETX_ERR_INVALID, "d_edge_enc must be 16-byte aligned");
   cudaSetDevice(c->device);
   const int H = c->desc.gnn_hidden;
   MlpArgs a;

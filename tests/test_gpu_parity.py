@@ -171,6 +171,24 @@ def test_radius_extremes_and_empty_inputs(B, c0, c0_oracle):
     assert len(out["src"]) == 0 and out["h"].shape == (2, cfg.gnn_hidden)
 
 
+def test_tc_refuses_misaligned_output(B, c1):
+    """The tensor-core path writes through TMA tensor maps: an output that is not 16-byte aligned is refused loudly."""
+    cfg, batch, blob = c1
+    tc = make_etx(B, cfg, blob, precision=3)
+    db = B.DeviceBatch(batch, tc.device)
+    tc.ensure_workspace(db.n_events, db.n_hits, 100000)
+    g = B.DeviceGraph(db.n_hits, 100000, tc.device)
+    E = tc.etx_build_graph(db, tc.etx_embed(db), synth.r2_max(cfg), cfg.max_plane_gap, g)
+    buf = torch.empty(E * cfg.gnn_hidden + 1, device=tc.device)
+    with pytest.raises(B.EtxError) as ei:
+        tc.etx_gnn_forward(db, g, buf[1:].view(E, cfg.gnn_hidden))
+    assert ei.value.status == B.ETX_ERR_INVALID
+    ok = torch.empty(E, cfg.gnn_hidden, device=tc.device)
+    tc.etx_gnn_forward(db, g, ok)                                 # the context is usable afterwards
+    torch.cuda.synchronize()
+    assert torch.isfinite(ok).all()
+
+
 def test_error_paths(B, c0):
     cfg, batch, blob = c0
     etx = make_etx(B, cfg, blob)
