@@ -137,7 +137,8 @@ struct TcArgs {
   int wide = 0;                                   // one layer, two 128-column output halves per row tile (bf16 modes)
   const unsigned char* wimg = nullptr;            // weight image: swizzled 16 KB tiles in consumption order
   const float* bias[kMaxLayers] = {nullptr};
-  const float* w_last = nullptr;                  // classifier: fp32 weights of the 1-unit output layer
+  const float* w_last = nullptr;                  // classifier: fp32 weights of the 1-unit output layer; narrow output: [128][n_out]
+  int n_out = 1;                                  // units of a narrow output layer (out_mode 2)
   int out_mode = 0; float* out = nullptr; const float* res = nullptr; int out_ld = 0;
   unsigned long long* dbg = nullptr;              // optional [grid][16] cycle counters (ETX_TC_DEBUG)
   int exp_flags = 0;                              // timing experiments only (ETX_TC_EXP): 1 skip gather stores, 2 skip weight copies

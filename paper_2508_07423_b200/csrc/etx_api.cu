@@ -232,18 +232,22 @@ int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
     t.K0 = a.mlp.dims[1];
     t.n_layers = a.mlp.n_layers - 1;
     for (int l = 0; l + 1 < a.mlp.n_layers; ++l) t.bias[l] = a.mlp.b[l + 1];
+    t.n_out = a.mlp.dims[a.mlp.n_layers];
   }
+  // the embedding (narrow linear output, out_mode 2) always runs the 3xTF32 kernel, whatever the GNN's mode:
+  // its result decides graph edges (DESIGN.md section 5 "Embedding on the tensor cores")
+  const int mode = (a.out_mode == 2) ? (int)ETX_PREC_TF32X3 : (int)c->desc.precision;
   t.w_last = a.mlp.Wt[a.mlp.n_layers - 1];         // [H][1] == [H]
   t.out_mode = a.out_mode; t.out = a.out; t.res = a.res; t.out_ld = a.out_ld;
   static const char* expv = getenv("ETX_TC_EXP");                  // developer aid: timing experiments (wrong results)
   t.exp_flags = expv ? atoi(expv) : 0;
   static const bool debug = getenv("ETX_TC_DEBUG") != nullptr;     // developer aid: per-role cycle counters
-  if (!debug) return launch_mlp_tc(t, c->desc.precision, c->sm_count, s);
+  if (!debug) return launch_mlp_tc(t, mode, c->sm_count, s);
   static unsigned long long* d_dbg = nullptr;
   if (!d_dbg) cudaMalloc(&d_dbg, sizeof(unsigned long long) * 32 * 256);
   cudaMemsetAsync(d_dbg, 0, sizeof(unsigned long long) * 32 * 256, s);
   t.dbg = d_dbg;
-  const int n = launch_mlp_tc(t, c->desc.precision, c->sm_count, s);
+  const int n = launch_mlp_tc(t, mode, c->sm_count, s);
   std::vector<unsigned long long> h(32 * 256);
   cudaStreamSynchronize(s);
   cudaMemcpy(h.data(), d_dbg, h.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
@@ -378,6 +382,11 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
     size_t wsrc = 0;
     for (size_t i = 0; i < mlps.size(); ++i) {
       const float* w = h_weights + wsrc;
+      if (i == 0 && mlps[i].n_layers >= 3 && mlps[i].dims[1] == 128 && !getenv("ETX_EMBED_FFMA")) {
+        // embedding: layers 2..L-1 as 3xTF32 MMA chain (layer 1 in the gather warps, the narrow last layer in the epilogue)
+        img_off[i] = img.size();
+        append_wimg(img, mlps[i], w, 1, 0, mlps[i].n_layers - 1, ETX_PREC_TF32X3);
+      }
       if (i == 1 && mlps[i].n_layers >= 2) {             // node encoder: layers 2.. (layer 1 runs in the gather warps)
         img_off[i] = img.size();
         append_wimg(img, mlps[i], w, 1, 0, mlps[i].n_layers, mode);
@@ -411,6 +420,7 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
       m.wimg = c->d_wimg + img_off[i];
       if (img_a[i] != (size_t)-1) { m.wimg_a = c->d_wimg + img_a[i]; m.wimg_b = c->d_wimg + img_b[i]; }
     };
+    if (img_off[0] != (size_t)-1) place(c->emb, 0);
     place(c->node_enc, 1);
     place(c->edge_enc, 2);
     for (int k = 0; k < desc->n_iter; ++k) { place(c->node_net[k], 3 + 2 * k); place(c->edge_net[k], 4 + 2 * k); }

@@ -144,7 +144,8 @@ __device__ __forceinline__ void tmem_cp_128x256b(uint32_t taddr, uint64_t desc) 
   asm volatile("tcgen05.cp.cta_group::1.128x256b [%0], %1;" ::"r"(taddr), "l"(desc) : "memory");
 }
 
-// VAR: 0 regular, 1 wide (one layer, 256 outputs), 2 feat (first-layer operand computed from 3 raw features)
+// VAR: 0 regular, 1 wide (one layer, 256 outputs), 2 feat (first-layer operand computed from 3 raw features),
+//      3 feat + narrow linear output layer of <= 8 units computed in the epilogue registers (embedding MLP)
 template <int MODE, int VAR>
 __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap tmap) {
   using C = Cfg<MODE>;
@@ -174,18 +175,19 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   unsigned char* gen = smem_raw + (base - raw);
   float* bias_s = reinterpret_cast<float*>(gen + (NSW + NSA) * kStageBytes + kAtomBytes);   // [kMaxLayers][128]
   float* wlast_s = bias_s + kMaxLayers * HW;                                                  // [128]
-  Bars* bars = reinterpret_cast<Bars*>(wlast_s + HW);
+  Bars* bars = reinterpret_cast<Bars*>(wlast_s + (VAR == 3 ? 8 * HW : HW));            // VAR 3: [128][8]
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_tiles = (a.n_rows + TM - 1) / TM;
-  const int n_gemm = (a.out_mode == 3) ? a.n_layers - 1 : a.n_layers;
+  const int n_gemm = (a.out_mode == 3 || VAR == 3) ? a.n_layers - 1 : a.n_layers;
   const int nc1 = a.K0 / KA;
   const int my_tiles = (n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles blockIdx.x + i * gridDim.x
   // Wide mode (one layer, 256 outputs: the per-hit projections [A h | B h] of the factorised edge MLPs):
   // the two slots of a "pair" are the two 128-column output halves of ONE row tile -- the operand entries
   // are gathered once and serve both halves, each half has its own weight chunks and accumulator.
   constexpr bool wide = (VAR == 1);             // (compile-time switches: the regular kernels carry none of it)
-  constexpr bool feat = (VAR == 2);
+  constexpr bool feat = (VAR == 2 || VAR == 3);
+  constexpr bool narrow = (VAR == 3);
   static_assert(!wide || NSLOT == 2, "wide mode needs two accumulator slots");
   const int n_pairs = wide ? my_tiles : (my_tiles + NSLOT - 1) / NSLOT;
   auto slots_of = [&](int pi) { return wide ? 2 : ((my_tiles - pi * NSLOT) < NSLOT ? (my_tiles - pi * NSLOT) : NSLOT); };
@@ -226,7 +228,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
     const int l = i / HW, j = i % HW;
     bias_s[i] = (l < n_gemm) ? __ldg(a.bias[l] + j) : 0.f;
   }
-  if (a.out_mode == 3)
+  if constexpr (narrow) {                        // last layer's weights [k][n_out] (k-major) padded to 8 units per k
+    for (int i = threadIdx.x; i < HW * 8; i += kThreads)
+      wlast_s[i] = (i % 8) < a.n_out ? __ldg(a.w_last + (i / 8) * a.n_out + (i % 8)) : 0.f;
+  } else if (a.out_mode == 3)
     for (int i = threadIdx.x; i < HW; i += kThreads) wlast_s[i] = __ldg(a.w_last + i);
   if (threadIdx.x == 0) {
     for (int i = 0; i < NSW; ++i) { mbar_init(smem_u32(&bars->w_full[i]), 1); mbar_init(smem_u32(&bars->w_empty[i]), 1); }
@@ -517,6 +522,36 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
           }
           tc_fence_before();
           mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
+        } else if (narrow) {
+          // ---- narrow linear output (embedding, Eq. 4.27 with identity output): last hidden layer, then
+          // n_out <= 8 units as fp32 FMA chains over the 128 hidden values of the row, in registers
+          if (hh == 0) {
+            float o8[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll 1
+            for (int q = 0; q < HW / 32; ++q) {
+              uint32_t v[32];
+              tmem_ld32(acc + q * 32, v);
+              tc_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 32; ++i) {
+                const float hv = fmaxf(__uint_as_float(v[i]) + bias[q * 32 + i], 0.f);
+                const float4 w0 = *reinterpret_cast<const float4*>(wlast_s + (q * 32 + i) * 8);
+                const float4 w1 = *reinterpret_cast<const float4*>(wlast_s + (q * 32 + i) * 8 + 4);
+                o8[0] = fmaf(hv, w0.x, o8[0]); o8[1] = fmaf(hv, w0.y, o8[1]); o8[2] = fmaf(hv, w0.z, o8[2]); o8[3] = fmaf(hv, w0.w, o8[3]);
+                o8[4] = fmaf(hv, w1.x, o8[4]); o8[5] = fmaf(hv, w1.y, o8[5]); o8[6] = fmaf(hv, w1.z, o8[6]); o8[7] = fmaf(hv, w1.w, o8[7]);
+              }
+            }
+            tc_fence_before();
+            mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
+            const int row = tile * TM + et;
+            if (row < a.n_rows) {
+#pragma unroll
+              for (int o = 0; o < 8; ++o)
+                if (o < a.n_out) a.out[(size_t)row * a.out_ld + o] = o8[o] + __ldg(a.bias[a.n_layers - 1] + o);
+            }
+          } else {
+            mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
+          }
         } else if (a.out_mode == 3) {
           // ---- classifier: last hidden layer, then 1 unit + sigmoid; column half 0
           // warps do all 128 columns of their rows (a cross-warp sum is not worth it for 1 unit).
@@ -792,7 +827,7 @@ int launch_mode(const TcArgs& a, int sm_count, cudaStream_t s) {
   using C = Cfg<MODE>;
   static bool configured = false;
   const size_t smem = 1024 + (size_t)(C::NSTAGE_W + C::NSTAGE_A) * C::PIECES * kAtomBytes + kAtomBytes +
-                      (kMaxLayers + 1) * HW * sizeof(float) + sizeof(Bars) + 64;
+                      (kMaxLayers + (VAR == 3 ? 8 : 1)) * HW * sizeof(float) + sizeof(Bars) + 64;
   if (!configured) {
     cudaFuncSetAttribute(mlp_tc_kernel<MODE, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
@@ -801,7 +836,7 @@ int launch_mode(const TcArgs& a, int sm_count, cudaStream_t s) {
   const int grid = n_tiles < sm_count ? n_tiles : sm_count;
   CUtensorMap tmap;
   std::memset(&tmap, 0, sizeof(tmap));
-  if (a.out_mode != 3 && !encode_out_map(&tmap, a.out, a.n_rows, VAR == 1 ? 2 * HW : HW, a.out_ld)) return -1;
+  if (a.out_mode != 3 && VAR != 3 && !encode_out_map(&tmap, a.out, a.n_rows, VAR == 1 ? 2 * HW : HW, a.out_ld)) return -1;
   mlp_tc_kernel<MODE, VAR><<<grid, kThreads, smem, s>>>(a, tmap);
   return 1;
 }
@@ -820,8 +855,12 @@ int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s) {
     if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, 1>(a, sm_count, s);
     return -1;
   }
-  if (a.w1) {                                    // first-layer operand computed from 3 features (node encoder)
+  if (a.w1) {                                    // first-layer operand computed from 3 features (node encoder, embedding)
     if (a.n_add != 0 || a.n_seg != 0 || a.K0 != HW || !a.b1 || !a.feat[0] || !a.feat[1] || !a.feat[2]) return -1;
+    if (a.out_mode == 2) {                       // narrow linear output (embedding): TF32X3 only
+      if (mode != ETX_PREC_TF32X3 || a.n_out < 1 || a.n_out > 8 || a.n_layers < 2) return -1;
+      return launch_mode<ETX_PREC_TF32X3, 3>(a, sm_count, s);
+    }
     if (mode == ETX_PREC_TF32X3) return launch_mode<ETX_PREC_TF32X3, 2>(a, sm_count, s);
     if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, 2>(a, sm_count, s);
     if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, 2>(a, sm_count, s);
