@@ -374,8 +374,9 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
     }
   }
   if (desc->precision != ETX_PREC_FP32) {
-    // tensor-core weight images for every MLP whose first-layer input is a multiple of the chunk
-    // (edge encoder, node/edge networks, classifier); embedding and node encoder (3 inputs) stay SIMT
+    // tensor-core weight images: edge encoder, node/edge networks, classifier (first-layer input a multiple of
+    // the chunk); node encoder and a 128-wide embedding with >= 2 hidden layers from their second layer on (their
+    // 3-feature first layer is computed in the gather warps).  Other embeddings keep the FFMA kernel.
     std::vector<unsigned char> img;
     std::vector<size_t> img_off(mlps.size(), (size_t)-1), img_a(mlps.size(), (size_t)-1), img_b(mlps.size(), (size_t)-1);
     const int H = desc->gnn_hidden, mode = desc->precision;

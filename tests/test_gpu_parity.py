@@ -325,3 +325,31 @@ def test_tc_rejects_unsupported_width(B, c0):
     with pytest.raises(B.EtxError) as ei:
         make_etx(B, cfg, blob, precision=1)                          # H = 64: tensor-core path needs H = 128
     assert ei.value.status == B.ETX_ERR_INVALID
+
+
+@pytest.mark.parametrize("widths", [(3, 128, 128, 3), (3, 128, 128, 128, 8), (3, 128, 128, 128, 128, 1), (3, 128, 128, 128, 4)])
+@pytest.mark.parametrize("prec", [synth.PREC_TF32X3, synth.PREC_BF16])
+def test_tc_embedding_shapes_and_ragged_tail(B, widths, prec):
+    """a0+a1 on the tensor cores (3xTF32 hidden layers, narrow linear output in the epilogue)
+    for 1..3 hidden MMA layers and 1..8 output units, on batches whose hit count is not a multiple of the 128-row
+    tile, in every GNN precision mode (the embedding is 3xTF32 in all of them): |emb - oracle| <= 2e-6 (section 6),
+    rows past n_hits untouched, and an empty batch is a no-op."""
+    cfg = dataclasses.replace(synth.CONFIGS["c2"], emb_widths=widths, precision=prec)
+    blob = synth.generate_weights(cfg)
+    spec = synth.model_layout(cfg)[0]
+    etx = B.Etx(B.make_desc(cfg, precision=prec), blob)
+    d = widths[-1]
+    for events in ([7], [3, 11, 200, 512, 999], []):
+        batch = synth.generate_events(cfg, events)
+        n = len(batch["r"])
+        db = B.DeviceBatch(batch, etx.device)
+        out = torch.full((n + 5, d), 7.0, device=etx.device)
+        etx.etx_embed(db, emb=out)
+        torch.cuda.synchronize()
+        assert torch.all(out[n:] == 7.0)
+        if n == 0:
+            continue
+        assert n % 128 != 0
+        fe, _ = orc.features(batch, synth.NORM_CENTER, synth.NORM_SCALE)
+        ora = orc.mlp(fe, spec.dims, blob, spec.offset)
+        assert np.abs(out[:n].cpu().numpy().astype(np.float64) - ora).max() <= 2e-6
