@@ -86,22 +86,34 @@ def test_full_batch_sampled_events(B, name, sample, precision):
     ev = check_properties(cfg, batch, out)
     assert abs(out["E"] / len(batch["r"]) - cfg.target_degree) < 0.08 * cfg.target_degree
     ep = batch["event_ptr"].astype(np.int64)
-    worst = 0.0
+    oras, emb2, n_border = {}, out["emb"].copy(), 0
     for e in sample:
         sub = synth.select_events(batch, [e])
-        ora = oracle_path(cfg, sub, blob)
+        ora = oras[e] = oracle_path(cfg, sub, blob)
         sel = ev[out["src"]] == e
         gs, gd = out["src"][sel] - ep[e], out["dst"][sel] - ep[e]
         np.testing.assert_allclose(out["emb"][ep[e]:ep[e + 1]], ora["emb"], rtol=0, atol=2e-6)
         _, _, border = orc.build_graph(sub["event_ptr"], sub["plane"], ora["emb"], synth.r2_max(cfg),
                                        cfg.max_plane_gap, band=1e-5, want_border=True)
         got, want = set(zip(gs.tolist(), gd.tolist())), set(zip(ora["src"].tolist(), ora["dst"].tolist()))
-        assert (got ^ want) <= set(map(tuple, border.tolist()))     # differences only inside the 1e-5 band
-        if got == want:
-            err = float(np.abs(out["scores"][sel].astype(np.float64) - ora["scores"]).max())
-            worst = max(worst, err)
-            assert err <= TOL[cfg.precision], (name, e, err)
-    print(f"{name} precision={cfg.precision}: N={len(batch['r'])} E={out['E']} worst sampled |score - oracle| = {worst:.3g}")
+        assert (got ^ want) <= set(map(tuple, border.tolist()))     # end to end: differences only inside the 1e-5 band
+        n_border += len(got ^ want)
+        emb2[ep[e]:ep[e + 1]] = ora["emb"]
+    # Scores: the same full batch again with the sampled events' embeddings replaced by the oracle's, so that their
+    # graphs must equal the oracle's bit for bit (BJ's graph gate) and EVERY sampled event's scores are compared
+    # (an event whose end-to-end graph differs by a border pair has legitimately different messages).
+    out2 = run_full(B, cfg, batch, blob, precision, emb_from=emb2)
+    worst = 0.0
+    for e in sample:
+        ora = oras[e]
+        sel = ev[out2["src"]] == e
+        np.testing.assert_array_equal(out2["src"][sel] - ep[e], ora["src"])
+        np.testing.assert_array_equal(out2["dst"][sel] - ep[e], ora["dst"])
+        err = float(np.abs(out2["scores"][sel].astype(np.float64) - ora["scores"]).max())
+        worst = max(worst, err)
+        assert err <= TOL[cfg.precision], (name, e, err)
+    print(f"{name} precision={cfg.precision}: N={len(batch['r'])} E={out['E']} worst sampled |score - oracle| = {worst:.3g} "
+          f"({n_border} border-pair differences end to end in the sampled events)")
 
 
 @pytest.mark.parametrize("name,precisions", [("c2", [synth.PREC_BF16X3, synth.PREC_TF32X3, synth.PREC_BF16]),
