@@ -327,6 +327,24 @@ def run_ours(args):
     if stages["scatter"]["ms"] > 0:
         stages["scatter"]["gbs"] = sc_bytes / (stages["scatter"]["ms"] * 1e-3) / 1e9
         stages["scatter"]["hbm_frac"] = stages["scatter"]["gbs"] / pk["hbm_gbs"]
+    # graph build (a2): the windowed all-pairs test is bound by plain fp32 ALU work, not by HBM: report
+    # both.  Pair tests = sum over events and planes p of n_p x (n_{p+1} + .. + n_{p+G}); 3d flop each (d subtractions,
+    # d multiplications, d-1 additions and the comparison, individually rounded: no FMA); the kernels sweep the
+    # candidates twice (count pass, fill pass).  Bytes: embeddings + plane ids read, both CSR structures written.
+    if stages["graph"]["ms"] > 0:
+        n_pl = int(batch["plane"].max()) + 1 if N else 1
+        ev_of = np.repeat(np.arange(n_ev), np.diff(batch["event_ptr"]))
+        cnt = np.bincount(ev_of * n_pl + batch["plane"].astype(np.int64), minlength=n_ev * n_pl).reshape(n_ev, n_pl)
+        pairs = sum(int((cnt[:, :n_pl - k].astype(np.int64) * cnt[:, k:]).sum()) for k in range(1, gap + 1))
+        d_emb = cfg.emb_widths[-1]
+        t_s = stages["graph"]["ms"] * 1e-3
+        alu_peak = 148 * 128 * pk["sm_max_mhz"] * 1e6           # unfused fp32 operations per second
+        g_bytes = N * (4 * d_emb + 1) + 2 * (4 * (N + 1) + 8 * E)
+        stages["graph"].update({"pair_tests": pairs, "pair_tests_per_s": pairs / t_s,
+                                "alu_frac": pairs * 3 * d_emb / t_s / alu_peak,
+                                "alu_frac_executed": 2 * pairs * 3 * d_emb / t_s / alu_peak,
+                                "gbs": g_bytes / t_s / 1e9, "hbm_frac": g_bytes / t_s / 1e9 / pk["hbm_gbs"],
+                                "bound": "alu (fp32, unfused): 148 SM x 128 lanes x %.0f MHz" % pk["sm_max_mhz"]})
     gnn_ms = sum(stages[k]["ms"] for k in ("node_enc", "edge_enc", "scatter", "node_net", "edge_net", "edge_proj"))
     stages["message_passing_total"] = {"ms": gnn_ms, "events_per_s": n_ev / (gnn_ms * 1e-3) if gnn_ms else None}
 

@@ -481,37 +481,35 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
               tmem_st32(hid + c * 32, w);
               tmem_st32(hid + HID_COLS + c * 32, v);
             } else if constexpr (P == 2) {       // BF16X3: 64 accumulator columns -> 32 hi + 32 lo packed columns
-              uint32_t v0[32], wh[32], wl[32];
-              tmem_ld32(acc + c * 64, v0);
-              tc_wait_ld();
-#pragma unroll
-              for (int i = 0; i < 16; ++i)
-                split_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 2 * i], 0.f),
-                             fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 2 * i + 1], 0.f), wh[i], wl[i]);
-              tmem_ld32(acc + c * 64 + 32, v0);
+              uint32_t va[32], vb[32], wh[32], wl[32];     // both loads in flight, one wait (va/vb die pair by pair as wh/wl are born)
+              tmem_ld32(acc + c * 64, va);
+              tmem_ld32(acc + c * 64 + 32, vb);
               tc_wait_ld();
               EP_ACC(0);
 #pragma unroll
               for (int i = 0; i < 16; ++i)
-                split_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
-                             fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f), wh[16 + i], wl[16 + i]);
+                split_bf16x2(fmaxf(__uint_as_float(va[2 * i]) + bias[c * 64 + 2 * i], 0.f),
+                             fmaxf(__uint_as_float(va[2 * i + 1]) + bias[c * 64 + 2 * i + 1], 0.f), wh[i], wl[i]);
+#pragma unroll
+              for (int i = 0; i < 16; ++i)
+                split_bf16x2(fmaxf(__uint_as_float(vb[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
+                             fmaxf(__uint_as_float(vb[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f), wh[16 + i], wl[16 + i]);
               tmem_st32(hid + c * 32, wh);
               tmem_st32(hid + HID_COLS + c * 32, wl);
             } else {
-              uint32_t v0[32], w[32];
-              tmem_ld32(acc + c * 64, v0);
-              tc_wait_ld();
-#pragma unroll
-              for (int i = 0; i < 16; ++i)
-                w[i] = pack_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 2 * i], 0.f),
-                                   fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 2 * i + 1], 0.f));
-              tmem_ld32(acc + c * 64 + 32, v0);
+              uint32_t va[32], vb[32], w[32];
+              tmem_ld32(acc + c * 64, va);
+              tmem_ld32(acc + c * 64 + 32, vb);
               tc_wait_ld();
               EP_ACC(0);
 #pragma unroll
               for (int i = 0; i < 16; ++i)
-                w[16 + i] = pack_bf16x2(fmaxf(__uint_as_float(v0[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
-                                        fmaxf(__uint_as_float(v0[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f));
+                w[i] = pack_bf16x2(fmaxf(__uint_as_float(va[2 * i]) + bias[c * 64 + 2 * i], 0.f),
+                                   fmaxf(__uint_as_float(va[2 * i + 1]) + bias[c * 64 + 2 * i + 1], 0.f));
+#pragma unroll
+              for (int i = 0; i < 16; ++i)
+                w[16 + i] = pack_bf16x2(fmaxf(__uint_as_float(vb[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
+                                        fmaxf(__uint_as_float(vb[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f));
               tmem_st32(hid + c * 32, w);
             }
             EP_ACC(1);
