@@ -46,6 +46,9 @@ struct Workspace {            // carved from the caller's buffer by carve_worksp
   size_t total = 0;
 };
 
+int launch_scatter_atomic(int n_nodes, long long n_edges, int H, const int32_t* src, const int32_t* dst,
+                          const float* e, float* m, cudaStream_t s);   // measured comparison only (ETX_SCATTER_ATOMIC)
+
 }  // namespace etx
 
 struct etx_ctx {
@@ -166,5 +169,8 @@ int launch_embed_int8(const Int8Args& a, int H, cudaStream_t s);
 // ---- scatter.cu
 int launch_scatter(int n_nodes, int H, const int32_t* row_ptr, const int32_t* in_ptr,
                    const int32_t* in_perm, const float* e, float* m, int32_t* counter /*device, 1 int*/, cudaStream_t s);
+
+int launch_scatter_atomic(int n_nodes, long long n_edges, int H, const int32_t* src, const int32_t* dst,
+                          const float* e, float* m, cudaStream_t s);   // measured comparison only (ETX_SCATTER_ATOMIC)
 
 }  // namespace etx

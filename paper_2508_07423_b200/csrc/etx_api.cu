@@ -669,6 +669,9 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
     // a4: m = [sum out, sum in] of e^k
     {
       ProfScope ps(c, ETX_K_SCATTER, s);
+      static const bool atomic = getenv("ETX_SCATTER_ATOMIC") != nullptr;   // developer aid: the measured alternative
+      if (atomic && H == 128) c->launches += launch_scatter_atomic(N, E, H, g->d_src, g->d_dst, (const float*)d_edge_enc, w.m, s);
+      else
       c->launches += launch_scatter(N, H, g->d_row_ptr, g->d_in_ptr, g->d_in_perm, d_edge_enc, w.m, w.sched, s);
     }
     {  // a5: h += phi_k([h, m])

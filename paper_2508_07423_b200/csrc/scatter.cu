@@ -75,7 +75,35 @@ __global__ void __launch_bounds__(256) scatter_kernel(int n_nodes, const int32_t
   }
 }
 
+// The alternative the thesis' pipeline used (scatter_add), kept ONLY as a measured comparison
+// (ETX_SCATTER_ATOMIC=1, developer aid): one warp per edge row, one vector reduction
+// (red.global.add.v4.f32) per lane into m[src] (outgoing half) and m[dst] (incoming half) of a zeroed m.
+// Summation order is whatever the L2 serialises: not deterministic, and measured slower.
+__global__ void __launch_bounds__(256) scatter_atomic_kernel(long long n_edges, const int32_t* __restrict__ src,
+                                                             const int32_t* __restrict__ dst,
+                                                             const float* __restrict__ e, float* __restrict__ m) {
+  const int lane = threadIdx.x & 31;
+  const long long n_warps = (long long)gridDim.x * (blockDim.x >> 5);
+  for (long long k = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); k < n_edges; k += n_warps) {
+    const float4 v = __ldg(reinterpret_cast<const float4*>(e) + k * 32 + lane);
+    float* po = m + (size_t)__ldg(src + k) * 256 + lane * 4;
+    float* pi = m + (size_t)__ldg(dst + k) * 256 + 128 + lane * 4;
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(po), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(pi), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+  }
+}
+
 }  // namespace
+
+int launch_scatter_atomic(int n_nodes, long long n_edges, int H, const int32_t* src, const int32_t* dst,
+                          const float* e, float* m, cudaStream_t s) {
+  if (n_nodes <= 0 || H != 128) return n_nodes <= 0 ? 0 : -1;
+  cudaMemsetAsync(m, 0, sizeof(float) * (size_t)n_nodes * 2 * H, s);
+  if (n_edges <= 0) return 0;
+  const long long need = (n_edges + 7) / 8;
+  scatter_atomic_kernel<<<(int)(need < 148 * 8 ? need : 148 * 8), 256, 0, s>>>(n_edges, src, dst, e, m);
+  return 1;
+}
 
 int launch_scatter(int n_nodes, int H, const int32_t* row_ptr, const int32_t* in_ptr,
                    const int32_t* in_perm, const float* e, float* m, int32_t* counter, cudaStream_t s) {
