@@ -101,13 +101,12 @@ search_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t*
       const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
       const int j1 = pp[top + 1];
       const int base_out = (MODE == 1) ? row_ptr[i] : 0;
+      const float r2 = a.r2_max;
       for (int base = j0; base < j1; base += 32) {
         const int j = base + lane;
-        bool ok = false;
-        if (j < j1) {
-          load_emb<D>(a.emb, j, a.d, other);
-          ok = dist2<D>(me, other, a.d) < a.r2_max;
-        }
+        // branch-free body: lanes past the end test the last candidate again and are masked out of the vote
+        load_emb<D>(a.emb, j < j1 ? j : j1 - 1, a.d, other);
+        const bool ok = (dist2<D>(me, other, a.d) < r2) & (j < j1);
         const unsigned b = __ballot_sync(kFull, ok);
         if (ok) {
           if (MODE == 0) {
