@@ -59,6 +59,35 @@ __device__ __forceinline__ void load_emb(const float* __restrict__ emb, int i, i
   }
 }
 
+// Packed fp32 pairs (sm_100 add/mul.rn.f32x2): two IEEE round-to-nearest operations per instruction, each lane
+// rounded on its own, never contracted -- the same values as the scalar __fsub_rn / __fmul_rn, half the issue slots.
+__device__ __forceinline__ unsigned long long pack2(float x, float y) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y));
+  return r;
+}
+__device__ __forceinline__ unsigned long long add2_rn(unsigned long long a, unsigned long long b) {
+  unsigned long long r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ unsigned long long mul2_rn(unsigned long long a, unsigned long long b) {
+  unsigned long long r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+// d = 4: d^2 = ((q0 + q1) + q2) + q3 with q_c = (b_c - a_c)^2 = (a_c - b_c)^2 exactly (negation is exact), the
+// differences and squares as packed pairs, the sum left to right as Eq. 8.1's oracle evaluates it.
+// na01 / na23 hold the NEGATED coordinates of the source hit.
+__device__ __forceinline__ float dist2_d4(unsigned long long na01, unsigned long long na23, const float4& b) {
+  const unsigned long long t01 = add2_rn(pack2(b.x, b.y), na01), t23 = add2_rn(pack2(b.z, b.w), na23);
+  const unsigned long long q01 = mul2_rn(t01, t01), q23 = mul2_rn(t23, t23);
+  float q0, q1, q2, q3;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(q0), "=f"(q1) : "l"(q01));
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(q2), "=f"(q3) : "l"(q23));
+  return __fadd_rn(__fadd_rn(__fadd_rn(q0, q1), q2), q3);
+}
+
 template <int D>
 __device__ __forceinline__ float dist2(const float (&a)[8], const float (&b)[8], int d) {
   float s = 0.0f;
@@ -102,11 +131,18 @@ search_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t*
       const int j1 = pp[top + 1];
       const int base_out = (MODE == 1) ? row_ptr[i] : 0;
       const float r2 = a.r2_max;
+      const unsigned long long nme01 = pack2(-me[0], -me[1]), nme23 = pack2(-me[2], -me[3]);
       for (int base = j0; base < j1; base += 32) {
         const int j = base + lane;
         // branch-free body: lanes past the end test the last candidate again and are masked out of the vote
-        load_emb<D>(a.emb, j < j1 ? j : j1 - 1, a.d, other);
-        const bool ok = (dist2<D>(me, other, a.d) < r2) & (j < j1);
+        const int jc = j < j1 ? j : j1 - 1;
+        bool ok;
+        if constexpr (D == 4) {
+          ok = (dist2_d4(nme01, nme23, __ldg(reinterpret_cast<const float4*>(a.emb) + jc)) < r2) & (j < j1);
+        } else {
+          load_emb<D>(a.emb, jc, a.d, other);
+          ok = (dist2<D>(me, other, a.d) < r2) & (j < j1);
+        }
         const unsigned b = __ballot_sync(kFull, ok);
         if (ok) {
           if (MODE == 0) {
