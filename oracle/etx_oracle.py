@@ -227,6 +227,43 @@ def wcc(n_hits: int, src, dst, scores, score_min: float) -> np.ndarray:
     return labels
 
 
+def triplets(n_hits: int, src, dst, scores, score_min: float) -> Dict[str, np.ndarray]:
+    """NEXT-4 (triplet building, Fig. 8.13): the edge connections of the purified hit graph (edges
+    with score >= score_min, the same cut as ``wcc``).  A triplet is two kept edges sharing a hit C:
+
+    * articulation: A -> C and C -> B (the common hit in the middle)        -> rows (edge A->C, edge C->B)
+    * left elbow:   C -> A and C -> B (the common hit on the left)          -> rows (e1, e2), e1 < e2
+    * right elbow:  A -> C and B -> C (the common hit on the right)         -> rows (e1, e2), e1 < e2
+
+    Plain definition, pure Python loops: for every hit C in ascending order, its kept incoming edges I(C) and
+    kept outgoing edges O(C) in ascending edge id; articulations = I(C) x O(C) (first index slowest), elbows =
+    the unordered pairs of O(C) / of I(C) in lexicographic order.  Returns int32 arrays [n, 2] of EDGE IDS under
+    "articulation", "left_elbow", "right_elbow".  The thesis fixes no order (several listings are correct);
+    this one is the order the GPU path is required to reproduce, so the comparison is an array comparison."""
+    src = np.asarray(src, np.int64)
+    dst = np.asarray(dst, np.int64)
+    keep = _f32(scores) >= np.float32(score_min)
+    ins: List[List[int]] = [[] for _ in range(n_hits)]
+    outs: List[List[int]] = [[] for _ in range(n_hits)]
+    for e in range(len(src)):                       # ascending edge id
+        if keep[e]:
+            outs[src[e]].append(e)
+            ins[dst[e]].append(e)
+    art, left, right = [], [], []
+    for c in range(n_hits):
+        for a in ins[c]:
+            for b in outs[c]:
+                art.append((a, b))
+        for i, a in enumerate(outs[c]):
+            for b in outs[c][i + 1:]:
+                left.append((a, b))
+        for i, a in enumerate(ins[c]):
+            for b in ins[c][i + 1:]:
+                right.append((a, b))
+    as_arr = lambda t: np.asarray(t, np.int32).reshape(-1, 2)
+    return {"articulation": as_arr(art), "left_elbow": as_arr(left), "right_elbow": as_arr(right)}
+
+
 def run_path(batch: Dict[str, np.ndarray], blob: np.ndarray, layout: Dict[str, Tuple[Tuple[int, ...], int]],
              H: int, n_iter: int, r2_max: float, gap: int, center, scale, n_planes: int = 26,
              graph: Optional[Tuple[np.ndarray, np.ndarray]] = None) -> Dict[str, np.ndarray]:
