@@ -272,6 +272,14 @@ def run_ours(args):
         sizes = torch.bincount(labels[:N].long(), minlength=1)
         next_rows["wcc_tracks"] = {"ms": wcc_ms, "events_per_s": n_ev / (wcc_ms * 1e-3), "score_min": 0.5,
                                    "components_ge3_hits": int((sizes >= 3).sum().item())}
+        # NEXT-4 (triplet part): triplet building on the same purified graph
+        tr = etx.etx_build_triplets(db, g, scores, 0.5)
+        n_tr = [int(tr[k].shape[0]) for k in ("articulation", "left_elbow", "right_elbow")]
+        del tr
+        tms, _ = time3(lambda: etx.etx_build_triplets(db, g, scores, 0.5, capacity=sum(n_tr)) and None)
+        next_rows["triplets"] = {"ms": tms, "events_per_s": n_ev / (tms * 1e-3), "score_min": 0.5,
+                                 "articulations": n_tr[0], "left_elbows": n_tr[1], "right_elbows": n_tr[2],
+                                 "rows_per_s": sum(n_tr) / (tms * 1e-3)}
         # NEXT-2: k_max-capped search (the thesis' k_max = 50, which rarely binds, and a cap that does)
         g2 = binding.DeviceGraph(N, cap, dev)
         for kk in (50, 4):

@@ -152,6 +152,26 @@ etx_status etx_edge_scores(etx_ctx* ctx, const etx_graph* g, const float* d_edge
 etx_status etx_build_tracks(etx_ctx* ctx, const etx_batch* batch, const etx_graph* g, const float* d_scores,
                             float score_min, int32_t* d_labels, void* stream);
 
+/* Next row: triplet building (Fig. 8.13).  Two edges of the purified hit graph (score >= score_min,
+ * the cut of etx_build_tracks) that share a hit C form an articulation (A -> C, C -> B), a left elbow (C -> A,
+ * C -> B) or a right elbow (A -> C, B -> C).  Rows are pairs of EDGE IDS (d_first[i], d_second[i]) in three
+ * consecutive sections -- n[0] articulations (first = the incoming edge A -> C, second = the outgoing edge
+ * C -> B), then n[1] left elbows, then n[2] right elbows (first < second) -- each section ordered by (shared hit,
+ * first, second).  d_ptr [3][n_hits + 1] receives, per kind, the offset of every shared hit's rows inside its
+ * section (CSR by shared hit; d_ptr[k][n_hits] = n[k]).  All buffers are caller-owned DEVICE memory.
+ * Synchronises the stream to return the counts.  n[0] + n[1] + n[2] > capacity: ETX_ERR_CAPACITY with n filled
+ * and d_first / d_second untouched.  A kind with more than 2^31 - 1 rows is ETX_ERR_CAPACITY as well.
+ * Needs the workspace of etx_build_graph.  Deterministic (integer work, one fixed order).                     */
+typedef struct {
+  int64_t capacity;           /* in: rows available in d_first / d_second                                   */
+  int64_t n[3];               /* out: articulations, left elbows, right elbows                              */
+  int32_t* d_ptr;             /* [3][n_hits + 1]                                                            */
+  int32_t* d_first;           /* [capacity]                                                                 */
+  int32_t* d_second;          /* [capacity]                                                                 */
+} etx_triplets;
+etx_status etx_build_triplets(etx_ctx* ctx, const etx_batch* batch, const etx_graph* g, const float* d_scores,
+                              float score_min, etx_triplets* t, void* stream);
+
 /* Whole path with HOST buffers: copies the batch host->device, runs a0..a7, copies src/dst/scores
  * back (h_src, h_dst may be NULL).  Needs a workspace sized with with_host_path = 1.  Host buffers
  * should be pinned for the copies to be asynchronous.  Synchronises the stream before returning.  */

@@ -21,7 +21,8 @@ ETX_OK, ETX_ERR_INVALID, ETX_ERR_CAPACITY, ETX_ERR_CUDA, ETX_ERR_UNSORTED, ETX_E
 
 EXPORTS = ["etx_weight_count", "etx_create", "etx_destroy", "etx_last_error", "etx_workspace_bytes",
            "etx_set_workspace", "etx_embed", "etx_build_graph", "etx_gnn_forward", "etx_edge_scores",
-           "etx_infer_host", "etx_launch_count", "etx_profile_enable", "etx_profile_read", "etx_build_tracks"]
+           "etx_infer_host", "etx_launch_count", "etx_profile_enable", "etx_profile_read", "etx_build_tracks",
+           "etx_build_triplets"]
 KERNEL_CLASSES = ["embed", "graph", "node_enc", "edge_enc", "scatter", "node_net", "edge_net", "cls", "tracks", "edge_proj"]
 
 
@@ -54,6 +55,11 @@ class Graph(C.Structure):
     _fields_ = [("edge_capacity", C.c_int64), ("n_edges", C.c_int64), ("d_row_ptr", C.c_void_p),
                 ("d_src", C.c_void_p), ("d_dst", C.c_void_p), ("d_in_ptr", C.c_void_p),
                 ("d_in_perm", C.c_void_p)]
+
+
+class Triplets(C.Structure):
+    _fields_ = [("capacity", C.c_int64), ("n", C.c_int64 * 3), ("d_ptr", C.c_void_p), ("d_first", C.c_void_p),
+                ("d_second", C.c_void_p)]
 
 
 _lib = None
@@ -99,6 +105,9 @@ def load_library():
         lib.etx_build_tracks.restype = C.c_int
         lib.etx_build_tracks.argtypes = [C.c_void_p, C.POINTER(Batch), C.POINTER(Graph), C.c_void_p, C.c_float,
                                          C.c_void_p, C.c_void_p]
+        lib.etx_build_triplets.restype = C.c_int
+        lib.etx_build_triplets.argtypes = [C.c_void_p, C.POINTER(Batch), C.POINTER(Graph), C.c_void_p, C.c_float,
+                                           C.POINTER(Triplets), C.c_void_p]
         lib.etx_profile_enable.restype = C.c_int
         lib.etx_profile_enable.argtypes = [C.c_void_p, C.c_int]
         lib.etx_profile_read.restype = C.c_int
@@ -256,6 +265,32 @@ class Etx:
         self._check(self.lib.etx_build_tracks(self.handle, C.byref(batch.c), C.byref(graph.c), _ptr(scores),
                                               score_min, _ptr(labels), self._stream()))
         return labels
+
+    def etx_build_triplets(self, batch: DeviceBatch, graph: DeviceGraph, scores: torch.Tensor, score_min: float,
+                           capacity: Optional[int] = None) -> Dict[str, torch.Tensor]:
+        """Rows of edge ids per kind ("articulation", "left_elbow", "right_elbow": int32 [n, 2] views of one
+        buffer) and "ptr" [3, n_hits + 1].  capacity=None sizes the row buffer from a first counting call."""
+        ptr = torch.empty(3, batch.n_hits + 1, dtype=torch.int32, device=self.device)
+        t = Triplets()
+        t.d_ptr = ptr.data_ptr()
+
+        def call(cap):
+            rows = torch.empty(2, max(cap, 1), dtype=torch.int32, device=self.device)
+            t.capacity, t.d_first, t.d_second = cap, rows[0].data_ptr(), rows[1].data_ptr()
+            st = self.lib.etx_build_triplets(self.handle, C.byref(batch.c), C.byref(graph.c), _ptr(scores), score_min,
+                                             C.byref(t), self._stream())
+            return st, rows
+
+        st, rows = call(0 if capacity is None else capacity)
+        if st == ETX_ERR_CAPACITY and capacity is None and min(t.n) >= 0:
+            st, rows = call(sum(t.n))
+        self._check(st)
+        n = [int(x) for x in t.n]
+        o = [0, n[0], n[0] + n[1], n[0] + n[1] + n[2]]
+        out = {"ptr": ptr}
+        for k, name in enumerate(("articulation", "left_elbow", "right_elbow")):
+            out[name] = torch.stack([rows[0, o[k]:o[k + 1]], rows[1, o[k]:o[k + 1]]], dim=1)
+        return out
 
     # ---- whole path with host buffers (pinned torch tensors or numpy arrays)
     def etx_infer_host(self, host: Dict[str, torch.Tensor], r2_max: float, max_plane_gap: int,

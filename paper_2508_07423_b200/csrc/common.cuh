@@ -46,6 +46,13 @@ struct Workspace {            // carved from the caller's buffer by carve_worksp
   size_t total = 0;
 };
 
+// ---- triplets.cu (next row: triplet building)
+int launch_triplet_count(int n_hits, const int32_t* row_ptr, const int32_t* in_ptr, const int32_t* in_perm,
+                         const float* scores, float score_min, int32_t* ptr /*[3][n_hits+1]*/, cudaStream_t s);
+int launch_triplet_fill(int n_hits, const int32_t* row_ptr, const int32_t* in_ptr, const int32_t* in_perm,
+                        const float* scores, float score_min, const int32_t* ptr, int32_t* first, int32_t* second,
+                        cudaStream_t s);
+
 int launch_scatter_atomic(int n_nodes, long long n_edges, int H, const int32_t* src, const int32_t* dst,
                           const float* e, float* m, cudaStream_t s);   // measured comparison only (ETX_SCATTER_ATOMIC)
 

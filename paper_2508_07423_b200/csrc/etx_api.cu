@@ -744,6 +744,44 @@ etx_status etx_build_tracks(etx_ctx* c, const etx_batch* b, const etx_graph* g, 
   return check_cuda(c, "etx_build_tracks");
 }
 
+etx_status etx_build_triplets(etx_ctx* c, const etx_batch* b, const etx_graph* g, const float* d_scores,
+                              float score_min, etx_triplets* t, void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (etx_status st = check_batch(c, b)) return st;
+  if (!g || g->n_edges < 0 || !g->d_row_ptr || !g->d_in_ptr) return fail(c, ETX_ERR_INVALID, "graph is NULL or not built");
+  if (!t || !t->d_ptr || t->capacity < 0) return fail(c, ETX_ERR_INVALID, "triplet buffers are NULL");
+  if (t->capacity > 0 && (!t->d_first || !t->d_second)) return fail(c, ETX_ERR_INVALID, "triplet row arrays are NULL");
+  if (g->n_edges > 0 && (!d_scores || !g->d_in_perm)) return fail(c, ETX_ERR_INVALID, "scores / in_perm are NULL");
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  if (etx_status st = need_ws(c, carve(c, b->n_events, b->n_hits, 0, false, nullptr))) return st;
+  const Workspace w = carve(c, b->n_events, b->n_hits, 0, false, (char*)c->ws);
+  const int N = b->n_hits;
+  const size_t ld = (size_t)N + 1;
+  {
+    ProfScope ps(c, ETX_K_TRACKS, s);
+    c->launches += launch_triplet_count(N, g->d_row_ptr, g->d_in_ptr, g->d_in_perm, d_scores, score_min, t->d_ptr, s);
+    for (int k = 0; k < 3; ++k) c->launches += launch_exclusive_scan(t->d_ptr + k * ld, N + 1, w.scan_tmp, s);
+  }
+  int32_t host[3] = {0, 0, 0};
+  for (int k = 0; k < 3; ++k)
+    cudaMemcpyAsync(&host[k], t->d_ptr + k * ld + N, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+  if (cudaStreamSynchronize(s) != cudaSuccess) return check_cuda(c, "etx_build_triplets (count)");
+  if (etx_status st = check_cuda(c, "etx_build_triplets (count)")) return st;
+  bool overflow = false;
+  for (int k = 0; k < 3; ++k) { t->n[k] = host[k]; overflow |= host[k] < 0; }
+  if (overflow) return fail(c, ETX_ERR_CAPACITY, "more than 2^31 - 1 triplets of one kind");
+  const int64_t total = t->n[0] + t->n[1] + t->n[2];
+  if (total > t->capacity)
+    return fail(c, ETX_ERR_CAPACITY, "triplets need " + std::to_string(total) + " rows, capacity " + std::to_string(t->capacity));
+  if (total > 0) {
+    ProfScope ps(c, ETX_K_TRACKS, s);
+    c->launches += launch_triplet_fill(N, g->d_row_ptr, g->d_in_ptr, g->d_in_perm, d_scores, score_min, t->d_ptr,
+                                       t->d_first, t->d_second, s);
+  }
+  return check_cuda(c, "etx_build_triplets (fill)");
+}
+
 etx_status etx_infer_host(etx_ctx* c, const etx_batch_host* hb, float r2_max, int32_t max_plane_gap,
                           int64_t edge_capacity, int64_t* n_edges, int32_t* h_src, int32_t* h_dst,
                           float* h_scores, void* stream) {
