@@ -91,6 +91,18 @@ def path_flops(cfg, N, E):
             "edge_proj": (cfg.n_iter + 1) * N * 2 * H * 2 * H}
 
 
+def pair_tests(batch, gap):
+    """Candidate pairs of the windowed search: sum over events and planes p of n_p x (n_{p+1} + .. + n_{p+gap})
+    (= the edge count at r -> infinity, SURVEY 8(c) closed form)."""
+    n_ev = len(batch["event_ptr"]) - 1
+    if len(batch["plane"]) == 0:
+        return 0
+    n_pl = int(batch["plane"].max()) + 1
+    ev_of = np.repeat(np.arange(n_ev), np.diff(batch["event_ptr"]))
+    cnt = np.bincount(ev_of * n_pl + batch["plane"].astype(np.int64), minlength=n_ev * n_pl).reshape(n_ev, n_pl)
+    return sum(int((cnt[:, :n_pl - k].astype(np.int64) * cnt[:, k:]).sum()) for k in range(1, gap + 1))
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -340,10 +352,7 @@ def run_ours(args):
     # d multiplications, d-1 additions and the comparison, individually rounded: no FMA); the kernels sweep the
     # candidates twice (count pass, fill pass).  Bytes: embeddings + plane ids read, both CSR structures written.
     if stages["graph"]["ms"] > 0:
-        n_pl = int(batch["plane"].max()) + 1 if N else 1
-        ev_of = np.repeat(np.arange(n_ev), np.diff(batch["event_ptr"]))
-        cnt = np.bincount(ev_of * n_pl + batch["plane"].astype(np.int64), minlength=n_ev * n_pl).reshape(n_ev, n_pl)
-        pairs = sum(int((cnt[:, :n_pl - k].astype(np.int64) * cnt[:, k:]).sum()) for k in range(1, gap + 1))
+        pairs = pair_tests(batch, gap)
         d_emb = cfg.emb_widths[-1]
         t_s = stages["graph"]["ms"] * 1e-3
         alu_peak = 148 * 128 * pk["sm_max_mhz"] * 1e6           # unfused fp32 operations per second

@@ -55,3 +55,18 @@ def test_single_process_helpers():
     H = 128
     assert fl["edge_net"] == 6 * 60 * 2 * (3 * H * H + H * H + H * H)      # 10 H^2 FLOP per edge and step
     assert fl["scatter"] == 6 * 2 * 60 * H
+
+
+def test_pair_test_count_is_the_edge_count_at_infinite_radius():
+    """bench.py's pair-test count (the denominator of the graph stage's ALU fraction) against the oracle's search
+    with r -> infinity on a ragged multi-event batch, for G = 1..3 (SURVEY 8(c) closed form)."""
+    import bench
+    from oracle import etx_oracle as orc
+    from paper_2508_07423_b200 import synth
+    cfg = synth.CONFIGS["c2"]
+    batch = synth.generate_events(cfg, [5, 6, 300])
+    emb = np.zeros((len(batch["r"]), 4), np.float32)
+    for gap in (1, 2, 3):
+        s, _ = orc.build_graph(batch["event_ptr"], batch["plane"], emb, np.inf, gap)
+        assert bench.pair_tests(batch, gap) == len(s)
+    assert bench.pair_tests(synth.generate_events(cfg, []), 3) == 0
