@@ -130,9 +130,12 @@ search_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t*
       const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
       const int j1 = pp[top + 1];
       const int base_out = (MODE == 1) ? row_ptr[i] : 0;
+      // fill pass: the count pass already fixed this hit's out-degree -- stop as soon as all its edges are written
+      // (a hit without neighbours tests nothing, the others skip the candidates behind their last neighbour)
+      const int deg = (MODE == 1) ? row_ptr[i + 1] - base_out : 0x7fffffff;
       const float r2 = a.r2_max;
       const unsigned long long nme01 = pack2(-me[0], -me[1]), nme23 = pack2(-me[2], -me[3]);
-      for (int base = j0; base < j1; base += 32) {
+      for (int base = j0; base < j1 && cnt < deg; base += 32) {
         const int j = base + lane;
         // branch-free body: lanes past the end test the last candidate again and are masked out of the vote
         const int jc = j < j1 ? j : j1 - 1;
