@@ -139,3 +139,53 @@ def test_full_batch_every_edge(B, name, precisions):
         print(f"{name} precision={prec}: all {out['E']} edges, max |score - FFMA| = {d.max():.3g}, "
               f"p99.99 = {np.quantile(d, 0.9999):.3g}, median = {np.median(d):.3g}")
         assert d.max() <= TOL[prec] - 3e-6, (name, prec, float(d.max()))
+
+
+def test_full_batch_next_rows_tracks_and_triplets(B):
+    """The next rows at bench.py's size and launch configuration (c2, 1000 events, default precision): closed-form
+    triplet counts and CSR offsets from the kept degrees on ALL hits, and tracks / triplets of sampled events
+    against the oracle run on that event alone (integer work: bit-equal)."""
+    cfg = synth.CONFIGS["c2"]
+    batch = synth.generate_events(cfg)
+    blob = synth.generate_weights(cfg)
+    etx = B.Etx(B.make_desc(cfg), blob)
+    dev = etx.device
+    db = B.DeviceBatch(batch, dev)
+    N = db.n_hits
+    cap = int(N * (cfg.target_degree * 1.25 + 2))
+    etx.ensure_workspace(db.n_events, N, cap)
+    g = B.DeviceGraph(N, cap, dev)
+    E = etx.etx_build_graph(db, etx.etx_embed(db), synth.r2_max(cfg), cfg.max_plane_gap, g)
+    enc = torch.empty(cap, cfg.gnn_hidden, device=dev)
+    sc = torch.empty(cap, device=dev)
+    etx.etx_gnn_forward(db, g, enc)
+    etx.etx_edge_scores(g, enc, sc)
+    s_min = 0.5
+    lab = etx.etx_build_tracks(db, g, sc, s_min)[:N].cpu().numpy()
+    tr = etx.etx_build_triplets(db, g, sc, s_min)
+    torch.cuda.synchronize()
+    src, dst, s = g.src[:E].cpu().numpy().astype(np.int64), g.dst[:E].cpu().numpy().astype(np.int64), sc[:E].cpu().numpy()
+    keep = s >= np.float32(s_min)
+    kout, kin = np.bincount(src[keep], minlength=N), np.bincount(dst[keep], minlength=N)
+    ptr = tr["ptr"].cpu().numpy()
+    rows = {k: tr[k].cpu().numpy() for k in ("articulation", "left_elbow", "right_elbow")}
+    for k, per_hit in enumerate((kin * kout, kout * (kout - 1) // 2, kin * (kin - 1) // 2)):
+        off = np.zeros(N + 1, np.int64); np.cumsum(per_hit, out=off[1:])
+        np.testing.assert_array_equal(ptr[k], off)
+    assert [len(rows[k]) for k in rows] == [int(ptr[k][-1]) for k in range(3)]
+    a, l, r = rows["articulation"], rows["left_elbow"], rows["right_elbow"]
+    assert np.all(keep[a]) and np.all(keep[l]) and np.all(keep[r])
+    assert np.array_equal(dst[a[:, 0]], src[a[:, 1]]) and np.array_equal(src[l[:, 0]], src[l[:, 1]])
+    assert np.array_equal(dst[r[:, 0]], dst[r[:, 1]]) and np.all(l[:, 0] < l[:, 1]) and np.all(r[:, 0] < r[:, 1])
+    ep = batch["event_ptr"].astype(np.int64)
+    rp = g.row_ptr.cpu().numpy().astype(np.int64)
+    ev = np.repeat(np.arange(len(ep) - 1), np.diff(ep))
+    assert np.array_equal(ev[lab], ev) and np.all(lab <= np.arange(N))          # tracks stay inside their event
+    for e in (0, 421, 999):
+        h0, h1, e0, e1 = ep[e], ep[e + 1], rp[ep[e]], rp[ep[e + 1]]
+        ls, ld, lsc = (src[e0:e1] - h0).astype(np.int32), (dst[e0:e1] - h0).astype(np.int32), s[e0:e1]
+        np.testing.assert_array_equal(lab[h0:h1] - h0, orc.wcc(int(h1 - h0), ls, ld, lsc, s_min))
+        want = orc.triplets(int(h1 - h0), ls, ld, lsc, s_min)
+        for k, name in enumerate(rows):
+            got = rows[name][ptr[k][h0]:ptr[k][h1]] - e0                         # the event's rows, local edge ids
+            np.testing.assert_array_equal(got, want[name])
