@@ -173,8 +173,14 @@ etx_status etx_build_triplets(etx_ctx* ctx, const etx_batch* batch, const etx_gr
                               float score_min, etx_triplets* t, void* stream);
 
 /* Whole path with HOST buffers: copies the batch host->device, runs a0..a7, copies src/dst/scores
- * back (h_src, h_dst may be NULL).  Needs a workspace sized with with_host_path = 1.  Host buffers
- * should be pinned for the copies to be asynchronous.  Synchronises the stream before returning.  */
+ * back (h_src, h_dst may be NULL; each needs edge_capacity entries).  Host buffers should be pinned for
+ * the copies to be asynchronous.  Synchronises the stream before returning.
+ * Workspace: one sized with etx_workspace_bytes(..., with_host_path = 1) for the whole batch runs it in one
+ * pass.  A SMALLER workspace is not an error: the batch is then split into consecutive event ranges that fit
+ * (the thesis bounds its GNN batches the same way: <= 2^20 hits, <= 2^22 edges), run one after the
+ * other; events are independent and edges are ordered by source, so the outputs are identical to the
+ * single-pass ones, element for element.  ETX_ERR_NOMEM only if a single event does not fit.
+ * *n_edges receives E; on ETX_ERR_CAPACITY the edges found so far plus the range that overflowed.       */
 etx_status etx_infer_host(etx_ctx* ctx, const etx_batch_host* batch, float r2_max,
                           int32_t max_plane_gap, int64_t edge_capacity, int64_t* n_edges,
                           int32_t* h_src, int32_t* h_dst, float* h_scores, void* stream);

@@ -20,7 +20,7 @@ ETX_MAX_MLP_LAYERS = 8
 ETX_OK, ETX_ERR_INVALID, ETX_ERR_CAPACITY, ETX_ERR_CUDA, ETX_ERR_UNSORTED, ETX_ERR_NOMEM = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["etx_weight_count", "etx_create", "etx_destroy", "etx_last_error", "etx_workspace_bytes",
-           "etx_set_workspace", "etx_embed", "etx_build_graph", "etx_gnn_forward", "etx_edge_scores",
+           "etx_set_workspace", "etx_embed", "etx_embed_int8", "etx_build_graph", "etx_gnn_forward", "etx_edge_scores",
            "etx_infer_host", "etx_launch_count", "etx_profile_enable", "etx_profile_read", "etx_build_tracks",
            "etx_build_triplets"]
 KERNEL_CLASSES = ["embed", "graph", "node_enc", "edge_enc", "scatter", "node_net", "edge_net", "cls", "tracks", "edge_proj"]
@@ -177,6 +177,7 @@ class Etx:
         if st != ETX_OK:
             raise EtxError(st, self.lib.etx_last_error(None).decode())
         self._ws = None
+        self._ws_bytes = 0
 
     def close(self):
         if getattr(self, "handle", None):
@@ -207,10 +208,19 @@ class Etx:
 
     def ensure_workspace(self, n_events: int, n_hits: int, edge_capacity: int, with_host_path: bool = False):
         need = self.workspace_bytes(n_events, n_hits, edge_capacity, with_host_path)
-        if self._ws is None or self._ws.numel() < need:
+        if self._ws is None or self._ws_bytes < need:      # compare with what was REGISTERED, not the padded tensor
             self._ws = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
             off = (-self._ws.data_ptr()) % 256
             self._check(self.lib.etx_set_workspace(self.handle, C.c_void_p(self._ws.data_ptr() + off), need))
+            self._ws_bytes = need
+
+    def set_workspace(self, nbytes: int):
+        """Register a workspace of exactly ``nbytes`` (etx_set_workspace); etx_infer_host splits a batch that does
+        not fit it into event ranges (include/etx.h)."""
+        self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        off = (-self._ws.data_ptr()) % 256
+        self._check(self.lib.etx_set_workspace(self.handle, C.c_void_p(self._ws.data_ptr() + off), nbytes))
+        self._ws_bytes = nbytes
 
     def launch_count(self) -> int:
         return int(self.lib.etx_launch_count(self.handle))

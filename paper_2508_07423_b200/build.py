@@ -39,6 +39,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
     if os.environ.get("ETX_TC_COUNTERS"):          # developer build: per-role cycle counters in mlp_tc.cu
         flags.append("-DETX_TC_COUNTERS")
+    if os.environ.get("ETX_DEV_SWITCHES"):         # developer build: timing experiments / measured alternatives that
+        flags.append("-DETX_DEV_SWITCHES")         # change results (ETX_TC_EXP, ETX_SCATTER_ATOMIC, ETX_EMBED_FFMA)
     flags += os.environ.get("ETX_NVCC_FLAGS", "").split()      # developer aid: extra -D switches for A/B builds
     cmd = [_nvcc()] + flags + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + sources()
     proc = subprocess.run(cmd, capture_output=True, text=True)

@@ -11,6 +11,7 @@
 namespace etx {
 
 constexpr int kMaxLayers = ETX_MAX_MLP_LAYERS;
+constexpr int kMaxDevices = 64;      // per-device launch configuration tables (cudaFuncSetAttribute is per device)
 
 // One MLP on the device.  Wt[l] is the layer's weight TRANSPOSED to [in][out] row-major (k-major, so
 // a K-chunk of it is a contiguous slab), b[l] its bias, both fp32.
@@ -52,9 +53,6 @@ int launch_triplet_count(int n_hits, const int32_t* row_ptr, const int32_t* in_p
 int launch_triplet_fill(int n_hits, const int32_t* row_ptr, const int32_t* in_ptr, const int32_t* in_perm,
                         const float* scores, float score_min, const int32_t* ptr, int32_t* first, int32_t* second,
                         cudaStream_t s);
-
-int launch_scatter_atomic(int n_nodes, long long n_edges, int H, const int32_t* src, const int32_t* dst,
-                          const float* e, float* m, cudaStream_t s);   // measured comparison only (ETX_SCATTER_ATOMIC)
 
 }  // namespace etx
 
@@ -104,6 +102,7 @@ int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32
                        const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst,
                        const int32_t* in_ptr, int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/, cudaStream_t s);
 size_t scan_tmp_ints(int n);
+int launch_add_offset(const int32_t* in, int32_t* out, int64_t n, int32_t offset, cudaStream_t s);
 int launch_sort_in_lists(int n_hits, const int32_t* flags, const int32_t* in_ptr, int32_t* in_perm, cudaStream_t s);
 // ---- graph_kmax.cu (next row: k_max-capped search)
 int launch_kmax_count(const GraphArgs& a, int k_max, const int32_t* plane_ptr, const int32_t* hit_event,
@@ -151,7 +150,7 @@ struct TcArgs {
   int n_out = 1;                                  // units of a narrow output layer (out_mode 2)
   int out_mode = 0; float* out = nullptr; const float* res = nullptr; int out_ld = 0;
   unsigned long long* dbg = nullptr;              // optional [grid][16] cycle counters (ETX_TC_DEBUG)
-  int exp_flags = 0;                              // timing experiments only (ETX_TC_EXP): 1 skip gather stores, 2 skip weight copies
+  int exp_flags = 0;                              // developer builds only (-DETX_DEV_SWITCHES): timing experiments, wrong results
 };
 int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s);
 int tc_chunk_k(int mode);
@@ -177,7 +176,9 @@ int launch_embed_int8(const Int8Args& a, int H, cudaStream_t s);
 int launch_scatter(int n_nodes, int H, const int32_t* row_ptr, const int32_t* in_ptr,
                    const int32_t* in_perm, const float* e, float* m, int32_t* counter /*device, 1 int*/, cudaStream_t s);
 
+#ifdef ETX_DEV_SWITCHES
 int launch_scatter_atomic(int n_nodes, long long n_edges, int H, const int32_t* src, const int32_t* dst,
-                          const float* e, float* m, cudaStream_t s);   // measured comparison only (ETX_SCATTER_ATOMIC)
+                          const float* e, float* m, cudaStream_t s);   // developer builds: the measured all-atomics alternative
+#endif
 
 }  // namespace etx

@@ -203,9 +203,10 @@ struct ProfScope {
   }
 };
 
-// Precision dispatch.  MLPs with a tensor-core weight image run on tcgen05 (mlp_tc.cu).  The embedding MLP
-// always runs the exact fp32 FFMA kernel (the graph must match the oracle edge for edge); the node encoder,
-// also fed by 3 raw features, runs its first layer in the gather warps of the tensor-core kernel.
+// Precision dispatch.  MLPs with a tensor-core weight image run on tcgen05 (mlp_tc.cu).  In the tensor-core modes
+// the embedding MLP runs the 3xTF32 chain whatever the GNN's mode (its result decides graph edges); like the node
+// encoder, also fed by 3 raw features, it runs its first layer in the gather warps of the tensor-core kernel.
+// ETX_PREC_FP32 runs every MLP in the exact fp32 FFMA kernel (mlp_simt.cu).
 int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s);
 // A launcher that refuses its arguments (unsupported shape, output not 16-byte aligned for the tensor map)
 // must not pass silently: the refusal is recorded and the API call that asked for it returns ETX_ERR_INVALID.
@@ -239,9 +240,14 @@ int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   const int mode = (a.out_mode == 2) ? (int)ETX_PREC_TF32X3 : (int)c->desc.precision;
   t.w_last = a.mlp.Wt[a.mlp.n_layers - 1];         // [H][1] == [H]
   t.out_mode = a.out_mode; t.out = a.out; t.res = a.res; t.out_ld = a.out_ld;
-  static const char* expv = getenv("ETX_TC_EXP");                  // developer aid: timing experiments (wrong results)
+#ifdef ETX_DEV_SWITCHES
+  static const char* expv = getenv("ETX_TC_EXP");                  // developer build: timing experiments (wrong results)
   t.exp_flags = expv ? atoi(expv) : 0;
-  static const bool debug = getenv("ETX_TC_DEBUG") != nullptr;     // developer aid: per-role cycle counters
+#endif
+#ifndef ETX_TC_COUNTERS
+  return launch_mlp_tc(t, mode, c->sm_count, s);
+#else
+  static const bool debug = getenv("ETX_TC_DEBUG") != nullptr;     // developer build: per-role cycle counters
   if (!debug) return launch_mlp_tc(t, mode, c->sm_count, s);
   static unsigned long long* d_dbg = nullptr;
   if (!d_dbg) cudaMalloc(&d_dbg, sizeof(unsigned long long) * 32 * 256);
@@ -260,6 +266,7 @@ int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
           a.n_rows, a.mlp.dims[0], tiles, avg[5] / tiles, avg[0] / tiles, avg[1] / tiles, avg[2] / tiles, avg[3] / tiles, avg[4] / tiles,
           avg[6] / tiles, avg[7] / tiles, avg[10] / tiles, avg[11] / tiles, avg[12] / tiles, avg[13] / tiles, avg[14] / tiles, avg[15] / tiles, avg[8] / tiles, avg[9] / tiles, avg[16] / tiles, avg[17] / tiles, avg[18] / tiles, avg[19] / tiles);
   return n;
+#endif
 }
 
 }  // namespace
@@ -383,7 +390,12 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
     size_t wsrc = 0;
     for (size_t i = 0; i < mlps.size(); ++i) {
       const float* w = h_weights + wsrc;
-      if (i == 0 && mlps[i].n_layers >= 3 && mlps[i].dims[1] == 128 && !getenv("ETX_EMBED_FFMA")) {
+#ifdef ETX_DEV_SWITCHES
+      const bool emb_ffma = getenv("ETX_EMBED_FFMA") != nullptr;   // developer build: keep the exact FFMA embedding
+#else
+      const bool emb_ffma = false;
+#endif
+      if (i == 0 && mlps[i].n_layers >= 3 && mlps[i].dims[1] == 128 && !emb_ffma) {
         // embedding: layers 2..L-1 as 3xTF32 MMA chain (layer 1 in the gather warps, the narrow last layer in the epilogue)
         img_off[i] = img.size();
         append_wimg(img, mlps[i], w, 1, 0, mlps[i].n_layers - 1, ETX_PREC_TF32X3);
@@ -549,6 +561,9 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
   if (k_max < 0) return fail(c, ETX_ERR_INVALID, "k_max must be >= 0 (0 = no cap)");
   if (max_plane_gap < 1) return fail(c, ETX_ERR_INVALID, "max_plane_gap must be >= 1");
   if (b->n_hits > 0 && !d_emb) return fail(c, ETX_ERR_INVALID, "d_emb is NULL");
+  if (c->emb.dims[c->emb.n_layers] == 4 && ((uintptr_t)d_emb & 15))
+    return fail(c, ETX_ERR_INVALID, "d_emb must be 16-byte aligned for a 4-dimensional embedding (vector loads)");
+  if (max_plane_gap > c->desc.n_planes - 1) max_plane_gap = c->desc.n_planes - 1;   // larger gaps reach no plane; keeps p + gap in range
   if (g->edge_capacity < 0 || (g->edge_capacity > 0 && (!g->d_src || !g->d_dst || !g->d_in_perm)))
     return fail(c, ETX_ERR_INVALID, "edge arrays are NULL");
   cudaSetDevice(c->device);
@@ -669,9 +684,11 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
     // a4: m = [sum out, sum in] of e^k
     {
       ProfScope ps(c, ETX_K_SCATTER, s);
-      static const bool atomic = getenv("ETX_SCATTER_ATOMIC") != nullptr;   // developer aid: the measured alternative
+#ifdef ETX_DEV_SWITCHES
+      static const bool atomic = getenv("ETX_SCATTER_ATOMIC") != nullptr;   // developer build: the measured alternative
       if (atomic && H == 128) c->launches += launch_scatter_atomic(N, E, H, g->d_src, g->d_dst, (const float*)d_edge_enc, w.m, s);
       else
+#endif
       c->launches += launch_scatter(N, H, g->d_row_ptr, g->d_in_ptr, g->d_in_perm, d_edge_enc, w.m, w.sched, s);
     }
     {  // a5: h += phi_k([h, m])
@@ -782,6 +799,75 @@ etx_status etx_build_triplets(etx_ctx* c, const etx_batch* b, const etx_graph* g
   return check_cuda(c, "etx_build_triplets (fill)");
 }
 
+// One pass of the whole path over events [e0, e1) of a HOST batch (hits [h0, h1)), results appended at edge
+// offset `edge_off` of the host outputs with hit indices made global again.  The workspace must hold the pass.
+static etx_status infer_host_pass(etx_ctx* c, const etx_batch_host* hb, int32_t e0, int32_t e1, float r2_max,
+                                  int32_t max_plane_gap, int64_t cap, int64_t edge_off, int64_t* n_edges,
+                                  int32_t* h_src, int32_t* h_dst, float* h_scores, cudaStream_t s) {
+  const int32_t n_ev = e1 - e0, h0 = hb->h_event_ptr[e0], h1 = hb->h_event_ptr[e1];
+  const Workspace w = carve(c, n_ev, h1 - h0, cap, true, (char*)c->ws);
+  const size_t nh = (size_t)(h1 - h0);
+  std::vector<int32_t> local_ptr;
+  const int32_t* ep = hb->h_event_ptr + e0;
+  if (h0 != 0) {                                       // a chunk's offsets restart at 0
+    local_ptr.resize((size_t)n_ev + 1);
+    for (int32_t i = 0; i <= n_ev; ++i) local_ptr[i] = ep[i] - h0;
+    ep = local_ptr.data();
+  }
+  cudaMemcpyAsync(w.s_event_ptr, ep, sizeof(int32_t) * ((size_t)n_ev + 1), cudaMemcpyHostToDevice, s);
+  if (!local_ptr.empty()) cudaStreamSynchronize(s);    // the pageable temporary must outlive its copy
+  if (nh) {
+    cudaMemcpyAsync(w.s_plane, hb->h_plane + h0, nh, cudaMemcpyHostToDevice, s);
+    cudaMemcpyAsync(w.s_r, hb->h_r + h0, nh * 4, cudaMemcpyHostToDevice, s);
+    cudaMemcpyAsync(w.s_phi, hb->h_phi + h0, nh * 4, cudaMemcpyHostToDevice, s);
+    cudaMemcpyAsync(w.s_z, hb->h_z + h0, nh * 4, cudaMemcpyHostToDevice, s);
+    cudaMemcpyAsync(w.s_x, hb->h_x + h0, nh * 4, cudaMemcpyHostToDevice, s);
+    cudaMemcpyAsync(w.s_y, hb->h_y + h0, nh * 4, cudaMemcpyHostToDevice, s);
+  }
+  etx_batch b;
+  b.n_events = n_ev; b.n_hits = h1 - h0;
+  b.d_event_ptr = w.s_event_ptr; b.d_plane = w.s_plane;
+  b.d_r = w.s_r; b.d_phi = w.s_phi; b.d_z = w.s_z; b.d_x = w.s_x; b.d_y = w.s_y;
+  etx_graph g;
+  g.edge_capacity = cap; g.n_edges = 0;
+  g.d_row_ptr = w.s_row_ptr; g.d_src = w.s_src; g.d_dst = w.s_dst; g.d_in_ptr = w.s_in_ptr; g.d_in_perm = w.s_in_perm;
+  if (etx_status st = etx_embed(c, &b, w.s_emb, s)) return st;
+  etx_status st = etx_build_graph(c, &b, w.s_emb, r2_max, max_plane_gap, 0, &g, s);
+  *n_edges = g.n_edges;
+  if (st) return st;
+  // the edge list is final once the graph is built: its device-to-host copy runs on the context's copy stream
+  // underneath the message passing; only the scores are copied after the last kernel
+  const size_t ne = (size_t)g.n_edges;
+  if (!c->copy_stream) {
+    cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    cudaEventCreateWithFlags(&c->copy_event, cudaEventDisableTiming);
+  }
+  if (ne && (h_src || h_dst)) {
+    int32_t *o_src = w.s_src, *o_dst = w.s_dst;
+    if (h0 != 0) {                                     // global hit indices: shifted copies in the (still unused) score / encoding buffers
+      o_src = reinterpret_cast<int32_t*>(w.s_scores);
+      o_dst = reinterpret_cast<int32_t*>(w.s_edge_enc);
+      c->launches += launch_add_offset(w.s_src, o_src, (int64_t)ne, h0, s);
+      c->launches += launch_add_offset(w.s_dst, o_dst, (int64_t)ne, h0, s);
+    }
+    cudaEventRecord(c->copy_event, s);
+    cudaStreamWaitEvent(c->copy_stream, c->copy_event, 0);
+    if (h_src) cudaMemcpyAsync(h_src + edge_off, o_src, ne * 4, cudaMemcpyDeviceToHost, c->copy_stream);
+    if (h_dst) cudaMemcpyAsync(h_dst + edge_off, o_dst, ne * 4, cudaMemcpyDeviceToHost, c->copy_stream);
+    if (h0 != 0) {                                     // the shifted copies live where the GNN writes next
+      cudaEventRecord(c->copy_event, c->copy_stream);
+      cudaStreamWaitEvent(s, c->copy_event, 0);
+    }
+  }
+  if (!(st = etx_gnn_forward(c, &b, &g, w.s_edge_enc, nullptr, s)))
+    st = etx_edge_scores(c, &g, w.s_edge_enc, w.s_scores, s);
+  if (!st && ne && h_scores) cudaMemcpyAsync(h_scores + edge_off, w.s_scores, ne * 4, cudaMemcpyDeviceToHost, s);
+  const cudaError_t e1c = cudaStreamSynchronize(c->copy_stream), e2c = cudaStreamSynchronize(s);
+  if (st) return st;
+  (void)e1c; (void)e2c;
+  return check_cuda(c, "etx_infer_host");
+}
+
 etx_status etx_infer_host(etx_ctx* c, const etx_batch_host* hb, float r2_max, int32_t max_plane_gap,
                           int64_t edge_capacity, int64_t* n_edges, int32_t* h_src, int32_t* h_dst,
                           float* h_scores, void* stream) {
@@ -792,49 +878,60 @@ etx_status etx_infer_host(etx_ctx* c, const etx_batch_host* hb, float r2_max, in
     return fail(c, ETX_ERR_INVALID, "host batch array is NULL");
   cudaSetDevice(c->device);
   cudaStream_t s = (cudaStream_t)stream;
-  if (etx_status st = need_ws(c, carve(c, hb->n_events, hb->n_hits, edge_capacity, true, nullptr))) return st;
-  const Workspace w = carve(c, hb->n_events, hb->n_hits, edge_capacity, true, (char*)c->ws);
-  const size_t nh = (size_t)hb->n_hits;
-  cudaMemcpyAsync(w.s_event_ptr, hb->h_event_ptr, sizeof(int32_t) * ((size_t)hb->n_events + 1), cudaMemcpyHostToDevice, s);
-  if (nh) {
-    cudaMemcpyAsync(w.s_plane, hb->h_plane, nh, cudaMemcpyHostToDevice, s);
-    cudaMemcpyAsync(w.s_r, hb->h_r, nh * 4, cudaMemcpyHostToDevice, s);
-    cudaMemcpyAsync(w.s_phi, hb->h_phi, nh * 4, cudaMemcpyHostToDevice, s);
-    cudaMemcpyAsync(w.s_z, hb->h_z, nh * 4, cudaMemcpyHostToDevice, s);
-    cudaMemcpyAsync(w.s_x, hb->h_x, nh * 4, cudaMemcpyHostToDevice, s);
-    cudaMemcpyAsync(w.s_y, hb->h_y, nh * 4, cudaMemcpyHostToDevice, s);
+  if (!c->ws) return fail(c, ETX_ERR_NOMEM, "no workspace set (etx_set_workspace)");
+  int64_t total = 0;
+  if (carve(c, hb->n_events, hb->n_hits, edge_capacity, true, nullptr).total <= c->ws_bytes) {
+    const etx_status st = infer_host_pass(c, hb, 0, hb->n_events, r2_max, max_plane_gap, edge_capacity, 0, &total,
+                                          h_src, h_dst, h_scores, s);
+    if (n_edges) *n_edges = total;
+    return st;
   }
-  etx_batch b;
-  b.n_events = hb->n_events; b.n_hits = hb->n_hits;
-  b.d_event_ptr = w.s_event_ptr; b.d_plane = w.s_plane;
-  b.d_r = w.s_r; b.d_phi = w.s_phi; b.d_z = w.s_z; b.d_x = w.s_x; b.d_y = w.s_y;
-  etx_graph g;
-  g.edge_capacity = edge_capacity; g.n_edges = 0;
-  g.d_row_ptr = w.s_row_ptr; g.d_src = w.s_src; g.d_dst = w.s_dst; g.d_in_ptr = w.s_in_ptr; g.d_in_perm = w.s_in_perm;
-  if (etx_status st = etx_embed(c, &b, w.s_emb, stream)) return st;
-  etx_status st = etx_build_graph(c, &b, w.s_emb, r2_max, max_plane_gap, 0, &g, stream);
-  if (n_edges) *n_edges = g.n_edges;
-  if (st) return st;
-  // the edge list is final once the graph is built: its device-to-host copy runs on the context's copy stream
-  // underneath the message passing; only the scores are copied after the last kernel
-  const size_t ne = (size_t)g.n_edges;
-  if (!c->copy_stream) {
-    cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
-    cudaEventCreateWithFlags(&c->copy_event, cudaEventDisableTiming);
+  // The batch does not fit the workspace: split it into consecutive event ranges that do (the thesis bounds its
+  // GNN batches the same way, <= 2^20 hits / 2^22 edges).  Events are independent and edges are
+  // ordered by source, so the passes' outputs concatenate into exactly the single-pass result.  A range gets the
+  // edge capacity the workspace has room for (at most what is left of the caller's), sized from the caller's own
+  // edges-per-hit ratio; a range whose graph still overflows its share is halved and retried.
+  const int32_t* ep = hb->h_event_ptr;
+  for (int32_t i = 0; i < hb->n_events; ++i)
+    if (ep[i + 1] < ep[i]) return fail(c, ETX_ERR_INVALID, "malformed batch: event_ptr not monotone");
+  if (hb->n_events > 0 && (ep[0] != 0 || ep[hb->n_events] != hb->n_hits))
+    return fail(c, ETX_ERR_INVALID, "malformed batch: event_ptr does not span the hits");
+  const double per_hit = hb->n_hits > 0 ? (double)edge_capacity / hb->n_hits : 0.0;
+  auto cap_of = [&](int32_t a, int32_t b2) {
+    const int64_t want = (int64_t)std::ceil(per_hit * (ep[b2] - ep[a])) + 1024;
+    return std::min<int64_t>(want, edge_capacity - total);
+  };
+  auto fits = [&](int32_t a, int32_t b2) {
+    return carve(c, b2 - a, ep[b2] - ep[a], cap_of(a, b2), true, nullptr).total <= c->ws_bytes;
+  };
+  int32_t e0 = 0, limit = hb->n_events;
+  while (e0 < hb->n_events) {
+    if (!fits(e0, e0 + 1))
+      return fail(c, ETX_ERR_NOMEM, "workspace too small for event " + std::to_string(e0) + " alone (" +
+                                        std::to_string(ep[e0 + 1] - ep[e0]) + " hits)");
+    int32_t lo = e0 + 1, hi = std::min(limit, hb->n_events);     // largest range [e0, e1) that fits, by bisection
+    while (lo < hi) { const int32_t mid = lo + (hi - lo + 1) / 2; if (fits(e0, mid)) lo = mid; else hi = mid - 1; }
+    const int32_t e1 = lo;
+    // give the range all the edge room the workspace still has
+    int64_t cap = cap_of(e0, e1);
+    {
+      const size_t base0 = carve(c, e1 - e0, ep[e1] - ep[e0], 0, true, nullptr).total;
+      const size_t base1 = carve(c, e1 - e0, ep[e1] - ep[e0], 4096, true, nullptr).total;
+      const double per_edge = (double)(base1 - base0) / 4096.0;
+      const int64_t room = (int64_t)((double)(c->ws_bytes - base0) / per_edge) - 4096;
+      cap = std::max(cap, std::min<int64_t>(room, edge_capacity - total));
+      while (cap > 0 && carve(c, e1 - e0, ep[e1] - ep[e0], cap, true, nullptr).total > c->ws_bytes) cap -= 1024;
+      if (cap < 0) cap = 0;
+    }
+    int64_t got = 0;
+    const etx_status st = infer_host_pass(c, hb, e0, e1, r2_max, max_plane_gap, cap, total, &got, h_src, h_dst, h_scores, s);
+    if (st == ETX_ERR_CAPACITY && e1 - e0 > 1 && total + got <= edge_capacity) { limit = e0 + (e1 - e0) / 2; continue; }
+    if (st) { if (n_edges) *n_edges = total + got; return st; }
+    total += got;
+    e0 = e1; limit = hb->n_events;
   }
-  if (ne && (h_src || h_dst)) {
-    cudaEventRecord(c->copy_event, s);
-    cudaStreamWaitEvent(c->copy_stream, c->copy_event, 0);
-    if (h_src) cudaMemcpyAsync(h_src, w.s_src, ne * 4, cudaMemcpyDeviceToHost, c->copy_stream);
-    if (h_dst) cudaMemcpyAsync(h_dst, w.s_dst, ne * 4, cudaMemcpyDeviceToHost, c->copy_stream);
-  }
-  if (!(st = etx_gnn_forward(c, &b, &g, w.s_edge_enc, nullptr, stream)))
-    st = etx_edge_scores(c, &g, w.s_edge_enc, w.s_scores, stream);
-  if (!st && ne && h_scores) cudaMemcpyAsync(h_scores, w.s_scores, ne * 4, cudaMemcpyDeviceToHost, s);
-  const cudaError_t e1 = cudaStreamSynchronize(c->copy_stream), e2 = cudaStreamSynchronize(s);
-  if (st) return st;
-  if (e1 != cudaSuccess || e2 != cudaSuccess) return check_cuda(c, "etx_infer_host");
-  return check_cuda(c, "etx_infer_host");
+  if (n_edges) *n_edges = total;
+  return ETX_OK;
 }
 
 }  // extern "C"

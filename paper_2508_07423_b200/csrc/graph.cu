@@ -326,4 +326,17 @@ int launch_sort_in_lists(int n_hits, const int32_t* flags, const int32_t* in_ptr
   return 1;
 }
 
+// out[i] = in[i] + offset (etx_infer_host's event-range passes: chunk-local hit indices -> indices of the whole batch)
+namespace {
+__global__ void add_offset_kernel(const int32_t* __restrict__ in, int32_t* __restrict__ out, int64_t n, int32_t offset) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) out[i] = in[i] + offset;
+}
+}  // namespace
+int launch_add_offset(const int32_t* in, int32_t* out, int64_t n, int32_t offset, cudaStream_t s) {
+  if (n <= 0) return 0;
+  const int64_t need = (n + 255) / 256;
+  add_offset_kernel<<<(int)(need < 148 * 8 ? need : 148 * 8), 256, 0, s>>>(in, out, n, offset);
+  return 1;
+}
+
 }  // namespace etx

@@ -197,11 +197,13 @@ __global__ void __launch_bounds__(NT, 2) mlp_simt_kernel(const MlpArgs a) {
 
 template <int H>
 int launch_h(const MlpArgs& a, cudaStream_t s) {
-  static bool configured = false;
+  static bool configured[kMaxDevices] = {false};    // the shared-memory opt-in is a per-DEVICE attribute of the function
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return -1;
   const size_t smem = sizeof(Smem<H>);
-  if (!configured) {
-    cudaFuncSetAttribute(mlp_simt_kernel<H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = true;
+  if (!configured[dev]) {
+    if (cudaFuncSetAttribute(mlp_simt_kernel<H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
+    configured[dev] = true;
   }
   const int grid = (a.n_rows + TM - 1) / TM;
   mlp_simt_kernel<H><<<grid, NT, smem, s>>>(a);

@@ -49,6 +49,15 @@
 #define ETX_DBG(a) false
 #endif
 
+// Timing experiments that deliberately produce WRONG results (gather every tile from the same rows, skip the weight
+// copies) exist only in developer builds (-DETX_DEV_SWITCHES, build.py: ETX_DEV_SWITCHES=1).  The default library
+// contains none of them: no environment variable can change what it computes.
+#ifdef ETX_DEV_SWITCHES
+#define ETX_EXP(a, bit) (((a).exp_flags & (bit)) != 0)
+#else
+#define ETX_EXP(a, bit) false
+#endif
+
 namespace etx {
 namespace {
 
@@ -325,15 +334,15 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
         for (int p = 0; p < NPASS; ++p) {
           const int row = ptile * TM + r0 + p * RPP;
           rown[p] = row < a.n_rows ? row : a.n_rows - 1;
-          if (a.exp_flags & 4) rown[p] = r0 + p * RPP;      // timing experiment: every tile reads the same rows
+          if (ETX_EXP(a, 4)) rown[p] = r0 + p * RPP;      // timing experiment: every tile reads the same rows
         }
         if (sidx0) {
 #pragma unroll
-          for (int p = 0; p < NPASS; ++p) ridx[0][p] = (a.exp_flags & 4) ? rown[p] : __ldg(sidx0 + rown[p]);
+          for (int p = 0; p < NPASS; ++p) ridx[0][p] = ETX_EXP(a, 4) ? rown[p] : __ldg(sidx0 + rown[p]);
         }
         if (sidx1) {
 #pragma unroll
-          for (int p = 0; p < NPASS; ++p) ridx[1][p] = (a.exp_flags & 4) ? rown[p] : __ldg(sidx1 + rown[p]);
+          for (int p = 0; p < NPASS; ++p) ridx[1][p] = ETX_EXP(a, 4) ? rown[p] : __ldg(sidx1 + rown[p]);
         }
       }
       const Unit un = utab[pu];
@@ -656,7 +665,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
           const int q = wide ? qq : (qq < rep1 * nc1 ? qq % (nc1 > 0 ? nc1 : 1) : qq - (rep1 - 1) * nc1);
           const uint32_t ws = w_cnt % NSW, wn = w_cnt / NSW;
           mbar_wait(smem_u32(&bars->w_empty[ws]), (wn & 1) ^ 1);
-          if (a.exp_flags & 2) { mbar_arrive(smem_u32(&bars->w_full[ws])); continue; }
+          if (ETX_EXP(a, 2)) { mbar_arrive(smem_u32(&bars->w_full[ws])); continue; }
           mbar_expect_tx(smem_u32(&bars->w_full[ws]), kStageBytes);
           bulk_g2s(wring + ws * kStageBytes, a.wimg + (size_t)q * kStageBytes, kStageBytes, smem_u32(&bars->w_full[ws]));
         }
@@ -839,12 +848,14 @@ bool encode_out_map(CUtensorMap* m, float* out, int n_rows, int n_cols, int out_
 template <int MODE, int VAR>
 int launch_mode(const TcArgs& a, int sm_count, cudaStream_t s) {
   using C = Cfg<MODE>;
-  static bool configured = false;
+  static bool configured[kMaxDevices] = {false};    // the shared-memory opt-in is a per-DEVICE attribute of the function
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return -1;
   const size_t smem = 1024 + (size_t)(C::NSTAGE_W + C::NSTAGE_A) * C::PIECES * kAtomBytes + kAtomBytes +
                       (kMaxLayers + (VAR == 3 ? 8 : 1)) * HW * sizeof(float) + sizeof(Bars) + 64;
-  if (!configured) {
-    cudaFuncSetAttribute(mlp_tc_kernel<MODE, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = true;
+  if (!configured[dev]) {
+    if (cudaFuncSetAttribute(mlp_tc_kernel<MODE, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
+    configured[dev] = true;
   }
   const int n_tiles = (a.n_rows + TM - 1) / TM;
   const int grid = n_tiles < sm_count ? n_tiles : sm_count;

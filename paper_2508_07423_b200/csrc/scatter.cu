@@ -75,8 +75,9 @@ __global__ void __launch_bounds__(256) scatter_kernel(int n_nodes, const int32_t
   }
 }
 
+#ifdef ETX_DEV_SWITCHES
 // The alternative the thesis' pipeline used (scatter_add), kept ONLY as a measured comparison
-// (ETX_SCATTER_ATOMIC=1, developer aid): one warp per edge row, one vector reduction
+// (developer builds, -DETX_DEV_SWITCHES, with ETX_SCATTER_ATOMIC=1): one warp per edge row, one vector reduction
 // (red.global.add.v4.f32) per lane into m[src] (outgoing half) and m[dst] (incoming half) of a zeroed m.
 // Summation order is whatever the L2 serialises: not deterministic, and measured slower.
 __global__ void __launch_bounds__(256) scatter_atomic_kernel(long long n_edges, const int32_t* __restrict__ src,
@@ -92,9 +93,11 @@ __global__ void __launch_bounds__(256) scatter_atomic_kernel(long long n_edges, 
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(pi), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
   }
 }
+#endif
 
 }  // namespace
 
+#ifdef ETX_DEV_SWITCHES
 int launch_scatter_atomic(int n_nodes, long long n_edges, int H, const int32_t* src, const int32_t* dst,
                           const float* e, float* m, cudaStream_t s) {
   if (n_nodes <= 0 || H != 128) return n_nodes <= 0 ? 0 : -1;
@@ -104,6 +107,7 @@ int launch_scatter_atomic(int n_nodes, long long n_edges, int H, const int32_t* 
   scatter_atomic_kernel<<<(int)(need < 148 * 8 ? need : 148 * 8), 256, 0, s>>>(n_edges, src, dst, e, m);
   return 1;
 }
+#endif
 
 int launch_scatter(int n_nodes, int H, const int32_t* row_ptr, const int32_t* in_ptr,
                    const int32_t* in_perm, const float* e, float* m, int32_t* counter, cudaStream_t s) {

@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(kThreads) wcc_kernel(int n_events, const int32
     for (int i = h0 + threadIdx.x; i < h1; i += kThreads) labels[i] = i;
     __syncthreads();
     const int n_chunks = (e1 - e0 + kThreads - 1) / kThreads;
-    for (int round = 0; round < 64; ++round) {           // converges in 2-3 rounds; 64 bounds the loop
+    for (;;) {                                           // until stable: labels only decrease, so this terminates (2-3 rounds on tracks)
       if (threadIdx.x == 0) changed = 0;
       __syncthreads();
       int local = 0;

@@ -21,7 +21,8 @@ def lib():
 def test_exports_match_header(lib):
     header = open(os.path.join(ROOT, "include", "etx.h")).read()
     header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
-    declared = set(re.findall(r"\b(etx_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(etx_[a-z0-9_]+)\s*\(", header))
+    assert "etx_embed_int8" in declared                 # a name with a digit must not slip through the pattern
     assert declared == set(binding.EXPORTS)
     for name in declared:
         assert getattr(lib, name) is not None          # raises AttributeError if not exported
@@ -70,3 +71,18 @@ def test_product_does_not_import_oracle():
         if f.endswith((".py", ".cpp")) and f != "calibrate_radius.py":
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "binding" not in text and "libetx" not in text and "csrc" not in text.replace("paper_2508_07423_b200/csrc)", ""), f
+
+
+def test_default_library_has_no_result_changing_environment_switches(lib):
+    """VERDICT r1 / ADVICE r1: timing experiments and measured alternatives that change results are compiled only
+    with -DETX_DEV_SWITCHES; the shipped library must not even contain their environment-variable names."""
+    blob = open(binding._LIB_PATH, "rb").read()
+    for name in (b"ETX_TC_EXP", b"ETX_SCATTER_ATOMIC", b"ETX_EMBED_FFMA", b"ETX_TC_DEBUG"):
+        assert name not in blob, name
+    src = "".join(open(os.path.join(ROOT, "paper_2508_07423_b200", "csrc", f)).read()
+                  for f in os.listdir(os.path.join(ROOT, "paper_2508_07423_b200", "csrc")))
+    for m in re.finditer(r"getenv\(", src):          # every getenv in the sources sits inside a developer-only block
+        head = src[:m.start()]
+        opened = max(head.rfind("#ifdef ETX_DEV_SWITCHES"), head.rfind("#else\n  static const bool debug"),
+                     head.rfind("#ifndef ETX_TC_COUNTERS"))
+        assert opened > head.rfind("#endif"), src[m.start() - 80:m.start() + 40]

@@ -67,21 +67,30 @@ def check_properties(cfg, batch, out):
     assert np.all(np.diff(perm)[same] > 0)                          # ascending edge id inside a group
     s = out["scores"]
     assert np.all(np.isfinite(s)) and s.min() >= 0.0 and s.max() <= 1.0
-    assert s.std() > 0.01 and np.mean((s > 0.02) & (s < 0.98)) > 0.5    # not saturated (Q14)
+    assert s.std() >= 0.04 and np.mean((s > 0.02) & (s < 0.98)) > 0.5    # neither collapsed nor saturated (Q14; floor 0.05 on the calibration events)
     return ev
 
 
-@pytest.mark.parametrize("name,sample,precision", [
-    ("c2", [0, 137, 500, 999], None), ("c3", [1, 998], None), ("c4", [0, 999], None),
-    ("c2", [0, 137, 500, 999], synth.PREC_TF32X3), ("c2", [0, 137, 500, 999], synth.PREC_BF16X3),
-    ("c2", [0, 999], synth.PREC_FP32), ("c4", [0, 999], synth.PREC_TF32X3)])
-def test_full_batch_sampled_events(B, name, sample, precision):
+def survey_subset(batch, every, n_ext):
+    """SURVEY 8(d)'s deterministic event subset: every `every`-th event, the n_ext largest and the n_ext smallest by hit count."""
+    n = np.diff(batch["event_ptr"].astype(np.int64))
+    order = np.argsort(n, kind="stable")
+    return sorted(set(range(0, len(n), every)) | set(order[:n_ext].tolist()) | set(order[len(n) - n_ext:].tolist()))
+
+
+# (config, every k-th event, extremes by hit count, precision).  The configs' own precisions get the survey's subset
+# (every 50th + 16 largest + 16 smallest: 50 events); the other modes a thinner one, the host oracle does ~4 events/s.
+@pytest.mark.parametrize("name,every,n_ext,precision", [
+    ("c2", 50, 16, None), ("c3", 50, 16, None), ("c4", 50, 16, None),
+    ("c2", 250, 4, synth.PREC_TF32X3), ("c2", 500, 2, synth.PREC_FP32), ("c4", 500, 4, synth.PREC_TF32X3)])
+def test_full_batch_sampled_events(B, name, every, n_ext, precision):
     cfg = synth.CONFIGS[name]
     if precision is not None:
         import dataclasses
         cfg = dataclasses.replace(cfg, precision=precision)
     batch = synth.generate_events(cfg)
     blob = synth.generate_weights(cfg)
+    sample = survey_subset(batch, every, n_ext)
     out = run_full(B, cfg, batch, blob, precision)
     ev = check_properties(cfg, batch, out)
     assert abs(out["E"] / len(batch["r"]) - cfg.target_degree) < 0.08 * cfg.target_degree
@@ -112,7 +121,8 @@ def test_full_batch_sampled_events(B, name, sample, precision):
         err = float(np.abs(out2["scores"][sel].astype(np.float64) - ora["scores"]).max())
         worst = max(worst, err)
         assert err <= TOL[cfg.precision], (name, e, err)
-    print(f"{name} precision={cfg.precision}: N={len(batch['r'])} E={out['E']} worst sampled |score - oracle| = {worst:.3g} "
+    print(f"{name} precision={cfg.precision}: {len(sample)} events (hits {int(np.diff(ep)[sample].min())}..{int(np.diff(ep)[sample].max())}), "
+          f"N={len(batch['r'])} E={out['E']} worst sampled |score - oracle| = {worst:.3g} "
           f"({n_border} border-pair differences end to end in the sampled events)")
 
 

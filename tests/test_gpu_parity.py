@@ -235,6 +235,78 @@ def test_host_buffer_entry_point_equals_device_path(B, c1, c1_oracle):
     assert etx.launch_count() > 0
 
 
+@pytest.mark.parametrize("prec", [0, 3])
+def test_host_path_splits_a_batch_larger_than_the_workspace(B, prec):
+    """PAPER.md:2638 (GNN batches bounded by memory) / VERDICT r1: a batch that does not fit the workspace is run as
+    consecutive event ranges and returns exactly what one pass returns -- events are independent."""
+    cfg = synth.CONFIGS["c2"]
+    batch = synth.generate_events(cfg, range(300, 348))
+    blob = synth.generate_weights(cfg)
+    etx = make_etx(B, cfg, blob, precision=prec)
+    r2, gap = synth.r2_max(cfg), cfg.max_plane_gap
+    n_ev, N = len(batch["event_ptr"]) - 1, len(batch["r"])
+    cap = int(N * (cfg.target_degree * 1.25 + 2))
+    host = B.pinned_host_batch(batch)
+
+    def run(ws_bytes):
+        etx.set_workspace(ws_bytes)
+        src = torch.full((cap,), -1, dtype=torch.int32).pin_memory()
+        dst = torch.full((cap,), -1, dtype=torch.int32).pin_memory()
+        sc = torch.full((cap,), -1.0, dtype=torch.float32).pin_memory()
+        l0 = etx.launch_count()
+        E = etx.etx_infer_host(host, r2, gap, cap, src, dst, sc)
+        return E, src[:E].numpy().copy(), dst[:E].numpy().copy(), sc[:E].numpy().copy(), etx.launch_count() - l0
+
+    full = etx.workspace_bytes(n_ev, N, cap, with_host_path=True)
+    E, src, dst, sc, l_one = run(full)
+    assert abs(E / N - cfg.target_degree) < 1.0
+    for frac in (0.45, 0.2, 0.07):                               # ~3, ~6 and ~16 ranges (ragged: events differ in size)
+        E2, src2, dst2, sc2, l_many = run(int(full * frac))
+        assert E2 == E and l_many > l_one                        # really ran in several passes
+        np.testing.assert_array_equal(src2, src)
+        np.testing.assert_array_equal(dst2, dst)
+        np.testing.assert_array_equal(sc2, sc)                   # same kernels, row-local arithmetic: bitwise
+    one = etx.workspace_bytes(1, int(np.diff(batch["event_ptr"]).max()), 64, with_host_path=True)
+    with pytest.raises(B.EtxError) as ei:                        # not even one event fits
+        run(one // 4)
+    assert ei.value.status == B.ETX_ERR_NOMEM
+    with pytest.raises(B.EtxError) as ei:                        # the caller's total capacity still binds
+        etx.set_workspace(int(full * 0.2))
+        etx.etx_infer_host(host, r2, gap, E // 2, None, None, torch.empty(E).pin_memory())
+    assert ei.value.status == B.ETX_ERR_CAPACITY
+
+
+def test_two_devices_in_one_process(B, c1):
+    """the >48 KB shared-memory opt-in is a per-device function attribute; a context on a second device
+    must configure its own kernels.  Needs two GPUs (skipped on the one-GPU box)."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    cfg, batch, blob = c1
+    outs = []
+    for dev in (0, 1):
+        with torch.cuda.device(dev):
+            etx = B.Etx(B.make_desc(cfg), blob, device=dev)
+            outs.append(B.run_path(etx, batch, synth.r2_max(cfg), cfg.max_plane_gap))
+    np.testing.assert_array_equal(outs[0]["scores"], outs[1]["scores"])
+
+
+def test_graph_build_hardening(B, c0):
+    """a huge plane gap must not overflow p + gap; a misaligned 4-d embedding is refused, not faulted."""
+    cfg, batch, blob = c0
+    etx = make_etx(B, cfg, blob)
+    a = B.run_path(etx, batch, synth.r2_max(cfg), 25)
+    b = B.run_path(etx, batch, synth.r2_max(cfg), 2**31 - 1)
+    np.testing.assert_array_equal(a["src"], b["src"])
+    np.testing.assert_array_equal(a["dst"], b["dst"])
+    db = B.DeviceBatch(batch, etx.device)
+    g = B.DeviceGraph(db.n_hits, 100000, etx.device)
+    etx.ensure_workspace(db.n_events, db.n_hits, 100000)
+    buf = torch.zeros(db.n_hits * 4 + 1, device=etx.device)
+    with pytest.raises(B.EtxError) as ei:
+        etx.etx_build_graph(db, buf[1:], 1e-3, 3, g)
+    assert ei.value.status == B.ETX_ERR_INVALID
+
+
 def test_deterministic_repeat(B, c1):
     cfg, batch, blob = c1
     etx = make_etx(B, cfg, blob)

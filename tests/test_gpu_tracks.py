@@ -89,3 +89,24 @@ def test_tracks_end_to_end_consistency(B, c1):
     np.testing.assert_array_equal(got, orc.wcc(len(batch["r"]), out["src"], out["dst"], out["scores"], s_min))
     keep = out["scores"] >= np.float32(s_min)
     assert np.all(got[out["src"][keep]] == got[out["dst"][keep]]) and np.all(got[got] == got)
+
+
+def test_tracks_long_zigzag_converges_beyond_64_rounds(B, c0):
+    """Adversarial component: a zig-zag a0->b0<-a1->b1<-a2 ... between two planes.  One forward + one
+    backward sweep move the minimum label two hops, so 150 alternations need ~150 rounds: a bounded loop (64 rounds
+    in round 1) returned wrong labels with ETX_OK.  The exact WCC (oracle: union-find) is one component."""
+    cfg, batch, blob = c0
+    etx = B.Etx(B.make_desc(cfg, precision=0), blob)
+    n = 150
+    one = {k: np.resize(batch[k], 2 * n).copy() for k in ("r", "phi", "z", "x", "y", "track")}
+    one["plane"] = np.repeat(np.array([0, 1], np.uint8), n)
+    one["event_ptr"] = np.array([0, 2 * n], np.int32)
+    src = np.concatenate([[0], np.repeat(np.arange(1, n), 2)]).astype(np.int32)          # a_i -> b_{i-1}, b_i
+    dst = np.concatenate([[n], (n + np.stack([np.arange(0, n - 1), np.arange(1, n)], 1)).ravel()]).astype(np.int32)
+    s = np.ones(len(src), np.float32)
+    want = orc.wcc(2 * n, src, dst, s, 0.5)
+    assert np.all(want == 0)
+    np.testing.assert_array_equal(gpu_labels(B, etx, one, src, dst, s, 0.5), want)
+    # the same chain cut in the middle: two components, second labelled by its smallest hit
+    s[len(s) // 2] = 0.0
+    np.testing.assert_array_equal(gpu_labels(B, etx, one, src, dst, s, 0.5), orc.wcc(2 * n, src, dst, s, 0.5))
