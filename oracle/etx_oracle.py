@@ -264,6 +264,103 @@ def triplets(n_hits: int, src, dst, scores, score_min: float) -> Dict[str, np.nd
     return {"articulation": as_arr(art), "left_elbow": as_arr(left), "right_elbow": as_arr(right)}
 
 
+def triplet_scores(e, trip: Dict[str, np.ndarray], H: int, n_layers: int, blob: np.ndarray, off_art: int,
+                   off_elb: int) -> Dict[str, np.ndarray]:
+    """NEXT-4 (triplet classifiers, "edge encodings are sufficient for both the edge classifier and triplet
+    classifier"; Fig. 8.12 caption P:2330 "[.,.] represents concatenation"; "separate triplet classifiers for
+    articulations and elbows ... each an MLP ending with a layer with 1 unit, and a sigmoid").  Reading (DESIGN Q23):
+    s = sigmoid(MLP_k([e_first, e_second])) on the rows ``triplets`` lists, MLP_art for articulations
+    (first = A->C, second = C->B), MLP_elb for BOTH elbow kinds (first < second edge id); each MLP is 2H -> H .. H -> 1
+    with the GNN's layer count, ReLU hidden layers, weights at blob[off_*].  Double accumulation (orc_mlp), sigmoid in
+    double, stored fp32 -- the same arithmetic convention as ``edge_scores``."""
+    e = _f32(e)
+    dims = [2 * H] + [H] * (n_layers - 1) + [1]
+    out = {}
+    for name, off in (("articulation", off_art), ("left_elbow", off_elb), ("right_elbow", off_elb)):
+        rows = np.asarray(trip[name], np.int64).reshape(-1, 2)
+        if len(rows) == 0:
+            out[name] = np.zeros(0, np.float32)
+            continue
+        x = np.concatenate([e[rows[:, 0]], e[rows[:, 1]]], axis=1)
+        logit = mlp(x, dims, blob, off)[:, 0].astype(np.float64)
+        out[name] = (1.0 / (1.0 + np.exp(-logit))).astype(np.float32)
+    return out
+
+
+def tracks_from_triplets(n_hits: int, src, dst, scores, score_min: float, trip: Dict[str, np.ndarray],
+                         trip_scores: Dict[str, np.ndarray], trip_min: float) -> Dict[str, object]:
+    """NEXT-4 (track building from triplets, the four steps of P:2363, section 8.3.5).  Plain Python, step by step.
+
+    Nodes of the EDGE graph are the kept edges (score >= score_min); its connections are the kept triplets
+    (triplet score >= trip_min, inclusive like the edge cut).  Reading of the four steps (DESIGN Q23):
+
+    1. "the left elbows and right elbows are connected ... Duplicate edges resulting from elbow connections are removed":
+       the two edges of every kept elbow are merged into one super-edge (union-find); every kept articulation (a, b)
+       becomes the pair (S(a), S(b)) of super-edges, pairs with S(a) == S(b) vanish and equal pairs count once.
+    2. "a WCC algorithm is applied to the edge graph, excluding these shared articulations": an articulation pair (u, v)
+       is SHARED iff u has two or more distinct successors or v has two or more distinct predecessors among the pairs
+       ("two articulations sharing an edge").  Connected sets = components of the super-edges under the unshared pairs.
+    3. "a new track is formed for each remaining articulation, effectively duplicating the shared set of connected
+       edges": every distinct pair (set of u, set of v) of a shared articulation gives the track  set(u) U set(v);  a
+       connected set touched by no shared articulation is a track by itself.
+    4. "edges are replaced by their corresponding hits": a track is the ascending list of the hits of its edges.
+
+    Labels: a connected set is named by its smallest edge id.  Returns
+      "edge_set"  int32 [E]   the set of every edge (-1 for an edge cut by score_min),
+      "joins"     int32 [J,2] the distinct (set of u, set of v) pairs of the shared articulations, ascending,
+      "tracks"    list of ascending hit tuples, ordered: untouched sets by label, then the joins in order."""
+    src = np.asarray(src, np.int64)
+    dst = np.asarray(dst, np.int64)
+    E = len(src)
+    keep = _f32(scores) >= np.float32(score_min)
+    parent = list(range(E))
+
+    def find(parent, x):
+        while parent[x] != x:
+            parent[x] = parent[parent[x]]
+            x = parent[x]
+        return x
+
+    def union(parent, a, b):
+        ra, rb = find(parent, a), find(parent, b)
+        if ra != rb:
+            parent[max(ra, rb)] = min(ra, rb)              # the root is the smallest edge id
+
+    tmin = np.float32(trip_min)
+    for kind in ("left_elbow", "right_elbow"):             # step 1: connect the elbows
+        for (a, b), s in zip(np.asarray(trip[kind], np.int64).reshape(-1, 2), _f32(trip_scores[kind])):
+            if s >= tmin:
+                union(parent, int(a), int(b))
+    pairs = set()
+    for (a, b), s in zip(np.asarray(trip["articulation"], np.int64).reshape(-1, 2), _f32(trip_scores["articulation"])):
+        if s >= tmin:
+            u, v = find(parent, int(a)), find(parent, int(b))
+            if u != v:
+                pairs.add((u, v))                          # duplicates removed
+    succ: Dict[int, set] = {}
+    pred: Dict[int, set] = {}
+    for u, v in pairs:
+        succ.setdefault(u, set()).add(v)
+        pred.setdefault(v, set()).add(u)
+    shared = {(u, v) for (u, v) in pairs if len(succ[u]) > 1 or len(pred[v]) > 1}
+    comp = list(parent)                                    # step 2: WCC without the shared articulations
+    for u, v in sorted(pairs - shared):
+        union(comp, u, v)
+    edge_set = np.full(E, -1, np.int32)
+    for e in range(E):
+        if keep[e]:
+            edge_set[e] = find(comp, e)
+    joins = sorted({(int(edge_set[u]), int(edge_set[v])) for (u, v) in shared})      # step 3
+    touched = {c for j in joins for c in j}
+    hits_of: Dict[int, set] = {}
+    for e in range(E):                                     # step 4: edges -> hits
+        if keep[e]:
+            hits_of.setdefault(int(edge_set[e]), set()).update((int(src[e]), int(dst[e])))
+    tracks = [tuple(sorted(hits_of[c])) for c in sorted(hits_of) if c not in touched]
+    tracks += [tuple(sorted(hits_of[a] | hits_of[b])) for (a, b) in joins]
+    return {"edge_set": edge_set, "joins": np.asarray(joins, np.int32).reshape(-1, 2), "tracks": tracks}
+
+
 def run_path(batch: Dict[str, np.ndarray], blob: np.ndarray, layout: Dict[str, Tuple[Tuple[int, ...], int]],
              H: int, n_iter: int, r2_max: float, gap: int, center, scale, n_planes: int = 26,
              graph: Optional[Tuple[np.ndarray, np.ndarray]] = None) -> Dict[str, np.ndarray]:

@@ -346,6 +346,35 @@ def generate_weights(cfg: Config) -> np.ndarray:
     return blob
 
 
+def triplet_layout(cfg: Config) -> Dict[str, Tuple[Tuple[int, ...], int]]:
+    """Next row (triplet classifiers): a SEPARATE blob holding two MLPs 2H -> H .. H -> 1, first the articulation
+    classifier, then the elbow classifier; name -> (dims, float offset)."""
+    H, hl = cfg.gnn_hidden, cfg.gnn_mlp_hidden_layers
+    dims = (2 * H,) + (H,) * hl + (1,)
+    n = sum(dims[i] * dims[i + 1] + dims[i + 1] for i in range(len(dims) - 1))
+    return {"trip_art": (dims, 0), "trip_elb": (dims, n)}
+
+
+def generate_triplet_weights(cfg: Config) -> np.ndarray:
+    """Xavier-uniform weights / U(-0.05, 0.05) biases of the two triplet classifiers, from their own key stream
+    (MLP indices 1000 and 1001), so the hot path's blob is unchanged."""
+    lay = triplet_layout(cfg)
+    dims = lay["trip_art"][0]
+    n = lay["trip_elb"][1]
+    blob = np.zeros(2 * n, dtype=np.float32)
+    for mi, (name, (_, off)) in enumerate(lay.items()):
+        o = off
+        for li in range(len(dims) - 1):
+            fi, fo = dims[li], dims[li + 1]
+            bound = np.sqrt(6.0 / (fi + fo))
+            kw = make_key(MASTER_SEED, cfg.seed_id, _P_WEIGHTS, 1000 + mi, li, 0)
+            kb = make_key(MASTER_SEED, cfg.seed_id, _P_WEIGHTS, 1000 + mi, li, 1)
+            blob[o:o + fi * fo] = ((2.0 * uniform01(kw, np.arange(fi * fo)) - 1.0) * bound).astype(np.float32)
+            blob[o + fi * fo:o + fi * fo + fo] = ((2.0 * uniform01(kb, np.arange(fo)) - 1.0) * 0.05).astype(np.float32)
+            o += fi * fo + fo
+    return blob
+
+
 # ----------------------------------------------------------------------------------------------
 # stored constants (radius per config), written by oracle/calibrate_radius.py (oracle-only script)
 # ----------------------------------------------------------------------------------------------
