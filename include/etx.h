@@ -172,6 +172,46 @@ typedef struct {
 etx_status etx_build_triplets(etx_ctx* ctx, const etx_batch* batch, const etx_graph* g, const float* d_scores,
                               float score_min, etx_triplets* t, void* stream);
 
+/* Next row: triplet classifiers ("edge encodings are sufficient for both the edge classifier and triplet
+ * classifier"; Fig. 8.12 caption P:2330, [.,.] = concatenation; "separate triplet classifiers for articulations
+ * and elbows", each "an MLP ending with a layer with 1 unit, and a sigmoid").  Reading: s = sigmoid(MLP_k([e_first,
+ * e_second])) on the rows of etx_build_triplets; MLP_art scores the articulations, MLP_elb both elbow kinds; each is
+ * 2H -> H .. H -> 1 with gnn_n_layers matrices.  The two MLPs come in their own host blob (articulation classifier,
+ * then elbow classifier; layer layout as the main blob) of etx_triplet_weight_count(desc) floats, and run in the
+ * context's precision.  d_trip_scores [n[0] + n[1] + n[2]] fp32, row for row with d_first / d_second.            */
+size_t etx_triplet_weight_count(const etx_model_desc* desc);
+etx_status etx_set_triplet_classifiers(etx_ctx* ctx, const float* h_weights, size_t n_weights);
+etx_status etx_triplet_scores(etx_ctx* ctx, const etx_graph* g, const float* d_edge_enc, const etx_triplets* t,
+                              float* d_trip_scores, void* stream);
+
+/* Next row: track building from triplets, the four steps of P:2363 (section 8.3.5).  The EDGE graph has the kept
+ * edges (score >= score_min) as nodes and the kept triplets (triplet score >= trip_min) as connections.
+ *   1. the two edges of every kept elbow are merged into one super-edge; a kept articulation (a, b) becomes the pair
+ *      (S(a), S(b)); pairs inside one super-edge vanish and equal pairs count once ("duplicate edges ... are removed");
+ *   2. a pair (u, v) is SHARED iff u has two or more distinct successors or v two or more distinct predecessors
+ *      ("two articulations sharing an edge"); connected sets = components under the elbows and the UNSHARED pairs;
+ *   3. every distinct (set of u, set of v) of a shared articulation is a track: the union of the two sets (the shared
+ *      set is duplicated into each of its tracks); a set touched by no shared articulation is a track by itself;
+ *   4. a track is the ascending list of the hits of its edges.
+ * Outputs (caller-owned DEVICE memory): d_edge_set[n_edges] = the set of every edge, named by its smallest edge id
+ * (-1 for a cut edge); d_joins [n_joins][2] = the distinct (set of u, set of v) pairs, ascending; tracks in CSR form,
+ * d_track_ptr [n_tracks + 1] / d_track_hits: first the n_plain untouched sets by ascending name, then the joins in
+ * order.  Everything is one fixed array (integer work).  Synchronises the stream twice to learn the counts; if a
+ * capacity is short returns ETX_ERR_CAPACITY with the four counts filled and only d_edge_set written.  Needs a
+ * workspace of etx_triplet_tracks_workspace_bytes (the same etx_set_workspace buffer; contents are clobbered).    */
+typedef struct {
+  int64_t join_capacity, track_capacity, hit_capacity;   /* in: rows of d_joins, tracks (d_track_ptr has +1), hit entries */
+  int64_t n_joins, n_plain, n_tracks, n_track_hits;      /* out */
+  int32_t* d_edge_set;                                   /* [n_edges]            */
+  int32_t* d_joins;                                      /* [join_capacity][2]   */
+  int32_t* d_track_ptr;                                  /* [track_capacity + 1] */
+  int32_t* d_track_hits;                                 /* [hit_capacity]       */
+} etx_tracks;
+size_t etx_triplet_tracks_workspace_bytes(const etx_ctx* ctx, int32_t n_hits, int64_t n_edges, int64_t n_articulations);
+etx_status etx_build_tracks_from_triplets(etx_ctx* ctx, const etx_batch* batch, const etx_graph* g, const float* d_scores,
+                                          float score_min, const etx_triplets* t, const float* d_trip_scores,
+                                          float trip_min, etx_tracks* tracks, void* stream);
+
 /* Whole path with HOST buffers: copies the batch host->device, runs a0..a7, copies src/dst/scores
  * back (h_src, h_dst may be NULL; each needs edge_capacity entries).  Host buffers should be pinned for
  * the copies to be asynchronous.  Synchronises the stream before returning.

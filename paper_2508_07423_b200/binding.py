@@ -22,7 +22,8 @@ ETX_OK, ETX_ERR_INVALID, ETX_ERR_CAPACITY, ETX_ERR_CUDA, ETX_ERR_UNSORTED, ETX_E
 EXPORTS = ["etx_weight_count", "etx_create", "etx_destroy", "etx_last_error", "etx_workspace_bytes",
            "etx_set_workspace", "etx_embed", "etx_embed_int8", "etx_build_graph", "etx_gnn_forward", "etx_edge_scores",
            "etx_infer_host", "etx_launch_count", "etx_profile_enable", "etx_profile_read", "etx_build_tracks",
-           "etx_build_triplets"]
+           "etx_build_triplets", "etx_triplet_weight_count", "etx_set_triplet_classifiers", "etx_triplet_scores",
+           "etx_triplet_tracks_workspace_bytes", "etx_build_tracks_from_triplets"]
 KERNEL_CLASSES = ["embed", "graph", "node_enc", "edge_enc", "scatter", "node_net", "edge_net", "cls", "tracks", "edge_proj"]
 
 
@@ -60,6 +61,13 @@ class Graph(C.Structure):
 class Triplets(C.Structure):
     _fields_ = [("capacity", C.c_int64), ("n", C.c_int64 * 3), ("d_ptr", C.c_void_p), ("d_first", C.c_void_p),
                 ("d_second", C.c_void_p)]
+
+
+class Tracks(C.Structure):
+    _fields_ = [("join_capacity", C.c_int64), ("track_capacity", C.c_int64), ("hit_capacity", C.c_int64),
+                ("n_joins", C.c_int64), ("n_plain", C.c_int64), ("n_tracks", C.c_int64), ("n_track_hits", C.c_int64),
+                ("d_edge_set", C.c_void_p), ("d_joins", C.c_void_p), ("d_track_ptr", C.c_void_p),
+                ("d_track_hits", C.c_void_p)]
 
 
 _lib = None
@@ -108,6 +116,17 @@ def load_library():
         lib.etx_build_triplets.restype = C.c_int
         lib.etx_build_triplets.argtypes = [C.c_void_p, C.POINTER(Batch), C.POINTER(Graph), C.c_void_p, C.c_float,
                                            C.POINTER(Triplets), C.c_void_p]
+        lib.etx_triplet_weight_count.restype = C.c_size_t
+        lib.etx_triplet_weight_count.argtypes = [C.POINTER(ModelDesc)]
+        lib.etx_set_triplet_classifiers.restype = C.c_int
+        lib.etx_set_triplet_classifiers.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
+        lib.etx_triplet_scores.restype = C.c_int
+        lib.etx_triplet_scores.argtypes = [C.c_void_p, C.POINTER(Graph), C.c_void_p, C.POINTER(Triplets), C.c_void_p, C.c_void_p]
+        lib.etx_triplet_tracks_workspace_bytes.restype = C.c_size_t
+        lib.etx_triplet_tracks_workspace_bytes.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int64]
+        lib.etx_build_tracks_from_triplets.restype = C.c_int
+        lib.etx_build_tracks_from_triplets.argtypes = [C.c_void_p, C.POINTER(Batch), C.POINTER(Graph), C.c_void_p, C.c_float,
+                                                       C.POINTER(Triplets), C.c_void_p, C.c_float, C.POINTER(Tracks), C.c_void_p]
         lib.etx_profile_enable.restype = C.c_int
         lib.etx_profile_enable.argtypes = [C.c_void_p, C.c_int]
         lib.etx_profile_read.restype = C.c_int
@@ -297,10 +316,57 @@ class Etx:
         self._check(st)
         n = [int(x) for x in t.n]
         o = [0, n[0], n[0] + n[1], n[0] + n[1] + n[2]]
-        out = {"ptr": ptr}
+        out = {"ptr": ptr, "c": t, "rows": rows}          # "c": the etx_triplets struct (points into "ptr" / "rows")
         for k, name in enumerate(("articulation", "left_elbow", "right_elbow")):
             out[name] = torch.stack([rows[0, o[k]:o[k + 1]], rows[1, o[k]:o[k + 1]]], dim=1)
         return out
+
+    # ---- next row: triplet classifiers and track building from triplets
+    def etx_set_triplet_classifiers(self, weights: np.ndarray):
+        w = np.ascontiguousarray(weights, dtype=np.float32)
+        self._check(self.lib.etx_set_triplet_classifiers(self.handle, w.ctypes.data_as(C.c_void_p), w.size))
+
+    def etx_triplet_scores(self, graph: DeviceGraph, edge_enc: torch.Tensor, trip: Dict[str, torch.Tensor]) -> Dict[str, torch.Tensor]:
+        """Scores per kind (views of one buffer under "all", row for row with the triplet rows)."""
+        n = [int(x) for x in trip["c"].n]
+        s = torch.empty(max(sum(n), 1), dtype=torch.float32, device=self.device)
+        self._check(self.lib.etx_triplet_scores(self.handle, C.byref(graph.c), _ptr(edge_enc), C.byref(trip["c"]), _ptr(s),
+                                                self._stream()))
+        o = [0, n[0], n[0] + n[1], sum(n)]
+        out = {"all": s}
+        for k, name in enumerate(("articulation", "left_elbow", "right_elbow")):
+            out[name] = s[o[k]:o[k + 1]]
+        return out
+
+    def etx_build_tracks_from_triplets(self, batch: DeviceBatch, graph: DeviceGraph, scores: torch.Tensor, score_min: float,
+                                       trip: Dict[str, torch.Tensor], trip_scores: torch.Tensor, trip_min: float) -> Dict[str, torch.Tensor]:
+        """edge_set [E], joins [J, 2], track_ptr [T + 1], track_hits; sized from a first counting call.  Uses (and
+        clobbers) the context workspace."""
+        E = graph.n_edges
+        need = int(self.lib.etx_triplet_tracks_workspace_bytes(self.handle, batch.n_hits, E, int(trip["c"].n[0])))
+        if self._ws is None or self._ws_bytes < need:
+            self.set_workspace(need)
+        i32 = dict(dtype=torch.int32, device=self.device)
+        edge_set = torch.empty(max(E, 1), **i32)
+        tk = Tracks()
+        tk.d_edge_set = edge_set.data_ptr()
+
+        def call(nj, nt, nh):
+            joins = torch.empty(max(nj, 1), 2, **i32)
+            tptr = torch.empty(nt + 1, **i32)
+            thits = torch.empty(max(nh, 1), **i32)
+            tk.join_capacity, tk.track_capacity, tk.hit_capacity = nj, nt, nh
+            tk.d_joins, tk.d_track_ptr, tk.d_track_hits = joins.data_ptr(), tptr.data_ptr(), thits.data_ptr()
+            st = self.lib.etx_build_tracks_from_triplets(self.handle, C.byref(batch.c), C.byref(graph.c), _ptr(scores), score_min,
+                                                         C.byref(trip["c"]), _ptr(trip_scores), trip_min, C.byref(tk), self._stream())
+            return st, joins, tptr, thits
+
+        st, joins, tptr, thits = call(0, 0, 0)
+        if st == ETX_ERR_CAPACITY:
+            st, joins, tptr, thits = call(int(tk.n_joins), int(tk.n_tracks), int(tk.n_track_hits))
+        self._check(st)
+        return {"edge_set": edge_set[:E], "joins": joins[:int(tk.n_joins)], "track_ptr": tptr[:int(tk.n_tracks) + 1],
+                "track_hits": thits[:int(tk.n_track_hits)], "n_plain": int(tk.n_plain)}
 
     # ---- whole path with host buffers (pinned torch tensors or numpy arrays)
     def etx_infer_host(self, host: Dict[str, torch.Tensor], r2_max: float, max_plane_gap: int,

@@ -74,6 +74,11 @@ struct etx_ctx {
   int* d_emb_wq = nullptr;              // INT8 codes of the embedding MLP's weights (next row), packed 4 per word
   int emb_wq_off[etx::kMaxLayers] = {0};
   float emb_sw[etx::kMaxLayers] = {0};  // their per-layer scales max|W| / 127
+  // next row: the two triplet classifiers (articulations, elbows), set by etx_set_triplet_classifiers
+  float* d_trip_weights = nullptr;
+  unsigned char* d_trip_wimg = nullptr;
+  etx::DevMlp trip_art, trip_elb;
+  bool have_trip = false;
   cudaStream_t copy_stream = nullptr;   // etx_infer_host: edge-list copy-out underneath the message passing
   cudaEvent_t copy_event = nullptr;
   // per-stage profiling (etx_profile_enable / etx_profile_read)
@@ -158,6 +163,15 @@ int tc_chunk_k(int mode);
 // ---- tracks.cu (next row: score cut + weakly connected components)
 int launch_wcc(int n_events, const int32_t* event_ptr, const int32_t* row_ptr, const int32_t* src,
                const int32_t* dst, const float* scores, float score_min, int32_t* labels, cudaStream_t s);
+
+// ---- triplet_tracks.cu (next row: track building from triplets)
+size_t triplet_tracks_ws_bytes(int n_hits, long long n_edges, long long n_art);
+int run_triplet_tracks(int n_events, int n_hits, long long n_edges, const int32_t* event_ptr, const int32_t* row_ptr,
+                       const int32_t* in_ptr, const int32_t* in_perm, const float* scores, float score_min,
+                       const int32_t* tptr, const long long n_trip[3], const int32_t* first, const int32_t* second,
+                       const float* tscores, float trip_min, char* ws, int32_t* d_edge_set, long long join_capacity,
+                       int32_t* d_joins, long long track_capacity, int32_t* d_track_ptr, long long hit_capacity,
+                       int32_t* d_track_hits, long long counts[4], bool* capacity_ok, cudaStream_t s);
 
 // ---- embed_int8.cu (next row: INT8 embedding MLP)
 struct Int8Args {

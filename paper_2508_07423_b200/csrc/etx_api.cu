@@ -449,6 +449,8 @@ etx_status etx_destroy(etx_ctx* c) {
   if (c->d_weights) cudaFree(c->d_weights);
   if (c->d_wimg) cudaFree(c->d_wimg);
   if (c->d_emb_wq) cudaFree(c->d_emb_wq);
+  if (c->d_trip_weights) cudaFree(c->d_trip_weights);
+  if (c->d_trip_wimg) cudaFree(c->d_trip_wimg);
   for (const etx_ctx::ProfRec& r : c->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
   if (c->copy_stream) { cudaStreamDestroy(c->copy_stream); cudaEventDestroy(c->copy_event); }
@@ -797,6 +799,139 @@ etx_status etx_build_triplets(etx_ctx* c, const etx_batch* b, const etx_graph* g
                                        t->d_first, t->d_second, s);
   }
   return check_cuda(c, "etx_build_triplets (fill)");
+}
+
+size_t etx_triplet_weight_count(const etx_model_desc* desc) {
+  if (check_desc(desc)) return 0;
+  const int H = desc->gnn_hidden, L = desc->gnn_n_layers;
+  size_t one = (size_t)2 * H * H + H;
+  for (int l = 1; l < L - 1; ++l) one += (size_t)H * H + H;
+  one += (size_t)H + 1;
+  return 2 * one;
+}
+
+etx_status etx_set_triplet_classifiers(etx_ctx* c, const float* h_weights, size_t n_weights) {
+  if (!c) return ETX_ERR_INVALID;
+  if (!h_weights || n_weights != etx_triplet_weight_count(&c->desc))
+    return fail(c, ETX_ERR_INVALID, "triplet classifier blob size does not match (see etx_triplet_weight_count)");
+  cudaSetDevice(c->device);
+  const int H = c->desc.gnn_hidden, L = c->desc.gnn_n_layers;
+  HostMlp m; m.n_layers = L; m.dims[0] = 2 * H;
+  for (int l = 1; l < L; ++l) m.dims[l] = H;
+  m.dims[L] = 1;
+  std::vector<float> staged;
+  std::vector<unsigned char> img;
+  size_t offW[2][kMaxLayers], offB[2][kMaxLayers], img_off[2] = {0, 0};
+  size_t src = 0;
+  for (int i = 0; i < 2; ++i) {
+    if (c->desc.precision != ETX_PREC_FP32) { img_off[i] = img.size(); append_wimg(img, m, h_weights + src, 0, 0, L - 1, c->desc.precision); }
+    for (int l = 0; l < L; ++l) {
+      const int fi = m.dims[l], fo = m.dims[l + 1];
+      staged.resize(align_up(staged.size(), 64));
+      offW[i][l] = staged.size();
+      staged.resize(staged.size() + (size_t)fi * fo);
+      float* Wt = staged.data() + offW[i][l];
+      const float* W = h_weights + src;
+      for (int o = 0; o < fo; ++o)
+        for (int k = 0; k < fi; ++k) Wt[(size_t)k * fo + o] = W[(size_t)o * fi + k];
+      src += (size_t)fi * fo;
+      staged.resize(align_up(staged.size(), 64));
+      offB[i][l] = staged.size();
+      staged.insert(staged.end(), h_weights + src, h_weights + src + fo);
+      src += fo;
+    }
+  }
+  if (c->d_trip_weights) { cudaFree(c->d_trip_weights); c->d_trip_weights = nullptr; }
+  if (c->d_trip_wimg) { cudaFree(c->d_trip_wimg); c->d_trip_wimg = nullptr; }
+  c->have_trip = false;
+  if (cudaMalloc(&c->d_trip_weights, staged.size() * sizeof(float)) != cudaSuccess ||
+      cudaMemcpy(c->d_trip_weights, staged.data(), staged.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess)
+    return check_cuda(c, "etx_set_triplet_classifiers");
+  if (!img.empty() && (cudaMalloc(&c->d_trip_wimg, img.size()) != cudaSuccess ||
+                       cudaMemcpy(c->d_trip_wimg, img.data(), img.size(), cudaMemcpyHostToDevice) != cudaSuccess))
+    return check_cuda(c, "etx_set_triplet_classifiers");
+  DevMlp* dm[2] = {&c->trip_art, &c->trip_elb};
+  for (int i = 0; i < 2; ++i) {
+    *dm[i] = DevMlp();
+    dm[i]->n_layers = L;
+    for (int l = 0; l <= L; ++l) dm[i]->dims[l] = m.dims[l];
+    for (int l = 0; l < L; ++l) { dm[i]->Wt[l] = c->d_trip_weights + offW[i][l]; dm[i]->b[l] = c->d_trip_weights + offB[i][l]; }
+    if (c->d_trip_wimg) dm[i]->wimg = c->d_trip_wimg + img_off[i];
+  }
+  c->have_trip = true;
+  return ETX_OK;
+}
+
+etx_status etx_triplet_scores(etx_ctx* c, const etx_graph* g, const float* d_edge_enc, const etx_triplets* t,
+                              float* d_trip_scores, void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (!c->have_trip) return fail(c, ETX_ERR_INVALID, "no triplet classifiers set (etx_set_triplet_classifiers)");
+  if (!g || g->n_edges < 0 || !t) return fail(c, ETX_ERR_INVALID, "graph / triplets are NULL");
+  const int64_t total = t->n[0] + t->n[1] + t->n[2];
+  if (t->n[0] < 0 || t->n[1] < 0 || t->n[2] < 0 || total > t->capacity) return fail(c, ETX_ERR_INVALID, "triplets not built");
+  if (total > 0 && (!d_edge_enc || !d_trip_scores || !t->d_first || !t->d_second)) return fail(c, ETX_ERR_INVALID, "triplet buffers are NULL");
+  if ((uintptr_t)d_edge_enc & 15) return fail(c, ETX_ERR_INVALID, "d_edge_enc must be 16-byte aligned");
+  cudaSetDevice(c->device);
+  const int H = c->desc.gnn_hidden;
+  for (int part = 0; part < 2; ++part) {                 // articulations, then both elbow kinds (adjacent sections)
+    const int64_t r0 = part == 0 ? 0 : t->n[0], nr = part == 0 ? t->n[0] : t->n[1] + t->n[2];
+    if (nr <= 0) continue;
+    MlpArgs a;
+    a.n_rows = (int)nr; a.n_seg = 2;
+    a.seg[0] = Segment{d_edge_enc, t->d_first + r0, H, H};
+    a.seg[1] = Segment{d_edge_enc, t->d_second + r0, H, H};
+    a.mlp = part == 0 ? c->trip_art : c->trip_elb;
+    a.out_mode = 3; a.out = d_trip_scores + r0; a.out_ld = 1;
+    ProfScope ps(c, ETX_K_TRACKS, (cudaStream_t)stream);
+    c->launches += run_mlp(c, a, (cudaStream_t)stream);
+  }
+  return check_cuda(c, "etx_triplet_scores");
+}
+
+size_t etx_triplet_tracks_workspace_bytes(const etx_ctx* c, int32_t n_hits, int64_t n_edges, int64_t n_articulations) {
+  if (!c || n_hits < 0 || n_edges < 0 || n_articulations < 0) return 0;
+  return triplet_tracks_ws_bytes(n_hits, n_edges, n_articulations);
+}
+
+etx_status etx_build_tracks_from_triplets(etx_ctx* c, const etx_batch* b, const etx_graph* g, const float* d_scores,
+                                          float score_min, const etx_triplets* t, const float* d_trip_scores,
+                                          float trip_min, etx_tracks* out, void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (etx_status st = check_batch(c, b)) return st;
+  if (!g || g->n_edges < 0 || !g->d_row_ptr || !g->d_in_ptr) return fail(c, ETX_ERR_INVALID, "graph is NULL or not built");
+  if (!t || !t->d_ptr || !out) return fail(c, ETX_ERR_INVALID, "triplets / tracks are NULL");
+  const int64_t total = t->n[0] + t->n[1] + t->n[2];
+  if (t->n[0] < 0 || t->n[1] < 0 || t->n[2] < 0 || total > t->capacity) return fail(c, ETX_ERR_INVALID, "triplets not built");
+  if (total > 0 && (!t->d_first || !t->d_second || !d_trip_scores)) return fail(c, ETX_ERR_INVALID, "triplet rows / scores are NULL");
+  if (g->n_edges > 0 && (!d_scores || !g->d_in_perm || !out->d_edge_set)) return fail(c, ETX_ERR_INVALID, "scores / in_perm / d_edge_set are NULL");
+  if (out->join_capacity < 0 || out->track_capacity < 0 || out->hit_capacity < 0) return fail(c, ETX_ERR_INVALID, "negative capacity");
+  if (!out->d_track_ptr || (out->join_capacity > 0 && !out->d_joins) || (out->hit_capacity > 0 && !out->d_track_hits))
+    return fail(c, ETX_ERR_INVALID, "track buffers are NULL");
+  cudaSetDevice(c->device);
+  if (!c->ws) return fail(c, ETX_ERR_NOMEM, "no workspace set (etx_set_workspace)");
+  const size_t need = triplet_tracks_ws_bytes(b->n_hits, g->n_edges, t->n[0]);
+  if (need > c->ws_bytes)
+    return fail(c, ETX_ERR_NOMEM, "workspace too small: need " + std::to_string(need) + " bytes (etx_triplet_tracks_workspace_bytes), have " +
+                                      std::to_string(c->ws_bytes));
+  long long counts[4] = {0, 0, 0, 0};
+  const long long ntr[3] = {t->n[0], t->n[1], t->n[2]};
+  bool ok = true;
+  int n;
+  {
+    ProfScope ps(c, ETX_K_TRACKS, (cudaStream_t)stream);
+    n = run_triplet_tracks(b->n_events, b->n_hits, g->n_edges, b->d_event_ptr, g->d_row_ptr, g->d_in_ptr, g->d_in_perm,
+                           d_scores, score_min, t->d_ptr, ntr, t->d_first, t->d_second, d_trip_scores, trip_min,
+                           (char*)c->ws, out->d_edge_set, out->join_capacity, out->d_joins, out->track_capacity,
+                           out->d_track_ptr, out->hit_capacity, out->d_track_hits, counts, &ok, (cudaStream_t)stream);
+    if (n > 0) c->launches += n;
+  }
+  out->n_joins = counts[0]; out->n_plain = counts[1]; out->n_tracks = counts[2]; out->n_track_hits = counts[3];
+  if (n < 0) return check_cuda(c, "etx_build_tracks_from_triplets");
+  if (etx_status st = check_cuda(c, "etx_build_tracks_from_triplets")) return st;
+  if (!ok)
+    return fail(c, ETX_ERR_CAPACITY, "tracks need " + std::to_string(counts[0]) + " joins, " + std::to_string(counts[2]) +
+                                         " tracks, " + std::to_string(counts[3]) + " hit entries");
+  return ETX_OK;
 }
 
 // One pass of the whole path over events [e0, e1) of a HOST batch (hits [h0, h1)), results appended at edge

@@ -155,8 +155,11 @@ CONFIGS: Dict[str, Config] = {
                  precision=PREC_BF16X3),
     "c3": Config("c3", 2, 1000, 150, True, 0.05, (3, 128, 128, 128, 4), 128, 2, 6, 6.0, gain=_stored_gain("c3"),
                  precision=PREC_BF16),
+    # C4 runs the exact-fp32 FFMA mode: at the oracle-calibrated gain its activations reach |h| ~ 2e2 over 8 steps and
+    # the split tensor-core modes (whose fp32 accumulation truncates) miss BASELINE.json's 1e-4 on the worst edges
+    # (measured 4.5e-4 max, 1.4e-4 at p99.99 of 35.6 M edges; profiles/r02_parity.md); FFMA holds 2e-6.
     "c4": Config("c4", 4, 1000, 300, True, 0.10, (3, 128, 128, 128, 4), 128, 2, 8, 10.0, gain=_stored_gain("c4"),
-                 precision=PREC_BF16X3),
+                 precision=PREC_FP32),
 }
 
 _P_EVENTS, _P_WEIGHTS = 1, 2
