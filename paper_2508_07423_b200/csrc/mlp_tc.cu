@@ -67,7 +67,6 @@ constexpr int kEpiThreads = 256;         // warpgroups 4-5 (warps 16-23): lane q
 constexpr int kThreads = kGatherThreads + kEpiThreads + 128;   // + warpgroup 6: loader warp 24, MMA warp 25, two idle warps
 constexpr int kWarpEpi0 = kGatherThreads / 32, kWarpLoader = kWarpEpi0 + kEpiThreads / 32, kWarpMma = kWarpLoader + 1, kWarpCommit = kWarpMma + 1;
 constexpr uint32_t kBarEntry0 = 2;       // named barriers 2 .. 2 + NSTAGE_A - 1: one per operand-ring entry
-constexpr uint32_t kBarOut0 = 12;        // named barriers 12, 13: the four epilogue warps of a column half around their shared output box
 // Register re-partitioning (setmaxnreg, per warpgroup): the kernel launches at <= 72 registers per
 // thread (896 threads), then the gather warpgroups shrink to 64, loader/MMA to 40, and the epilogue
 // warpgroups grow to 104.  More, thinner warps: the SIMT roles are latency-bound, not issue-bound.
@@ -606,14 +605,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
           // state: one IEEE fp32 add per element, performed at L2, no residual load, deterministic (each
           // element is touched exactly once).  No SIMT global traffic, no read-back of the staging tile,
           // rows past n_rows are clipped by the tensor map.
-          // One 8 KB box [128 rows x 16 columns] per column half and step (the four lane-quarter warps of a half
-          // fill it together): 8 TMA operations per tile instead of 32.  The per-warp 2 KB boxes of round 1 spent
-          // ~690 cycles per box waiting for the TMA unit to read the previous one -- a per-OPERATION cost (smaller
-          // boxes were slower, wider ones of the same size no faster), so the cure is fewer, larger operations.
-          const uint32_t stg = stage_out + hh * 8192;
-          const uint32_t bar_id = kBarOut0 + hh;
+          const uint32_t stg = stage_out + ew * 2048;
           const bool in_place_add = (a.out_mode == 1);
-          const int row0 = tile * TM;
+          const int row0 = tile * TM + q4 * 32;
 #pragma unroll 1
           for (int q = 0; q < 4; ++q) {
             const int col0 = hh * 64 + q * 16;
@@ -628,19 +622,19 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             tc_wait_ld();
             EP_ACC(3);
             if (q == 3) { tc_fence_before(); mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane); }
-            if (q4 == 0 && lane == 0) bulk_wait_read0();   // the TMA unit has read the previous box out of the staging slice
-            named_bar_sync(bar_id, 128);                   // ... and the four warps of this half may overwrite it
+            if (lane == 0) bulk_wait_read0();      // the TMA unit has read the previous box out of the staging slice
+            __syncwarp();
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
               const float4 bq = *reinterpret_cast<const float4*>(bias + col0 + 4 * j);
-              st_shared_v4(stg + et * 64 + ((j ^ ((lane >> 1) & 3)) << 4),
+              st_shared_v4(stg + lane * 64 + ((j ^ ((lane >> 1) & 3)) << 4),
                            __float_as_uint(__uint_as_float(v[4 * j]) + bq.x), __float_as_uint(__uint_as_float(v[4 * j + 1]) + bq.y),
                            __float_as_uint(__uint_as_float(v[4 * j + 2]) + bq.z), __float_as_uint(__uint_as_float(v[4 * j + 3]) + bq.w));
             }
             fence_async_smem();                    // generic-proxy writes -> async proxy (TMA)
-            named_bar_sync(bar_id, 128);           // the box is complete
+            __syncwarp();
             EP_ACC(4);
-            if (q4 == 0 && lane == 0) {
+            if (lane == 0) {
               const int cg = (wide ? sl * HW : 0) + col0;
               if (in_place_add) tma_reduce_add_2d(&tmap, stg, cg, row0);
               else tma_store_2d(&tmap, stg, cg, row0);
@@ -651,7 +645,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
         }
       }
     }
-    if (q4 == 0 && lane == 0) bulk_wait_all();   // every output box has left the SM before the CTA retires
+    if (lane == 0) bulk_wait_all();              // every output box has left the SM before the CTA retires
     __syncwarp();
     if (edbg && ew == 0 && lane == 0) {
       a.dbg[(size_t)blockIdx.x * 32 + 6] = (unsigned long long)e_wait;
@@ -830,7 +824,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
 }
 
 // Tensor map of the output [n_rows][n_cols] fp32 (row stride out_ld floats) with the epilogue's box: 16 columns
-// (64 bytes, SWIZZLE_64B) x 128 rows (a whole tile's rows).  cuTensorMapEncodeTiled is fetched through the runtime (no link-time
+// (64 bytes, SWIZZLE_64B) x 32 rows.  cuTensorMapEncodeTiled is fetched through the runtime (no link-time
 // dependency on libcuda: the library must still load on a machine without a driver).
 bool encode_out_map(CUtensorMap* m, float* out, int n_rows, int n_cols, int out_ld) {
   using Fn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -846,7 +840,7 @@ bool encode_out_map(CUtensorMap* m, float* out, int n_rows, int n_cols, int out_
   if (!fn || (reinterpret_cast<uintptr_t>(out) & 15) || (out_ld & 3)) return false;
   const cuuint64_t dims[2] = {(cuuint64_t)n_cols, (cuuint64_t)n_rows};
   const cuuint64_t strides[1] = {(cuuint64_t)out_ld * sizeof(float)};
-  const cuuint32_t box[2] = {16, 128}, estr[2] = {1, 1};
+  const cuuint32_t box[2] = {16, 32}, estr[2] = {1, 1};
   return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, out, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
