@@ -147,6 +147,21 @@ void orc_mlp_int8(int64_t n, int32_t n_layers, const int32_t* dims, const float*
   }
 }
 
+// ---- next row (GNN part): the message aggregation of Eq. 8.5 in PLAIN fp32 -- every sum
+//      starts from 0 and adds its edges' encodings one by one in ascending edge id, each add a single rounded fp32
+//      operation ("fp32 scatter").  The hot path's oracle (orc_scatter) accumulates in double; the
+//      quantised path needs the aggregate itself reproducible bit for bit, because it feeds a quantiser (a last-bit
+//      difference in m can move an INT8 code).  m [n_nodes, 2H] = [outgoing sum, incoming sum].
+void orc_scatter_f32(int64_t n_nodes, int64_t n_edges, const int32_t* src, const int32_t* dst, const float* e, int32_t H,
+                     float* m) {
+  for (int64_t i = 0; i < n_nodes * 2 * H; ++i) m[i] = 0.0f;
+  for (int64_t k = 0; k < n_edges; ++k) {               // ascending edge id
+    float* mo = m + (int64_t)src[k] * 2 * H;
+    float* mi = m + (int64_t)dst[k] * 2 * H + H;
+    for (int c = 0; c < H; ++c) { mo[c] = mo[c] + e[k * H + c]; mi[c] = mi[c] + e[k * H + c]; }
+  }
+}
+
 // ---- a2 rough graph: hit i on plane p connects to hits j of the same event on planes
 //      p+1 .. min(p+G, L-1) iff d^2(i,j) < r2_max (Eq. 8.1; strict "<": P:2674).
 //      Sequential loop over candidates in ascending index, as P:2674 describes, so edges come out in

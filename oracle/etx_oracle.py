@@ -215,6 +215,86 @@ def edge_scores(e, H: int, n_layers: int, blob: np.ndarray, off_cls: int, want_l
     return (s, lg) if want_logits else s
 
 
+def scatter_f32(n_nodes: int, src, dst, e) -> np.ndarray:
+    """NEXT-3 (GNN part): Eq. 8.5 in plain fp32, sequential adds in ascending edge id (see orc_scatter_f32)."""
+    e = _f32(e)
+    src = np.ascontiguousarray(src, np.int32)
+    dst = np.ascontiguousarray(dst, np.int32)
+    H = e.shape[1]
+    m = np.empty((n_nodes, 2 * H), np.float32)
+    lib().orc_scatter_f32(C.c_int64(n_nodes), C.c_int64(len(src)), _p(src, C.c_int32), _p(dst, C.c_int32),
+                          _p(e, C.c_float), C.c_int32(H), _p(m, C.c_float))
+    return m
+
+
+GNN_MLPS = ("node_enc", "edge_enc", "node_net", "edge_net", "cls")
+
+
+def gnn_mlp_names(n_iter: int) -> List[str]:
+    """The GNN's MLPs in the order their calibrated ranges are stored / handed to the library."""
+    return ["node_enc", "edge_enc"] + [f"{n}_{k}" for k in range(n_iter) for n in ("node_net", "edge_net")] + ["cls"]
+
+
+def _relu(x):
+    return np.where(x > 0, x, np.float32(0.0)).astype(np.float32)
+
+
+def gnn_forward_steps(f_node, src, dst, n_iter: int, mlp_fn, scatter_fn):
+    """a3-a7 written out step by step in the thesis' order on top of an MLP
+    evaluator ``mlp_fn(name, x) -> y`` and an aggregator ``scatter_fn(n_nodes, src, dst, e) -> m``; the concatenation
+    orders are those of the hot path (Q10: [h, m_out, m_in], [h_src, h_dst, e], [h_src, h_dst]); residual adds are
+    single fp32 additions.  Returns h^n, e^n and the classifier's logits."""
+    f_node = _f32(f_node)
+    src = np.asarray(src, np.int64)
+    dst = np.asarray(dst, np.int64)
+    n = f_node.shape[0]
+    h = mlp_fn("node_enc", f_node)
+    e = mlp_fn("edge_enc", np.concatenate([h[src], h[dst]], axis=1))
+    for k in range(n_iter):
+        m = scatter_fn(n, src, dst, e)
+        h = (h + mlp_fn(f"node_net_{k}", np.concatenate([h, m], axis=1))).astype(np.float32)
+        e = (e + mlp_fn(f"edge_net_{k}", np.concatenate([h[src], h[dst], e], axis=1))).astype(np.float32)
+    return h, e, mlp_fn("cls", e)[:, 0]
+
+
+def gnn_int8_calibration(f_node, src, dst, n_iter: int, blob: np.ndarray, layout) -> Dict[str, List[float]]:
+    """Static PTQ calibration of the GNN's MLPs with a max observer: the fp32 model (this module's
+    plain MLP and double-accumulating scatter) runs on the sample and the range of every layer's INPUT is recorded."""
+    blob = _f32(blob)
+    ranges: Dict[str, List[float]] = {}
+
+    def fp32_mlp(name, x):
+        dims, off = layout[name]
+        ranges[name] = [float(a) for a in int8_calibration(x, dims, blob, off)]
+        return mlp(x, dims, blob, off)
+
+    gnn_forward_steps(f_node, src, dst, n_iter, fp32_mlp, scatter)
+    return ranges
+
+
+def gnn_forward_int8(f_node, src, dst, n_iter: int, blob: np.ndarray, layout, act_alpha: Dict[str, Sequence[float]]):
+    """NEXT-3 (GNN part; "quantization of the GNN holds the most potential"; scheme of Eqs. 4.31-4.33): every MLP
+    of the GNN evaluated by ``mlp_int8`` (INT8 codes for every layer's input and weight, exact integer sums, fp32
+    de-quantisation and biases), state h, e and the aggregate m in fp32, fp32 scatter (``scatter_f32``), fp32 residual
+    adds.  One exception (DESIGN Q24): the node encoder's FIRST layer -- 3 raw geometry features in -- stays the fp32
+    layer of the hot path (double accumulation), its ReLU output is the first quantised tensor.  act_alpha[name][l] is
+    the calibrated range of layer l's input (entry 0 of node_enc is unused).  Returns h^n, e^n, logits, scores."""
+    blob = _f32(blob)
+
+    def q_mlp(name, x):
+        dims, off = layout[name]
+        al = list(act_alpha[name])
+        if name == "node_enc":
+            x = _relu(mlp(x, dims[:2], blob, off))
+            off += dims[0] * dims[1] + dims[1]
+            dims, al = dims[1:], al[1:]
+        return mlp_int8(x, dims, blob, off, al)
+
+    h, e, logit = gnn_forward_steps(f_node, src, dst, n_iter, q_mlp, scatter_f32)
+    s = (1.0 / (1.0 + np.exp(-logit.astype(np.float64)))).astype(np.float32)
+    return h, e, logit, s
+
+
 def wcc(n_hits: int, src, dst, scores, score_min: float) -> np.ndarray:
     """NEXT-1: labels [n_hits] = smallest hit index of the weakly connected
     component of the purified graph (edges with score >= score_min)."""

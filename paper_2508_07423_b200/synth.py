@@ -387,6 +387,13 @@ def int8_act_alpha(cfg: Config) -> np.ndarray:
     return np.asarray(load_constants()[key]["int8_act_alpha"], np.float32)
 
 
+def int8_gnn_alpha(cfg: Config) -> Dict[str, List[float]]:
+    """Stored calibrated activation ranges of the INT8 GNN (next row; oracle/calibrate_int8_gnn.py): MLP name -> one
+    range per layer input."""
+    key = {"c3": "c2"}.get(cfg.name, cfg.name)
+    return load_constants()[key]["int8_gnn_alpha"]
+
+
 def r2_max(cfg: Config) -> float:
     """Stored fp32 r^2 for the config; both paths read this constant."""
     key = {"c3": "c2"}.get(cfg.name, cfg.name)

@@ -5,7 +5,7 @@ Nothing in this file touches the CUDA library."""
 import numpy as np
 import pytest
 
-from oracle import calibrate_gain, calibrate_int8, calibrate_radius
+from oracle import calibrate_gain, calibrate_int8, calibrate_int8_gnn, calibrate_radius
 from paper_2508_07423_b200 import synth
 
 NAMES = ("c0", "c1", "c2", "c4")
@@ -40,6 +40,14 @@ def test_gain_is_regenerated_by_the_oracle_script(stored, name):
     # ... and every smaller grid value was rejected (the rule takes the smallest accepted one)
     assert all(not calibrate_gain.accept(t) for t in got["gain_tried"][:-1])
     assert [t["gain"] for t in got["gain_tried"]] == calibrate_gain.GRID[:len(got["gain_tried"])]
+
+
+@pytest.mark.parametrize("name", NAMES)
+def test_int8_gnn_ranges_are_regenerated_by_the_oracle_script(stored, name):
+    got = calibrate_int8_gnn.calibrate(name)
+    assert sorted(got) == sorted(stored[name]["int8_gnn_alpha"])
+    for k, v in got.items():
+        np.testing.assert_array_equal(np.float32(v), np.float32(stored[name]["int8_gnn_alpha"][k]))
 
 
 def test_c3_shares_c2_constants():
