@@ -51,9 +51,12 @@ typedef enum {
   ETX_PREC_FP32 = 0,    /* fp32 operands, FFMA on the CUDA cores, fp32 accumulate                 */
   ETX_PREC_TF32X3 = 1,  /* tcgen05 tensor cores, error-compensated 3xTF32 split (fp32-equivalent) */
   ETX_PREC_BF16 = 2,    /* tcgen05 tensor cores, bf16 operands, fp32 accumulate, fp32 state       */
-  ETX_PREC_BF16X3 = 3   /* tcgen05, operands split x = hi + lo into two bf16 (16 significand bits),
+  ETX_PREC_BF16X3 = 3,  /* tcgen05, operands split x = hi + lo into two bf16 (16 significand bits),
                            three kind::f16 MMAs (lo.hi + hi.lo + hi.hi), fp32 accumulate and state:
                            meets the fp32 tolerance at half the tensor-core work of 3xTF32          */
+  ETX_PREC_INT8 = 4     /* next row (NEXT-3, GNN part): tcgen05 kind::i8 -- INT8 codes for every GNN MLP layer
+                           input and weight (static ranges: etx_set_int8_ranges), exact int32 sums, fp32
+                           de-quantisation, biases, state and scatter-sum; the embedding stays 3xTF32      */
 } etx_precision;
 
 typedef struct {
@@ -122,6 +125,20 @@ etx_status etx_embed(etx_ctx* ctx, const etx_batch* batch, float* d_emb, void* s
  * layers, every float step one rounded fp32 operation.  d_emb[n_hits, emb_dim] fp32 as etx_embed.               */
 etx_status etx_embed_int8(etx_ctx* ctx, const etx_batch* batch, const float* h_act_alpha, int32_t n_alpha,
                           float* d_emb, void* stream);
+
+/* Next row (NEXT-3, GNN part; "the quantization of the GNN holds the most potential"): a context created with
+ * ETX_PREC_INT8 runs every GNN MLP (encoders, node / edge networks, classifier) as an INT8 chain on the tensor cores
+ * (tcgen05.mma.kind::i8): static post-training quantisation with the symmetric per-tensor scheme of Eqs. 4.31-4.33
+ * exactly as etx_embed_int8 -- layer input codes with S_a = alpha / 127 (calibrated ranges, below), weight
+ * codes with S_w = max|W_l| / 127, exact int32 sums, y = float(sum) * (S_a S_w) + b in single rounded fp32 steps.  The
+ * state h, e, the aggregate m (sequential fp32 sums in ascending edge id) and the residual adds stay fp32.  Exception: the
+ * node encoder's first layer (3 geometry features in) stays fp32 with double accumulation; its ReLU output is the first
+ * quantised tensor.  The first layer of the edge MLPs is factorised as in the other tensor-core modes, in exact integer
+ * arithmetic (int32 per-hit projections).  etx_set_int8_ranges hands over the ranges: HOST array of (3 + 2 n_iter) x
+ * gnn_n_layers positive floats, MLPs in the order node encoder, edge encoder, (node network k, edge network k) for
+ * k = 0..n_iter-1, classifier; entry l of an MLP = range of layer l's input (entry 0 of the node encoder is unused).
+ * Without it etx_gnn_forward / etx_edge_scores return ETX_ERR_INVALID in this precision.  Needs gnn_hidden = 128.      */
+etx_status etx_set_int8_ranges(etx_ctx* ctx, const float* h_alpha, size_t n);
 
 /* a2: fixed-radius search in embedding space.  Edge (i -> j) iff same event,
  * 1 <= plane(j) - plane(i) <= max_plane_gap, and d^2 < r2_max with d^2 evaluated in fp32 as

@@ -23,7 +23,7 @@ EXPORTS = ["etx_weight_count", "etx_create", "etx_destroy", "etx_last_error", "e
            "etx_set_workspace", "etx_embed", "etx_embed_int8", "etx_build_graph", "etx_gnn_forward", "etx_edge_scores",
            "etx_infer_host", "etx_launch_count", "etx_profile_enable", "etx_profile_read", "etx_build_tracks",
            "etx_build_triplets", "etx_triplet_weight_count", "etx_set_triplet_classifiers", "etx_triplet_scores",
-           "etx_triplet_tracks_workspace_bytes", "etx_build_tracks_from_triplets"]
+           "etx_triplet_tracks_workspace_bytes", "etx_build_tracks_from_triplets", "etx_set_int8_ranges"]
 KERNEL_CLASSES = ["embed", "graph", "node_enc", "edge_enc", "scatter", "node_net", "edge_net", "cls", "tracks", "edge_proj"]
 
 
@@ -127,6 +127,8 @@ def load_library():
         lib.etx_build_tracks_from_triplets.restype = C.c_int
         lib.etx_build_tracks_from_triplets.argtypes = [C.c_void_p, C.POINTER(Batch), C.POINTER(Graph), C.c_void_p, C.c_float,
                                                        C.POINTER(Triplets), C.c_void_p, C.c_float, C.POINTER(Tracks), C.c_void_p]
+        lib.etx_set_int8_ranges.restype = C.c_int
+        lib.etx_set_int8_ranges.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
         lib.etx_profile_enable.restype = C.c_int
         lib.etx_profile_enable.argtypes = [C.c_void_p, C.c_int]
         lib.etx_profile_read.restype = C.c_int
@@ -320,6 +322,14 @@ class Etx:
         for k, name in enumerate(("articulation", "left_elbow", "right_elbow")):
             out[name] = torch.stack([rows[0, o[k]:o[k + 1]], rows[1, o[k]:o[k + 1]]], dim=1)
         return out
+
+    # ---- next row: INT8 GNN (context created with precision ETX_PREC_INT8 = 4)
+    def etx_set_int8_ranges(self, alpha: Dict[str, list]):
+        """alpha: MLP name -> per-layer input ranges (synth.int8_gnn_alpha); flattened in the library's MLP order."""
+        n_iter = int(self.desc.n_iter)
+        names = ["node_enc", "edge_enc"] + [f"{n}_{k}" for k in range(n_iter) for n in ("node_net", "edge_net")] + ["cls"]
+        flat = np.ascontiguousarray(np.concatenate([np.asarray(alpha[n], np.float32) for n in names]))
+        self._check(self.lib.etx_set_int8_ranges(self.handle, flat.ctypes.data_as(C.c_void_p), flat.size))
 
     # ---- next row: triplet classifiers and track building from triplets
     def etx_set_triplet_classifiers(self, weights: np.ndarray):

@@ -26,6 +26,10 @@ struct DevMlp {
   // one-layer images of A and B (applied once per HIT), wimg then holds C (if any) and the other layers.
   const unsigned char* wimg_a = nullptr;
   const unsigned char* wimg_b = nullptr;
+  // ETX_PREC_INT8 (next row): per-layer weight scales S_w = max|W_l| / 127, and the integer codes of a 1-unit last
+  // layer held as floats (the classifier's output unit is evaluated in the epilogue registers)
+  float sw[kMaxLayers] = {0};
+  const float* wq_last = nullptr;
 };
 
 struct Workspace {            // carved from the caller's buffer by carve_workspace()
@@ -79,6 +83,9 @@ struct etx_ctx {
   unsigned char* d_trip_wimg = nullptr;
   etx::DevMlp trip_art, trip_elb;
   bool have_trip = false;
+  // next row: calibrated activation ranges of ETX_PREC_INT8, [n_mlps][gnn_n_layers] in the order node encoder, edge
+  // encoder, (node network k, edge network k)..., classifier (etx_set_int8_ranges)
+  std::vector<float> q_alpha;
   cudaStream_t copy_stream = nullptr;   // etx_infer_host: edge-list copy-out underneath the message passing
   cudaEvent_t copy_event = nullptr;
   // per-stage profiling (etx_profile_enable / etx_profile_read)
@@ -135,6 +142,7 @@ struct MlpArgs {
   // output: mode 0 store, 1 residual add (out = res + y; res may alias out), 2 small-N linear,
   // 3 small-N sigmoid
   int out_mode = 0; float* out = nullptr; const float* res = nullptr; int out_ld = 0;
+  float q_sa0 = 1.f; float q_sc[kMaxLayers] = {0}; float q_sn[kMaxLayers] = {0};   // ETX_PREC_INT8 scales (see TcArgs)
 };
 int launch_mlp_simt(const MlpArgs& a, cudaStream_t s);
 
@@ -154,6 +162,9 @@ struct TcArgs {
   const float* w_last = nullptr;                  // classifier: fp32 weights of the 1-unit output layer; narrow output: [128][n_out]
   int n_out = 1;                                  // units of a narrow output layer (out_mode 2)
   int out_mode = 0; float* out = nullptr; const float* res = nullptr; int out_ld = 0;
+  // ETX_PREC_INT8 (next row): q_sa0 = scale of the first layer's input (the gather warps quantise with it); per GEMM
+  // layer l: q_sc[l] = S_a S_w (de-quantisation), q_sn[l] = the NEXT layer's input scale (re-quantisation)
+  float q_sa0 = 1.f; float q_sc[kMaxLayers] = {0}; float q_sn[kMaxLayers] = {0};
   unsigned long long* dbg = nullptr;              // optional [grid][16] cycle counters (ETX_TC_DEBUG)
   int exp_flags = 0;                              // developer builds only (-DETX_DEV_SWITCHES): timing experiments, wrong results
 };
@@ -172,6 +183,10 @@ int run_triplet_tracks(int n_events, int n_hits, long long n_edges, const int32_
                        const float* tscores, float trip_min, char* ws, int32_t* d_edge_set, long long join_capacity,
                        int32_t* d_joins, long long track_capacity, int32_t* d_track_ptr, long long hit_capacity,
                        int32_t* d_track_hits, long long counts[4], bool* capacity_ok, cudaStream_t s);
+
+// ---- q8_aux.cu (next row: ETX_PREC_INT8)
+int launch_node_l1(int n_rows, int H, const float* const feat[3], const float fc[3], const float fs[3], const float* Wt,
+                   const float* b, float* out, cudaStream_t s);
 
 // ---- embed_int8.cu (next row: INT8 embedding MLP)
 struct Int8Args {

@@ -28,7 +28,7 @@ const char* check_desc(const etx_model_desc* d) {
   if (d->gnn_n_layers < 2 || d->gnn_n_layers > kMaxLayers) return "gnn_n_layers must be 2..8";
   if (d->n_iter < 0 || d->n_iter > 64) return "n_iter must be 0..64";
   if (d->n_planes < 2 || d->n_planes > 255) return "n_planes must be 2..255";
-  if (d->precision < ETX_PREC_FP32 || d->precision > ETX_PREC_BF16X3) return "unknown precision";
+  if (d->precision < ETX_PREC_FP32 || d->precision > ETX_PREC_INT8) return "unknown precision";
   for (int i = 0; i < 5; ++i)
     if (!(d->norm_scale[i] != 0.0f)) return "norm_scale entries must be non-zero";
   return nullptr;
@@ -72,10 +72,36 @@ uint16_t bf16_rne(float f) {
   return (uint16_t)(u >> 16);
 }
 
+float layer_weight_scale(const float* W, int fi, int fo) {
+  float mx = 0.0f;
+  for (size_t i = 0; i < (size_t)fi * fo; ++i) mx = std::max(mx, std::fabs(W[i]));
+  return mx / 127.0f;
+}
+int quant_code_host(float x, float S) {
+  float q = std::nearbyintf(x / S);
+  q = std::min(std::max(q, -127.0f), 127.0f);
+  return (int)q;
+}
+
 // Appends the image of input columns [k_begin, k_end) of one layer W [fo = 128][fi] (row-major, fp32).
 void append_wimg_slab(std::vector<unsigned char>& img, const float* W, int fi, int fo, int k_begin, int k_end, int mode) {
   const int KA = tc_chunk_k(mode);
-  const int pieces = mode == ETX_PREC_BF16 ? 1 : 2;
+  const int pieces = (mode == ETX_PREC_BF16 || mode == ETX_PREC_INT8) ? 1 : 2;
+  if (mode == ETX_PREC_INT8) {
+    // INT8 codes (Eqs. 4.31-4.33): S_w = max|W| / 127 over the WHOLE layer (per-tensor scale), code =
+    // clip(round(w / S_w)); one byte per weight, 128 codes per 128-byte row of the swizzled tile
+    const float sw = layer_weight_scale(W, fi, fo);
+    for (int k0 = k_begin; k0 < k_end; k0 += KA) {
+      const size_t base = img.size();
+      img.resize(base + 128 * 128, 0);
+      for (int n = 0; n < fo; ++n)
+        for (int kk = 0; kk < KA; ++kk) {
+          const signed char q = (signed char)quant_code_host(W[(size_t)n * fi + k0 + kk], sw);
+          img[base + (size_t)n * 128 + (size_t)(((kk / 16) ^ (n & 7)) * 16) + (kk % 16)] = (unsigned char)q;
+        }
+    }
+    return;
+  }
   for (int k0 = k_begin; k0 < k_end; k0 += KA) {
     const size_t base = img.size();
     img.resize(base + (size_t)pieces * 128 * 128, 0);
@@ -239,6 +265,11 @@ int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   // its result decides graph edges (DESIGN.md section 5 "Embedding on the tensor cores")
   const int mode = (a.out_mode == 2) ? (int)ETX_PREC_TF32X3 : (int)c->desc.precision;
   t.w_last = a.mlp.Wt[a.mlp.n_layers - 1];         // [H][1] == [H]
+  if (mode == ETX_PREC_INT8) {
+    if (a.out_mode == 3) { if (!a.mlp.wq_last) return -1; t.w_last = a.mlp.wq_last; }
+    t.q_sa0 = a.q_sa0;
+    for (int l = 0; l < kMaxLayers; ++l) { t.q_sc[l] = a.q_sc[l]; t.q_sn[l] = a.q_sn[l]; }
+  }
   t.out_mode = a.out_mode; t.out = a.out; t.res = a.res; t.out_ld = a.out_ld;
 #ifdef ETX_DEV_SWITCHES
   static const char* expv = getenv("ETX_TC_EXP");                  // developer build: timing experiments (wrong results)
@@ -332,6 +363,23 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
   staged.resize(align_up(staged.size(), 64));
   const size_t off_zero = staged.size();               // 128 zeros: bias of the per-hit projection launches
   staged.resize(staged.size() + 128, 0.0f);
+  // ETX_PREC_INT8: per-layer weight scales of every GNN MLP, and the classifier's 1-unit output layer as integer codes
+  // held in floats (evaluated in the epilogue registers: 128 products of codes sum exactly in fp32)
+  const size_t off_clsq = staged.size();
+  {
+    size_t wsrc = 0;
+    for (size_t i = 0; i < mlps.size(); ++i) {
+      const float* W = h_weights + wsrc;
+      for (int l = 0; l < mlps[i].n_layers; ++l) {
+        const int fi = mlps[i].dims[l], fo = mlps[i].dims[l + 1];
+        dev[i].sw[l] = layer_weight_scale(W, fi, fo);
+        if (i + 1 == mlps.size() && l == mlps[i].n_layers - 1)
+          for (int k = 0; k < fi; ++k) staged.push_back((float)quant_code_host(W[k], dev[i].sw[l]));
+        W += (size_t)fi * fo + fo;
+      }
+      wsrc += mlp_floats(mlps[i]);
+    }
+  }
   c->d_weights_floats = staged.size();
   if (cudaMalloc(&c->d_weights, staged.size() * sizeof(float)) != cudaSuccess ||
       cudaMemcpy(c->d_weights, staged.data(), staged.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) {
@@ -351,6 +399,7 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
   c->edge_enc = dev[2];
   for (int k = 0; k < desc->n_iter; ++k) { c->node_net.push_back(dev[3 + 2 * k]); c->edge_net.push_back(dev[4 + 2 * k]); }
   c->cls = dev.back();
+  c->cls.wq_last = c->d_weights + off_clsq;
   {
     // next row: INT8 codes of the embedding MLP's weights (Eqs. 4.31-4.33): S_w = max|W| / 127,
     // w_q = clip(round(W / S_w), -127, 127), packed 4 consecutive inputs per word, rows padded with zeros
@@ -503,6 +552,28 @@ etx_status etx_profile_read(etx_ctx* c, double* ms, int64_t* launches) {
   return ETX_OK;
 }
 
+etx_status etx_set_int8_ranges(etx_ctx* c, const float* h_alpha, size_t n) {
+  if (!c) return ETX_ERR_INVALID;
+  const size_t need = (size_t)(3 + 2 * c->desc.n_iter) * c->desc.gnn_n_layers;
+  if (!h_alpha || n != need) return fail(c, ETX_ERR_INVALID, "etx_set_int8_ranges needs (3 + 2 n_iter) x gnn_n_layers ranges");
+  for (size_t i = 0; i < n; ++i)
+    if (!(h_alpha[i] > 0.0f)) return fail(c, ETX_ERR_INVALID, "activation ranges must be positive");
+  c->q_alpha.assign(h_alpha, h_alpha + n);
+  return ETX_OK;
+}
+
+// ETX_PREC_INT8: scales of one launch covering layers [shift, shift + n_l) of GNN MLP number mi (order of etx_set_int8_ranges)
+static void fill_q(const etx_ctx* c, MlpArgs& a, int mi, const DevMlp& full, int shift, int n_l) {
+  const int L = c->desc.gnn_n_layers;
+  const float* al = c->q_alpha.data() + (size_t)mi * L;
+  a.q_sa0 = al[shift] / 127.0f;
+  for (int l = 0; l < n_l; ++l) {
+    const float sa = al[shift + l] / 127.0f;
+    a.q_sc[l] = sa * full.sw[shift + l];
+    a.q_sn[l] = (shift + l + 1 < L) ? al[shift + l + 1] / 127.0f : 1.0f;
+  }
+}
+
 etx_status etx_embed(etx_ctx* c, const etx_batch* b, float* d_emb, void* stream) {
   if (!c) return ETX_ERR_INVALID;
   if (etx_status st = check_batch(c, b)) return st;
@@ -632,6 +703,8 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
   const int H = c->desc.gnn_hidden, N = b->n_hits;
   const int E = (int)g->n_edges;
 
+  const bool q8 = c->desc.precision == ETX_PREC_INT8;
+  if (q8 && c->q_alpha.empty()) return fail(c, ETX_ERR_INVALID, "ETX_PREC_INT8 needs calibrated ranges (etx_set_int8_ranges)");
   {  // a3: h0 = MLP_n((x,y,z) normalised)
     MlpArgs a;
     a.n_rows = N; a.n_seg = 0;
@@ -640,6 +713,17 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
     for (int i = 0; i < 3; ++i) { a.fc[i] = c->desc.norm_center[id[i]]; a.fs[i] = c->desc.norm_scale[id[i]]; }
     a.mlp = c->node_enc; a.out_mode = 0; a.out = w.h; a.out_ld = H;
     ProfScope ps(c, ETX_K_NODE_ENC, s);
+    if (q8) {
+      // the 3-feature first layer stays fp32 (double accumulation: q8_aux.cu); its ReLU output, parked in m, is the
+      // first quantised tensor; layers 2.. run as an INT8 chain
+      c->launches += launch_node_l1(N, H, a.feat, a.fc, a.fs, c->node_enc.Wt[0], c->node_enc.b[0], w.m, s);
+      const DevMlp& f = c->node_enc;
+      a.n_seg = 1; a.seg[0] = Segment{w.m, nullptr, H, H};
+      a.mlp.n_layers = f.n_layers - 1;
+      for (int l = 0; l < f.n_layers; ++l) { a.mlp.dims[l] = f.dims[l + 1]; }
+      for (int l = 0; l + 1 < f.n_layers; ++l) { a.mlp.Wt[l] = f.Wt[l + 1]; a.mlp.b[l] = f.b[l + 1]; }
+      fill_q(c, a, 0, f, 1, f.n_layers - 1);
+    }
     c->launches += run_mlp(c, a, s);
   }
   // Tensor-core modes factorise the first layer of the edge MLPs: with W1 = [A | B | C]
@@ -647,7 +731,7 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
   // p_l = [A h_l | B h_l] cost 4 H^2 flop per HIT instead of per EDGE; the edge kernel gathers the two
   // 128-wide rows, adds them and starts its layer-1 accumulator from the sum.
   const bool fact = c->desc.precision != ETX_PREC_FP32;
-  auto project = [&](const DevMlp& mlp) {              // p = [A h | B h] over the hits
+  auto project = [&](const DevMlp& mlp, int mi) {      // p = [A h | B h] over the hits (mi: the MLP's number, for its INT8 ranges)
     ProfScope ps(c, ETX_K_EDGE_PROJ, s);
     // bf16 modes: ONE launch, h read once, both 128-column halves (the images of A and B are adjacent);
     // TF32X3 (one tile in flight, no second accumulator slot): one launch per half
@@ -660,6 +744,7 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
       a.mlp.wimg = part == 0 ? mlp.wimg_a : mlp.wimg_b;
       a.mlp.b[0] = c->d_zero_bias; a.mlp.Wt[0] = c->d_zero_bias;
       a.wide = wide ? 1 : 0;
+      if (q8) a.q_sa0 = c->q_alpha[(size_t)mi * c->desc.gnn_n_layers] / 127.0f;   // the edge MLP's layer-1 input scale; raw int32 out
       a.out_mode = 0; a.out = w.p + part * H; a.out_ld = 2 * H;
       c->launches += run_mlp(c, a, s);
     }
@@ -669,7 +754,8 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
     a.n_rows = E;
     a.mlp = c->edge_enc; a.out_mode = 0; a.out = d_edge_enc; a.out_ld = H;
     if (fact) {
-      if (E > 0) project(c->edge_enc);
+      if (E > 0) project(c->edge_enc, 1);
+      if (q8) fill_q(c, a, 1, c->edge_enc, 0, c->edge_enc.n_layers);
       a.n_seg = 0; a.n_add = 2;
       a.add[0] = Segment{w.p, g->d_src, H, 2 * H};
       a.add[1] = Segment{w.p + H, g->d_dst, H, 2 * H};
@@ -699,6 +785,7 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
       a.seg[0] = Segment{w.h, nullptr, H, H};
       a.seg[1] = Segment{w.m, nullptr, 2 * H, 2 * H};
       a.mlp = c->node_net[k]; a.out_mode = 1; a.out = w.h; a.res = w.h; a.out_ld = H;
+      if (q8) fill_q(c, a, 2 + 2 * k, c->node_net[k], 0, c->node_net[k].n_layers);
       ProfScope ps(c, ETX_K_NODE_NET, s);
       c->launches += run_mlp(c, a, s);
     }
@@ -707,7 +794,8 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
       a.n_rows = E;
       a.mlp = c->edge_net[k]; a.out_mode = 1; a.out = d_edge_enc; a.res = d_edge_enc; a.out_ld = H;
       if (fact) {
-        if (E > 0) project(c->edge_net[k]);
+        if (E > 0) project(c->edge_net[k], 3 + 2 * k);
+        if (q8) fill_q(c, a, 3 + 2 * k, c->edge_net[k], 0, c->edge_net[k].n_layers);
         a.n_seg = 1; a.n_add = 2;
         a.seg[0] = Segment{d_edge_enc, nullptr, H, H};
         a.add[0] = Segment{w.p, g->d_src, H, 2 * H};
@@ -740,6 +828,10 @@ etx_status etx_edge_scores(etx_ctx* c, const etx_graph* g, const float* d_edge_e
   a.n_rows = (int)g->n_edges; a.n_seg = 1;
   a.seg[0] = Segment{d_edge_enc, nullptr, H, H};
   a.mlp = c->cls; a.out_mode = 3; a.out = d_scores; a.out_ld = 1;
+  if (c->desc.precision == ETX_PREC_INT8) {
+    if (c->q_alpha.empty()) return fail(c, ETX_ERR_INVALID, "ETX_PREC_INT8 needs calibrated ranges (etx_set_int8_ranges)");
+    fill_q(c, a, 2 + 2 * c->desc.n_iter, c->cls, 0, c->cls.n_layers);
+  }
   {
     ProfScope ps(c, ETX_K_CLS, (cudaStream_t)stream);
     c->launches += run_mlp(c, a, (cudaStream_t)stream);
@@ -866,6 +958,7 @@ etx_status etx_triplet_scores(etx_ctx* c, const etx_graph* g, const float* d_edg
                               float* d_trip_scores, void* stream) {
   if (!c) return ETX_ERR_INVALID;
   if (!c->have_trip) return fail(c, ETX_ERR_INVALID, "no triplet classifiers set (etx_set_triplet_classifiers)");
+  if (c->desc.precision == ETX_PREC_INT8) return fail(c, ETX_ERR_INVALID, "the triplet classifiers have no ETX_PREC_INT8 path");
   if (!g || g->n_edges < 0 || !t) return fail(c, ETX_ERR_INVALID, "graph / triplets are NULL");
   const int64_t total = t->n[0] + t->n[1] + t->n[2];
   if (t->n[0] < 0 || t->n[1] < 0 || t->n[2] < 0 || total > t->capacity) return fail(c, ETX_ERR_INVALID, "triplets not built");

@@ -77,6 +77,7 @@ constexpr int kAtomBytes = 128 * 128;         // one operand tile: 128 rows x 12
 template <int MODE> struct Cfg;
 template <> struct Cfg<ETX_PREC_TF32X3> {
   static constexpr int KA = 32;               // K elements per 128-byte swizzle atom
+  static constexpr int KG = 32;               // columns of one gather unit (= KA except for 8-bit operands)
   static constexpr int PIECES = 2;            // hi, lo
   // Ring split (measured, edge network at C2): the operand ring wants depth (a whole tile of entries in
   // flight), the weight ring does not (2 stages = one hidden layer; weights are never late): 4+2 -> 2+4
@@ -89,6 +90,7 @@ template <> struct Cfg<ETX_PREC_TF32X3> {
 };
 template <> struct Cfg<ETX_PREC_BF16> {
   static constexpr int KA = 64;
+  static constexpr int KG = 64;
   static constexpr int PIECES = 1;
   static constexpr int NSTAGE_W = 4;          // 16 KB each
   static constexpr int NSTAGE_A = 8;          // 16 KB each
@@ -98,6 +100,7 @@ template <> struct Cfg<ETX_PREC_BF16> {
 };
 template <> struct Cfg<ETX_PREC_BF16X3> {
   static constexpr int KA = 64;
+  static constexpr int KG = 64;
   static constexpr int PIECES = 2;            // hi, lo (bf16 each)
   static constexpr int NSTAGE_W = 2;          // 32 KB each
   static constexpr int NSTAGE_A = 4;          // 32 KB each
@@ -106,7 +109,35 @@ template <> struct Cfg<ETX_PREC_BF16X3> {
   static constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);
 };
 
+// Next row (NEXT-3, GNN part): INT8 codes for every layer input and weight (Eqs. 4.31-4.33), one
+// kind::i8 MMA per K-step (K = 32), int32 accumulators, fp32 de-quantisation / bias / state.  A 128-byte atom holds 128
+// codes, so a K-chunk is 128 wide; the fp32 rows are still gathered in 64-column units (two units fill one ring entry),
+// which keeps the gather geometry -- and the fp32 / int32 addend path -- of the single-pass bf16 mode.
+template <> struct Cfg<ETX_PREC_INT8> {
+  static constexpr int KA = 128;
+  static constexpr int KG = 64;
+  static constexpr int PIECES = 1;
+  static constexpr int NSTAGE_W = 4;          // 16 KB each
+  static constexpr int NSTAGE_A = 8;          // 16 KB each
+  static constexpr int PREFETCH = 2;
+  static constexpr int HID_COLS = 32;         // 128 codes = 32 columns
+  static constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);   // D = s32, A = B = s8
+};
+
 using namespace tcp;
+
+// Eq. 4.33 with alpha_q = 127: clip(round(x / S), -127, 127); fp32 division, round half to even -- the oracle's arithmetic
+__device__ __forceinline__ float quant_f(float x, float S) {
+  return fminf(fmaxf(rintf(__fdiv_rn(x, S)), -127.0f), 127.0f);
+}
+__device__ __forceinline__ uint32_t quant_pack4(float a, float b, float c, float d, float S) {
+  return ((uint32_t)(int)quant_f(a, S) & 0xffu) | (((uint32_t)(int)quant_f(b, S) & 0xffu) << 8) |
+         (((uint32_t)(int)quant_f(c, S) & 0xffu) << 16) | (((uint32_t)(int)quant_f(d, S) & 0xffu) << 24);
+}
+// y = float(sum) * (S_a S_w) + b, each step one rounded fp32 operation
+__device__ __forceinline__ float dequant(uint32_t acc_bits, float sc, float b) {
+  return __fadd_rn(__fmul_rn(__int2float_rn((int)acc_bits), sc), b);
+}
 
 // D[tmem] (+)= A * B^T with B in shared memory; A in shared memory (SS) or tensor memory (TS)
 template <int MODE>
@@ -114,6 +145,10 @@ __device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_
   if constexpr (MODE == ETX_PREC_TF32X3)
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                  "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
+  else if constexpr (MODE == ETX_PREC_INT8)
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
   else
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
@@ -125,6 +160,10 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
   if constexpr (MODE == ETX_PREC_TF32X3)
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                  "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
+  else if constexpr (MODE == ETX_PREC_INT8)
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
   else
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
@@ -169,8 +208,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   // and keeps one tile in flight with ping-pong accumulators.
   constexpr int NSLOT = (MODE == ETX_PREC_TF32X3) ? 1 : 2;
   constexpr uint32_t HIDW = P * HID_COLS;       // TMEM columns of one hidden operand region (256 / 128 / 64)
-  constexpr int HCH = HW / KA;                  // K-chunks per hidden layer (4 / 2)
-  constexpr int LPR = KA * 4 / 16;              // gather lanes per row: 16-byte pieces of a chunk row (8 / 16)
+  constexpr int HCH = HW / KA;                  // K-chunks per hidden layer (4 / 2; 1 for 8-bit operands)
+  constexpr int KG = C::KG;                     // columns of one gather unit
+  constexpr int GCH = HW / KG;                  // gather units per 128 columns
+  constexpr int UPE = KA / KG;                  // gather units per ring entry (2 for 8-bit operands, else 1)
+  constexpr bool q8 = (MODE == ETX_PREC_INT8);
+  constexpr int LPR = KG * 4 / 16;              // gather lanes per row: 16-byte pieces of a unit row (8 / 16)
   constexpr int RPP = kGatherThreads / LPR;     // rows covered by one pass of the gather threads (32 / 16)
   constexpr int NPASS = TM / RPP;               // passes per chunk (4 / 8)
   constexpr int D = C::PREFETCH;                // nc1 is a multiple of D for every MLP this kernel serves
@@ -204,9 +247,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   const bool share1 = !wide && nc1 <= NSW;      // first-layer weight stages shared by the tiles of a pair
   // Addend (first-layer factorisation): the accumulator of layer 1 starts from
   // add[0][idx0[row]] + add[1][idx1[row]] (128 fp32 columns) instead of zero.
-  const int n_addu = a.n_add ? 2 * HCH : 0;     // addend gather units per tile (two sources x 128 / KA column chunks)
+  const int n_addu = a.n_add ? 2 * GCH : 0;     // addend gather units per tile (two sources x 128 / KG column chunks)
   const int n_addg = n_addu / D;                // = 2 groups of 64 columns
-  const int n_units = n_addu + nc1;
+  const int n_units = n_addu + a.K0 / KG;
   Unit* utab = bars->utab;
   if ((int)threadIdx.x < n_units) {
     const int u = threadIdx.x;
@@ -216,11 +259,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
       const float* b = second ? a.add[1].base : a.add[0].base;
       const int ld = second ? a.add[1].ld : a.add[0].ld;
       const bool has_idx = (second ? a.add[1].idx : a.add[0].idx) != nullptr;
-      un.base = reinterpret_cast<const char*>(b + (u >> 1) * KA);
+      un.base = reinterpret_cast<const char*>(b + (u >> 1) * KG);
       un.ldb = (uint32_t)ld * 4u;
       un.sel = has_idx ? (u & 1) : -1;
     } else {
-      int k = (u - n_addu) * KA, sg = 0;
+      int k = (u - n_addu) * KG, sg = 0;
       if (a.n_seg > 1 && k >= a.seg[0].width) { k -= a.seg[0].width; sg = 1; }
       if (sg == 1 && a.n_seg > 2 && k >= a.seg[1].width) { k -= a.seg[1].width; sg = 2; }
       const float* b = sg == 0 ? a.seg[0].base : (sg == 1 ? a.seg[1].base : a.seg[2].base);
@@ -246,7 +289,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
     for (int i = 0; i < NSW; ++i) { mbar_init(smem_u32(&bars->w_full[i]), 1); mbar_init(smem_u32(&bars->w_empty[i]), 1); }
     for (int i = 0; i < NSA; ++i) { mbar_init(smem_u32(&bars->a_full[i]), 1); mbar_init(smem_u32(&bars->a_empty[i]), 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&bars->acc_full[i]), 1); mbar_init(smem_u32(&bars->acc_free[i]), kEpiThreads / 32); }
-    for (int i = 0; i < 8; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), 4);
+    for (int i = 0; i < 8; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), q8 ? 8 : 4);   // 8-bit: ONE chunk per layer, written by all 8 warps
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == kWarpMma) {                        // TMEM: all 512 columns of this SM (1 CTA per SM)
@@ -418,6 +461,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             const uint32_t tbase = (P == 2) ? aring + (ecnt % NSA) * kStageBytes + tsel * kAtomBytes
                                             : aring + ((ecnt + tsel) % NSA) * kStageBytes;
             const float4 x = buf[0][p], y = buf[1][p];
+            if constexpr (q8)                  // the projections are exact int32 sums: integer add of the bit patterns
+              st_shared_v4(tbase + r * 128 + (((jl & 7) ^ (r & 7)) << 4),
+                           (uint32_t)(__float_as_int(x.x) + __float_as_int(y.x)), (uint32_t)(__float_as_int(x.y) + __float_as_int(y.y)),
+                           (uint32_t)(__float_as_int(x.z) + __float_as_int(y.z)), (uint32_t)(__float_as_int(x.w) + __float_as_int(y.w)));
+            else
             st_shared_v4(tbase + r * 128 + (((jl & 7) ^ (r & 7)) << 4),
                          __float_as_uint(x.x + y.x), __float_as_uint(x.y + y.y), __float_as_uint(x.z + y.z), __float_as_uint(x.w + y.w));
           }
@@ -429,6 +477,32 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
         named_bar_arrive(kBarEntry0 + ecnt % NSA, kGatherThreads + 32);
         if constexpr (ENT == 2) named_bar_arrive(kBarEntry0 + (ecnt + 1) % NSA, kGatherThreads + 32);
         ecnt += ENT;
+        GP_ACC(2);
+        if (more) {
+#pragma unroll
+          for (int d = 0; d < D; ++d) load_unit(buf[d]);
+        }
+        GP_ACC(3);
+      } else if constexpr (UPE == 2) {
+        // 8-bit operands: the D = 2 units of a group are the two 64-column halves of ONE K-chunk (128 codes per row)
+        static_assert(UPE == 1 || D == UPE, "a group of gather units fills exactly one ring entry");
+        wait_entry(ecnt);
+        GP_T0();
+        const uint32_t tile_q = aring + (ecnt % NSA) * kStageBytes;
+#pragma unroll
+        for (int d = 0; d < D; ++d) {
+#pragma unroll
+          for (int p = 0; p < NPASS; ++p) {
+            const int r = r0 + p * RPP;
+            const float4 v = buf[d][p];
+            const uint32_t byte = d * 64 + jl * 4;          // K position of this thread's 4 codes inside the 128-byte row
+            asm volatile("st.shared.b32 [%0], %1;" ::"r"(tile_q + r * 128 + (((byte >> 4) ^ (r & 7)) << 4) + (byte & 15)),
+                         "r"(quant_pack4(v.x, v.y, v.z, v.w, a.q_sa0)) : "memory");
+          }
+        }
+        GP_ACC(1);
+        named_bar_arrive(kBarEntry0 + ecnt % NSA, kGatherThreads + 32);
+        ++ecnt;
         GP_ACC(2);
         if (more) {
 #pragma unroll
@@ -489,6 +563,36 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
         if (l < n_gemm - 1) {
           // ---- hidden layer: ReLU(x + b) -> next A operand in TMEM, released chunk by chunk.
           // This warp's column half holds K-chunks hh*HCH/2 .. of the next layer.
+          if constexpr (q8) {
+            // 8-bit: de-quantise the int32 sums, bias, ReLU, re-quantise with the NEXT layer's input scale (the Q -> node
+            // -> DQ chain of P:2725); this warp's 64 columns become 16 packed columns of the single K-chunk
+            EP_T0();
+            uint32_t va[32], vb[32], w[16];
+            tmem_ld32(acc + hh * 64, va);
+            tmem_ld32(acc + hh * 64 + 32, vb);
+            tc_wait_ld();
+            EP_ACC(0);
+            const float sc = a.q_sc[l], sn = a.q_sn[l];
+            const float* bq = bias + hh * 64;
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+              w[i] = quant_pack4(fmaxf(dequant(va[4 * i], sc, bq[4 * i]), 0.f), fmaxf(dequant(va[4 * i + 1], sc, bq[4 * i + 1]), 0.f),
+                                 fmaxf(dequant(va[4 * i + 2], sc, bq[4 * i + 2]), 0.f), fmaxf(dequant(va[4 * i + 3], sc, bq[4 * i + 3]), 0.f), sn);
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+              w[8 + i] = quant_pack4(fmaxf(dequant(vb[4 * i], sc, bq[32 + 4 * i]), 0.f), fmaxf(dequant(vb[4 * i + 1], sc, bq[32 + 4 * i + 1]), 0.f),
+                                     fmaxf(dequant(vb[4 * i + 2], sc, bq[32 + 4 * i + 2]), 0.f), fmaxf(dequant(vb[4 * i + 3], sc, bq[32 + 4 * i + 3]), 0.f), sn);
+            asm volatile(
+                "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+                "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+                ::"r"(hid + hh * 16), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7]),
+                  "r"(w[8]), "r"(w[9]), "r"(w[10]), "r"(w[11]), "r"(w[12]), "r"(w[13]), "r"(w[14]), "r"(w[15]) : "memory");
+            EP_ACC(1);
+            tc_wait_st();
+            tc_fence_before();
+            mbar_arrive_relaxed_warp(smem_u32(&hid_ready[0]), lane);
+            EP_ACC(2);
+          }
 #pragma unroll 1
           for (int c = hh * (HCH / 2); c < (hh + 1) * (HCH / 2); ++c) {
             EP_T0();
@@ -586,11 +690,18 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
               tmem_ld32(acc + q * 32, v);
               tc_wait_ld();
 #pragma unroll
-              for (int i = 0; i < 32; ++i)
+              for (int i = 0; i < 32; ++i) {
+                if constexpr (q8)              // codes of the last hidden activation x integer weight codes (held as floats):
+                  logit = fmaf(quant_f(fmaxf(dequant(v[i], a.q_sc[l], bias[q * 32 + i]), 0.f), a.q_sn[l]),   // exact below 2^24
+                               wlast_s[q * 32 + i], logit);
+                else
                 logit = fmaf(fmaxf(__uint_as_float(v[i]) + bias[q * 32 + i], 0.f), wlast_s[q * 32 + i], logit);
+              }
             }
             tc_fence_before();
             mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
+            if constexpr (q8) logit = __fadd_rn(__fmul_rn(logit, a.q_sc[a.n_layers - 1]), __ldg(a.bias[a.n_layers - 1]));
+            else
             logit += __ldg(a.bias[a.n_layers - 1]);
             const int row = tile * TM + et;
             if (row < a.n_rows) a.out[row] = 1.0f / (1.0f + expf(-logit));
@@ -627,6 +738,14 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
               const float4 bq = *reinterpret_cast<const float4*>(bias + col0 + 4 * j);
+              if constexpr (q8 && wide)        // 8-bit per-hit projections: the raw int32 sums (they are added as integers)
+                st_shared_v4(stg + lane * 64 + ((j ^ ((lane >> 1) & 3)) << 4), v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+              else if constexpr (q8) {
+                const float sc = a.q_sc[l];
+                st_shared_v4(stg + lane * 64 + ((j ^ ((lane >> 1) & 3)) << 4),
+                             __float_as_uint(dequant(v[4 * j], sc, bq.x)), __float_as_uint(dequant(v[4 * j + 1], sc, bq.y)),
+                             __float_as_uint(dequant(v[4 * j + 2], sc, bq.z)), __float_as_uint(dequant(v[4 * j + 3], sc, bq.w)));
+              } else
               st_shared_v4(stg + lane * 64 + ((j ^ ((lane >> 1) & 3)) << 4),
                            __float_as_uint(__uint_as_float(v[4 * j]) + bq.x), __float_as_uint(__uint_as_float(v[4 * j + 1]) + bq.y),
                            __float_as_uint(__uint_as_float(v[4 * j + 2]) + bq.z), __float_as_uint(__uint_as_float(v[4 * j + 3]) + bq.w));
@@ -868,7 +987,9 @@ int launch_mode(const TcArgs& a, int sm_count, cudaStream_t s) {
 
 }  // namespace
 
-int tc_chunk_k(int mode) { return mode == ETX_PREC_TF32X3 ? Cfg<ETX_PREC_TF32X3>::KA : Cfg<ETX_PREC_BF16>::KA; }
+int tc_chunk_k(int mode) {
+  return mode == ETX_PREC_TF32X3 ? Cfg<ETX_PREC_TF32X3>::KA : (mode == ETX_PREC_INT8 ? Cfg<ETX_PREC_INT8>::KA : Cfg<ETX_PREC_BF16>::KA);
+}
 
 // Requirements (checked by the caller): hidden width 128; K0 a multiple of the chunk (32 / 64) and
 // segment widths multiples of it; out_mode 0/1 needs dims[L] == 128; out_mode 3 needs dims[L] == 1.
@@ -878,6 +999,7 @@ int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s) {
     if (a.n_layers != 1 || a.n_add != 0 || a.out_mode != 0) return -1;
     if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, 1>(a, sm_count, s);
     if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, 1>(a, sm_count, s);
+    if (mode == ETX_PREC_INT8) return launch_mode<ETX_PREC_INT8, 1>(a, sm_count, s);
     return -1;
   }
   if (a.w1) {                                    // first-layer operand computed from 3 features (node encoder, embedding)
@@ -894,6 +1016,7 @@ int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s) {
   if (mode == ETX_PREC_TF32X3) return launch_mode<ETX_PREC_TF32X3, 0>(a, sm_count, s);
   if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, 0>(a, sm_count, s);
   if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, 0>(a, sm_count, s);
+  if (mode == ETX_PREC_INT8) return launch_mode<ETX_PREC_INT8, 0>(a, sm_count, s);
   return -1;
 }
 
