@@ -337,6 +337,33 @@ def run_ours(args):
         if etx._ws_bytes != ws_before:                 # the track building may have grown (and clobbered) the workspace
             etx.ensure_workspace(db.n_events, N, cap, with_host_path=True)
 
+    if not args.no_next_rows and H == 128:
+        # NEXT-3 (GNN part): the same graph through the INT8 GNN (ETX_PREC_INT8, tcgen05.mma.kind::i8) with the stored
+        # calibrated ranges; the default mode's scores of this run are the comparison
+        ref_scores = scores[:E].clone()
+        q = binding.Etx(binding.make_desc(cfg, precision=synth.PREC_INT8), blob, device=local)
+        q.etx_set_int8_ranges(synth.int8_gnn_alpha(cfg))
+        q.ensure_workspace(db.n_events, N, cap)
+        sc8 = torch.empty(cap, device=dev)
+
+        def q_step():
+            q.etx_gnn_forward(db, g, enc)
+            q.etx_edge_scores(g, enc, sc8)
+
+        q.profile_enable(True)
+        q.profile_read()
+        qms, _ = time3(q_step)
+        qprof = q.profile_read()
+        d8 = (sc8[:E] - ref_scores).abs()
+        next_rows["gnn_int8"] = {"ms": qms, "events_per_s": n_ev / (qms * 1e-3),
+                                 "default_mode_gnn_ms": sum(prof[k][0] for k in ("node_enc", "edge_enc", "scatter", "node_net", "edge_net", "edge_proj", "cls")) / args.steps,
+                                 "edge_net_ms_per_launch": qprof["edge_net"][0] / max(qprof["edge_net"][1], 1),
+                                 "stages_ms": {k: v[0] / 4 for k, v in qprof.items() if v[1]},
+                                 "score_err_vs_default_mode": {"max": float(d8.max()), "median": float(d8.median()),
+                                                               "p99": float(torch.quantile(d8[::16].float(), 0.99))},
+                                 "kept_edges_at_0.5": {"int8": int((sc8[:E] >= 0.5).sum()), "default": int((ref_scores >= 0.5).sum())}}
+        del q, sc8, ref_scores
+
     # ---- end to end through the host-buffer entry point
     host = binding.pinned_host_batch(batch)
     o_src = torch.empty(cap, dtype=torch.int32).pin_memory()

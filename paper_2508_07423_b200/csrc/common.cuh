@@ -39,6 +39,7 @@ struct Workspace {            // carved from the caller's buffer by carve_worksp
   int32_t* scan_tmp = nullptr;    // block sums for the device scan
   int32_t* flags = nullptr;       // [8] validation flags / counters
   int32_t* sched = nullptr;       // [8] work counters of the dynamically scheduled kernels (scatter)
+  uint32_t* ballots = nullptr;    // [n_hits][kBallotWords] vote words of the search's count pass (4-d embeddings)
   float* h = nullptr;             // [n_hits, H]
   float* m = nullptr;             // [n_hits, 2H]
   float* p = nullptr;             // [n_hits, 2H] per-hit first-layer projections [A h | B h] (tensor-core modes)
@@ -78,6 +79,10 @@ struct etx_ctx {
   int* d_emb_wq = nullptr;              // INT8 codes of the embedding MLP's weights (next row), packed 4 per word
   int emb_wq_off[etx::kMaxLayers] = {0};
   float emb_sw[etx::kMaxLayers] = {0};  // their per-layer scales max|W| / 127
+  // the same embedding for the tensor-core INT8 kernel (128-wide hidden layers): kind::i8 image of the hidden layers,
+  // and the 3-input first layer / the narrow last layer as integer codes held in floats (k-major)
+  unsigned char* d_embq_img = nullptr;
+  float* d_embq_f = nullptr;            // [3][128] first-layer codes, then [128][n_out] last-layer codes
   // next row: the two triplet classifiers (articulations, elbows), set by etx_set_triplet_classifiers
   float* d_trip_weights = nullptr;
   unsigned char* d_trip_wimg = nullptr;
@@ -107,12 +112,15 @@ struct GraphArgs {
 };
 // each returns the number of kernels launched; errors are reported through cudaGetLastError
 int launch_plane_index(const GraphArgs& a, int32_t* plane_ptr, int32_t* hit_event, int32_t* flags, cudaStream_t s);
+constexpr int kBallotWords = 32;   // vote words (32 candidates each) the count pass keeps per source for the fill pass
 int launch_search_count(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
-                        const int32_t* flags, int32_t* out_deg, int32_t* in_deg, cudaStream_t s);
+                        const int32_t* flags, int32_t* out_deg, int32_t* in_deg, uint32_t* ballots /*[n_hits][kBallotWords] or null*/,
+                        cudaStream_t s);
 int launch_exclusive_scan(int32_t* data /*[n+1], in place, data[n] = total*/, int n, int32_t* tmp, cudaStream_t s);
 int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
                        const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst,
-                       const int32_t* in_ptr, int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/, cudaStream_t s);
+                       const int32_t* in_ptr, int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/,
+                       const uint32_t* ballots, cudaStream_t s);
 size_t scan_tmp_ints(int n);
 int launch_add_offset(const int32_t* in, int32_t* out, int64_t n, int32_t offset, cudaStream_t s);
 int launch_sort_in_lists(int n_hits, const int32_t* flags, const int32_t* in_ptr, int32_t* in_perm, cudaStream_t s);
@@ -165,6 +173,8 @@ struct TcArgs {
   // ETX_PREC_INT8 (next row): q_sa0 = scale of the first layer's input (the gather warps quantise with it); per GEMM
   // layer l: q_sc[l] = S_a S_w (de-quantisation), q_sn[l] = the NEXT layer's input scale (re-quantisation)
   float q_sa0 = 1.f; float q_sc[kMaxLayers] = {0}; float q_sn[kMaxLayers] = {0};
+  float q_sf = 1.f, q_sc0 = 1.f;                  // feature mode (INT8 embedding): scale of the 3 features, S_a S_w of the MLP's own first layer
+  float q_rsa0 = 1.f, q_rsn[kMaxLayers] = {0}, q_rsf = 1.f;   // fl(1 / scale) of q_sa0, q_sn[], q_sf (filled by launch_mlp_tc)
   unsigned long long* dbg = nullptr;              // optional [grid][16] cycle counters (ETX_TC_DEBUG)
   int exp_flags = 0;                              // developer builds only (-DETX_DEV_SWITCHES): timing experiments, wrong results
 };

@@ -153,6 +153,7 @@ Workspace carve(const etx_ctx* c, int32_t n_events, int32_t n_hits, int64_t cap,
   w.scan_tmp = (int32_t*)take(sizeof(int32_t) * scan_tmp_ints(n_hits + 1));
   w.flags = (int32_t*)take(sizeof(int32_t) * 8);
   w.sched = (int32_t*)take(sizeof(int32_t) * 8);
+  if (d == 4) w.ballots = (uint32_t*)take(sizeof(uint32_t) * (size_t)n_hits * kBallotWords);
   w.h = (float*)take(sizeof(float) * (size_t)n_hits * H);
   w.m = (float*)take(sizeof(float) * (size_t)n_hits * 2 * H);
   if (c->desc.precision != ETX_PREC_FP32) w.p = (float*)take(sizeof(float) * (size_t)n_hits * 2 * H);
@@ -429,6 +430,29 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
       return fail(nullptr, ETX_ERR_CUDA, msg);
     }
   }
+  if (mlps[0].n_layers >= 3 && mlps[0].dims[1] == 128) {
+    // INT8 embedding on the tensor cores (etx_embed_int8): kind::i8 image of layers 2..L-1, float-held codes of the
+    // 3-input first layer [k][128] and of the narrow last layer [k][n_out]
+    const HostMlp& m = mlps[0];
+    std::vector<unsigned char> qimg;
+    append_wimg(qimg, m, h_weights, 1, 0, m.n_layers - 1, ETX_PREC_INT8);
+    const int n_out = m.dims[m.n_layers];
+    std::vector<float> qf((size_t)3 * 128 + (size_t)128 * n_out);
+    const float* W = h_weights;
+    for (int o = 0; o < 128; ++o)
+      for (int k = 0; k < 3; ++k) qf[(size_t)k * 128 + o] = (float)quant_code_host(W[(size_t)o * 3 + k], c->emb_sw[0]);
+    for (int l = 0; l + 1 < m.n_layers; ++l) W += (size_t)m.dims[l] * m.dims[l + 1] + m.dims[l + 1];
+    for (int o = 0; o < n_out; ++o)
+      for (int k = 0; k < 128; ++k) qf[(size_t)3 * 128 + (size_t)k * n_out + o] = (float)quant_code_host(W[(size_t)o * 128 + k], c->emb_sw[m.n_layers - 1]);
+    if (cudaMalloc(&c->d_embq_img, qimg.size()) != cudaSuccess ||
+        cudaMemcpy(c->d_embq_img, qimg.data(), qimg.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMalloc(&c->d_embq_f, qf.size() * sizeof(float)) != cudaSuccess ||
+        cudaMemcpy(c->d_embq_f, qf.data(), qf.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) {
+      const std::string msg = std::string("int8 embedding image upload failed: ") + cudaGetErrorString(cudaGetLastError());
+      etx_destroy(c);
+      return fail(nullptr, ETX_ERR_CUDA, msg);
+    }
+  }
   if (desc->precision != ETX_PREC_FP32) {
     // tensor-core weight images: edge encoder, node/edge networks, classifier (first-layer input a multiple of
     // the chunk); node encoder and a 128-wide embedding with >= 2 hidden layers from their second layer on (their
@@ -498,6 +522,8 @@ etx_status etx_destroy(etx_ctx* c) {
   if (c->d_weights) cudaFree(c->d_weights);
   if (c->d_wimg) cudaFree(c->d_wimg);
   if (c->d_emb_wq) cudaFree(c->d_emb_wq);
+  if (c->d_embq_img) cudaFree(c->d_embq_img);
+  if (c->d_embq_f) cudaFree(c->d_embq_f);
   if (c->d_trip_weights) cudaFree(c->d_trip_weights);
   if (c->d_trip_wimg) cudaFree(c->d_trip_wimg);
   for (const etx_ctx::ProfRec& r : c->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -617,6 +643,27 @@ etx_status etx_embed_int8(etx_ctx* c, const etx_batch* b, const float* h_act_alp
     a.sc[l] = a.sa[l] * c->emb_sw[l];
   }
   a.out = d_emb;
+  if (c->d_embq_img) {
+    // 128-wide hidden layers: the tcgen05 kernel -- first layer in exact integer arithmetic in the gather warps, hidden
+    // layers as kind::i8 MMAs, the narrow last layer in the epilogue registers (mlp_tc.cu); same codes, same result
+    TcArgs t;
+    t.n_rows = b->n_hits; t.K0 = 128;
+    for (int i = 0; i < 3; ++i) { t.feat[i] = a.feat[i]; t.fc[i] = a.fc[i]; t.fs[i] = a.fs[i]; }
+    t.w1 = c->d_embq_f; t.b1 = c->emb.b[0];
+    t.n_layers = L - 1;
+    for (int l = 0; l + 1 < L; ++l) t.bias[l] = c->emb.b[l + 1];
+    t.n_out = c->emb.dims[L];
+    t.wimg = c->d_embq_img;
+    t.w_last = c->d_embq_f + 3 * 128;
+    t.out_mode = 2; t.out = d_emb; t.out_ld = c->emb.dims[L];
+    t.q_sf = a.sa[0]; t.q_sc0 = a.sc[0]; t.q_sa0 = a.sa[1];
+    for (int l = 0; l + 1 < L; ++l) { t.q_sc[l] = a.sc[l + 1]; t.q_sn[l] = (l + 2 < L) ? a.sa[l + 2] : 1.0f; }
+    ProfScope ps(c, ETX_K_EMBED, (cudaStream_t)stream);
+    const int n = launch_mlp_tc(t, ETX_PREC_INT8, c->sm_count, (cudaStream_t)stream);
+    if (n < 0) return fail(c, ETX_ERR_INVALID, "the INT8 tensor-core embedding refused its arguments");
+    c->launches += n;
+    return check_cuda(c, "etx_embed_int8");
+  }
   {
     ProfScope ps(c, ETX_K_EMBED, (cudaStream_t)stream);
     const int n = launch_embed_int8(a, c->emb.dims[1], (cudaStream_t)stream);
@@ -652,7 +699,7 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
     ProfScope ps(c, ETX_K_GRAPH, s);
     c->launches += launch_plane_index(a, w.plane_ptr, w.hit_event, w.flags, s);
     if (k_max == 0) {
-      c->launches += launch_search_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_in_ptr, s);
+      c->launches += launch_search_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_in_ptr, w.ballots, s);
       c->launches += launch_exclusive_scan(g->d_row_ptr, b->n_hits + 1, w.scan_tmp, s);
       c->launches += launch_exclusive_scan(g->d_in_ptr, b->n_hits + 1, w.scan_tmp, s);
     } else {                                       // next row: capped search (graph_kmax.cu)
@@ -683,7 +730,7 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
   } else if (g->n_edges > 0) {
     ProfScope ps(c, ETX_K_GRAPH, s);
     c->launches += launch_search_fill(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_src, g->d_dst,
-                                      g->d_in_ptr, g->d_in_perm, w.cursor, s);
+                                      g->d_in_ptr, g->d_in_perm, w.cursor, w.ballots, s);
   }
   return check_cuda(c, "etx_build_graph (fill)");
 }

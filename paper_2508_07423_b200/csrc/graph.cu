@@ -165,6 +165,118 @@ search_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t*
   if (MODE == 0 && blockIdx.x == 0 && threadIdx.x == 0) out_deg[a.n_hits] = 0;
 }
 
+// ------------------------------------------------------------------ d = 4: tiled count pass + ballot fill pass
+// One CTA owns an (event, source plane) window: the candidates -- the hits of planes p+1..p+G of the event, a
+// contiguous index range -- are staged ONCE in shared memory as float4 and every warp tests them against FOUR source
+// hits at a time (register-blocked: one shared-memory load per candidate and four distance tests), instead of one warp
+// per source re-reading its ~190-candidate window from L1/L2.  The count pass also KEEPS its vote words (kBallotWords
+// 32-candidate words per source), so the fill pass expands bits into edges and computes no distance at all; a window
+// longer than kBallotWords x 32 candidates re-tests only the words that did not fit.
+constexpr int kTileCand = 1024;                    // candidates staged per chunk (16 KB)
+
+__device__ __forceinline__ unsigned sel4(unsigned b0, unsigned b1, unsigned b2, unsigned b3, int k) {
+  return k == 0 ? b0 : (k == 1 ? b1 : (k == 2 ? b2 : b3));
+}
+
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+search_tile_count_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t* __restrict__ flags,
+                         int32_t* __restrict__ out_deg /*zeroed*/, int32_t* __restrict__ in_deg /*zeroed*/,
+                         uint32_t* __restrict__ ballots /*[n_hits][kBallotWords]*/) {
+  if (flags[0] != 0) return;
+  __shared__ float4 cand[kTileCand];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int L = a.n_planes;
+  const long long n_work = (long long)a.n_events * (L - 1);
+  const float4* __restrict__ emb4 = reinterpret_cast<const float4*>(a.emb);
+  const float r2 = a.r2_max;
+  for (long long work = blockIdx.x; work < n_work; work += gridDim.x) {
+    const int ev = (int)(work / (L - 1)), p = (int)(work % (L - 1));
+    const int32_t* pp = plane_ptr + (size_t)ev * (L + 1);
+    const int s0 = pp[p], s1 = pp[p + 1];
+    const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
+    const int j0 = s1, j1 = pp[top + 1];
+    if (s1 <= s0 || j1 <= j0) continue;            // uniform over the CTA
+    for (int c0 = 0; c0 < j1 - j0; c0 += kTileCand) {
+      const int ncc = (j1 - j0 - c0) < kTileCand ? (j1 - j0 - c0) : kTileCand;
+      __syncthreads();                             // the previous chunk / window is no longer read
+      for (int t = threadIdx.x; t < ncc; t += blockDim.x) cand[t] = __ldg(emb4 + j0 + c0 + t);
+      __syncthreads();
+      const int nw = (ncc + 31) >> 5;
+      for (int i0 = s0 + 4 * warp; i0 < s1; i0 += 4 * kWarpsPerBlock) {
+        unsigned long long n01[4], n23[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const float4 m = __ldg(emb4 + (i0 + k < s1 ? i0 + k : s1 - 1));
+          n01[k] = pack2(-m.x, -m.y); n23[k] = pack2(-m.z, -m.w);
+        }
+        int cnt = 0;                               // lane k < 4 keeps source i0 + k's count
+        for (int t = 0; t < nw; ++t) {
+          const int idx = t * 32 + lane;
+          const bool vld = idx < ncc;
+          const float4 cq = cand[vld ? idx : ncc - 1];
+          const bool ok0 = (dist2_d4(n01[0], n23[0], cq) < r2) & vld, ok1 = (dist2_d4(n01[1], n23[1], cq) < r2) & vld;
+          const bool ok2 = (dist2_d4(n01[2], n23[2], cq) < r2) & vld, ok3 = (dist2_d4(n01[3], n23[3], cq) < r2) & vld;
+          const unsigned b0 = __ballot_sync(kFull, ok0), b1 = __ballot_sync(kFull, ok1);
+          const unsigned b2 = __ballot_sync(kFull, ok2), b3 = __ballot_sync(kFull, ok3);
+          const int tw = (c0 >> 5) + t;
+          const unsigned mine = sel4(b0, b1, b2, b3, lane & 3);
+          if (lane < 4 && i0 + lane < s1) {
+            if (tw < kBallotWords) ballots[(size_t)(i0 + lane) * kBallotWords + tw] = mine;
+            cnt += __popc(mine);
+          }
+          const int n_in = (int)ok0 + (int)(ok1 & (i0 + 1 < s1)) + (int)(ok2 & (i0 + 2 < s1)) + (int)(ok3 & (i0 + 3 < s1));
+          if (n_in) atomicAdd(&in_deg[j0 + c0 + idx], n_in);
+        }
+        if (lane < 4 && i0 + lane < s1) out_deg[i0 + lane] += cnt;      // one owner per source: plain add across chunks
+      }
+    }
+  }
+}
+
+// Fill pass for d = 4: one warp per source expands its vote words into edges (ascending candidate index, so the CSR is
+// the same unique array) and drops each edge id into its destination's list; words past kBallotWords are re-tested.
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+search_ballot_fill_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t* __restrict__ hit_event,
+                          const int32_t* __restrict__ flags, const uint32_t* __restrict__ ballots,
+                          const int32_t* __restrict__ row_ptr, int32_t* __restrict__ src, int32_t* __restrict__ dst,
+                          const int32_t* __restrict__ in_ptr, int32_t* __restrict__ in_perm, int32_t* __restrict__ cursor) {
+  if (flags[0] != 0) return;
+  const int lane = threadIdx.x & 31;
+  const int n_warps = gridDim.x * kWarpsPerBlock;
+  const unsigned lt = (1u << lane) - 1u;
+  const int L = a.n_planes;
+  for (int i = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5); i < a.n_hits; i += n_warps) {
+    const int base_out = row_ptr[i], deg = row_ptr[i + 1] - base_out;
+    if (deg == 0) continue;
+    const int p = a.plane[i];
+    const int32_t* pp = plane_ptr + (size_t)hit_event[i] * (L + 1);
+    const int j0 = pp[p + 1];
+    const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
+    const int j1 = pp[top + 1];
+    unsigned long long n01 = 0, n23 = 0;
+    if (j1 - j0 > kBallotWords * 32) {
+      const float4 m = __ldg(reinterpret_cast<const float4*>(a.emb) + i);
+      n01 = pack2(-m.x, -m.y); n23 = pack2(-m.z, -m.w);
+    }
+    int cnt = 0;
+    for (int t = 0; cnt < deg; ++t) {
+      unsigned b;
+      if (t < kBallotWords) b = __ldg(ballots + (size_t)i * kBallotWords + t);
+      else {
+        const int j = j0 + t * 32 + lane, jc = j < j1 ? j : j1 - 1;
+        b = __ballot_sync(kFull, (dist2_d4(n01, n23, __ldg(reinterpret_cast<const float4*>(a.emb) + jc)) < a.r2_max) & (j < j1));
+      }
+      if ((b >> lane) & 1u) {
+        const int pos = base_out + cnt + __popc(b & lt), j = j0 + t * 32 + lane;
+        src[pos] = i;
+        dst[pos] = j;
+        in_perm[in_ptr[j] + atomicAdd(&cursor[j], 1)] = pos;
+      }
+      cnt += __popc(b);
+    }
+  }
+}
+
 // Orders every destination's list of edge ids ascending.  One warp per hit: a list of <= 32 ids (in-degrees are
 // ~6-10) sits one id per lane, each lane ranks its id with shuffles and writes it to its place (coalesced both
 // ways); a longer list is insertion-sorted by one lane.
@@ -297,8 +409,16 @@ static void launch_search(const GraphArgs& a, const int32_t* plane_ptr, const in
 }
 
 int launch_search_count(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
-                        const int32_t* flags, int32_t* out_deg, int32_t* in_deg, cudaStream_t s) {
+                        const int32_t* flags, int32_t* out_deg, int32_t* in_deg, uint32_t* ballots, cudaStream_t s) {
   cudaMemsetAsync(in_deg, 0, sizeof(int32_t) * ((size_t)a.n_hits + 1), s);
+  if (a.d == 4 && ballots) {                       // tiled count pass (shared-memory candidate windows, kept vote words)
+    cudaMemsetAsync(out_deg, 0, sizeof(int32_t) * ((size_t)a.n_hits + 1), s);
+    const long long n_work = (long long)a.n_events * (a.n_planes - 1);
+    const int cap = 148 * 8;
+    search_tile_count_kernel<<<(int)(n_work < 1 ? 1 : (n_work < cap ? n_work : cap)), kWarpsPerBlock * 32, 0, s>>>(
+        a, plane_ptr, flags, out_deg, in_deg, ballots);
+    return 1;
+  }
   launch_search<0>(a, plane_ptr, hit_event, flags, out_deg, in_deg, nullptr, nullptr, nullptr, nullptr,
                    nullptr, nullptr, s);
   return 1;
@@ -314,8 +434,14 @@ int launch_exclusive_scan(int32_t* data, int n, int32_t* tmp, cudaStream_t s) {
 
 int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
                        const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst,
-                       const int32_t* in_ptr, int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/, cudaStream_t s) {
+                       const int32_t* in_ptr, int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/,
+                       const uint32_t* ballots, cudaStream_t s) {
   cudaMemsetAsync(cursor, 0, sizeof(int32_t) * (size_t)a.n_hits, s);
+  if (a.d == 4 && ballots) {
+    search_ballot_fill_kernel<<<search_grid(a.n_hits), kWarpsPerBlock * 32, 0, s>>>(a, plane_ptr, hit_event, flags, ballots,
+                                                                                    row_ptr, src, dst, in_ptr, in_perm, cursor);
+    return 1 + launch_sort_in_lists(a.n_hits, flags, in_ptr, in_perm, s);
+  }
   launch_search<1>(a, plane_ptr, hit_event, flags, nullptr, nullptr, row_ptr, src, dst, in_ptr, in_perm, cursor, s);
   return 1 + launch_sort_in_lists(a.n_hits, flags, in_ptr, in_perm, s);
 }

@@ -127,12 +127,38 @@ template <> struct Cfg<ETX_PREC_INT8> {
 using namespace tcp;
 
 // Eq. 4.33 with alpha_q = 127: clip(round(x / S), -127, 127); fp32 division, round half to even -- the oracle's arithmetic
-__device__ __forceinline__ float quant_f(float x, float S) {
-  return fminf(fmaxf(rintf(__fdiv_rn(x, S)), -127.0f), 127.0f);
+// The definition divides (x / S in fp32, then round half to even); an IEEE division per activation made the INT8 chain
+// slower than the fp32-equivalent one (and a ZERO numerator -- half of all post-ReLU values -- even takes div.rn's
+// slow path: 10x on the classifier).  The code is computed from t = x * fl(1/S) instead, which is within
+// |t| * 2^-22.9 <= 1.6e-5 of the exact quotient for |t| < 127.5, as is the fp32 quotient itself (<= 7.6e-6): unless t
+// lies within 3e-5 of a tie k + 1/2 all three round to the same integer.  Only those rare lanes (~6e-5 of the
+// values) evaluate the real division, so the result is the definition's, bit for bit.
+// The tie test of N values is folded into ONE rarely-taken branch, so the common path is straight-line code with N
+// independent chains (a branch per value serialised them: the INT8 chain ran latency-bound, 3x slower).
+struct QScale { float S, r; };                  // scale and fl(1 / S)
+template <int N>
+__device__ __forceinline__ void quant_codes(const float (&x)[N], float (&q)[N], QScale s) {
+  bool amb = false;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    const float t = x[i] * s.r;
+    q[i] = rintf(t);
+    amb |= (fabsf(t - q[i]) > 0.49997f) & (fabsf(t) < 127.6f);
+  }
+  if (amb) {                                    // some value sits within 3e-5 of a tie: the definition's division decides
+#pragma unroll
+    for (int i = 0; i < N; ++i) q[i] = (x[i] == 0.0f) ? 0.0f : rintf(__fdiv_rn(x[i], s.S));
+  }
+#pragma unroll
+  for (int i = 0; i < N; ++i) q[i] = fminf(fmaxf(q[i], -127.0f), 127.0f);
 }
-__device__ __forceinline__ uint32_t quant_pack4(float a, float b, float c, float d, float S) {
-  return ((uint32_t)(int)quant_f(a, S) & 0xffu) | (((uint32_t)(int)quant_f(b, S) & 0xffu) << 8) |
-         (((uint32_t)(int)quant_f(c, S) & 0xffu) << 16) | (((uint32_t)(int)quant_f(d, S) & 0xffu) << 24);
+__device__ __forceinline__ uint32_t pack_codes(float a, float b, float c, float d) {
+  return ((uint32_t)(int)a & 0xffu) | (((uint32_t)(int)b & 0xffu) << 8) | (((uint32_t)(int)c & 0xffu) << 16) | (((uint32_t)(int)d & 0xffu) << 24);
+}
+__device__ __forceinline__ float quant_f(float x, QScale s) {
+  float xi[1] = {x}, q[1];
+  quant_codes<1>(xi, q, s);
+  return q[0];
 }
 // y = float(sum) * (S_a S_w) + b, each step one rounded fp32 operation
 __device__ __forceinline__ float dequant(uint32_t acc_bits, float sc, float b) {
@@ -330,6 +356,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
         // Feature mode (node encoder): the operand of the first tensor-core layer is the output of the
         // MLP's own first layer, ReLU(W1 f + b1) with f = the 3 normalised features of the row -- 3 FMAs per
         // value, computed here instead of being loaded.  ridx[0..1] / rown hold the row's 3 features.
+        // 8-bit (INT8 embedding): the features become INT8 codes (held as floats), w1 holds weight codes as floats, so
+        // the 3-term sums below are exact integers; de-quantisation + bias + ReLU follow the oracle's single steps and
+        // the store path re-quantises with the next layer's scale
+        auto feat_val = [&](float f) { if constexpr (q8) return quant_f(f, QScale{a.q_sf, a.q_rsf}); else return f; };
         if (pu == 0) {
           // all feature loads first, then the normalisations: the IEEE division has a slow-path branch the loads are
           // not hoisted across, and a load -> divide -> load chain costs one DRAM latency per feature (12 per tile)
@@ -342,21 +372,21 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             row = row < a.n_rows ? row : a.n_rows - 1;
             f0[p] = __ldg(a.feat[0] + row); f1[p] = __ldg(a.feat[1] + row); f2[p] = __ldg(a.feat[2] + row);
             if constexpr (NPASS <= 2) {
-              ridx[0][p] = __float_as_int(__fdiv_rn(__fsub_rn(f0[p], a.fc[0]), a.fs[0]));
-              ridx[1][p] = __float_as_int(__fdiv_rn(__fsub_rn(f1[p], a.fc[1]), a.fs[1]));
-              rown[p] = __float_as_int(__fdiv_rn(__fsub_rn(f2[p], a.fc[2]), a.fs[2]));
+              ridx[0][p] = __float_as_int(feat_val(__fdiv_rn(__fsub_rn(f0[p], a.fc[0]), a.fs[0])));
+              ridx[1][p] = __float_as_int(feat_val(__fdiv_rn(__fsub_rn(f1[p], a.fc[1]), a.fs[1])));
+              rown[p] = __float_as_int(feat_val(__fdiv_rn(__fsub_rn(f2[p], a.fc[2]), a.fs[2])));
             }
           }
           if constexpr (NPASS > 2) {
 #pragma unroll
             for (int p = 0; p < NPASS; ++p) {
-              ridx[0][p] = __float_as_int(__fdiv_rn(__fsub_rn(f0[p], a.fc[0]), a.fs[0]));
-              ridx[1][p] = __float_as_int(__fdiv_rn(__fsub_rn(f1[p], a.fc[1]), a.fs[1]));
-              rown[p] = __float_as_int(__fdiv_rn(__fsub_rn(f2[p], a.fc[2]), a.fs[2]));
+              ridx[0][p] = __float_as_int(feat_val(__fdiv_rn(__fsub_rn(f0[p], a.fc[0]), a.fs[0])));
+              ridx[1][p] = __float_as_int(feat_val(__fdiv_rn(__fsub_rn(f1[p], a.fc[1]), a.fs[1])));
+              rown[p] = __float_as_int(feat_val(__fdiv_rn(__fsub_rn(f2[p], a.fc[2]), a.fs[2])));
             }
           }
         }
-        const int c0 = pu * KA + jl * 4;             // this thread's 4 columns of the layer-1 output
+        const int c0 = pu * KG + jl * 4;             // this thread's 4 columns of the layer-1 output
         const float4 w0 = __ldg(reinterpret_cast<const float4*>(a.w1 + c0));
         const float4 w1 = __ldg(reinterpret_cast<const float4*>(a.w1 + HW + c0));
         const float4 w2 = __ldg(reinterpret_cast<const float4*>(a.w1 + 2 * HW + c0));
@@ -364,10 +394,17 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
 #pragma unroll
         for (int p = 0; p < NPASS; ++p) {
           const float fx = __int_as_float(ridx[0][p]), fy = __int_as_float(ridx[1][p]), fz = __int_as_float(rown[p]);
+          if constexpr (q8) {
+            dst[p].x = fmaxf(__fadd_rn(__fmul_rn(fmaf(w2.x, fz, fmaf(w1.x, fy, w0.x * fx)), a.q_sc0), bb.x), 0.f);
+            dst[p].y = fmaxf(__fadd_rn(__fmul_rn(fmaf(w2.y, fz, fmaf(w1.y, fy, w0.y * fx)), a.q_sc0), bb.y), 0.f);
+            dst[p].z = fmaxf(__fadd_rn(__fmul_rn(fmaf(w2.z, fz, fmaf(w1.z, fy, w0.z * fx)), a.q_sc0), bb.z), 0.f);
+            dst[p].w = fmaxf(__fadd_rn(__fmul_rn(fmaf(w2.w, fz, fmaf(w1.w, fy, w0.w * fx)), a.q_sc0), bb.w), 0.f);
+          } else {
           dst[p].x = fmaxf(fmaf(w2.x, fz, fmaf(w1.x, fy, fmaf(w0.x, fx, bb.x))), 0.f);
           dst[p].y = fmaxf(fmaf(w2.y, fz, fmaf(w1.y, fy, fmaf(w0.y, fx, bb.y))), 0.f);
           dst[p].z = fmaxf(fmaf(w2.z, fz, fmaf(w1.z, fy, fmaf(w0.z, fx, bb.z))), 0.f);
           dst[p].w = fmaxf(fmaf(w2.w, fz, fmaf(w1.w, fy, fmaf(w0.w, fx, bb.w))), 0.f);
+          }
         }
         if (++pu == n_units) { pu = 0; ptile += gridDim.x; }
         return;
@@ -492,23 +529,25 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
 #pragma unroll
         for (int d = 0; d < D; ++d) {
 #pragma unroll
-          for (int p = 0; p < NPASS; ++p) {
-            const int r = r0 + p * RPP;
-            const float4 v = buf[d][p];
-            const uint32_t byte = d * 64 + jl * 4;          // K position of this thread's 4 codes inside the 128-byte row
-            asm volatile("st.shared.b32 [%0], %1;" ::"r"(tile_q + r * 128 + (((byte >> 4) ^ (r & 7)) << 4) + (byte & 15)),
-                         "r"(quant_pack4(v.x, v.y, v.z, v.w, a.q_sa0)) : "memory");
+          for (int p2 = 0; p2 < NPASS; p2 += 2) {           // 8 values per tie test (these warps have 64 registers)
+            float xq[8] = {buf[d][p2].x, buf[d][p2].y, buf[d][p2].z, buf[d][p2].w,
+                           buf[d][p2 + 1].x, buf[d][p2 + 1].y, buf[d][p2 + 1].z, buf[d][p2 + 1].w};
+            float cq[8];
+            quant_codes<8>(xq, cq, QScale{a.q_sa0, a.q_rsa0});
+#pragma unroll
+            for (int h2 = 0; h2 < 2; ++h2) {
+              const int r = r0 + (p2 + h2) * RPP;
+              const uint32_t byte = d * 64 + jl * 4;        // K position of this thread's 4 codes inside the 128-byte row
+              asm volatile("st.shared.b32 [%0], %1;" ::"r"(tile_q + r * 128 + (((byte >> 4) ^ (r & 7)) << 4) + (byte & 15)),
+                           "r"(pack_codes(cq[4 * h2], cq[4 * h2 + 1], cq[4 * h2 + 2], cq[4 * h2 + 3])) : "memory");
+            }
           }
+          if (more) load_unit(buf[d]);                       // this buffer's next loads fly while the other half is converted
         }
         GP_ACC(1);
         named_bar_arrive(kBarEntry0 + ecnt % NSA, kGatherThreads + 32);
         ++ecnt;
         GP_ACC(2);
-        if (more) {
-#pragma unroll
-          for (int d = 0; d < D; ++d) load_unit(buf[d]);
-        }
-        GP_ACC(3);
       } else {
 #pragma unroll
         for (int d = 0; d < D; ++d) {
@@ -572,16 +611,19 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             tmem_ld32(acc + hh * 64 + 32, vb);
             tc_wait_ld();
             EP_ACC(0);
-            const float sc = a.q_sc[l], sn = a.q_sn[l];
+            const float sc = a.q_sc[l];
+            const QScale sn{a.q_sn[l], a.q_rsn[l]};
             const float* bq = bias + hh * 64;
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
-              w[i] = quant_pack4(fmaxf(dequant(va[4 * i], sc, bq[4 * i]), 0.f), fmaxf(dequant(va[4 * i + 1], sc, bq[4 * i + 1]), 0.f),
-                                 fmaxf(dequant(va[4 * i + 2], sc, bq[4 * i + 2]), 0.f), fmaxf(dequant(va[4 * i + 3], sc, bq[4 * i + 3]), 0.f), sn);
+            for (int g4 = 0; g4 < 4; ++g4) {         // 16 values per tie test
+              float xv[16], cv[16];
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
-              w[8 + i] = quant_pack4(fmaxf(dequant(vb[4 * i], sc, bq[32 + 4 * i]), 0.f), fmaxf(dequant(vb[4 * i + 1], sc, bq[32 + 4 * i + 1]), 0.f),
-                                     fmaxf(dequant(vb[4 * i + 2], sc, bq[32 + 4 * i + 2]), 0.f), fmaxf(dequant(vb[4 * i + 3], sc, bq[32 + 4 * i + 3]), 0.f), sn);
+              for (int i = 0; i < 16; ++i)
+                xv[i] = fmaxf(dequant(g4 < 2 ? va[16 * g4 + i] : vb[16 * (g4 - 2) + i], sc, bq[16 * g4 + i]), 0.f);
+              quant_codes<16>(xv, cv, sn);
+#pragma unroll
+              for (int i = 0; i < 4; ++i) w[4 * g4 + i] = pack_codes(cv[4 * i], cv[4 * i + 1], cv[4 * i + 2], cv[4 * i + 3]);
+            }
             asm volatile(
                 "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
                 "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
@@ -661,7 +703,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
               tc_wait_ld();
 #pragma unroll
               for (int i = 0; i < 32; ++i) {
-                const float hv = fmaxf(__uint_as_float(v[i]) + bias[q * 32 + i], 0.f);
+                float hv;
+                if constexpr (q8) hv = quant_f(fmaxf(dequant(v[i], a.q_sc[l], bias[q * 32 + i]), 0.f), QScale{a.q_sn[l], a.q_rsn[l]});   // code x weight codes: exact
+                else hv = fmaxf(__uint_as_float(v[i]) + bias[q * 32 + i], 0.f);
                 const float4 w0 = *reinterpret_cast<const float4*>(wlast_s + (q * 32 + i) * 8);
                 const float4 w1 = *reinterpret_cast<const float4*>(wlast_s + (q * 32 + i) * 8 + 4);
                 o8[0] = fmaf(hv, w0.x, o8[0]); o8[1] = fmaf(hv, w0.y, o8[1]); o8[2] = fmaf(hv, w0.z, o8[2]); o8[3] = fmaf(hv, w0.w, o8[3]);
@@ -674,7 +718,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             if (row < a.n_rows) {
 #pragma unroll
               for (int o = 0; o < 8; ++o)
-                if (o < a.n_out) a.out[(size_t)row * a.out_ld + o] = o8[o] + __ldg(a.bias[a.n_layers - 1] + o);
+                if (o < a.n_out) {
+                  if constexpr (q8) a.out[(size_t)row * a.out_ld + o] = __fadd_rn(__fmul_rn(o8[o], a.q_sc[a.n_layers - 1]), __ldg(a.bias[a.n_layers - 1] + o));
+                  else a.out[(size_t)row * a.out_ld + o] = o8[o] + __ldg(a.bias[a.n_layers - 1] + o);
+                }
             }
           } else {
             mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
@@ -689,12 +736,16 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
               uint32_t v[32];
               tmem_ld32(acc + q * 32, v);
               tc_wait_ld();
+              if constexpr (q8) {              // codes of the last hidden activation x integer weight codes (held as floats):
+                float xv[32], cv[32];          // exact below 2^24
 #pragma unroll
-              for (int i = 0; i < 32; ++i) {
-                if constexpr (q8)              // codes of the last hidden activation x integer weight codes (held as floats):
-                  logit = fmaf(quant_f(fmaxf(dequant(v[i], a.q_sc[l], bias[q * 32 + i]), 0.f), a.q_sn[l]),   // exact below 2^24
-                               wlast_s[q * 32 + i], logit);
-                else
+                for (int i = 0; i < 32; ++i) xv[i] = fmaxf(dequant(v[i], a.q_sc[l], bias[q * 32 + i]), 0.f);
+                quant_codes<32>(xv, cv, QScale{a.q_sn[l], a.q_rsn[l]});
+#pragma unroll
+                for (int i = 0; i < 32; ++i) logit = fmaf(cv[i], wlast_s[q * 32 + i], logit);
+              } else {
+#pragma unroll
+              for (int i = 0; i < 32; ++i)
                 logit = fmaf(fmaxf(__uint_as_float(v[i]) + bias[q * 32 + i], 0.f), wlast_s[q * 32 + i], logit);
               }
             }
@@ -993,8 +1044,13 @@ int tc_chunk_k(int mode) {
 
 // Requirements (checked by the caller): hidden width 128; K0 a multiple of the chunk (32 / 64) and
 // segment widths multiples of it; out_mode 0/1 needs dims[L] == 128; out_mode 3 needs dims[L] == 1.
-int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s) {
-  if (a.n_rows <= 0) return 0;
+int launch_mlp_tc(const TcArgs& a_in, int mode, int sm_count, cudaStream_t s) {
+  if (a_in.n_rows <= 0) return 0;
+  TcArgs a = a_in;
+  if (mode == ETX_PREC_INT8) {
+    a.q_rsa0 = 1.0f / a.q_sa0; a.q_rsf = 1.0f / a.q_sf;
+    for (int l = 0; l < kMaxLayers; ++l) a.q_rsn[l] = a.q_sn[l] != 0.0f ? 1.0f / a.q_sn[l] : 0.0f;
+  }
   if (a.wide) {                                  // one layer, no addend, two output halves; bf16 modes only
     if (a.n_layers != 1 || a.n_add != 0 || a.out_mode != 0) return -1;
     if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, 1>(a, sm_count, s);
@@ -1004,8 +1060,9 @@ int launch_mlp_tc(const TcArgs& a, int mode, int sm_count, cudaStream_t s) {
   }
   if (a.w1) {                                    // first-layer operand computed from 3 features (node encoder, embedding)
     if (a.n_add != 0 || a.n_seg != 0 || a.K0 != HW || !a.b1 || !a.feat[0] || !a.feat[1] || !a.feat[2]) return -1;
-    if (a.out_mode == 2) {                       // narrow linear output (embedding): TF32X3 only
-      if (mode != ETX_PREC_TF32X3 || a.n_out < 1 || a.n_out > 8 || a.n_layers < 2) return -1;
+    if (a.out_mode == 2) {                       // narrow linear output (embedding): 3xTF32, or the INT8 embedding
+      if ((mode != ETX_PREC_TF32X3 && mode != ETX_PREC_INT8) || a.n_out < 1 || a.n_out > 8 || a.n_layers < 2) return -1;
+      if (mode == ETX_PREC_INT8) return launch_mode<ETX_PREC_INT8, 3>(a, sm_count, s);
       return launch_mode<ETX_PREC_TF32X3, 3>(a, sm_count, s);
     }
     if (mode == ETX_PREC_TF32X3) return launch_mode<ETX_PREC_TF32X3, 2>(a, sm_count, s);
