@@ -294,9 +294,9 @@ int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   for (int b = 0; b < grid; ++b) for (int i = 0; i < 32; ++i) avg[i] += (double)h[b * 32 + i] / grid;
   const double tiles = (double)((a.n_rows + 127) / 128) / grid;
   fprintf(stderr, "[tc dbg] rows=%d K0=%d tiles/cta=%.1f | per tile cycles: mma total %.0f = wait acc_free %.0f + a_full %.0f + "
-          "hid_ready %.0f + w_full %.0f + issue %.0f | epi: wait acc_full %.0f of %.0f [hid ld %.0f math %.0f st+arrive %.0f | fin ld %.0f bar+sts %.0f io %.0f] | gather: wait a_empty %.0f of %.0f [data wait %.0f cvt+sts %.0f fence+arrive %.0f issue loads %.0f]\n",
+          "hid_ready %.0f + w_full %.0f + issue %.0f | epi: wait acc_full %.0f of %.0f [hid ld %.0f math %.0f st+arrive %.0f | fin ld %.0f fence %.0f io %.0f rdwait %.0f sts %.0f] | gather: wait a_empty %.0f of %.0f [data wait %.0f cvt+sts %.0f fence+arrive %.0f issue loads %.0f]\n",
           a.n_rows, a.mlp.dims[0], tiles, avg[5] / tiles, avg[0] / tiles, avg[1] / tiles, avg[2] / tiles, avg[3] / tiles, avg[4] / tiles,
-          avg[6] / tiles, avg[7] / tiles, avg[10] / tiles, avg[11] / tiles, avg[12] / tiles, avg[13] / tiles, avg[14] / tiles, avg[15] / tiles, avg[8] / tiles, avg[9] / tiles, avg[16] / tiles, avg[17] / tiles, avg[18] / tiles, avg[19] / tiles);
+          avg[6] / tiles, avg[7] / tiles, avg[10] / tiles, avg[11] / tiles, avg[12] / tiles, avg[13] / tiles, avg[14] / tiles, avg[15] / tiles, avg[20] / tiles, avg[21] / tiles, avg[8] / tiles, avg[9] / tiles, avg[16] / tiles, avg[17] / tiles, avg[18] / tiles, avg[19] / tiles);
   return n;
 #endif
 }

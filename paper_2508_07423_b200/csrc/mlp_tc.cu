@@ -73,6 +73,7 @@ constexpr uint32_t kBarEntry0 = 2;       // named barriers 2 .. 2 + NSTAGE_A - 1
 constexpr int kRegGather = 64, kRegEpi = 104, kRegCtl = 40;
 constexpr int HW = 128;                       // hidden width handled by this kernel
 constexpr int kAtomBytes = 128 * 128;         // one operand tile: 128 rows x 128 bytes (one swizzle atom wide)
+constexpr int kStageOutBytes = 8 * 4096;      // output staging: one 4 KB box [32 rows x 32 fp32 columns] per epilogue warp
 
 template <int MODE> struct Cfg;
 template <> struct Cfg<ETX_PREC_TF32X3> {
@@ -197,6 +198,8 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
                  ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
 }
 
+constexpr int kTcLayers = 4;                    // layers whose biases fit in shared memory beside the rings and the output staging
+
 struct Unit {                                   // one gather unit: KA columns of one source (16 bytes)
   const char* base;                             // source base + column offset (bytes)
   uint32_t ldb;                                 // row stride in bytes
@@ -244,16 +247,18 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   constexpr int NPASS = TM / RPP;               // passes per chunk (4 / 8)
   constexpr int D = C::PREFETCH;                // nc1 is a multiple of D for every MLP this kernel serves
 
-  extern __shared__ unsigned char smem_raw[];
-  const uint32_t raw = smem_u32(smem_raw);
-  const uint32_t base = (raw + 1023u) & ~1023u;                          // SWIZZLE_128B needs 1024-byte alignment
+  // SWIZZLE_128B tiles need 1024-byte alignment: the dynamic window is declared with that alignment (checked below), so
+  // no slack is reserved -- every byte of the 227 KB counts (rings 192 KB + output staging + biases + barriers)
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const uint32_t base = smem_u32(smem_raw);
   const uint32_t wring = base;
   const uint32_t aring = wring + NSW * kStageBytes;
-  const uint32_t stage_out = aring + NSA * kStageBytes;                  // 16 KB swizzled staging tile
-  unsigned char* gen = smem_raw + (base - raw);
-  float* bias_s = reinterpret_cast<float*>(gen + (NSW + NSA) * kStageBytes + kAtomBytes);   // [kMaxLayers][128]
-  float* wlast_s = bias_s + kMaxLayers * HW;                                                  // [128]
-  Bars* bars = reinterpret_cast<Bars*>(wlast_s + (VAR == 3 ? 8 * HW : HW));            // VAR 3: [128][8]
+  const uint32_t stage_out = aring + NSA * kStageBytes;                  // 32 KB: one swizzled 4 KB staging box per epilogue warp
+  unsigned char* gen = smem_raw;
+  float* wlast_s = reinterpret_cast<float*>(gen + (NSW + NSA) * kStageBytes);   // [128] / [128][8]: classifier and narrow-output launches stage no output, so this aliases the staging boxes
+  float* bias_s = reinterpret_cast<float*>(gen + (NSW + NSA) * kStageBytes + kStageOutBytes);   // [kTcLayers][128]
+  Bars* bars = reinterpret_cast<Bars*>(bias_s + kTcLayers * HW);
+  if (base & 1023u) __trap();
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_tiles = (a.n_rows + TM - 1) / TM;
@@ -302,10 +307,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
     utab[u] = un;
   }
 
-  for (int i = threadIdx.x; i < a.n_layers * HW; i += kThreads) {
-    const int l = i / HW, j = i % HW;
-    bias_s[i] = (l < n_gemm) ? __ldg(a.bias[l] + j) : 0.f;
-  }
+  for (int i = threadIdx.x; i < n_gemm * HW; i += kThreads) bias_s[i] = __ldg(a.bias[i / HW] + i % HW);
   if constexpr (narrow) {                        // last layer's weights [k][n_out] (k-major) padded to 8 units per k
     for (int i = threadIdx.x; i < HW * 8; i += kThreads)
       wlast_s[i] = (i % 8) < a.n_out ? __ldg(a.w_last + (i / 8) * a.n_out + (i % 8)) : 0.f;
@@ -578,7 +580,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
     const int et = q4 * 32 + lane;               // tile row = TMEM lane
     const uint32_t lane_addr = tmem + ((uint32_t)(q4 * 32) << 16);
     uint32_t g = 0;
-    long long e_wait = 0, ep[6] = {0, 0, 0, 0, 0, 0}, tp = 0;
+    long long e_wait = 0, ep[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, tp = 0;
     const bool edbg = ETX_DBG(a);
 #define EP_T0() if (edbg) tp = clock64()
 #define EP_ACC(i) if (edbg) { const long long tn = clock64(); ep[i] += tn - tp; tp = tn; }
@@ -592,28 +594,30 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
         const int tile = tile_of(pi, sl);
         const uint32_t hid = lane_addr + COL_HID + (NSLOT == 2 ? sl * HIDW : 0);
         uint64_t* hid_ready = bars->hid_ready + (NSLOT == 2 ? sl * 4 : 0);
-        const float* bias = bias_s + l * HW;
         long long te0 = edbg ? clock64() : 0;
         mbar_wait_warp(smem_u32(&bars->acc_full[b]), uacc[b] & 1, lane);
         ++uacc[b];
         if (edbg) e_wait += clock64() - te0;
         tc_fence_after();
         const uint32_t acc = lane_addr + COL_ACC + b * 128;
-        if (l < n_gemm - 1) {
+        {
+        const int L = l, HH = hh;
+        const float* bias = bias_s + L * HW;
+        if (L < n_gemm - 1) {
           // ---- hidden layer: ReLU(x + b) -> next A operand in TMEM, released chunk by chunk.
-          // This warp's column half holds K-chunks hh*HCH/2 .. of the next layer.
+          // This warp's column half holds K-chunks HH*HCH/2 .. of the next layer.
           if constexpr (q8) {
             // 8-bit: de-quantise the int32 sums, bias, ReLU, re-quantise with the NEXT layer's input scale (the Q -> node
             // -> DQ chain of P:2725); this warp's 64 columns become 16 packed columns of the single K-chunk
             EP_T0();
             uint32_t va[32], vb[32], w[16];
-            tmem_ld32(acc + hh * 64, va);
-            tmem_ld32(acc + hh * 64 + 32, vb);
+            tmem_ld32(acc + HH * 64, va);
+            tmem_ld32(acc + HH * 64 + 32, vb);
             tc_wait_ld();
             EP_ACC(0);
-            const float sc = a.q_sc[l];
-            const QScale sn{a.q_sn[l], a.q_rsn[l]};
-            const float* bq = bias + hh * 64;
+            const float sc = a.q_sc[L];
+            const QScale sn{a.q_sn[L], a.q_rsn[L]};
+            const float* bq = bias + HH * 64;
 #pragma unroll
             for (int g4 = 0; g4 < 4; ++g4) {         // 16 values per tie test
               float xv[16], cv[16];
@@ -627,7 +631,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             asm volatile(
                 "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
                 "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
-                ::"r"(hid + hh * 16), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7]),
+                ::"r"(hid + HH * 16), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7]),
                   "r"(w[8]), "r"(w[9]), "r"(w[10]), "r"(w[11]), "r"(w[12]), "r"(w[13]), "r"(w[14]), "r"(w[15]) : "memory");
             EP_ACC(1);
             tc_wait_st();
@@ -635,8 +639,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             mbar_arrive_relaxed_warp(smem_u32(&hid_ready[0]), lane);
             EP_ACC(2);
           }
-#pragma unroll 1
-          for (int c = hh * (HCH / 2); c < (hh + 1) * (HCH / 2); ++c) {
+#pragma unroll
+          for (int c = HH * (HCH / 2); c < (HH + 1) * (HCH / 2); ++c) {
             EP_T0();
             if constexpr (MODE == ETX_PREC_TF32X3) {
               uint32_t v[32], w[32];
@@ -694,7 +698,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
         } else if (narrow) {
           // ---- narrow linear output (embedding, Eq. 4.27 with identity output): last hidden layer, then
           // n_out <= 8 units as fp32 FMA chains over the 128 hidden values of the row, in registers
-          if (hh == 0) {
+          if (HH == 0) {
             float o8[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll 1
             for (int q = 0; q < HW / 32; ++q) {
@@ -704,7 +708,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
 #pragma unroll
               for (int i = 0; i < 32; ++i) {
                 float hv;
-                if constexpr (q8) hv = quant_f(fmaxf(dequant(v[i], a.q_sc[l], bias[q * 32 + i]), 0.f), QScale{a.q_sn[l], a.q_rsn[l]});   // code x weight codes: exact
+                if constexpr (q8) hv = quant_f(fmaxf(dequant(v[i], a.q_sc[L], bias[q * 32 + i]), 0.f), QScale{a.q_sn[L], a.q_rsn[L]});   // code x weight codes: exact
                 else hv = fmaxf(__uint_as_float(v[i]) + bias[q * 32 + i], 0.f);
                 const float4 w0 = *reinterpret_cast<const float4*>(wlast_s + (q * 32 + i) * 8);
                 const float4 w1 = *reinterpret_cast<const float4*>(wlast_s + (q * 32 + i) * 8 + 4);
@@ -729,7 +733,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
         } else if (a.out_mode == 3) {
           // ---- classifier: last hidden layer, then 1 unit + sigmoid; column half 0
           // warps do all 128 columns of their rows (a cross-warp sum is not worth it for 1 unit).
-          if (hh == 0) {
+          if (HH == 0) {
             float logit = 0.f;
 #pragma unroll 1
             for (int q = 0; q < HW / 32; ++q) {
@@ -739,8 +743,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
               if constexpr (q8) {              // codes of the last hidden activation x integer weight codes (held as floats):
                 float xv[32], cv[32];          // exact below 2^24
 #pragma unroll
-                for (int i = 0; i < 32; ++i) xv[i] = fmaxf(dequant(v[i], a.q_sc[l], bias[q * 32 + i]), 0.f);
-                quant_codes<32>(xv, cv, QScale{a.q_sn[l], a.q_rsn[l]});
+                for (int i = 0; i < 32; ++i) xv[i] = fmaxf(dequant(v[i], a.q_sc[L], bias[q * 32 + i]), 0.f);
+                quant_codes<32>(xv, cv, QScale{a.q_sn[L], a.q_rsn[L]});
 #pragma unroll
                 for (int i = 0; i < 32; ++i) logit = fmaf(cv[i], wlast_s[q * 32 + i], logit);
               } else {
@@ -760,47 +764,52 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
           }
         } else {
-          // ---- linear output (+ residual).  Each warp moves 16 columns of its own 32 rows at a time:
-          // thread = row = TMEM lane writes its 64 bytes (+ bias) into a private 2 KB staging box laid out
-          // as the SWIZZLE_64B tensor-map box [32 rows x 16 columns], and one lane hands the box to the TMA
+          // ---- linear output (+ residual).  Each warp moves 32 columns of its own 32 rows at a time:
+          // thread = row = TMEM lane writes its 128 bytes (+ bias) into the warp's private 4 KB staging box, laid out
+          // as the SWIZZLE_128B tensor-map box [32 rows x 32 columns], and one lane hands the box to the TMA
           // unit -- a tensor store, or for the residual e += y a tensor REDUCE-ADD on the in-place
           // state: one IEEE fp32 add per element, performed at L2, no residual load, deterministic (each
           // element is touched exactly once).  No SIMT global traffic, no read-back of the staging tile,
           // rows past n_rows are clipped by the tensor map.
-          const uint32_t stg = stage_out + ew * 2048;
+          // The warp's 64 accumulator columns go to registers first and the accumulator is released at once (the MMA
+          // warp starts the next tile's first layer while the boxes drain).  Two TMA operations per warp and tile:
+          // in-kernel counters put the issue of one operation at ~420 cycles of the issuing warp with all eight
+          // epilogue warps at it (16 boxes of 4 KB per tile instead of round 1's 32 of 2 KB).
+          const uint32_t stg = stage_out + ew * 4096;
           const bool in_place_add = (a.out_mode == 1);
           const int row0 = tile * TM + q4 * 32;
-#pragma unroll 1
-          for (int q = 0; q < 4; ++q) {
-            const int col0 = hh * 64 + q * 16;
+          EP_T0();
+          uint32_t va[32], vb[32];
+          tmem_ld32(acc + HH * 64, va);
+          tmem_ld32(acc + HH * 64 + 32, vb);
+          tc_wait_ld();
+          tc_fence_before();
+          mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
+          EP_ACC(3);
+#pragma unroll
+          for (int q = 0; q < 2; ++q) {
+            const int col0 = HH * 64 + q * 32;
             EP_T0();
-            uint32_t v[16];
-            asm volatile(
-                "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-                "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-                : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                  "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                : "r"(acc + col0) : "memory");
-            tc_wait_ld();
-            EP_ACC(3);
-            if (q == 3) { tc_fence_before(); mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane); }
             if (lane == 0) bulk_wait_read0();      // the TMA unit has read the previous box out of the staging slice
             __syncwarp();
+            EP_ACC(6);
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 bq = *reinterpret_cast<const float4*>(bias + col0 + 4 * j);
+            for (int j = 0; j < 8; ++j) {
+              const uint32_t v0 = q == 0 ? va[4 * j] : vb[4 * j], v1 = q == 0 ? va[4 * j + 1] : vb[4 * j + 1];
+              const uint32_t v2 = q == 0 ? va[4 * j + 2] : vb[4 * j + 2], v3 = q == 0 ? va[4 * j + 3] : vb[4 * j + 3];
+              const int cb = col0 + 4 * j;
+              const uint32_t dst = stg + lane * 128 + ((j ^ (lane & 7)) << 4);
               if constexpr (q8 && wide)        // 8-bit per-hit projections: the raw int32 sums (they are added as integers)
-                st_shared_v4(stg + lane * 64 + ((j ^ ((lane >> 1) & 3)) << 4), v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+                st_shared_v4(dst, v0, v1, v2, v3);
               else if constexpr (q8) {
-                const float sc = a.q_sc[l];
-                st_shared_v4(stg + lane * 64 + ((j ^ ((lane >> 1) & 3)) << 4),
-                             __float_as_uint(dequant(v[4 * j], sc, bq.x)), __float_as_uint(dequant(v[4 * j + 1], sc, bq.y)),
-                             __float_as_uint(dequant(v[4 * j + 2], sc, bq.z)), __float_as_uint(dequant(v[4 * j + 3], sc, bq.w)));
+                const float sc = a.q_sc[L];
+                st_shared_v4(dst, __float_as_uint(dequant(v0, sc, bias[cb])), __float_as_uint(dequant(v1, sc, bias[cb + 1])),
+                             __float_as_uint(dequant(v2, sc, bias[cb + 2])), __float_as_uint(dequant(v3, sc, bias[cb + 3])));
               } else
-              st_shared_v4(stg + lane * 64 + ((j ^ ((lane >> 1) & 3)) << 4),
-                           __float_as_uint(__uint_as_float(v[4 * j]) + bq.x), __float_as_uint(__uint_as_float(v[4 * j + 1]) + bq.y),
-                           __float_as_uint(__uint_as_float(v[4 * j + 2]) + bq.z), __float_as_uint(__uint_as_float(v[4 * j + 3]) + bq.w));
+              st_shared_v4(dst, __float_as_uint(__uint_as_float(v0) + bias[cb]), __float_as_uint(__uint_as_float(v1) + bias[cb + 1]),
+                           __float_as_uint(__uint_as_float(v2) + bias[cb + 2]), __float_as_uint(__uint_as_float(v3) + bias[cb + 3]));
             }
+            EP_ACC(7);
             fence_async_smem();                    // generic-proxy writes -> async proxy (TMA)
             __syncwarp();
             EP_ACC(4);
@@ -813,6 +822,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             EP_ACC(5);
           }
         }
+        }
       }
     }
     if (lane == 0) bulk_wait_all();              // every output box has left the SM before the CTA retires
@@ -821,6 +831,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
       a.dbg[(size_t)blockIdx.x * 32 + 6] = (unsigned long long)e_wait;
       a.dbg[(size_t)blockIdx.x * 32 + 7] = (unsigned long long)(clock64() - e_start);
       for (int i = 0; i < 6; ++i) a.dbg[(size_t)blockIdx.x * 32 + 10 + i] = (unsigned long long)ep[i];
+      for (int i = 6; i < 9; ++i) a.dbg[(size_t)blockIdx.x * 32 + 14 + i] = (unsigned long long)ep[i];
     }
   } else if (warp == kWarpLoader) {
     // =========================== weight loader ===========================
@@ -993,8 +1004,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   }
 }
 
-// Tensor map of the output [n_rows][n_cols] fp32 (row stride out_ld floats) with the epilogue's box: 16 columns
-// (64 bytes, SWIZZLE_64B) x 32 rows.  cuTensorMapEncodeTiled is fetched through the runtime (no link-time
+// Tensor map of the output [n_rows][n_cols] fp32 (row stride out_ld floats) with the epilogue's box: 32 columns
+// (128 bytes, SWIZZLE_128B) x 32 rows.  cuTensorMapEncodeTiled is fetched through the runtime (no link-time
 // dependency on libcuda: the library must still load on a machine without a driver).
 bool encode_out_map(CUtensorMap* m, float* out, int n_rows, int n_cols, int out_ld) {
   using Fn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -1010,23 +1021,27 @@ bool encode_out_map(CUtensorMap* m, float* out, int n_rows, int n_cols, int out_
   if (!fn || (reinterpret_cast<uintptr_t>(out) & 15) || (out_ld & 3)) return false;
   const cuuint64_t dims[2] = {(cuuint64_t)n_cols, (cuuint64_t)n_rows};
   const cuuint64_t strides[1] = {(cuuint64_t)out_ld * sizeof(float)};
-  const cuuint32_t box[2] = {16, 32}, estr[2] = {1, 1};
+  const cuuint32_t box[2] = {32, 32}, estr[2] = {1, 1};
   return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, out, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 template <int MODE, int VAR>
 int launch_mode(const TcArgs& a, int sm_count, cudaStream_t s) {
   using C = Cfg<MODE>;
-  static bool configured[kMaxDevices] = {false};    // the shared-memory opt-in is a per-DEVICE attribute of the function
+  static int configured[kMaxDevices] = {0};         // the shared-memory opt-in is a per-DEVICE attribute of the function
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return -1;
-  const size_t smem = 1024 + (size_t)(C::NSTAGE_W + C::NSTAGE_A) * C::PIECES * kAtomBytes + kAtomBytes +
-                      (kMaxLayers + (VAR == 3 ? 8 : 1)) * HW * sizeof(float) + sizeof(Bars) + 64;
+  // rings (192 KB) + output staging (32 KB; the classifier's / narrow output's last-layer weights alias it) + biases +
+  // barriers: 226.8 of the 227 KB an SM offers
+  const size_t smem = (size_t)(C::NSTAGE_W + C::NSTAGE_A) * C::PIECES * kAtomBytes + kStageOutBytes +
+                      kTcLayers * HW * sizeof(float) + sizeof(Bars) + 16;
   if (!configured[dev]) {
     if (cudaFuncSetAttribute(mlp_tc_kernel<MODE, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
-    configured[dev] = true;
+    configured[dev] = 1;
   }
+  const int n_gemm = (a.out_mode == 3 || VAR == 3) ? a.n_layers - 1 : a.n_layers;
+  if (n_gemm > kTcLayers) return -1;                // the shared-memory bias table holds kTcLayers layers
   const int n_tiles = (a.n_rows + TM - 1) / TM;
   const int grid = n_tiles < sm_count ? n_tiles : sm_count;
   CUtensorMap tmap;
