@@ -51,6 +51,45 @@ def peaks():
             "source": "fallback"}
 
 
+def measured_alu_peaks(local: int):
+    """ALU denominators measured live by the library's microbenchmark (etx_measure_alu_peak, include/etx.h): unfused
+    fp32 add+mul as scalar and as packed-pair instructions (operations/s) and FFMA (flop/s)."""
+    from paper_2508_07423_b200 import binding
+    return {"scalar_ops": binding.etx_measure_alu_peak(local, 0), "packed_ops": binding.etx_measure_alu_peak(local, 1),
+            "ffma_flops": binding.etx_measure_alu_peak(local, 2)}
+
+
+def measured_tf32_peak(dev, seconds: float = 1.5):
+    """Dense TF32 tensor peak measured the way MEASURED_PEAKS.json's bf16 figure is: cuBLAS (torch.matmul on fp32 inputs
+    with TF32 allowed) 8192^3, best of 10 launches (burst) and back to back for `seconds` (sustained, power-capped)."""
+    import torch
+    old = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = True
+    try:
+        n = 8192
+        a = torch.randn(n, n, device=dev)
+        b = torch.randn(n, n, device=dev)
+        c = torch.empty(n, n, device=dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.matmul(a, b, out=c)
+        best = float("inf")
+        for _ in range(10):
+            e0.record(); torch.matmul(a, b, out=c); e1.record(); e1.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        reps, t_start = 0, time.perf_counter()
+        e0.record()
+        while time.perf_counter() - t_start < seconds:
+            for _ in range(10):
+                torch.matmul(a, b, out=c)
+            reps += 10
+            torch.cuda.synchronize()
+        e1.record(); e1.synchronize()
+        sus = e0.elapsed_time(e1) / max(reps, 1)
+        return {"burst": 2 * n ** 3 / (best * 1e-3) / 1e12, "sustained": 2 * n ** 3 / (sus * 1e-3) / 1e12}
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = old
+
+
 def shard_event_ids(cfg, rank: int, n_ev: int):
     """Events are independent: rank r takes event ids r*n_ev .. (r+1)*n_ev - 1 of the config's
     stream (weak scaling, no data-path collective)."""
@@ -233,6 +272,8 @@ def run_ours(args):
     blob = synth.generate_weights(cfg)
     etx = binding.Etx(binding.make_desc(cfg, precision=args.precision if args.precision is not None else cfg.precision),
                       blob, device=local)
+    if int(etx.desc.precision) == synth.PREC_INT8:     # next row NEXT-3 as the whole step: needs the stored calibrated ranges
+        etx.etx_set_int8_ranges(synth.int8_gnn_alpha(cfg))
     r2, gap, H = synth.r2_max(cfg), cfg.max_plane_gap, cfg.gnn_hidden
     N = len(batch["r"])
     cap = int(N * (cfg.target_degree * (1.25 if args.tracks_mean <= 0 else 4.0) + 2))   # r^2 is calibrated at the config's occupancy
@@ -411,13 +452,17 @@ def run_ours(args):
         pairs = pair_tests(batch, gap)
         d_emb = cfg.emb_widths[-1]
         t_s = stages["graph"]["ms"] * 1e-3
-        alu_peak = 148 * 128 * pk["sm_max_mhz"] * 1e6           # unfused fp32 operations per second
+        alu = measured_alu_peaks(local)
+        alu_peak = alu["packed_ops"] if d_emb == 4 else alu["scalar_ops"]     # unfused fp32 operations per second, measured
         g_bytes = N * (4 * d_emb + 1) + 2 * (4 * (N + 1) + 8 * E)
         stages["graph"].update({"pair_tests": pairs, "pair_tests_per_s": pairs / t_s,
                                 "alu_frac": pairs * 3 * d_emb / t_s / alu_peak,
                                 "alu_frac_executed": 2 * pairs * 3 * d_emb / t_s / alu_peak,
                                 "gbs": g_bytes / t_s / 1e9, "hbm_frac": g_bytes / t_s / 1e9 / pk["hbm_gbs"],
-                                "bound": "alu (fp32, unfused): 148 SM x 128 lanes x %.0f MHz" % pk["sm_max_mhz"]})
+                                "alu_peak_ops_per_s": alu_peak,
+                                "bound": "alu (fp32 add/mul, unfused, %s): measured by etx_measure_alu_peak; nominal 148 SM x 128 lanes x "
+                                         "%.0f MHz = %.3g/s" % ("packed pairs" if d_emb == 4 else "scalar", pk["sm_max_mhz"],
+                                                                148 * 128 * pk["sm_max_mhz"] * 1e6)})
     gnn_ms = sum(stages[k]["ms"] for k in ("node_enc", "edge_enc", "scatter", "node_net", "edge_net", "edge_proj"))
     stages["message_passing_total"] = {"ms": gnn_ms, "events_per_s": n_ev / (gnn_ms * 1e-3) if gnn_ms else None}
 
@@ -434,20 +479,28 @@ def run_ours(args):
     L = cfg.gnn_mlp_hidden_layers
     mma_flop = E * flops_mlp((H,) + (H,) * L + (H,))          # per launch, factorised first layer
     if prec == synth.PREC_FP32:
-        # FFMA: 148 SMs x 128 fp32 lanes x 2 FLOP x max SM clock (B200_PROFILING.md unit counts)
-        peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+        # FFMA: measured by the library's microbenchmark (nominal: 148 SMs x 128 fp32 lanes x 2 FLOP x max SM clock)
+        peak = measured_alu_peaks(local)["ffma_flops"] / 1e12
         roof = {"bound": "alu", "unit": "TFLOP/s", "peak": peak,
-                "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x %.0f MHz" % pk["sm_max_mhz"]}
+                "peak_source": "measured FFMA microbenchmark (etx_measure_alu_peak); nominal 148 SM x 128 lanes x 2 x %.0f MHz = %.1f"
+                               % (pk["sm_max_mhz"], 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12)}
         dtype, passes, mma_flop = "f32", 1, per_launch_flop
     elif prec == synth.PREC_TF32X3:
-        peak = pk["bf16_tflops_sustained"] * 0.5
+        tf = measured_tf32_peak(dev)
+        peak = tf["sustained"]
         roof = {"bound": "tensor", "unit": "TFLOP/s", "peak": peak,
-                "peak_source": f"{pk['source']} bf16 sustained x 0.5 (tf32 nominal ratio)"}
+                "peak_source": "measured in this run: cuBLAS TF32 8192^3 sustained (burst %.0f; bf16 sustained x 0.5 nominal ratio = %.0f)"
+                               % (tf["burst"], pk["bf16_tflops_sustained"] * 0.5)}
         dtype, passes = "tf32x3", 3
     elif prec == synth.PREC_BF16X3:
         peak = pk["bf16_tflops_sustained"]
         roof = {"bound": "tensor", "unit": "TFLOP/s", "peak": peak, "peak_source": f"{pk['source']} bf16 sustained"}
         dtype, passes = "bf16x3", 3
+    elif prec == synth.PREC_INT8:
+        peak = pk["bf16_tflops_sustained"] * 2.0
+        roof = {"bound": "tensor", "unit": "TOP/s", "peak": peak,
+                "peak_source": f"{pk['source']} bf16 sustained x 2 (8-bit nominal ratio)"}
+        dtype, passes = "i8", 1
     else:
         peak = pk["bf16_tflops_sustained"]
         roof = {"bound": "tensor", "unit": "TFLOP/s", "peak": peak, "peak_source": f"{pk['source']} bf16 sustained"}
@@ -533,7 +586,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c2", choices=sorted(synth.CONFIGS))
     ap.add_argument("--events", type=int, default=0, help="events per GPU (default: the config's)")
-    ap.add_argument("--precision", type=int, default=None, help="override etx_precision (0 fp32, 1 tf32x3, 2 bf16, 3 bf16x3)")
+    ap.add_argument("--precision", type=int, default=None, help="override etx_precision (0 fp32, 1 tf32x3, 2 bf16, 3 bf16x3, 4 int8)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the next-row timings (launch lists of the step only)")
     ap.add_argument("--tracks-mean", type=float, default=0.0,

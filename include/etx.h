@@ -245,6 +245,16 @@ etx_status etx_infer_host(etx_ctx* ctx, const etx_batch_host* batch, float r2_ma
 /* Number of kernels the library has launched on this context since creation (for accounting).     */
 int64_t etx_launch_count(const etx_ctx* ctx);
 
+/* Measurement utility (not a step of the path): the rate, in arithmetic operations per second, at which `device`
+ * retires the instruction mix of two of the library's ALU-bound kernels, measured with a register-resident
+ * microbenchmark (8 independent chains per thread, 8 CTAs of 256 threads per SM, best of 4 timed launches):
+ *   kind 0  unfused fp32 add + multiply as scalar instructions   -- the distance test of Eq. 8.1 for d != 4
+ *   kind 1  the same as packed pairs (add.rn.f32x2 / mul.rn.f32x2) -- the d = 4 distance test (graph.cu)
+ *   kind 2  fused multiply-add, 2 flop each                       -- the exact-fp32 MLP kernel (ETX_PREC_FP32)
+ * bench.py divides by these instead of a figure derived from unit counts and clocks.  Needs no context; returns
+ * ETX_ERR_CUDA without a device, ETX_ERR_INVALID for a bad kind or a NULL result pointer. */
+etx_status etx_measure_alu_peak(int32_t device, int32_t kind, double* ops_per_s);
+
 /* Per-stage device timing.  While enabled, every group of launches of one class is bracketed by CUDA
  * events on the call's stream.  etx_profile_read synchronises those events, returns the accumulated
  * milliseconds and launch counts per class since the last read (arrays of ETX_K_COUNT), and resets.  */

@@ -23,7 +23,8 @@ EXPORTS = ["etx_weight_count", "etx_create", "etx_destroy", "etx_last_error", "e
            "etx_set_workspace", "etx_embed", "etx_embed_int8", "etx_build_graph", "etx_gnn_forward", "etx_edge_scores",
            "etx_infer_host", "etx_launch_count", "etx_profile_enable", "etx_profile_read", "etx_build_tracks",
            "etx_build_triplets", "etx_triplet_weight_count", "etx_set_triplet_classifiers", "etx_triplet_scores",
-           "etx_triplet_tracks_workspace_bytes", "etx_build_tracks_from_triplets", "etx_set_int8_ranges"]
+           "etx_triplet_tracks_workspace_bytes", "etx_build_tracks_from_triplets", "etx_set_int8_ranges",
+           "etx_measure_alu_peak"]
 KERNEL_CLASSES = ["embed", "graph", "node_enc", "edge_enc", "scatter", "node_net", "edge_net", "cls", "tracks", "edge_proj"]
 
 
@@ -31,6 +32,15 @@ class EtxError(RuntimeError):
     def __init__(self, status: int, msg: str):
         super().__init__(f"libetx status {status}: {msg}")
         self.status = status
+
+
+def etx_measure_alu_peak(device: int, kind: int) -> float:
+    """Arithmetic operations per second of the ALU microbenchmark (etx.h): kind 0 scalar add+mul, 1 packed pairs, 2 FFMA."""
+    out = C.c_double(0.0)
+    st = load_library().etx_measure_alu_peak(int(device), int(kind), C.byref(out))
+    if st != 0:
+        raise EtxError(st, "etx_measure_alu_peak failed")
+    return float(out.value)
 
 
 class ModelDesc(C.Structure):
@@ -110,6 +120,8 @@ def load_library():
                                        C.POINTER(C.c_int64), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.etx_launch_count.restype = C.c_int64
         lib.etx_launch_count.argtypes = [C.c_void_p]
+        lib.etx_measure_alu_peak.restype = C.c_int
+        lib.etx_measure_alu_peak.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double)]
         lib.etx_build_tracks.restype = C.c_int
         lib.etx_build_tracks.argtypes = [C.c_void_p, C.POINTER(Batch), C.POINTER(Graph), C.c_void_p, C.c_float,
                                          C.c_void_p, C.c_void_p]

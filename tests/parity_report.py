@@ -1,7 +1,7 @@
 """Parity report at BASELINE.json's full sizes (needs a B200): writes the markdown that is committed as
 profiles/rNN_parity.md.  Test infrastructure: calls the CUDA library through the binding and the CPU oracle.
 
-  python -m tests.parity_report --out gpurun_out/parity.md [--quick]
+  python tests/parity_report.py --out gpurun_out/parity.md [--quick]
 
 Sections
   1. error vs gain: for C2/C3 and C4, at the oracle-calibrated gain g (config_constants.json,
@@ -51,7 +51,7 @@ def main():
     L = []
     w = L.append
     w("# Parity report (full-size batches, one B200)\n")
-    w(f"command: `python -m tests.parity_report --out {args.out}{' --quick' if args.quick else ''}`  \n"
+    w(f"command: `python tests/parity_report.py --out {args.out}{' --quick' if args.quick else ''}`  \n"
       f"device: {torch.cuda.get_device_name(0)}; gains from `config_constants.json` (oracle/calibrate_gain.py): "
       + ", ".join(f"{k} g={v.gain}" for k, v in synth.CONFIGS.items()) + "\n")
     w("## 1. Score error vs gain, EVERY edge, tensor-core modes against the exact-fp32 FFMA mode\n")
