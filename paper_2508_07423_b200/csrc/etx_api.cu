@@ -274,7 +274,16 @@ int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   t.out_mode = a.out_mode; t.out = a.out; t.res = a.res; t.out_ld = a.out_ld;
 #ifdef ETX_DEV_SWITCHES
   static const char* expv = getenv("ETX_TC_EXP");                  // developer build: timing experiments (wrong results)
-  t.exp_flags = expv ? atoi(expv) : 0;
+  t.exp_flags = (expv && a.out_mode != 2) ? atoi(expv) : 0;      // not the embedding: the graph must stay the real one
+#endif
+#ifdef ETX_DEV_SWITCHES
+  if (getenv("ETX_TC_SYNC")) {                                     // developer build: localise a faulting launch
+    const int n = launch_mlp_tc(t, mode, c->sm_count, s);
+    const cudaError_t e = cudaStreamSynchronize(s);
+    fprintf(stderr, "[tc sync] mode=%d rows=%d K0=%d n_add=%d wide=%d layers=%d out_mode=%d -> %d, %s\n", mode, t.n_rows, t.K0, t.n_add,
+            t.wide, t.n_layers, t.out_mode, n, cudaGetErrorString(e));
+    return n;
+  }
 #endif
 #ifndef ETX_TC_COUNTERS
   return launch_mlp_tc(t, mode, c->sm_count, s);

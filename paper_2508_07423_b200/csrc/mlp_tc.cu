@@ -210,6 +210,11 @@ constexpr int kMaxUnits = 24;
 struct Bars {                                   // mbarriers (8 bytes each) + TMEM base + gather unit table
   uint64_t w_full[8], w_empty[8], a_full[8], a_empty[8], acc_full[2], acc_free[2], hid_ready[8];
   uint32_t tmem_base;
+  // Progress counters for the two MMA issuer warps (see there): weight stages the loader has started to fill, operand
+  // entries the commit warp has published.  An mbarrier parity wait is only meaningful for the barrier's CURRENT phase;
+  // an issuer that reaches a stage / entry one ring revolution ahead of its sibling would read the other parity as
+  // "complete".  It first waits for the counter to pass its index, which implies the previous phase has completed.
+  uint32_t w_issued, a_produced;
   Unit utab[kMaxUnits];
 };
 
@@ -236,6 +241,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   // released, so the weight ring moves half the bytes.  TF32X3 needs 256 columns per hidden operand
   // and keeps one tile in flight with ping-pong accumulators.
   constexpr int NSLOT = (MODE == ETX_PREC_TF32X3) ? 1 : 2;
+  // MMA issuer warps.  2 (one per tile in flight, each walking its own tile's chain of waits) is implemented and correct,
+  // and measured SLOWER (edge network 23.5 -> 25.4 ms per step, classifier 1.9 -> 2.4): issued concurrently, the two tiles'
+  // MMAs interleave in the tensor pipe and both tiles finish their layer late and together, which destroys the stagger
+  // (layer l of tile A, then of tile B) that lets the epilogue warps work on one tile while the other one's MMAs run.
+  constexpr int NMW = 1;
   constexpr uint32_t HIDW = P * HID_COLS;       // TMEM columns of one hidden operand region (256 / 128 / 64)
   constexpr int HCH = HW / KA;                  // K-chunks per hidden layer (4 / 2; 1 for 8-bit operands)
   constexpr int KG = C::KG;                     // columns of one gather unit
@@ -314,10 +324,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   } else if (a.out_mode == 3)
     for (int i = threadIdx.x; i < HW; i += kThreads) wlast_s[i] = __ldg(a.w_last + i);
   if (threadIdx.x == 0) {
-    for (int i = 0; i < NSW; ++i) { mbar_init(smem_u32(&bars->w_full[i]), 1); mbar_init(smem_u32(&bars->w_empty[i]), 1); }
-    for (int i = 0; i < NSA; ++i) { mbar_init(smem_u32(&bars->a_full[i]), 1); mbar_init(smem_u32(&bars->a_empty[i]), 1); }
+    for (int i = 0; i < NSW; ++i) { mbar_init(smem_u32(&bars->w_full[i]), 1); mbar_init(smem_u32(&bars->w_empty[i]), NMW); }
+    for (int i = 0; i < NSA; ++i) { mbar_init(smem_u32(&bars->a_full[i]), 1); mbar_init(smem_u32(&bars->a_empty[i]), wide ? 2 : 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&bars->acc_full[i]), 1); mbar_init(smem_u32(&bars->acc_free[i]), kEpiThreads / 32); }
     for (int i = 0; i < 8; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), q8 ? 8 : 4);   // 8-bit: ONE chunk per layer, written by all 8 warps
+    bars->w_issued = 0; bars->a_produced = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == kWarpMma) {                        // TMEM: all 512 columns of this SM (1 CTA per SM)
@@ -429,6 +440,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
       }
       const Unit un = utab[pu];
       const char* base = un.base + jl * 16;
+      if (ETX_EXP(a, 32)) {                        // timing experiment (wrong results): no global loads in the gather warps
+#pragma unroll
+        for (int p = 0; p < NPASS; ++p) dst[p] = make_float4(1.f, 2.f, 3.f, 4.f);
+        if (++pu == n_units) { pu = 0; ptile += gridDim.x; }
+        return;
+      }
 #pragma unroll
       for (int p = 0; p < NPASS; ++p) {
         const uint32_t idx = (uint32_t)(un.sel == 0 ? ridx[0][p] : (un.sel == 1 ? ridx[1][p] : rown[p]));
@@ -439,6 +456,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
     // store one K-chunk of the MMA operand (converted / split) into ring entry `slot`
     auto store_operand = [&](const float4 (&src)[NPASS], uint32_t slot) {
       const uint32_t tile_hi = aring + slot * kStageBytes;
+      if (ETX_EXP(a, 512)) return;                 // timing experiment (wrong results): the gather warps store nothing
 #pragma unroll
       for (int p = 0; p < NPASS; ++p) {
         const int r = r0 + p * RPP;
@@ -488,7 +506,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
         if constexpr (ENT == 2) wait_entry(ecnt + 1);
         GP_T0();
 #pragma unroll
-        for (int p = 0; p < NPASS; ++p) {
+        for (int p = 0; p < (ETX_EXP(a, 512) ? 0 : NPASS); ++p) {
           const int r = r0 + p * RPP;
           if constexpr (LPR == 8) {            // unit = 32 columns: (buf0 + buf1) -> tile 0, (buf2 + buf3) -> tile 1
             const uint32_t dst0 = aring + (ecnt % NSA) * kStageBytes + r * 128 + ((jl ^ (r & 7)) << 4);
@@ -657,20 +675,37 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
               tmem_st32(hid + HID_COLS + c * 32, v);
             } else if constexpr (P == 2) {       // BF16X3: 64 accumulator columns -> 32 hi + 32 lo packed columns
               uint32_t va[32], vb[32], wh[32], wl[32];     // both loads in flight, one wait (va/vb die pair by pair as wh/wl are born)
+              if (ETX_EXP(a, 256)) {               // timing experiment (wrong results): no tensor-memory traffic in the hidden epilogue
+                tc_fence_before();
+                mbar_arrive_relaxed_warp(smem_u32(&hid_ready[c]), lane);
+                continue;
+              }
               tmem_ld32(acc + c * 64, va);
               tmem_ld32(acc + c * 64 + 32, vb);
+              // the first half's biases are fetched while the tensor-memory loads fly: tcgen05.wait::ld is an asm volatile
+              // with a memory clobber, so a load written after it is issued after it (ncu: the short scoreboard of these
+              // LDS was the epilogue warps' largest stall)
+              float4 bp[8];
+#pragma unroll
+              for (int i = 0; i < 8; ++i) bp[i] = *reinterpret_cast<const float4*>(bias + c * 64 + 4 * i);
               tc_wait_ld();
               EP_ACC(0);
+              if (ETX_EXP(a, 8)) {                 // timing experiment (wrong results): no bias / ReLU / split arithmetic
+                tmem_st32(hid + c * 32, va);
+                tmem_st32(hid + HID_COLS + c * 32, vb);
+              } else {
 #pragma unroll
-              for (int i = 0; i < 16; ++i)
-                split_bf16x2(fmaxf(__uint_as_float(va[2 * i]) + bias[c * 64 + 2 * i], 0.f),
-                             fmaxf(__uint_as_float(va[2 * i + 1]) + bias[c * 64 + 2 * i + 1], 0.f), wh[i], wl[i]);
+              for (int i = 0; i < 8; ++i) {
+                split_bf16x2(fmaxf(__uint_as_float(va[4 * i]) + bp[i].x, 0.f), fmaxf(__uint_as_float(va[4 * i + 1]) + bp[i].y, 0.f), wh[2 * i], wl[2 * i]);
+                split_bf16x2(fmaxf(__uint_as_float(va[4 * i + 2]) + bp[i].z, 0.f), fmaxf(__uint_as_float(va[4 * i + 3]) + bp[i].w, 0.f), wh[2 * i + 1], wl[2 * i + 1]);
+              }
 #pragma unroll
               for (int i = 0; i < 16; ++i)
                 split_bf16x2(fmaxf(__uint_as_float(vb[2 * i]) + bias[c * 64 + 32 + 2 * i], 0.f),
                              fmaxf(__uint_as_float(vb[2 * i + 1]) + bias[c * 64 + 32 + 2 * i + 1], 0.f), wh[16 + i], wl[16 + i]);
               tmem_st32(hid + c * 32, wh);
               tmem_st32(hid + HID_COLS + c * 32, wl);
+              }
             } else {
               uint32_t va[32], vb[32], w[32];
               tmem_ld32(acc + c * 64, va);
@@ -780,34 +815,42 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
           const int row0 = tile * TM + q4 * 32;
           EP_T0();
           uint32_t va[32], vb[32];
+          if (!ETX_EXP(a, 256)) {
           tmem_ld32(acc + HH * 64, va);
           tmem_ld32(acc + HH * 64 + 32, vb);
+          }
           tc_wait_ld();
           tc_fence_before();
           mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
           EP_ACC(3);
 #pragma unroll
-          for (int q = 0; q < 2; ++q) {
+          for (int q = 0; q < (ETX_EXP(a, 16) ? 0 : 2); ++q) {       // (timing experiment 16, wrong results: no output at all)
             const int col0 = HH * 64 + q * 32;
             EP_T0();
             if (lane == 0) bulk_wait_read0();      // the TMA unit has read the previous box out of the staging slice
             __syncwarp();
             EP_ACC(6);
+            // The box's 32 biases first, all eight 128-bit loads in flight together: st_shared_v4 is an asm volatile
+            // with a memory clobber, so a bias load written between two stores is issued only after the store before it
+            // and the loop pays one shared-memory latency per store (in-kernel counters: 2.2k cycles per tile for these
+            // 16 stores in the edge network, 3.7k for the 32 of the projection launches).
+            float4 bq[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) bq[j] = *reinterpret_cast<const float4*>(bias + col0 + 4 * j);
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
               const uint32_t v0 = q == 0 ? va[4 * j] : vb[4 * j], v1 = q == 0 ? va[4 * j + 1] : vb[4 * j + 1];
               const uint32_t v2 = q == 0 ? va[4 * j + 2] : vb[4 * j + 2], v3 = q == 0 ? va[4 * j + 3] : vb[4 * j + 3];
-              const int cb = col0 + 4 * j;
               const uint32_t dst = stg + lane * 128 + ((j ^ (lane & 7)) << 4);
               if constexpr (q8 && wide)        // 8-bit per-hit projections: the raw int32 sums (they are added as integers)
                 st_shared_v4(dst, v0, v1, v2, v3);
               else if constexpr (q8) {
                 const float sc = a.q_sc[L];
-                st_shared_v4(dst, __float_as_uint(dequant(v0, sc, bias[cb])), __float_as_uint(dequant(v1, sc, bias[cb + 1])),
-                             __float_as_uint(dequant(v2, sc, bias[cb + 2])), __float_as_uint(dequant(v3, sc, bias[cb + 3])));
+                st_shared_v4(dst, __float_as_uint(dequant(v0, sc, bq[j].x)), __float_as_uint(dequant(v1, sc, bq[j].y)),
+                             __float_as_uint(dequant(v2, sc, bq[j].z)), __float_as_uint(dequant(v3, sc, bq[j].w)));
               } else
-              st_shared_v4(dst, __float_as_uint(__uint_as_float(v0) + bias[cb]), __float_as_uint(__uint_as_float(v1) + bias[cb + 1]),
-                           __float_as_uint(__uint_as_float(v2) + bias[cb + 2]), __float_as_uint(__uint_as_float(v3) + bias[cb + 3]));
+              st_shared_v4(dst, __float_as_uint(__uint_as_float(v0) + bq[j].x), __float_as_uint(__uint_as_float(v1) + bq[j].y),
+                           __float_as_uint(__uint_as_float(v2) + bq[j].z), __float_as_uint(__uint_as_float(v3) + bq[j].w));
             }
             EP_ACC(7);
             fence_async_smem();                    // generic-proxy writes -> async proxy (TMA)
@@ -846,9 +889,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
           const int q = wide ? qq : (qq < rep1 * nc1 ? qq % (nc1 > 0 ? nc1 : 1) : qq - (rep1 - 1) * nc1);
           const uint32_t ws = w_cnt % NSW, wn = w_cnt / NSW;
           mbar_wait(smem_u32(&bars->w_empty[ws]), (wn & 1) ^ 1);
-          if (ETX_EXP(a, 2)) { mbar_arrive(smem_u32(&bars->w_full[ws])); continue; }
+          if (ETX_EXP(a, 2)) { mbar_arrive(smem_u32(&bars->w_full[ws])); if (NMW == 2) st_release_shared(smem_u32(&bars->w_issued), w_cnt + 1); continue; }
           mbar_expect_tx(smem_u32(&bars->w_full[ws]), kStageBytes);
           bulk_g2s(wring + ws * kStageBytes, a.wimg + (size_t)q * kStageBytes, kStageBytes, smem_u32(&bars->w_full[ws]));
+          if (NMW == 2) st_release_shared(smem_u32(&bars->w_issued), w_cnt + 1);
         }
       }
     }
@@ -864,20 +908,32 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
     for (uint32_t cnt = 0; cnt < total; ++cnt) {
       named_bar_sync(kBarEntry0 + cnt % NSA, kGatherThreads + 32);
       fence_async_smem();
-      if (lane == 0) mbar_arrive(smem_u32(&bars->a_full[cnt % NSA]));
+      if (lane == 0) {
+        mbar_arrive(smem_u32(&bars->a_full[cnt % NSA]));
+        if (NMW == 2) st_release_shared(smem_u32(&bars->a_produced), cnt + 1);
+      }
       __syncwarp();
     }
-  } else if (warp > kWarpMma) {
+  } else if (warp > kWarpMma && NMW == 1) {
     reg_dec<kRegCtl>();                          // idle warp that completes the control warpgroup
   } else {
-    // =========================== MMA issuer ===========================
+    // =========================== MMA issuers ===========================
     reg_dec<kRegCtl>();
     // Warp-uniform control flow: every lane waits on the barriers, one elected lane issues.  (Issuing
     // from a divergent `if (lane == 0)` region makes ptxas wrap every UTCHMMA in an election loop,
     // which left the tensor pipe idle half of the time.)
-    uint32_t w_cnt = 0, a_cnt = 0, g = 0;
+    // NMW == 2 (measured alternative, see NMW): the two tiles in flight have one issuer warp each (warp kWarpMma: slot 0,
+    // the control warpgroup's fourth warp: slot 1).  What the tiles share is counted: a weight stage is released by two
+    // arrivals (a stage only one tile uses is committed twice), the wide mode's operand entries likewise; the progress
+    // counters in Bars keep an issuer from waiting on a parity one ring revolution ahead.  The motivation: with
+    // everything else switched off (no MMAs, loads, stores or tensor-memory traffic: developer build, ETX_TC_EXP) the
+    // hand-shakes alone cost 4.3k cycles per tile -- one warp walks both tiles' chains of ~17 mbarrier waits (>= 90
+    // cycles each even when already complete), fences and commits.
+    const int mw = (warp == kWarpMma) ? 0 : 1;
+    const int ept = (a.n_add ? ((P == 2) ? 2 : 4) : 0) + nc1;      // operand-ring entries per tile
+    uint32_t w_base = 0, a_base = 0, g = 0;
     long long dt[6] = {0, 0, 0, 0, 0, 0};
-    const bool dbg = ETX_DBG(a);
+    const bool dbg = ETX_DBG(a) && mw == 0;
     long long t_start = dbg ? clock64() : 0, t0 = 0;
 #define DBG_T0() if (dbg) t0 = clock64()
 #define DBG_ACC(i) if (dbg) dt[i] += clock64() - t0
@@ -890,12 +946,14 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
        // ring (every hidden layer; a first layer of <= NSW/2 chunks); otherwise the loader streams the
        // layer once per tile.
        const bool shared_w = (l > 0) || share1;
-       const uint32_t w_cnt0 = w_cnt;              // first weight stage of this layer
        for (int sl = 0; sl < ns; ++sl, ++g) {
+        if (NMW == 2 && sl != mw) continue;         // the other issuer's tile
         const uint32_t b = (NSLOT == 2) ? (uint32_t)sl : (g & 1);
         const uint32_t hs = (NSLOT == 2) ? (uint32_t)sl : 0u;
-        if (shared_w) w_cnt = w_cnt0;
-        if (wide && sl == 1) a_cnt -= nch;          // second output half: the same operand entries again
+        uint32_t w_cnt = shared_w ? w_base : w_base + (uint32_t)(sl * nch);       // first weight stage this tile uses
+        uint32_t a_cnt = a_base + (wide ? 0u : (uint32_t)(sl * ept));             // first operand entry of this tile
+        // arrivals this issuer owes a weight stage: two complete it (one per issuer; both from the stage's only user)
+        const int n_wc = (NMW == 2) ? ((!shared_w || ns == 1) ? 2 : 1) : 1;
         DBG_T0();
         if (uacc[b] >= 1) mbar_wait(smem_u32(&bars->acc_free[b]), (uacc[b] - 1) & 1);   // epilogue done with acc[b]
         DBG_ACC(0);
@@ -906,6 +964,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
           for (int en = 0; en < NENT; ++en, ++a_cnt) {
             const uint32_t slot = a_cnt % NSA;
             DBG_T0();
+            if (NMW == 2) spin_until_above(smem_u32(&bars->a_produced), a_cnt);
             mbar_wait(smem_u32(&bars->a_full[slot]), (a_cnt / NSA) & 1);
             DBG_ACC(1);
             fence_async_smem();                  // gather warps' st.shared (generic proxy) -> tcgen05.cp (async proxy)
@@ -914,6 +973,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
 #pragma unroll
               for (int t = 0; t < TPE; ++t) {
                 const uint64_t sd = smem_desc(aring + slot * kStageBytes + t * kAtomBytes);
+                if (ETX_EXP(a, 128)) continue;     // timing experiment (wrong results): no tcgen05.cp of the addend
 #pragma unroll
                 for (int ks = 0; ks < 4; ++ks) tmem_cp_128x256b(d_tmem + (en * TPE + t) * 32 + ks * 8, sd + ks * 2);
               }
@@ -929,6 +989,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
           DBG_T0();
           if (l == 0) {
             slot = a_cnt % NSA;
+            if (NMW == 2) spin_until_above(smem_u32(&bars->a_produced), a_cnt);
             mbar_wait(smem_u32(&bars->a_full[slot]), (a_cnt / NSA) & 1);
             // The proxy fence that makes the gather warps' st.shared (generic proxy) visible to the
             // tensor core (async proxy) sits HERE, on the consumer side of the mbarrier: the writes are
@@ -942,14 +1003,16 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             DBG_ACC(2);
           }
           DBG_T0();
-          if (!shared_w || sl == 0) mbar_wait(smem_u32(&bars->w_full[ws]), wn & 1);   // shared: the pair's second tile finds it already there
+          if (NMW == 2) spin_until_above(smem_u32(&bars->w_issued), w_cnt);
+          if (NMW == 2 || !shared_w || sl == 0) mbar_wait(smem_u32(&bars->w_full[ws]), wn & 1);   // one issuer: the pair's second tile finds a shared stage already there
           DBG_ACC(3);
           tc_fence_after();
           DBG_T0();
           if (elect_one()) {
             const uint64_t wd = smem_desc(wring + ws * kStageBytes);          // weight tile (hi piece)
             const uint32_t accum0 = (c > 0 || (l == 0 && a.n_add)) ? 1u : 0u;
-            if (l == 0) {
+            if (ETX_EXP(a, 64)) {                  // timing experiment (wrong results): no MMAs, only the commits
+            } else if (l == 0) {
               const uint64_t ad = smem_desc(aring + slot * kStageBytes);      // gathered operand tile (hi piece)
 #pragma unroll
               for (int ks = 0; ks < 4; ++ks) {     // 4 MMA k-steps of 32 bytes inside the 128-byte atom
@@ -976,8 +1039,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
                 }
               }
             }
-            if (!shared_w || sl == ns - 1) tc_commit(smem_u32(&bars->w_empty[ws]));
-            if (l == 0 && (!wide || sl == 1)) tc_commit(smem_u32(&bars->a_empty[slot]));
+            if (NMW == 2 || !shared_w || sl == ns - 1) tc_commit(smem_u32(&bars->w_empty[ws]));   // one issuer: a shared stage is released after the pair's last tile
+            if (n_wc == 2) tc_commit(smem_u32(&bars->w_empty[ws]));
+            if (l == 0) tc_commit(smem_u32(&bars->a_empty[slot]));       // wide: the entry is released by both halves' arrivals
             if (c == nch - 1) tc_commit(smem_u32(&bars->acc_full[b]));
           }
           __syncwarp();
@@ -987,8 +1051,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
         ++uacc[b];
         if (l > 0) ++uhid[hs];
        }
-       if (shared_w) w_cnt = w_cnt0 + nch;
+       w_base += shared_w ? (uint32_t)nch : (uint32_t)(ns * nch);
       }
+      a_base += wide ? (uint32_t)ept : (uint32_t)(ns * ept);
     }
     if (dbg && lane == 0) {
       unsigned long long* o = a.dbg + (size_t)blockIdx.x * 32;

@@ -88,6 +88,16 @@ __device__ __forceinline__ void mbar_arrive_relaxed_warp(uint32_t bar, int lane)
   __syncwarp();
   if (lane == 0) mbar_arrive_relaxed(bar);
 }
+// Progress counters in shared memory: release store by the producer, acquire polling by the consumers.
+__device__ __forceinline__ void st_release_shared(uint32_t addr, uint32_t v) {
+  asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void spin_until_above(uint32_t addr, uint32_t v) {      // returns once [addr] > v
+  uint32_t x;
+  do {
+    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(x) : "r"(addr) : "memory");
+  } while (x <= v);
+}
 // Named barriers (bar.arrive does not block and does not wait for the caller's outstanding global loads).
 __device__ __forceinline__ void named_bar_arrive(uint32_t id, uint32_t count) {
   asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory");
