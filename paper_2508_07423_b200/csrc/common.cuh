@@ -116,6 +116,8 @@ constexpr int kBallotWords = 32;   // vote words (32 candidates each) the count 
 int launch_search_count(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
                         const int32_t* flags, int32_t* out_deg, int32_t* in_deg, uint32_t* ballots /*[n_hits][kBallotWords] or null*/,
                         cudaStream_t s);
+int launch_search_kmax_cap(const GraphArgs& a, int k_max, const int32_t* plane_ptr, const int32_t* hit_event, int32_t* flags,
+                           int32_t* out_deg, int32_t* in_deg, uint32_t* ballots, cudaStream_t s);
 int launch_exclusive_scan(int32_t* data /*[n+1], in place, data[n] = total*/, int n, int32_t* tmp, cudaStream_t s);
 int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
                        const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst,

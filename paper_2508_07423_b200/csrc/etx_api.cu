@@ -704,30 +704,41 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
   a.d = c->emb.dims[c->emb.n_layers]; a.gap = max_plane_gap; a.r2_max = r2_max;
   a.event_ptr = b->d_event_ptr; a.plane = b->d_plane; a.emb = d_emb;
 
-  {
-    ProfScope ps(c, ETX_K_GRAPH, s);
-    c->launches += launch_plane_index(a, w.plane_ptr, w.hit_event, w.flags, s);
-    if (k_max == 0) {
-      c->launches += launch_search_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_in_ptr, w.ballots, s);
-      c->launches += launch_exclusive_scan(g->d_row_ptr, b->n_hits + 1, w.scan_tmp, s);
-      c->launches += launch_exclusive_scan(g->d_in_ptr, b->n_hits + 1, w.scan_tmp, s);
-    } else {                                       // next row: capped search (graph_kmax.cu)
-      c->launches += launch_kmax_count(a, k_max, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, s);
-      c->launches += launch_exclusive_scan(g->d_row_ptr, b->n_hits + 1, w.scan_tmp, s);
+  // k_max > 0 on a 4-d embedding runs the tiled search too: a cap kernel clears the votes beyond the k_max nearest and
+  // the rest of the build is the hot path's (graph.cu); other dimensions, or a window with more candidates than kept vote
+  // words, use the one-warp-per-source kernels of graph_kmax.cu
+  bool kmax_tiled = k_max > 0 && a.d == 4 && w.ballots;
+  int32_t host[3] = {0, 0, 0};
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    {
+      ProfScope ps(c, ETX_K_GRAPH, s);
+      c->launches += launch_plane_index(a, w.plane_ptr, w.hit_event, w.flags, s);
+      if (k_max == 0 || kmax_tiled) {
+        c->launches += launch_search_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_in_ptr, w.ballots, s);
+        if (kmax_tiled)
+          c->launches += launch_search_kmax_cap(a, k_max, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_in_ptr, w.ballots, s);
+        c->launches += launch_exclusive_scan(g->d_row_ptr, b->n_hits + 1, w.scan_tmp, s);
+        c->launches += launch_exclusive_scan(g->d_in_ptr, b->n_hits + 1, w.scan_tmp, s);
+      } else {                                       // next row: capped search (graph_kmax.cu)
+        c->launches += launch_kmax_count(a, k_max, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, s);
+        c->launches += launch_exclusive_scan(g->d_row_ptr, b->n_hits + 1, w.scan_tmp, s);
+      }
     }
+    cudaMemcpyAsync(&host[0], w.flags, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+    cudaMemcpyAsync(&host[2], g->d_row_ptr + b->n_hits, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+    if (cudaStreamSynchronize(s) != cudaSuccess) return check_cuda(c, "etx_build_graph (count)");
+    if (etx_status st = check_cuda(c, "etx_build_graph (count)")) return st;
+    if (kmax_tiled && host[1] != 0) { kmax_tiled = false; continue; }   // a window longer than the kept vote words: redo
+    break;
   }
-  int32_t host[2] = {0, 0};
-  cudaMemcpyAsync(&host[0], w.flags, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
-  cudaMemcpyAsync(&host[1], g->d_row_ptr + b->n_hits, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
-  if (cudaStreamSynchronize(s) != cudaSuccess) return check_cuda(c, "etx_build_graph (count)");
-  if (etx_status st = check_cuda(c, "etx_build_graph (count)")) return st;
   if (host[0] & 1) return fail(c, ETX_ERR_INVALID, "malformed batch: event_ptr not monotone / plane id >= n_planes");
   if (host[0] & 2) return fail(c, ETX_ERR_UNSORTED, "hits of an event are not sorted by plane");
+  host[1] = host[2];
   g->n_edges = host[1];
   if (g->n_edges > g->edge_capacity)
     return fail(c, ETX_ERR_CAPACITY, "graph needs " + std::to_string(g->n_edges) + " edges, capacity " +
                                          std::to_string(g->edge_capacity));
-  if (k_max > 0) {
+  if (k_max > 0 && !kmax_tiled) {
     // the by-destination lists depend on which edges survived the cap: forward fill first, then in-degrees,
     // scan, and the incoming side from the capped edge list
     ProfScope ps(c, ETX_K_GRAPH, s);

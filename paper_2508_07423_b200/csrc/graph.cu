@@ -233,6 +233,96 @@ search_tile_count_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, con
   }
 }
 
+// Next row NEXT-2 on the tiled search (k_max > 0, d = 4; Algorithm 1): after the count pass a source
+// with more than k_max votes keeps its k_max nearest candidates by (d^2 in fp32, then hit index) -- the order of
+// graph_kmax.cu and of the oracle -- by CLEARING the other votes: the vote words then describe the capped graph and the scans,
+// the ballot fill pass and the in-list sort run unchanged.  One warp per hit, almost all of which leave at once (the thesis:
+// < 0.1 % of hits exceed k_max = 50); lane t owns vote word t (a window has at most kBallotWords = 32 words, else the
+// caller falls back to graph_kmax.cu: flags[1]).  <= 128 votes: their keys (d^2 bits : index) are compacted into a
+// per-warp shared-memory list and every lane ranks its keys against the list; more: the k_max-th smallest key by bitwise
+// bisection (64 counting sweeps over the lane's own word).  Dropped votes give their in-degree count back.
+constexpr int kCapListMax = 128;
+static_assert(kBallotWords <= 32, "one vote word per lane");
+
+__device__ __forceinline__ unsigned long long cap_key(float d2, int j) {
+  return ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned)j;   // d2 >= 0: the bit pattern is monotone
+}
+
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+search_kmax_cap_kernel(GraphArgs a, int k_max, const int32_t* __restrict__ plane_ptr, const int32_t* __restrict__ hit_event,
+                       int32_t* __restrict__ flags, int32_t* __restrict__ out_deg, int32_t* __restrict__ in_deg,
+                       uint32_t* __restrict__ ballots) {
+  if (flags[0] != 0) return;
+  __shared__ unsigned long long s_keys[kWarpsPerBlock][kCapListMax];
+  const int lane = threadIdx.x & 31;
+  const int n_warps = gridDim.x * kWarpsPerBlock;
+  const int L = a.n_planes;
+  const float4* __restrict__ emb4 = reinterpret_cast<const float4*>(a.emb);
+  unsigned long long* keys = s_keys[threadIdx.x >> 5];
+  for (int i = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5); i < a.n_hits; i += n_warps) {
+    const int total = out_deg[i];
+    if (total <= k_max) continue;
+    const int p = a.plane[i];                      // total > 0 implies p <= L - 2
+    const int32_t* pp = plane_ptr + (size_t)hit_event[i] * (L + 1);
+    const int j0 = pp[p + 1];
+    const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
+    const int j1 = pp[top + 1];
+    const int nw = (j1 - j0 + 31) >> 5;
+    if (nw > kBallotWords) {                       // some votes were not kept: the caller redoes the build with graph_kmax.cu
+      if (lane == 0) atomicOr(&flags[1], 1);
+      continue;
+    }
+    const float4 m = __ldg(emb4 + i);
+    const unsigned long long n01 = pack2(-m.x, -m.y), n23 = pack2(-m.z, -m.w);
+    const unsigned word = lane < nw ? ballots[(size_t)i * kBallotWords + lane] : 0u;
+    const int jw = j0 + lane * 32;                 // first candidate of this lane's word
+    unsigned keep = word;                          // votes that survive the cap
+    if (total <= kCapListMax) {
+      // short list: every lane writes its votes' keys behind the votes of the lanes before it (ascending index = ascending slot)
+      int off = __popc(word);
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(kFull, off, o);
+        if (lane >= o) off += t;
+      }
+      off -= __popc(word);
+      for (unsigned w = word; w; w &= w - 1) {
+        const int bit = __ffs(w) - 1;
+        keys[off++] = cap_key(dist2_d4(n01, n23, __ldg(emb4 + jw + bit)), jw + bit);
+      }
+      __syncwarp();
+      for (unsigned w = word; w; w &= w - 1) {
+        const int bit = __ffs(w) - 1;
+        const unsigned long long mine = cap_key(dist2_d4(n01, n23, __ldg(emb4 + jw + bit)), jw + bit);
+        int rank = 0;
+        for (int q = 0; q < total; ++q) rank += keys[q] < mine;
+        if (rank >= k_max) keep &= ~(1u << bit);
+      }
+      __syncwarp();
+    } else {
+      unsigned long long thr = 0ull;               // invariant: thr <= the k_max-th smallest key
+      for (int b = 63; b >= 0; --b) {
+        const unsigned long long cand = thr | (1ull << b);
+        int below = 0;
+        for (unsigned w = word; w; w &= w - 1) {
+          const int bit = __ffs(w) - 1;
+          below += cap_key(dist2_d4(n01, n23, __ldg(emb4 + jw + bit)), jw + bit) < cand;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) below += __shfl_xor_sync(kFull, below, o);
+        if (below < k_max) thr = cand;             // fewer than k_max keys below cand: the k_max-th one is >= cand
+      }
+      for (unsigned w = word; w; w &= w - 1) {
+        const int bit = __ffs(w) - 1;
+        if (cap_key(dist2_d4(n01, n23, __ldg(emb4 + jw + bit)), jw + bit) > thr) keep &= ~(1u << bit);
+      }
+    }
+    for (unsigned w = word & ~keep; w; w &= w - 1) atomicSub(&in_deg[jw + __ffs(w) - 1], 1);
+    if (lane < nw && keep != word) ballots[(size_t)i * kBallotWords + lane] = keep;
+    if (lane == 0) out_deg[i] = k_max;
+  }
+}
+
 // Fill pass for d = 4: one warp per source expands its vote words into edges (ascending candidate index, so the CSR is
 // the same unique array) and drops each edge id into its destination's list; words past kBallotWords are re-tested.
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
@@ -421,6 +511,13 @@ int launch_search_count(const GraphArgs& a, const int32_t* plane_ptr, const int3
   }
   launch_search<0>(a, plane_ptr, hit_event, flags, out_deg, in_deg, nullptr, nullptr, nullptr, nullptr,
                    nullptr, nullptr, s);
+  return 1;
+}
+
+int launch_search_kmax_cap(const GraphArgs& a, int k_max, const int32_t* plane_ptr, const int32_t* hit_event, int32_t* flags,
+                           int32_t* out_deg, int32_t* in_deg, uint32_t* ballots, cudaStream_t s) {
+  search_kmax_cap_kernel<<<search_grid(a.n_hits), kWarpsPerBlock * 32, 0, s>>>(a, k_max, plane_ptr, hit_event, flags, out_deg,
+                                                                               in_deg, ballots);
   return 1;
 }
 

@@ -13,6 +13,9 @@
 // are emitted in ascending index through the same ballot / popc compaction, so the CSR is again the unique
 // ordered array.  The by-destination lists are built from the
 // capped edge list with integer counters, a cursor and graph.cu's per-segment sort (no second search).
+//
+// Since round 2 a 4-dimensional embedding takes the tiled search of graph.cu with a vote-clearing cap kernel
+// (search_kmax_cap_kernel); these kernels serve the other dimensions and windows longer than the kept vote words.
 #include "common.cuh"
 
 namespace etx {

@@ -91,3 +91,28 @@ def test_kmax_empty_and_capacity(B, c0):
     with pytest.raises(B.EtxError) as ei:                              # one edge short: reported, nothing written past it
         etx.etx_build_graph(db, torch.from_numpy(emb).to(etx.device), 1e9, 3, g, k_max=3)
     assert ei.value.status == B.ETX_ERR_CAPACITY and g.n_edges == len(s)
+
+
+def crowded_event(n_src, n_cand, seed):
+    """One event: n_src hits on plane 0 and n_cand hits on plane 1 (a candidate window of n_cand hits per source)."""
+    rng = np.random.default_rng(seed)
+    n = n_src + n_cand
+    batch = {"event_ptr": np.array([0, n], np.int32), "plane": np.r_[np.zeros(n_src), np.ones(n_cand)].astype(np.uint8)}
+    for k in ("r", "phi", "z", "x", "y"):
+        batch[k] = rng.normal(size=n).astype(np.float32)
+    emb = rng.integers(-2, 3, size=(n, 4)).astype(np.float32) * np.float32(0.5)      # lattice: plenty of exact ties
+    return batch, emb
+
+
+@pytest.mark.parametrize("n_cand,k_max", [(700, 50), (700, 200), (1500, 50), (1024, 7)])
+def test_kmax_many_votes_and_windows_longer_than_the_kept_vote_words(B, c0, n_cand, k_max):
+    """The tiled capped search (d = 4): more than 128 votes per source select by bisection instead of the ranked list
+    (700 candidates, everything inside the radius); a window of more than 32 vote words (1500 candidates) is not kept
+    whole by the count pass, so the build falls back to graph_kmax.cu's kernels.  Same arrays as the oracle either way."""
+    cfg, _, blob = c0
+    etx = B.Etx(B.make_desc(cfg, precision=0), blob)
+    batch, emb = crowded_event(40, n_cand, n_cand + k_max)
+    for r2 in (1e9, 1.1):
+        s = compare(B, etx, batch, emb, r2, 3, k_max)
+        if r2 > 1e8:
+            assert np.bincount(s, minlength=40)[:40].tolist() == [k_max] * 40
