@@ -195,7 +195,7 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------------------
 # reference arm: the oracle as it stands, on the host cores
 # --------------------------------------------------------------------------------------------------
-def oracle_events_per_s(cfg, event_ids):
+def oracle_events_per_s(cfg, event_ids, keep=None):
     from oracle import etx_oracle as orc
     batch = synth.generate_events(cfg, event_ids)
     blob = synth.generate_weights(cfg)
@@ -204,7 +204,30 @@ def oracle_events_per_s(cfg, event_ids):
     out = orc.run_path(batch, blob, layout, cfg.gnn_hidden, cfg.n_iter, synth.r2_max(cfg), cfg.max_plane_gap,
                        synth.NORM_CENTER, synth.NORM_SCALE)
     dt = time.perf_counter() - t
+    if keep is not None:
+        keep.update(batch=batch, out=out)
     return len(event_ids) / dt, dt, len(batch["r"]), len(out["src"])
+
+
+CDF_AT = [1e-7, 1e-6, 1e-5, 1e-4, 1e-3, 1e-2, 2e-2, 5e-2]
+
+
+def compare_with_oracle(gpu, ora):
+    """End-to-end comparison of one GPU run with the oracle's on the same events (reading Q16): the edge sets
+    (symmetric difference: the two embeddings decide pairs near the radius differently) and the score error on the common edges
+    with its CDF and the oracle's score histogram (reading Q14)."""
+    n = int(max(gpu["src"].max(initial=0), gpu["dst"].max(initial=0), ora["src"].max(initial=0), ora["dst"].max(initial=0))) + 1
+    kg = gpu["src"].astype(np.int64) * n + gpu["dst"]
+    ko = ora["src"].astype(np.int64) * n + ora["dst"]
+    common, ig, io = np.intersect1d(kg, ko, assume_unique=True, return_indices=True)
+    d = np.abs(gpu["scores"][ig].astype(np.float64) - np.asarray(ora["scores"], np.float64)[io])
+    hist, _ = np.histogram(np.asarray(ora["scores"], np.float64), bins=10, range=(0.0, 1.0))
+    return {"edges_gpu": int(len(kg)), "edges_oracle": int(len(ko)), "common": int(len(common)),
+            "only_gpu": int(len(kg) - len(common)), "only_oracle": int(len(ko) - len(common)),
+            "score_err_on_common": {"max": float(d.max(initial=0.0)), "p99": float(np.quantile(d, 0.99)) if len(d) else 0.0,
+                                    "median": float(np.median(d)) if len(d) else 0.0},
+            "score_err_cdf": {f"{t:g}": float(np.mean(d <= t)) if len(d) else 1.0 for t in CDF_AT},
+            "oracle_score_hist_0_to_1_by_0.1": [float(x) / max(len(ko), 1) for x in hist]}
 
 
 def oracle_single_thread(config: str):
@@ -531,12 +554,30 @@ def run_ours(args):
                                        "6 H^2 per edge (first layer factorised; the per-hit part runs in edge_proj)")}})
 
     # ---- CPU baseline: the oracle on a bounded sample, rank 0, N=1 only
-    cpu = None
+    cpu, parity = None, None
     if world == 1 and not args.no_cpu_baseline:
         from oracle import etx_oracle as orc
         _, dt1, _, _ = oracle_events_per_s(cfg, [0])
         n_s = int(min(32, max(2, round(15.0 / max(dt1, 1e-3)))))
-        v, dt, nh, ne = oracle_events_per_s(cfg, list(range(n_s)))
+        kept = {}
+        v, dt, nh, ne = oracle_events_per_s(cfg, list(range(n_s)), keep=kept)
+        # parity on the same sample, end to end (the GPU's own embedding and graph): every config / mode that is benched
+        # carries its comparison with the oracle in the line
+        gpu_s = binding.run_path(etx, kept["batch"], r2, gap, edge_capacity=int(nh * (cfg.target_degree * 1.25 + 2)))
+        parity = {"sample": f"first {n_s} events of {args.config}, end to end (GPU embedding and graph) against the oracle",
+                  "note": "the gate is defined on identical graphs (tests/, profiles/r02_parity.md); end to end the few edges only one "
+                          "side has (pairs within 1e-5 of the radius) also move the scores of their neighbours, which is what the "
+                          "maximum shows when only_gpu + only_oracle > 0",
+                  "gate": {synth.PREC_BF16: 2e-2, synth.PREC_INT8: None}.get(int(etx.desc.precision), 1e-4),
+                  **compare_with_oracle(gpu_s, kept["out"])}
+        if H == 128 and int(etx.desc.precision) != synth.PREC_FP32:
+            # reading Q16's report: the same events with a bf16 EMBEDDING (etx_embed_bf16) -- which edges change, and the
+            # score error on the edges both graphs have
+            gpu_b = binding.run_path(etx, kept["batch"], r2, gap, edge_capacity=int(nh * (cfg.target_degree * 1.25 + 2) * 2),
+                                     embed="etx_embed_bf16")
+            next_rows["bf16_embedding_end_to_end"] = {
+                "note": "report only (reading Q16): the step with etx_embed_bf16 instead of the 3xTF32 embedding, same radius",
+                **compare_with_oracle(gpu_b, kept["out"])}
         cpu = {"value": v, "unit": "events/s", "cores": orc.n_threads(), "kind": "oracle",
                "sample": f"first {n_s} events of {args.config} ({nh} hits, {ne} edges) in {dt:.1f} s",
                "note": "the oracle is deliberately unoptimised (per-neuron loops, double accumulators, no BLAS/SIMD, OpenMP "
@@ -552,7 +593,7 @@ def run_ours(args):
                    "mean_out_degree": E / max(N, 1), "r2_max": r2, "hits_per_s": world * N / (ms_step * 1e-3),
                    "l2": "state larger than L2 (edge encodings %.1f GB), no flush needed" % (E * H * 4 / 1e9),
                    "parallelism": "events sharded across GPUs, no collective" if world > 1 else "single GPU"},
-        "roofline": roof, "cpu_baseline": cpu,
+        "roofline": roof, "cpu_baseline": cpu, "parity": parity,
         "e2e": {"value": aggregate_events_per_s(world, n_ev, e2e_ms), "unit": "events/s", "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms},
         "gpu_launches": int(launches), "clocks": clk.summary(), "stages": stages, "next_rows": next_rows}))

@@ -117,6 +117,14 @@ etx_status etx_set_workspace(etx_ctx* ctx, void* d_workspace, size_t bytes);
 /* a0+a1: d_emb[n_hits, emb_dim] fp32 row-major = embedding MLP of ((r,phi,z) - center) / scale.   */
 etx_status etx_embed(etx_ctx* ctx, const etx_batch* batch, float* d_emb, void* stream);
 
+/* Report-only variant of etx_embed (reading Q16; BASELINE.json's config 3 says "embedding ... in bf16"): the
+ * embedding MLP with its hidden layers' operands rounded to bf16 (round to nearest even), one tcgen05.mma.kind::f16 per
+ * K-step, fp32 accumulation; the 3-input first layer and the narrow output layer stay fp32 FMA chains as in etx_embed.
+ * The path itself always embeds in 3xTF32 because the embedding decides graph edges; this call exists so that bench.py
+ * can report what a bf16 embedding does to the edge set (thesis analogue: +5-10 % edges after INT8 calibration).
+ * Needs 128-wide hidden layers (ETX_ERR_INVALID otherwise).                                                           */
+etx_status etx_embed_bf16(etx_ctx* ctx, const etx_batch* batch, float* d_emb, void* stream);
+
 /* Next row (embedding part): the embedding MLP of etx_embed with INT8 weights and
  * activations, static post-training quantisation with the symmetric scheme of Eqs. 4.31-4.33:
  * S = alpha / 127, x_q = clip(round(x / S), -127, 127) (round half to even, fp32 division).  Per layer the input

@@ -20,7 +20,7 @@ ETX_MAX_MLP_LAYERS = 8
 ETX_OK, ETX_ERR_INVALID, ETX_ERR_CAPACITY, ETX_ERR_CUDA, ETX_ERR_UNSORTED, ETX_ERR_NOMEM = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["etx_weight_count", "etx_create", "etx_destroy", "etx_last_error", "etx_workspace_bytes",
-           "etx_set_workspace", "etx_embed", "etx_embed_int8", "etx_build_graph", "etx_gnn_forward", "etx_edge_scores",
+           "etx_set_workspace", "etx_embed", "etx_embed_bf16", "etx_embed_int8", "etx_build_graph", "etx_gnn_forward", "etx_edge_scores",
            "etx_infer_host", "etx_launch_count", "etx_profile_enable", "etx_profile_read", "etx_build_tracks",
            "etx_build_triplets", "etx_triplet_weight_count", "etx_set_triplet_classifiers", "etx_triplet_scores",
            "etx_triplet_tracks_workspace_bytes", "etx_build_tracks_from_triplets", "etx_set_int8_ranges",
@@ -105,6 +105,8 @@ def load_library():
         lib.etx_set_workspace.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
         lib.etx_embed.restype = C.c_int
         lib.etx_embed.argtypes = [C.c_void_p, C.POINTER(Batch), C.c_void_p, C.c_void_p]
+        lib.etx_embed_bf16.restype = C.c_int
+        lib.etx_embed_bf16.argtypes = [C.c_void_p, C.POINTER(Batch), C.c_void_p, C.c_void_p]
         lib.etx_embed_int8.restype = C.c_int
         lib.etx_embed_int8.argtypes = [C.c_void_p, C.POINTER(Batch), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
         lib.etx_build_graph.restype = C.c_int
@@ -276,6 +278,12 @@ class Etx:
         self._check(self.lib.etx_embed(self.handle, C.byref(batch.c), _ptr(emb), self._stream()))
         return emb
 
+    def etx_embed_bf16(self, batch: DeviceBatch, emb: Optional[torch.Tensor] = None) -> torch.Tensor:
+        if emb is None:
+            emb = torch.empty(batch.n_hits, self.emb_dim, dtype=torch.float32, device=self.device)
+        self._check(self.lib.etx_embed_bf16(self.handle, C.byref(batch.c), _ptr(emb), self._stream()))
+        return emb
+
     def etx_embed_int8(self, batch: DeviceBatch, act_alpha, emb: Optional[torch.Tensor] = None) -> torch.Tensor:
         if emb is None:
             emb = torch.empty(batch.n_hits, self.emb_dim, dtype=torch.float32, device=self.device)
@@ -411,13 +419,14 @@ def pinned_host_batch(batch: Dict[str, np.ndarray]) -> Dict[str, torch.Tensor]:
 
 
 def run_path(etx: Etx, batch: Dict[str, np.ndarray], r2_max: float, max_plane_gap: int,
-             edge_capacity: Optional[int] = None, graph_override=None) -> Dict[str, np.ndarray]:
-    """Convenience for tests: the four calls in order on device-resident inputs, results to numpy."""
+             edge_capacity: Optional[int] = None, graph_override=None, embed: str = "etx_embed") -> Dict[str, np.ndarray]:
+    """Convenience for tests: the four calls in order on device-resident inputs, results to numpy.  `embed` names the
+    embedding call (etx_embed, or the report-only etx_embed_bf16)."""
     dev = etx.device
     db = DeviceBatch(batch, dev)
     cap = edge_capacity if edge_capacity is not None else max(64 * db.n_hits, 1024)
     etx.ensure_workspace(db.n_events, db.n_hits, cap)
-    emb = etx.etx_embed(db)
+    emb = getattr(etx, embed)(db)
     g = DeviceGraph(db.n_hits, cap, dev)
     E = etx.etx_build_graph(db, emb, r2_max, max_plane_gap, g)
     H = int(etx.desc.gnn_hidden)

@@ -81,6 +81,7 @@ struct etx_ctx {
   float emb_sw[etx::kMaxLayers] = {0};  // their per-layer scales max|W| / 127
   // the same embedding for the tensor-core INT8 kernel (128-wide hidden layers): kind::i8 image of the hidden layers,
   // and the 3-input first layer / the narrow last layer as integer codes held in floats (k-major)
+  unsigned char* d_emb_bf16_img = nullptr;  // single-pass bf16 image of the embedding's hidden layers (etx_embed_bf16)
   unsigned char* d_embq_img = nullptr;
   float* d_embq_f = nullptr;            // [3][128] first-layer codes, then [128][n_out] last-layer codes
   // next row: the two triplet classifiers (articulations, elbows), set by etx_set_triplet_classifiers
@@ -152,6 +153,7 @@ struct MlpArgs {
   // output: mode 0 store, 1 residual add (out = res + y; res may alias out), 2 small-N linear,
   // 3 small-N sigmoid
   int out_mode = 0; float* out = nullptr; const float* res = nullptr; int out_ld = 0;
+  int emb_mode = -1;          // out_mode 2 (embedding): tensor-core mode to run instead of the default 3xTF32 (etx_embed_bf16)
   float q_sa0 = 1.f; float q_sc[kMaxLayers] = {0}; float q_sn[kMaxLayers] = {0};   // ETX_PREC_INT8 scales (see TcArgs)
 };
 int launch_mlp_simt(const MlpArgs& a, cudaStream_t s);

@@ -243,7 +243,7 @@ int run_mlp(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   return n;
 }
 int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
-  if (c->desc.precision == ETX_PREC_FP32 || !a.mlp.wimg) return launch_mlp_simt(a, s);
+  if ((c->desc.precision == ETX_PREC_FP32 && a.emb_mode < 0) || !a.mlp.wimg) return launch_mlp_simt(a, s);
   TcArgs t;
   t.n_rows = a.n_rows; t.n_seg = a.n_seg; t.K0 = a.mlp.dims[0];
   for (int i = 0; i < 3; ++i) t.seg[i] = a.seg[i];
@@ -264,7 +264,7 @@ int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   }
   // the embedding (narrow linear output, out_mode 2) always runs the 3xTF32 kernel, whatever the GNN's mode:
   // its result decides graph edges (DESIGN.md section 5 "Embedding on the tensor cores")
-  const int mode = (a.out_mode == 2) ? (int)ETX_PREC_TF32X3 : (int)c->desc.precision;
+  const int mode = (a.out_mode == 2) ? (a.emb_mode >= 0 ? a.emb_mode : (int)ETX_PREC_TF32X3) : (int)c->desc.precision;
   t.w_last = a.mlp.Wt[a.mlp.n_layers - 1];         // [H][1] == [H]
   if (mode == ETX_PREC_INT8) {
     if (a.out_mode == 3) { if (!a.mlp.wq_last) return -1; t.w_last = a.mlp.wq_last; }
@@ -462,6 +462,17 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
       return fail(nullptr, ETX_ERR_CUDA, msg);
     }
   }
+  if (mlps[0].n_layers >= 3 && mlps[0].dims[1] == 128) {
+    // report-only bf16 embedding (etx_embed_bf16, reading Q16): single-pass bf16 image of layers 2..L-1
+    std::vector<unsigned char> bimg;
+    append_wimg(bimg, mlps[0], h_weights, 1, 0, mlps[0].n_layers - 1, ETX_PREC_BF16);
+    if (cudaMalloc(&c->d_emb_bf16_img, bimg.size()) != cudaSuccess ||
+        cudaMemcpy(c->d_emb_bf16_img, bimg.data(), bimg.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+      const std::string msg = std::string("bf16 embedding image upload failed: ") + cudaGetErrorString(cudaGetLastError());
+      etx_destroy(c);
+      return fail(nullptr, ETX_ERR_CUDA, msg);
+    }
+  }
   if (desc->precision != ETX_PREC_FP32) {
     // tensor-core weight images: edge encoder, node/edge networks, classifier (first-layer input a multiple of
     // the chunk); node encoder and a 128-wide embedding with >= 2 hidden layers from their second layer on (their
@@ -532,6 +543,7 @@ etx_status etx_destroy(etx_ctx* c) {
   if (c->d_wimg) cudaFree(c->d_wimg);
   if (c->d_emb_wq) cudaFree(c->d_emb_wq);
   if (c->d_embq_img) cudaFree(c->d_embq_img);
+  if (c->d_emb_bf16_img) cudaFree(c->d_emb_bf16_img);
   if (c->d_embq_f) cudaFree(c->d_embq_f);
   if (c->d_trip_weights) cudaFree(c->d_trip_weights);
   if (c->d_trip_wimg) cudaFree(c->d_trip_wimg);
@@ -628,6 +640,30 @@ etx_status etx_embed(etx_ctx* c, const etx_batch* b, float* d_emb, void* stream)
     c->launches += run_mlp(c, a, (cudaStream_t)stream);
   }
   return check_cuda(c, "etx_embed");
+}
+
+etx_status etx_embed_bf16(etx_ctx* c, const etx_batch* b, float* d_emb, void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (etx_status st = check_batch(c, b)) return st;
+  if (b->n_hits > 0 && !d_emb) return fail(c, ETX_ERR_INVALID, "d_emb is NULL");
+  if (!c->d_emb_bf16_img) return fail(c, ETX_ERR_INVALID, "the bf16 embedding needs 128-wide hidden layers (two or more)");
+  cudaSetDevice(c->device);
+  MlpArgs a;
+  a.n_rows = b->n_hits;
+  a.n_seg = 0;
+  a.feat[0] = b->d_r; a.feat[1] = b->d_phi; a.feat[2] = b->d_z;
+  for (int i = 0; i < 3; ++i) { a.fc[i] = c->desc.norm_center[i]; a.fs[i] = c->desc.norm_scale[i]; }
+  a.mlp = c->emb;
+  a.mlp.wimg = c->d_emb_bf16_img;
+  a.emb_mode = ETX_PREC_BF16;
+  a.out_mode = 2;
+  a.out = d_emb;
+  a.out_ld = c->emb.dims[c->emb.n_layers];
+  {
+    ProfScope ps(c, ETX_K_EMBED, (cudaStream_t)stream);
+    c->launches += run_mlp(c, a, (cudaStream_t)stream);
+  }
+  return check_cuda(c, "etx_embed_bf16");
 }
 
 etx_status etx_embed_int8(etx_ctx* c, const etx_batch* b, const float* h_act_alpha, int32_t n_alpha, float* d_emb,

@@ -1141,8 +1141,9 @@ int launch_mlp_tc(const TcArgs& a_in, int mode, int sm_count, cudaStream_t s) {
   if (a.w1) {                                    // first-layer operand computed from 3 features (node encoder, embedding)
     if (a.n_add != 0 || a.n_seg != 0 || a.K0 != HW || !a.b1 || !a.feat[0] || !a.feat[1] || !a.feat[2]) return -1;
     if (a.out_mode == 2) {                       // narrow linear output (embedding): 3xTF32, or the INT8 embedding
-      if ((mode != ETX_PREC_TF32X3 && mode != ETX_PREC_INT8) || a.n_out < 1 || a.n_out > 8 || a.n_layers < 2) return -1;
+      if ((mode != ETX_PREC_TF32X3 && mode != ETX_PREC_INT8 && mode != ETX_PREC_BF16) || a.n_out < 1 || a.n_out > 8 || a.n_layers < 2) return -1;
       if (mode == ETX_PREC_INT8) return launch_mode<ETX_PREC_INT8, 3>(a, sm_count, s);
+      if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, 3>(a, sm_count, s);     // report-only (etx_embed_bf16)
       return launch_mode<ETX_PREC_TF32X3, 3>(a, sm_count, s);
     }
     if (mode == ETX_PREC_TF32X3) return launch_mode<ETX_PREC_TF32X3, 2>(a, sm_count, s);

@@ -425,3 +425,41 @@ def test_tc_embedding_shapes_and_ragged_tail(B, widths, prec):
         fe, _ = orc.features(batch, synth.NORM_CENTER, synth.NORM_SCALE)
         ora = orc.mlp(fe, spec.dims, blob, spec.offset)
         assert np.abs(out[:n].cpu().numpy().astype(np.float64) - ora).max() <= 2e-6
+
+
+def test_bf16_embedding_report_entry_point(B, c1, c1_oracle):
+    """etx_embed_bf16 (report-only, reading Q16): hidden-layer operands rounded to bf16, fp32 accumulation.  Checked against
+    the same arithmetic written with torch CPU ops (bf16 round-to-nearest-even operands, float64 accumulation) and against
+    the fp32 oracle embedding: close to both, and genuinely different from the fp32 one."""
+    cfg, batch, blob = c1
+    etx = make_etx(B, cfg, blob, precision=synth.PREC_BF16X3)
+    db = B.DeviceBatch(batch, etx.device)
+    etx.ensure_workspace(db.n_events, db.n_hits, 64 * db.n_hits)
+    got = etx.etx_embed_bf16(db).cpu().numpy().astype(np.float64)
+    lay = {s.name: (s.dims, s.offset) for s in synth.model_layout(cfg)}
+    dims, off = lay["emb"]
+    f = np.stack([(batch[k].astype(np.float32) - np.float32(synth.NORM_CENTER[i])) / np.float32(synth.NORM_SCALE[i])
+                  for i, k in enumerate(("r", "phi", "z"))], axis=1)
+    x = torch.from_numpy(f).double()
+    o = off
+    n_l = len(dims) - 1
+    for l in range(n_l):
+        fi, fo = dims[l], dims[l + 1]
+        W = torch.from_numpy(blob[o:o + fi * fo].reshape(fo, fi).copy()); o += fi * fo
+        b = torch.from_numpy(blob[o:o + fo].copy()).double(); o += fo
+        if 0 < l < n_l - 1:                            # tensor-core layers: bf16 operands
+            x = x.float().bfloat16().double() @ W.bfloat16().double().T + b
+        else:
+            x = x @ W.double().T + b
+        if l < n_l - 1:
+            x = torch.relu(x).float().double()         # every layer output is stored in fp32
+    want = x.numpy()
+    assert np.abs(got - want).max() <= 2e-3
+    ref = c1_oracle["emb"].astype(np.float64)
+    d = np.abs(got - ref).max()
+    assert 1e-5 < d <= 3e-2
+    # a context without tensor-core images of the embedding refuses
+    cfg0, batch0, blob0 = synth.CONFIGS["c0"], synth.generate_events(synth.CONFIGS["c0"]), synth.generate_weights(synth.CONFIGS["c0"])
+    etx0 = make_etx(B, cfg0, blob0)
+    with pytest.raises(B.EtxError):
+        etx0.etx_embed_bf16(B.DeviceBatch(batch0, etx0.device))
