@@ -377,4 +377,83 @@ void orc_wcc(int64_t n_hits, int64_t n_edges, const int32_t* src, const int32_t*
   for (int64_t i = 0; i < n_hits; ++i) labels[i] = uf_find(parent, (int32_t)i);
 }
 
+// ---- next row: the GNN's MLPs in FP8 (e4m3: 1 sign, 4 exponent, 3 mantissa bits, bias 7, no
+//      infinities, largest finite value 448, subnormals down to 2^-9) with static per-tensor scales.  The thesis treats INT8
+//      only (Eqs. 4.31-4.33; "the quantization of the GNN holds the most potential"); this is the same
+//      symmetric per-tensor scheme with the integer grid replaced by the e4m3 grid (reading Q26):
+//        S = alpha / 448 (alpha mapped to the largest e4m3 value, as P:1487 maps it to 127),
+//        x_q = e4m3( clip( x * fl(1 / S), -448, 448 ) ), round to nearest, ties to even (the scaling is ONE rounded fp32
+//        multiplication by the rounded reciprocal, the arithmetic of hardware FP8 pipelines; every x_q is decided in that
+//        precision on both sides),
+//        y_o = float(sum_k x_q[k] w_q[o][k]) * (S_a S_w) + b_o ;  ReLU on hidden layers, biases fp32.
+//      The products of two e4m3 values and their sum over <= 512 terms are exact in double, so the oracle's sum is the
+//      exact one, rounded to fp32 once; the tensor core accumulates in fp32, so the GPU is compared within a tolerance.
+static inline float e4m3_round(float t) {                // nearest e4m3 value of a finite t, ties to even, saturating
+  const float a = std::fabs(t);
+  if (!(a < 448.0f)) return t < 0.0f ? -448.0f : 448.0f;
+  int e;
+  std::frexp(a, &e);                                     // a = m 2^e, m in [0.5, 1)  ->  floor(log2 a) = e - 1
+  int le = (a == 0.0f) ? -6 : e - 1;
+  if (le < -6) le = -6;                                  // subnormal range: spacing 2^-9
+  const float ulp = std::ldexp(1.0f, le - 3);            // 3 mantissa bits
+  const float r = std::nearbyintf(a / ulp) * ulp;        // power-of-two scaling is exact; nearbyint rounds half to even
+  return t < 0.0f ? -r : r;
+}
+
+void orc_quantize_fp8(int64_t n, const float* x, float alpha, float* values, float* scale_out) {
+  const float S = alpha / 448.0f;
+  const float rS = 1.0f / S;
+  if (scale_out) *scale_out = S;
+  for (int64_t i = 0; i < n; ++i) values[i] = e4m3_round(x[i] * rS);
+}
+
+void orc_mlp_fp8(int64_t n, int32_t n_layers, const int32_t* dims, const float* w, const float* in,
+                 const float* act_alpha /*[n_layers]*/, float* out) {
+  int32_t maxw = 0;
+  for (int l = 0; l <= n_layers; ++l) maxw = dims[l] > maxw ? dims[l] : maxw;
+  std::vector<std::vector<float>> wq(n_layers);          // e4m3 VALUES of the scaled weights
+  std::vector<float> sw(n_layers);
+  {
+    const float* p = w;
+    for (int l = 0; l < n_layers; ++l) {
+      const int64_t cnt = (int64_t)dims[l] * dims[l + 1];
+      float m = 0.0f;
+      for (int64_t i = 0; i < cnt; ++i) m = std::fabs(p[i]) > m ? std::fabs(p[i]) : m;
+      sw[l] = m / 448.0f;
+      const float rs = 1.0f / sw[l];
+      wq[l].resize(cnt);
+      for (int64_t i = 0; i < cnt; ++i) wq[l][i] = e4m3_round(p[i] * rs);
+      p += cnt + dims[l + 1];
+    }
+  }
+#pragma omp parallel
+  {
+    std::vector<float> a(maxw), b(maxw), aq(maxw);
+#pragma omp for schedule(static)
+    for (int64_t row = 0; row < n; ++row) {
+      for (int i = 0; i < dims[0]; ++i) a[i] = in[row * dims[0] + i];
+      const float* p = w;
+      for (int l = 0; l < n_layers; ++l) {
+        const int fi = dims[l], fo = dims[l + 1];
+        const float* bias = p + (int64_t)fi * fo;
+        const float sa = act_alpha[l] / 448.0f;
+        const float rsa = 1.0f / sa;
+        const float sc = sa * sw[l];
+        for (int i = 0; i < fi; ++i) aq[i] = e4m3_round(a[i] * rsa);
+        for (int o = 0; o < fo; ++o) {
+          double acc = 0.0;                              // exact: products have <= 8 significant bits, <= 512 terms
+          for (int i = 0; i < fi; ++i) acc += (double)aq[i] * (double)wq[l][(int64_t)o * fi + i];
+          const float prod = (float)acc * sc;
+          float v = prod + bias[o];
+          if (l < n_layers - 1 && !(v > 0.0f)) v = 0.0f;
+          b[o] = v;
+        }
+        a.swap(b);
+        p = bias + fo;
+      }
+      for (int o = 0; o < dims[n_layers]; ++o) out[row * dims[n_layers] + o] = a[o];
+    }
+  }
+}
+
 }  // extern "C"

@@ -98,6 +98,31 @@ def mlp_int8(x: np.ndarray, dims: Sequence[int], blob: np.ndarray, offset: int, 
     return out
 
 
+def quantize_fp8(x: np.ndarray, alpha: float):
+    """Next row (NEXT-3, FP8; DESIGN reading Q26): S = alpha / 448, value = e4m3(clip(x * fl(1/S), -448, 448)), round to
+    nearest even.  Returns (e4m3 values as float32 -- multiply by S to de-quantise --, S)."""
+    x = _f32(x).ravel()
+    vals = np.empty(x.size, np.float32)
+    S = C.c_float(0.0)
+    lib().orc_quantize_fp8(C.c_int64(x.size), _p(x, C.c_float), C.c_float(alpha), _p(vals, C.c_float), C.byref(S))
+    return vals, float(S.value)
+
+
+def mlp_fp8(x: np.ndarray, dims: Sequence[int], blob: np.ndarray, offset: int, act_alpha: Sequence[float]) -> np.ndarray:
+    """The MLP chain with e4m3 weights and activations (static per-tensor scales, exact sums, fp32 de-quantisation and
+    biases); act_alpha[l] = calibrated range of layer l's input (the ranges of the INT8 row: a max observer)."""
+    x = _f32(x)
+    d = np.ascontiguousarray(dims, np.int32)
+    al = _f32(np.asarray(act_alpha, np.float32))
+    assert len(al) == len(d) - 1
+    n = x.shape[0]
+    out = np.empty((n, int(d[-1])), np.float32)
+    w = blob[offset:]
+    lib().orc_mlp_fp8(C.c_int64(n), C.c_int32(len(d) - 1), _p(d, C.c_int32), _p(w, C.c_float),
+                      _p(x, C.c_float), _p(al, C.c_float), _p(out, C.c_float))
+    return out
+
+
 def int8_calibration(x: np.ndarray, dims: Sequence[int], blob: np.ndarray, offset: int) -> np.ndarray:
     """Static PTQ calibration with a max observer: range of every layer's INPUT over the sample x,
     taken from the fp32 oracle MLP."""
@@ -289,6 +314,26 @@ def gnn_forward_int8(f_node, src, dst, n_iter: int, blob: np.ndarray, layout, ac
             off += dims[0] * dims[1] + dims[1]
             dims, al = dims[1:], al[1:]
         return mlp_int8(x, dims, blob, off, al)
+
+    h, e, logit = gnn_forward_steps(f_node, src, dst, n_iter, q_mlp, scatter_f32)
+    s = (1.0 / (1.0 + np.exp(-logit.astype(np.float64)))).astype(np.float32)
+    return h, e, logit, s
+
+
+def gnn_forward_fp8(f_node, src, dst, n_iter: int, blob: np.ndarray, layout, act_alpha: Dict[str, Sequence[float]]):
+    """NEXT-3 (GNN part) in FP8 e4m3: ``gnn_forward_int8`` with ``mlp_fp8`` in place of ``mlp_int8`` -- e4m3 values for every
+    layer's input and weight, fp32 state, fp32 sequential scatter, fp32 residual adds, the node encoder's first layer in
+    fp32; the same calibrated ranges.  Returns h^n, e^n, logits, scores."""
+    blob = _f32(blob)
+
+    def q_mlp(name, x):
+        dims, off = layout[name]
+        al = list(act_alpha[name])
+        if name == "node_enc":
+            x = _relu(mlp(x, dims[:2], blob, off))
+            off += dims[0] * dims[1] + dims[1]
+            dims, al = dims[1:], al[1:]
+        return mlp_fp8(x, dims, blob, off, al)
 
     h, e, logit = gnn_forward_steps(f_node, src, dst, n_iter, q_mlp, scatter_f32)
     s = (1.0 / (1.0 + np.exp(-logit.astype(np.float64)))).astype(np.float32)
