@@ -295,7 +295,7 @@ def run_ours(args):
     blob = synth.generate_weights(cfg)
     etx = binding.Etx(binding.make_desc(cfg, precision=args.precision if args.precision is not None else cfg.precision),
                       blob, device=local)
-    if int(etx.desc.precision) == synth.PREC_INT8:     # next row NEXT-3 as the whole step: needs the stored calibrated ranges
+    if int(etx.desc.precision) in (synth.PREC_INT8, synth.PREC_FP8):     # next row NEXT-3 as the whole step: needs the stored calibrated ranges
         etx.etx_set_int8_ranges(synth.int8_gnn_alpha(cfg))
     r2, gap, H = synth.r2_max(cfg), cfg.max_plane_gap, cfg.gnn_hidden
     N = len(batch["r"])
@@ -402,31 +402,34 @@ def run_ours(args):
             etx.ensure_workspace(db.n_events, N, cap, with_host_path=True)
 
     if not args.no_next_rows and H == 128:
-        # NEXT-3 (GNN part): the same graph through the INT8 GNN (ETX_PREC_INT8, tcgen05.mma.kind::i8) with the stored
-        # calibrated ranges; the default mode's scores of this run are the comparison
+        # NEXT-3 (GNN part): the same graph through the quantised GNNs -- INT8 (ETX_PREC_INT8, tcgen05.mma.kind::i8) and FP8 e4m3
+        # (ETX_PREC_FP8, kind::f8f6f4) -- with the stored calibrated ranges; the default mode's scores of this run are the comparison
         ref_scores = scores[:E].clone()
-        q = binding.Etx(binding.make_desc(cfg, precision=synth.PREC_INT8), blob, device=local)
-        q.etx_set_int8_ranges(synth.int8_gnn_alpha(cfg))
-        q.ensure_workspace(db.n_events, N, cap)
-        sc8 = torch.empty(cap, device=dev)
+        default_gnn_ms = sum(prof[k][0] for k in ("node_enc", "edge_enc", "scatter", "node_net", "edge_net", "edge_proj", "cls")) / args.steps
+        for row, qprec in (("gnn_int8", synth.PREC_INT8), ("gnn_fp8", synth.PREC_FP8)):
+            q = binding.Etx(binding.make_desc(cfg, precision=qprec), blob, device=local)
+            q.etx_set_int8_ranges(synth.int8_gnn_alpha(cfg))
+            q.ensure_workspace(db.n_events, N, cap)
+            sc8 = torch.empty(cap, device=dev)
 
-        def q_step():
-            q.etx_gnn_forward(db, g, enc)
-            q.etx_edge_scores(g, enc, sc8)
+            def q_step():
+                q.etx_gnn_forward(db, g, enc)
+                q.etx_edge_scores(g, enc, sc8)
 
-        q.profile_enable(True)
-        q.profile_read()
-        qms, _ = time3(q_step)
-        qprof = q.profile_read()
-        d8 = (sc8[:E] - ref_scores).abs()
-        next_rows["gnn_int8"] = {"ms": qms, "events_per_s": n_ev / (qms * 1e-3),
-                                 "default_mode_gnn_ms": sum(prof[k][0] for k in ("node_enc", "edge_enc", "scatter", "node_net", "edge_net", "edge_proj", "cls")) / args.steps,
-                                 "edge_net_ms_per_launch": qprof["edge_net"][0] / max(qprof["edge_net"][1], 1),
-                                 "stages_ms": {k: v[0] / 4 for k, v in qprof.items() if v[1]},
-                                 "score_err_vs_default_mode": {"max": float(d8.max()), "median": float(d8.median()),
-                                                               "p99": float(torch.quantile(d8[::16].float(), 0.99))},
-                                 "kept_edges_at_0.5": {"int8": int((sc8[:E] >= 0.5).sum()), "default": int((ref_scores >= 0.5).sum())}}
-        del q, sc8, ref_scores
+            q.profile_enable(True)
+            q.profile_read()
+            qms, _ = time3(q_step)
+            qprof = q.profile_read()
+            d8 = (sc8[:E] - ref_scores).abs()
+            next_rows[row] = {"ms": qms, "events_per_s": n_ev / (qms * 1e-3), "default_mode_gnn_ms": default_gnn_ms,
+                              "speed_vs_default_mode": default_gnn_ms / qms,
+                              "edge_net_ms_per_launch": qprof["edge_net"][0] / max(qprof["edge_net"][1], 1),
+                              "stages_ms": {k: v[0] / 4 for k, v in qprof.items() if v[1]},
+                              "score_err_vs_default_mode": {"max": float(d8.max()), "median": float(d8.median()),
+                                                            "p99": float(torch.quantile(d8[::16].float(), 0.99))},
+                              "kept_edges_at_0.5": {row[4:]: int((sc8[:E] >= 0.5).sum()), "default": int((ref_scores >= 0.5).sum())}}
+            del q, sc8
+        del ref_scores
 
     # ---- end to end through the host-buffer entry point
     host = binding.pinned_host_batch(batch)
@@ -519,11 +522,11 @@ def run_ours(args):
         peak = pk["bf16_tflops_sustained"]
         roof = {"bound": "tensor", "unit": "TFLOP/s", "peak": peak, "peak_source": f"{pk['source']} bf16 sustained"}
         dtype, passes = "bf16x3", 3
-    elif prec == synth.PREC_INT8:
+    elif prec in (synth.PREC_INT8, synth.PREC_FP8):
         peak = pk["bf16_tflops_sustained"] * 2.0
-        roof = {"bound": "tensor", "unit": "TOP/s", "peak": peak,
+        roof = {"bound": "tensor", "unit": "TOP/s" if prec == synth.PREC_INT8 else "TFLOP/s", "peak": peak,
                 "peak_source": f"{pk['source']} bf16 sustained x 2 (8-bit nominal ratio)"}
-        dtype, passes = "i8", 1
+        dtype, passes = ("i8" if prec == synth.PREC_INT8 else "f8e4m3"), 1
     else:
         peak = pk["bf16_tflops_sustained"]
         roof = {"bound": "tensor", "unit": "TFLOP/s", "peak": peak, "peak_source": f"{pk['source']} bf16 sustained"}
@@ -568,7 +571,7 @@ def run_ours(args):
                   "note": "the gate is defined on identical graphs (tests/, profiles/r02_parity.md); end to end the few edges only one "
                           "side has (pairs within 1e-5 of the radius) also move the scores of their neighbours, which is what the "
                           "maximum shows when only_gpu + only_oracle > 0",
-                  "gate": {synth.PREC_BF16: 2e-2, synth.PREC_INT8: None}.get(int(etx.desc.precision), 1e-4),
+                  "gate": {synth.PREC_BF16: 2e-2, synth.PREC_INT8: None, synth.PREC_FP8: None}.get(int(etx.desc.precision), 1e-4),
                   **compare_with_oracle(gpu_s, kept["out"])}
         if H == 128 and int(etx.desc.precision) != synth.PREC_FP32:
             # reading Q16's report: the same events with a bf16 EMBEDDING (etx_embed_bf16) -- which edges change, and the
@@ -627,7 +630,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c2", choices=sorted(synth.CONFIGS))
     ap.add_argument("--events", type=int, default=0, help="events per GPU (default: the config's)")
-    ap.add_argument("--precision", type=int, default=None, help="override etx_precision (0 fp32, 1 tf32x3, 2 bf16, 3 bf16x3, 4 int8)")
+    ap.add_argument("--precision", type=int, default=None, help="override etx_precision (0 fp32, 1 tf32x3, 2 bf16, 3 bf16x3, 4 int8, 5 fp8 e4m3)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-next-rows", action="store_true", help="skip the next-row timings (launch lists of the step only)")
     ap.add_argument("--tracks-mean", type=float, default=0.0,

@@ -54,8 +54,11 @@ typedef enum {
   ETX_PREC_BF16X3 = 3,  /* tcgen05, operands split x = hi + lo into two bf16 (16 significand bits),
                            three kind::f16 MMAs (lo.hi + hi.lo + hi.hi), fp32 accumulate and state:
                            meets the fp32 tolerance at half the tensor-core work of 3xTF32          */
-  ETX_PREC_INT8 = 4     /* next row (NEXT-3, GNN part): tcgen05 kind::i8 -- INT8 codes for every GNN MLP layer
+  ETX_PREC_INT8 = 4,    /* next row (NEXT-3, GNN part): tcgen05 kind::i8 -- INT8 codes for every GNN MLP layer
                            input and weight (static ranges: etx_set_int8_ranges), exact int32 sums, fp32
+                           de-quantisation, biases, state and scatter-sum; the embedding stays 3xTF32      */
+  ETX_PREC_FP8 = 5      /* next row (NEXT-3, GNN part): tcgen05 kind::f8f6f4 -- e4m3 values for every GNN MLP layer
+                           input and weight (the same static ranges, S = alpha / 448), fp32 accumulation,
                            de-quantisation, biases, state and scatter-sum; the embedding stays 3xTF32      */
 } etx_precision;
 
@@ -145,7 +148,12 @@ etx_status etx_embed_int8(etx_ctx* ctx, const etx_batch* batch, const float* h_a
  * arithmetic (int32 per-hit projections).  etx_set_int8_ranges hands over the ranges: HOST array of (3 + 2 n_iter) x
  * gnn_n_layers positive floats, MLPs in the order node encoder, edge encoder, (node network k, edge network k) for
  * k = 0..n_iter-1, classifier; entry l of an MLP = range of layer l's input (entry 0 of the node encoder is unused).
- * Without it etx_gnn_forward / etx_edge_scores return ETX_ERR_INVALID in this precision.  Needs gnn_hidden = 128.      */
+ * Without it etx_gnn_forward / etx_edge_scores return ETX_ERR_INVALID in this precision.  Needs gnn_hidden = 128.
+ * ETX_PREC_FP8 is the same scheme on the e4m3 grid (reading Q26): S = alpha / 448, value = e4m3(clip(x * fl(1 / S),
+ * -448, 448)) rounded to nearest even (cvt.rn.satfinite.e4m3x2.f32), weights likewise with S_w = max|W_l| / 448, products
+ * accumulated in fp32 by the tensor cores (tcgen05.mma.kind::f8f6f4), y = acc * (S_a S_w) + b; the first-layer projections of
+ * the edge MLPs are fp32 sums.  It takes the same ranges through etx_set_int8_ranges.  Results agree with the quantised oracle
+ * within a tolerance, not bit for bit: the oracle's sums are exact, the tensor cores' are fp32.                        */
 etx_status etx_set_int8_ranges(etx_ctx* ctx, const float* h_alpha, size_t n);
 
 /* a2: fixed-radius search in embedding space.  Edge (i -> j) iff same event,

@@ -28,7 +28,7 @@ const char* check_desc(const etx_model_desc* d) {
   if (d->gnn_n_layers < 2 || d->gnn_n_layers > kMaxLayers) return "gnn_n_layers must be 2..8";
   if (d->n_iter < 0 || d->n_iter > 64) return "n_iter must be 0..64";
   if (d->n_planes < 2 || d->n_planes > 255) return "n_planes must be 2..255";
-  if (d->precision < ETX_PREC_FP32 || d->precision > ETX_PREC_INT8) return "unknown precision";
+  if (d->precision < ETX_PREC_FP32 || d->precision > ETX_PREC_FP8) return "unknown precision";
   for (int i = 0; i < 5; ++i)
     if (!(d->norm_scale[i] != 0.0f)) return "norm_scale entries must be non-zero";
   return nullptr;
@@ -72,10 +72,35 @@ uint16_t bf16_rne(float f) {
   return (uint16_t)(u >> 16);
 }
 
-float layer_weight_scale(const float* W, int fi, int fo) {
+float layer_weight_scale(const float* W, int fi, int fo, float qmax = 127.0f) {
   float mx = 0.0f;
   for (size_t i = 0; i < (size_t)fi * fo; ++i) mx = std::max(mx, std::fabs(W[i]));
-  return mx / 127.0f;
+  return mx / qmax;
+}
+// e4m3 (1-4-3, bias 7, no infinities, max 448): nearest value of a finite t, ties to even, saturating; and its byte code
+float e4m3_round_host(float t) {
+  const float a = std::fabs(t);
+  if (!(a < 448.0f)) return t < 0.0f ? -448.0f : 448.0f;
+  int e;
+  std::frexp(a, &e);
+  int le = (a == 0.0f) ? -6 : e - 1;
+  if (le < -6) le = -6;
+  const float ulp = std::ldexp(1.0f, le - 3);
+  const float r = std::nearbyintf(a / ulp) * ulp;
+  return t < 0.0f ? -r : r;
+}
+unsigned char e4m3_code_host(float t) {
+  const float v = e4m3_round_host(t);
+  const float a = std::fabs(v);
+  unsigned char code;
+  if (a == 0.0f) code = 0;
+  else if (a < 0.015625f) code = (unsigned char)std::lround(a * 512.0f);               // subnormal: mantissa = a / 2^-9
+  else {
+    int e;
+    const float m = std::frexp(a, &e);                                                // a = m 2^e, m in [0.5, 1)
+    code = (unsigned char)(((e - 1 + 7) << 3) | (int)std::lround((m * 2.0f - 1.0f) * 8.0f));
+  }
+  return (unsigned char)(code | ((std::signbit(v) && a != 0.0f) ? 0x80 : 0));
 }
 int quant_code_host(float x, float S) {
   float q = std::nearbyintf(x / S);
@@ -86,7 +111,19 @@ int quant_code_host(float x, float S) {
 // Appends the image of input columns [k_begin, k_end) of one layer W [fo = 128][fi] (row-major, fp32).
 void append_wimg_slab(std::vector<unsigned char>& img, const float* W, int fi, int fo, int k_begin, int k_end, int mode) {
   const int KA = tc_chunk_k(mode);
-  const int pieces = (mode == ETX_PREC_BF16 || mode == ETX_PREC_INT8) ? 1 : 2;
+  const int pieces = (mode == ETX_PREC_BF16 || mode == ETX_PREC_INT8 || mode == ETX_PREC_FP8) ? 1 : 2;
+  if (mode == ETX_PREC_FP8) {
+    // e4m3 codes: S_w = max|W| / 448 over the whole layer, code = e4m3(w * fl(1 / S_w)); layout as the INT8 image
+    const float rs = 1.0f / layer_weight_scale(W, fi, fo, 448.0f);
+    for (int k0 = k_begin; k0 < k_end; k0 += KA) {
+      const size_t base = img.size();
+      img.resize(base + 128 * 128, 0);
+      for (int n = 0; n < fo; ++n)
+        for (int kk = 0; kk < KA; ++kk)
+          img[base + (size_t)n * 128 + (size_t)(((kk / 16) ^ (n & 7)) * 16) + (kk % 16)] = e4m3_code_host(W[(size_t)n * fi + k0 + kk] * rs);
+    }
+    return;
+  }
   if (mode == ETX_PREC_INT8) {
     // INT8 codes (Eqs. 4.31-4.33): S_w = max|W| / 127 over the WHOLE layer (per-tensor scale), code =
     // clip(round(w / S_w)); one byte per weight, 128 codes per 128-byte row of the swizzled tile
@@ -266,7 +303,7 @@ int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   // its result decides graph edges (DESIGN.md section 5 "Embedding on the tensor cores")
   const int mode = (a.out_mode == 2) ? (a.emb_mode >= 0 ? a.emb_mode : (int)ETX_PREC_TF32X3) : (int)c->desc.precision;
   t.w_last = a.mlp.Wt[a.mlp.n_layers - 1];         // [H][1] == [H]
-  if (mode == ETX_PREC_INT8) {
+  if (mode == ETX_PREC_INT8 || mode == ETX_PREC_FP8) {
     if (a.out_mode == 3) { if (!a.mlp.wq_last) return -1; t.w_last = a.mlp.wq_last; }
     t.q_sa0 = a.q_sa0;
     for (int l = 0; l < kMaxLayers; ++l) { t.q_sc[l] = a.q_sc[l]; t.q_sn[l] = a.q_sn[l]; }
@@ -382,9 +419,11 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
       const float* W = h_weights + wsrc;
       for (int l = 0; l < mlps[i].n_layers; ++l) {
         const int fi = mlps[i].dims[l], fo = mlps[i].dims[l + 1];
-        dev[i].sw[l] = layer_weight_scale(W, fi, fo);
+        const bool fp8 = desc->precision == ETX_PREC_FP8;
+        dev[i].sw[l] = layer_weight_scale(W, fi, fo, fp8 ? 448.0f : 127.0f);
         if (i + 1 == mlps.size() && l == mlps[i].n_layers - 1)
-          for (int k = 0; k < fi; ++k) staged.push_back((float)quant_code_host(W[k], dev[i].sw[l]));
+          for (int k = 0; k < fi; ++k)
+            staged.push_back(fp8 ? e4m3_round_host(W[k] * (1.0f / dev[i].sw[l])) : (float)quant_code_host(W[k], dev[i].sw[l]));
         W += (size_t)fi * fo + fo;
       }
       wsrc += mlp_floats(mlps[i]);
@@ -613,11 +652,12 @@ etx_status etx_set_int8_ranges(etx_ctx* c, const float* h_alpha, size_t n) {
 static void fill_q(const etx_ctx* c, MlpArgs& a, int mi, const DevMlp& full, int shift, int n_l) {
   const int L = c->desc.gnn_n_layers;
   const float* al = c->q_alpha.data() + (size_t)mi * L;
-  a.q_sa0 = al[shift] / 127.0f;
+  const float qmax = c->desc.precision == ETX_PREC_FP8 ? 448.0f : 127.0f;     // the range maps to the grid's largest value
+  a.q_sa0 = al[shift] / qmax;
   for (int l = 0; l < n_l; ++l) {
-    const float sa = al[shift + l] / 127.0f;
+    const float sa = al[shift + l] / qmax;
     a.q_sc[l] = sa * full.sw[shift + l];
-    a.q_sn[l] = (shift + l + 1 < L) ? al[shift + l + 1] / 127.0f : 1.0f;
+    a.q_sn[l] = (shift + l + 1 < L) ? al[shift + l + 1] / qmax : 1.0f;
   }
 }
 
@@ -806,8 +846,8 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
   const int H = c->desc.gnn_hidden, N = b->n_hits;
   const int E = (int)g->n_edges;
 
-  const bool q8 = c->desc.precision == ETX_PREC_INT8;
-  if (q8 && c->q_alpha.empty()) return fail(c, ETX_ERR_INVALID, "ETX_PREC_INT8 needs calibrated ranges (etx_set_int8_ranges)");
+  const bool q8 = c->desc.precision == ETX_PREC_INT8 || c->desc.precision == ETX_PREC_FP8;   // 8-bit operands, static ranges
+  if (q8 && c->q_alpha.empty()) return fail(c, ETX_ERR_INVALID, "ETX_PREC_INT8 / ETX_PREC_FP8 need calibrated ranges (etx_set_int8_ranges)");
   {  // a3: h0 = MLP_n((x,y,z) normalised)
     MlpArgs a;
     a.n_rows = N; a.n_seg = 0;
@@ -847,7 +887,7 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
       a.mlp.wimg = part == 0 ? mlp.wimg_a : mlp.wimg_b;
       a.mlp.b[0] = c->d_zero_bias; a.mlp.Wt[0] = c->d_zero_bias;
       a.wide = wide ? 1 : 0;
-      if (q8) a.q_sa0 = c->q_alpha[(size_t)mi * c->desc.gnn_n_layers] / 127.0f;   // the edge MLP's layer-1 input scale; raw int32 out
+      if (q8) a.q_sa0 = c->q_alpha[(size_t)mi * c->desc.gnn_n_layers] / (c->desc.precision == ETX_PREC_FP8 ? 448.0f : 127.0f);   // the edge MLP's layer-1 input scale; raw sums out
       a.out_mode = 0; a.out = w.p + part * H; a.out_ld = 2 * H;
       c->launches += run_mlp(c, a, s);
     }
@@ -931,8 +971,8 @@ etx_status etx_edge_scores(etx_ctx* c, const etx_graph* g, const float* d_edge_e
   a.n_rows = (int)g->n_edges; a.n_seg = 1;
   a.seg[0] = Segment{d_edge_enc, nullptr, H, H};
   a.mlp = c->cls; a.out_mode = 3; a.out = d_scores; a.out_ld = 1;
-  if (c->desc.precision == ETX_PREC_INT8) {
-    if (c->q_alpha.empty()) return fail(c, ETX_ERR_INVALID, "ETX_PREC_INT8 needs calibrated ranges (etx_set_int8_ranges)");
+  if (c->desc.precision == ETX_PREC_INT8 || c->desc.precision == ETX_PREC_FP8) {
+    if (c->q_alpha.empty()) return fail(c, ETX_ERR_INVALID, "ETX_PREC_INT8 / ETX_PREC_FP8 need calibrated ranges (etx_set_int8_ranges)");
     fill_q(c, a, 2 + 2 * c->desc.n_iter, c->cls, 0, c->cls.n_layers);
   }
   {
@@ -1061,7 +1101,8 @@ etx_status etx_triplet_scores(etx_ctx* c, const etx_graph* g, const float* d_edg
                               float* d_trip_scores, void* stream) {
   if (!c) return ETX_ERR_INVALID;
   if (!c->have_trip) return fail(c, ETX_ERR_INVALID, "no triplet classifiers set (etx_set_triplet_classifiers)");
-  if (c->desc.precision == ETX_PREC_INT8) return fail(c, ETX_ERR_INVALID, "the triplet classifiers have no ETX_PREC_INT8 path");
+  if (c->desc.precision == ETX_PREC_INT8 || c->desc.precision == ETX_PREC_FP8)
+    return fail(c, ETX_ERR_INVALID, "the triplet classifiers have no ETX_PREC_INT8 / ETX_PREC_FP8 path");
   if (!g || g->n_edges < 0 || !t) return fail(c, ETX_ERR_INVALID, "graph / triplets are NULL");
   const int64_t total = t->n[0] + t->n[1] + t->n[2];
   if (t->n[0] < 0 || t->n[1] < 0 || t->n[2] < 0 || total > t->capacity) return fail(c, ETX_ERR_INVALID, "triplets not built");

@@ -36,6 +36,7 @@
 //                    L2 bytes of TF32X3.  Measured score error is the same ~1e-5 as TF32X3, because both
 //                    are dominated by the tensor core's truncating fp32 accumulation.
 #include <cuda.h>
+#include <cuda_fp16.h>
 #include <cstring>
 
 #include "common.cuh"
@@ -125,7 +126,37 @@ template <> struct Cfg<ETX_PREC_INT8> {
   static constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);   // D = s32, A = B = s8
 };
 
+// Next row (NEXT-3, GNN part) in FP8: e4m3 values for every layer input and weight (reading Q26), one
+// kind::f8f6f4 MMA per K-step (K = 32), fp32 accumulators.  Same 8-bit operand geometry as the INT8 mode.
+template <> struct Cfg<ETX_PREC_FP8> {
+  static constexpr int KA = 128;
+  static constexpr int KG = 64;
+  static constexpr int PIECES = 1;
+  static constexpr int NSTAGE_W = 4;          // 16 KB each
+  static constexpr int NSTAGE_A = 8;          // 16 KB each
+  static constexpr int PREFETCH = 2;
+  static constexpr int HID_COLS = 32;         // 128 codes = 32 columns
+  static constexpr uint32_t IDESC = (1u << 4) | (0u << 7) | (0u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);   // D = f32, A = B = e4m3
+};
+
 using namespace tcp;
+
+// two floats -> two e4m3 codes (round to nearest even, saturating at +-448); `lo` goes to bits [0,8)
+__device__ __forceinline__ uint32_t cvt_e4m3x2(float lo, float hi) {
+  uint16_t d;
+  asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(d) : "f"(hi), "f"(lo));
+  return (uint32_t)d;
+}
+__device__ __forceinline__ uint32_t pack_e4m3x4(float a, float b, float c, float d) {
+  return cvt_e4m3x2(a, b) | (cvt_e4m3x2(c, d) << 16);
+}
+// the float value of the e4m3 rounding of t (exact: e4m3 is a subset of fp16)
+__device__ __forceinline__ float e4m3_value(float t) {
+  const uint16_t c = (uint16_t)cvt_e4m3x2(t, 0.0f);
+  uint32_t h2;
+  asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h2) : "h"(c));
+  return __half2float(__ushort_as_half((unsigned short)(h2 & 0xffffu)));
+}
 
 // Eq. 4.33 with alpha_q = 127: clip(round(x / S), -127, 127); fp32 division, round half to even -- the oracle's arithmetic
 // The definition divides (x / S in fp32, then round half to even); an IEEE division per activation made the INT8 chain
@@ -177,6 +208,10 @@ __device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                  "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
+  else if constexpr (MODE == ETX_PREC_FP8)
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
   else
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                  "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
@@ -191,6 +226,10 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
   else if constexpr (MODE == ETX_PREC_INT8)
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                  "tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
+  else if constexpr (MODE == ETX_PREC_FP8)
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], [%1], %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(Cfg<MODE>::IDESC), "r"(accumulate) : "memory");
   else
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
@@ -252,6 +291,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   constexpr int GCH = HW / KG;                  // gather units per 128 columns
   constexpr int UPE = KA / KG;                  // gather units per ring entry (2 for 8-bit operands, else 1)
   constexpr bool q8 = (MODE == ETX_PREC_INT8);
+  constexpr bool f8 = (MODE == ETX_PREC_FP8);
+  constexpr bool op8 = q8 || f8;                // 8-bit operands: one 128-code K-chunk per 128 inputs
   constexpr int LPR = KG * 4 / 16;              // gather lanes per row: 16-byte pieces of a unit row (8 / 16)
   constexpr int RPP = kGatherThreads / LPR;     // rows covered by one pass of the gather threads (32 / 16)
   constexpr int NPASS = TM / RPP;               // passes per chunk (4 / 8)
@@ -327,7 +368,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
     for (int i = 0; i < NSW; ++i) { mbar_init(smem_u32(&bars->w_full[i]), 1); mbar_init(smem_u32(&bars->w_empty[i]), NMW); }
     for (int i = 0; i < NSA; ++i) { mbar_init(smem_u32(&bars->a_full[i]), 1); mbar_init(smem_u32(&bars->a_empty[i]), wide ? 2 : 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&bars->acc_full[i]), 1); mbar_init(smem_u32(&bars->acc_free[i]), kEpiThreads / 32); }
-    for (int i = 0; i < 8; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), q8 ? 8 : 4);   // 8-bit: ONE chunk per layer, written by all 8 warps
+    for (int i = 0; i < 8; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), op8 ? 8 : 4);   // 8-bit: ONE chunk per layer, written by all 8 warps
     bars->w_issued = 0; bars->a_produced = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -553,13 +594,20 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             float xq[8] = {buf[d][p2].x, buf[d][p2].y, buf[d][p2].z, buf[d][p2].w,
                            buf[d][p2 + 1].x, buf[d][p2 + 1].y, buf[d][p2 + 1].z, buf[d][p2 + 1].w};
             float cq[8];
-            quant_codes<8>(xq, cq, QScale{a.q_sa0, a.q_rsa0});
+            if constexpr (f8) {                             // e4m3: scale by fl(1/S), the conversion rounds and saturates
+#pragma unroll
+              for (int i = 0; i < 8; ++i) cq[i] = __fmul_rn(xq[i], a.q_rsa0);
+            } else {
+              quant_codes<8>(xq, cq, QScale{a.q_sa0, a.q_rsa0});
+            }
 #pragma unroll
             for (int h2 = 0; h2 < 2; ++h2) {
               const int r = r0 + (p2 + h2) * RPP;
               const uint32_t byte = d * 64 + jl * 4;        // K position of this thread's 4 codes inside the 128-byte row
+              const uint32_t word = f8 ? pack_e4m3x4(cq[4 * h2], cq[4 * h2 + 1], cq[4 * h2 + 2], cq[4 * h2 + 3])
+                                       : pack_codes(cq[4 * h2], cq[4 * h2 + 1], cq[4 * h2 + 2], cq[4 * h2 + 3]);
               asm volatile("st.shared.b32 [%0], %1;" ::"r"(tile_q + r * 128 + (((byte >> 4) ^ (r & 7)) << 4) + (byte & 15)),
-                           "r"(pack_codes(cq[4 * h2], cq[4 * h2 + 1], cq[4 * h2 + 2], cq[4 * h2 + 3])) : "memory");
+                           "r"(word) : "memory");
             }
           }
           if (more) load_unit(buf[d]);                       // this buffer's next loads fly while the other half is converted
@@ -624,9 +672,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
         if (L < n_gemm - 1) {
           // ---- hidden layer: ReLU(x + b) -> next A operand in TMEM, released chunk by chunk.
           // This warp's column half holds K-chunks HH*HCH/2 .. of the next layer.
-          if constexpr (q8) {
-            // 8-bit: de-quantise the int32 sums, bias, ReLU, re-quantise with the NEXT layer's input scale (the Q -> node
-            // -> DQ chain of P:2725); this warp's 64 columns become 16 packed columns of the single K-chunk
+          if constexpr (op8) {
+            // 8-bit: de-quantise the int32 (INT8) / fp32 (FP8) sums, bias, ReLU, re-quantise with the NEXT layer's input scale
+            // (the Q -> node -> DQ chain of P:2725); this warp's 64 columns become 16 packed columns of the single K-chunk
             EP_T0();
             uint32_t va[32], vb[32], w[16];
             tmem_ld32(acc + HH * 64, va);
@@ -640,11 +688,21 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             for (int g4 = 0; g4 < 4; ++g4) {         // 16 values per tie test
               float xv[16], cv[16];
 #pragma unroll
-              for (int i = 0; i < 16; ++i)
-                xv[i] = fmaxf(dequant(g4 < 2 ? va[16 * g4 + i] : vb[16 * (g4 - 2) + i], sc, bq[16 * g4 + i]), 0.f);
+              for (int i = 0; i < 16; ++i) {
+                const uint32_t acc_bits = g4 < 2 ? va[16 * g4 + i] : vb[16 * (g4 - 2) + i];
+                if constexpr (f8) xv[i] = fmaxf(__fadd_rn(__fmul_rn(__uint_as_float(acc_bits), sc), bq[16 * g4 + i]), 0.f);
+                else xv[i] = fmaxf(dequant(acc_bits, sc, bq[16 * g4 + i]), 0.f);
+              }
+              if constexpr (f8) {
+#pragma unroll
+                for (int i = 0; i < 16; ++i) cv[i] = __fmul_rn(xv[i], sn.r);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) w[4 * g4 + i] = pack_e4m3x4(cv[4 * i], cv[4 * i + 1], cv[4 * i + 2], cv[4 * i + 3]);
+              } else {
               quant_codes<16>(xv, cv, sn);
 #pragma unroll
               for (int i = 0; i < 4; ++i) w[4 * g4 + i] = pack_codes(cv[4 * i], cv[4 * i + 1], cv[4 * i + 2], cv[4 * i + 3]);
+              }
             }
             asm volatile(
                 "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
@@ -782,6 +840,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
                 quant_codes<32>(xv, cv, QScale{a.q_sn[L], a.q_rsn[L]});
 #pragma unroll
                 for (int i = 0; i < 32; ++i) logit = fmaf(cv[i], wlast_s[q * 32 + i], logit);
+              } else if constexpr (f8) {       // e4m3 values of the last hidden activation x e4m3 values of the weights, fp32 sum
+#pragma unroll
+                for (int i = 0; i < 32; ++i) {
+                  const float x = fmaxf(__fadd_rn(__fmul_rn(__uint_as_float(v[i]), a.q_sc[L]), bias[q * 32 + i]), 0.f);
+                  logit = fmaf(e4m3_value(__fmul_rn(x, a.q_rsn[L])), wlast_s[q * 32 + i], logit);
+                }
               } else {
 #pragma unroll
               for (int i = 0; i < 32; ++i)
@@ -790,7 +854,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             }
             tc_fence_before();
             mbar_arrive_relaxed_warp(smem_u32(&bars->acc_free[b]), lane);
-            if constexpr (q8) logit = __fadd_rn(__fmul_rn(logit, a.q_sc[a.n_layers - 1]), __ldg(a.bias[a.n_layers - 1]));
+            if constexpr (op8) logit = __fadd_rn(__fmul_rn(logit, a.q_sc[a.n_layers - 1]), __ldg(a.bias[a.n_layers - 1]));
             else
             logit += __ldg(a.bias[a.n_layers - 1]);
             const int row = tile * TM + et;
@@ -848,6 +912,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
                 const float sc = a.q_sc[L];
                 st_shared_v4(dst, __float_as_uint(dequant(v0, sc, bq[j].x)), __float_as_uint(dequant(v1, sc, bq[j].y)),
                              __float_as_uint(dequant(v2, sc, bq[j].z)), __float_as_uint(dequant(v3, sc, bq[j].w)));
+              } else if constexpr (f8 && !wide) {   // fp32 sums of e4m3 products: y = acc * (S_a S_w) + b (the projections stay raw sums)
+                const float sc = a.q_sc[L];
+                st_shared_v4(dst, __float_as_uint(__fadd_rn(__fmul_rn(__uint_as_float(v0), sc), bq[j].x)),
+                             __float_as_uint(__fadd_rn(__fmul_rn(__uint_as_float(v1), sc), bq[j].y)),
+                             __float_as_uint(__fadd_rn(__fmul_rn(__uint_as_float(v2), sc), bq[j].z)),
+                             __float_as_uint(__fadd_rn(__fmul_rn(__uint_as_float(v3), sc), bq[j].w)));
               } else
               st_shared_v4(dst, __float_as_uint(__uint_as_float(v0) + bq[j].x), __float_as_uint(__uint_as_float(v1) + bq[j].y),
                            __float_as_uint(__uint_as_float(v2) + bq[j].z), __float_as_uint(__uint_as_float(v3) + bq[j].w));
@@ -1119,7 +1189,8 @@ int launch_mode(const TcArgs& a, int sm_count, cudaStream_t s) {
 }  // namespace
 
 int tc_chunk_k(int mode) {
-  return mode == ETX_PREC_TF32X3 ? Cfg<ETX_PREC_TF32X3>::KA : (mode == ETX_PREC_INT8 ? Cfg<ETX_PREC_INT8>::KA : Cfg<ETX_PREC_BF16>::KA);
+  return mode == ETX_PREC_TF32X3 ? Cfg<ETX_PREC_TF32X3>::KA
+                                 : ((mode == ETX_PREC_INT8 || mode == ETX_PREC_FP8) ? Cfg<ETX_PREC_INT8>::KA : Cfg<ETX_PREC_BF16>::KA);
 }
 
 // Requirements (checked by the caller): hidden width 128; K0 a multiple of the chunk (32 / 64) and
@@ -1127,7 +1198,7 @@ int tc_chunk_k(int mode) {
 int launch_mlp_tc(const TcArgs& a_in, int mode, int sm_count, cudaStream_t s) {
   if (a_in.n_rows <= 0) return 0;
   TcArgs a = a_in;
-  if (mode == ETX_PREC_INT8) {
+  if (mode == ETX_PREC_INT8 || mode == ETX_PREC_FP8) {
     a.q_rsa0 = 1.0f / a.q_sa0; a.q_rsf = 1.0f / a.q_sf;
     for (int l = 0; l < kMaxLayers; ++l) a.q_rsn[l] = a.q_sn[l] != 0.0f ? 1.0f / a.q_sn[l] : 0.0f;
   }
@@ -1136,6 +1207,7 @@ int launch_mlp_tc(const TcArgs& a_in, int mode, int sm_count, cudaStream_t s) {
     if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, 1>(a, sm_count, s);
     if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, 1>(a, sm_count, s);
     if (mode == ETX_PREC_INT8) return launch_mode<ETX_PREC_INT8, 1>(a, sm_count, s);
+    if (mode == ETX_PREC_FP8) return launch_mode<ETX_PREC_FP8, 1>(a, sm_count, s);
     return -1;
   }
   if (a.w1) {                                    // first-layer operand computed from 3 features (node encoder, embedding)
@@ -1155,6 +1227,7 @@ int launch_mlp_tc(const TcArgs& a_in, int mode, int sm_count, cudaStream_t s) {
   if (mode == ETX_PREC_BF16) return launch_mode<ETX_PREC_BF16, 0>(a, sm_count, s);
   if (mode == ETX_PREC_BF16X3) return launch_mode<ETX_PREC_BF16X3, 0>(a, sm_count, s);
   if (mode == ETX_PREC_INT8) return launch_mode<ETX_PREC_INT8, 0>(a, sm_count, s);
+  if (mode == ETX_PREC_FP8) return launch_mode<ETX_PREC_FP8, 0>(a, sm_count, s);
   return -1;
 }
 

@@ -53,6 +53,7 @@ PREC_TF32X3 = 1    # tensor cores, error-compensated 3xTF32 (fp32-equivalent)
 PREC_BF16 = 2      # tensor cores, bf16 operands, fp32 accumulate
 PREC_BF16X3 = 3    # tensor cores, bf16 hi/lo split, 3 MMAs (fp32 tolerance at half the work of 3xTF32)
 PREC_INT8 = 4      # next row: INT8 GNN MLPs on the tensor cores (kind::i8), fp32 state and scatter
+PREC_FP8 = 5       # next row: FP8 e4m3 GNN MLPs on the tensor cores (kind::f8f6f4), fp32 state and scatter; the same ranges
 
 _U64 = np.uint64
 _GOLDEN = _U64(0x9E3779B97F4A7C15)
