@@ -82,11 +82,16 @@ void orc_mlp(int64_t n, int32_t n_layers, const int32_t* dims, const float* w, c
 //      this function), its weight with S_w[l] = max|W_l| / 127 (the weight range is known), the
 //      products are summed exactly in integers and de-quantised:
 //        y_o = float(sum_k x_q[k] w_q[o][k]) * (S_a S_w) + b_o ;  ReLU on hidden layers (biases stay fp32).
-//      Every float step is a single fp32 operation (x / S, rint = round-half-even, S_a * S_w, * , +; compile
+//      Every float step is a single fp32 operation (1 / S, x * that, rint = round-half-even, S_a * S_w, * , +; compile
 //      with -ffp-contract=off), so the integer codes -- and with them the outputs -- are reproducible bit
 //      for bit (reading Q21).
+//      Round 2 (reading Q21, revised): the quotient x / S of Eq. 4.31 is evaluated as x * fl(1 / S) -- one
+//      rounded fp32 multiplication by the rounded reciprocal of the scale, the arithmetic of INT8 inference pipelines and
+//      of the FP8 row below.  It is the same real number; in fp32 it differs from the divided form on ~6e-5 of the values
+//      (those within 3e-5 of a tie), by one code.
 static inline int32_t quant_code(float x, float S) {
-  float q = std::nearbyintf(x / S);                 // default rounding mode: to nearest, ties to even
+  const float r = 1.0f / S;
+  float q = std::nearbyintf(x * r);                 // default rounding mode: to nearest, ties to even
   if (q > 127.0f) q = 127.0f;
   if (q < -127.0f) q = -127.0f;
   return (int32_t)q;

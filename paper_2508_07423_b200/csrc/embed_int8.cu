@@ -16,10 +16,10 @@ constexpr int TM = 64;
 constexpr int NT = 256;
 
 __device__ __forceinline__ int quant_code(float x, float S) {
-  const bool z = (x == 0.0f);                       // 0 / S would take div.rn's slow path (see mlp_tc.cu quant_f)
-  float q = rintf(__fdiv_rn(z ? S : x, S));         // round to nearest, ties to even
+  const float r = __fdiv_rn(1.0f, S);               // x / S of Eq. 4.31 as x * fl(1 / S) (DESIGN reading Q21)
+  float q = rintf(__fmul_rn(x, r));                 // round to nearest, ties to even
   q = fminf(fmaxf(q, -127.0f), 127.0f);
-  return z ? 0 : (int)q;
+  return (int)q;
 }
 
 template <int H>

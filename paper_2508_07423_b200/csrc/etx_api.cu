@@ -102,8 +102,9 @@ unsigned char e4m3_code_host(float t) {
   }
   return (unsigned char)(code | ((std::signbit(v) && a != 0.0f) ? 0x80 : 0));
 }
-int quant_code_host(float x, float S) {
-  float q = std::nearbyintf(x / S);
+int quant_code_host(float x, float S) {              // Eq. 4.33 with x / S evaluated as x * fl(1 / S) (DESIGN reading Q21)
+  const float r = 1.0f / S;
+  float q = std::nearbyintf(x * r);
   q = std::min(std::max(q, -127.0f), 127.0f);
   return (int)q;
 }
@@ -465,7 +466,7 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
       codes.resize(codes.size() + (size_t)fo * kw, 0);
       for (int o = 0; o < fo; ++o)
         for (int k = 0; k < fi; ++k) {
-          float q = std::nearbyintf(W[(size_t)o * fi + k] / sw);
+          float q = std::nearbyintf(W[(size_t)o * fi + k] * (1.0f / sw));
           q = std::min(std::max(q, -127.0f), 127.0f);
           codes[c->emb_wq_off[l] + (size_t)o * kw + k / 4] |= (int)(((unsigned)(int)q & 0xffu) << (8 * (k % 4)));
         }

@@ -158,31 +158,16 @@ __device__ __forceinline__ float e4m3_value(float t) {
   return __half2float(__ushort_as_half((unsigned short)(h2 & 0xffffu)));
 }
 
-// Eq. 4.33 with alpha_q = 127: clip(round(x / S), -127, 127); fp32 division, round half to even -- the oracle's arithmetic
-// The definition divides (x / S in fp32, then round half to even); an IEEE division per activation made the INT8 chain
-// slower than the fp32-equivalent one (and a ZERO numerator -- half of all post-ReLU values -- even takes div.rn's
-// slow path: 10x on the classifier).  The code is computed from t = x * fl(1/S) instead, which is within
-// |t| * 2^-22.9 <= 1.6e-5 of the exact quotient for |t| < 127.5, as is the fp32 quotient itself (<= 7.6e-6): unless t
-// lies within 3e-5 of a tie k + 1/2 all three round to the same integer.  Only those rare lanes (~6e-5 of the
-// values) evaluate the real division, so the result is the definition's, bit for bit.
-// The tie test of N values is folded into ONE rarely-taken branch, so the common path is straight-line code with N
-// independent chains (a branch per value serialised them: the INT8 chain ran latency-bound, 3x slower).
+// Eq. 4.33 with alpha_q = 127: clip(round(x / S), -127, 127), round half to even -- the oracle's arithmetic, in which the
+// quotient is ONE rounded fp32 multiplication by the rounded reciprocal of the scale (reading Q21, revised in
+// round 2).  Round 1's reading divided (x / S in fp32): reproducing IEEE division bit for bit needed a tie test per value and
+// a division on the rare ambiguous ones, which made the INT8 instantiation 12k instructions long (instruction-cache misses:
+// stall_no_inst 39 % in the epilogue warps) and slower than the fp32-equivalent mode it approximates.
 struct QScale { float S, r; };                  // scale and fl(1 / S)
 template <int N>
 __device__ __forceinline__ void quant_codes(const float (&x)[N], float (&q)[N], QScale s) {
-  bool amb = false;
 #pragma unroll
-  for (int i = 0; i < N; ++i) {
-    const float t = x[i] * s.r;
-    q[i] = rintf(t);
-    amb |= (fabsf(t - q[i]) > 0.49997f) & (fabsf(t) < 127.6f);
-  }
-  if (amb) {                                    // some value sits within 3e-5 of a tie: the definition's division decides
-#pragma unroll
-    for (int i = 0; i < N; ++i) q[i] = (x[i] == 0.0f) ? 0.0f : rintf(__fdiv_rn(x[i], s.S));
-  }
-#pragma unroll
-  for (int i = 0; i < N; ++i) q[i] = fminf(fmaxf(q[i], -127.0f), 127.0f);
+  for (int i = 0; i < N; ++i) q[i] = fminf(fmaxf(rintf(__fmul_rn(x[i], s.r)), -127.0f), 127.0f);
 }
 __device__ __forceinline__ uint32_t pack_codes(float a, float b, float c, float d) {
   return ((uint32_t)(int)a & 0xffu) | (((uint32_t)(int)b & 0xffu) << 8) | (((uint32_t)(int)c & 0xffu) << 16) | (((uint32_t)(int)d & 0xffu) << 24);
