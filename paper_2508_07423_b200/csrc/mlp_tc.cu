@@ -232,7 +232,7 @@ struct Unit {                                   // one gather unit: KA columns o
 constexpr int kMaxUnits = 24;
 
 struct Bars {                                   // mbarriers (8 bytes each) + TMEM base + gather unit table
-  uint64_t w_full[8], w_empty[8], a_full[8], a_empty[8], acc_full[2], acc_free[2], hid_ready[8];
+  uint64_t w_full[8], w_empty[8], a_full[8], a_empty[8], acc_full[3], acc_free[3], hid_ready[12];
   uint32_t tmem_base;
   // Progress counters for the two MMA issuer warps (see there): weight stages the loader has started to fill, operand
   // entries the commit warp has published.  An mbarrier parity wait is only meaningful for the barrier's CURRENT phase;
@@ -258,13 +258,18 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   constexpr int KA = C::KA, P = C::PIECES, NSW = C::NSTAGE_W, NSA = C::NSTAGE_A, HID_COLS = C::HID_COLS;
   constexpr uint32_t kStageBytes = P * kAtomBytes;
   static_assert(NSW <= 8 && NSA <= 8, "Bars holds 8 mbarriers per ring");
-  constexpr uint32_t COL_ACC = 0, COL_HID = 256;
+  constexpr uint32_t COL_ACC = 0;
   // Tiles in flight per CTA.  The bf16 modes keep TWO 128-row tiles in flight (slot s: accumulator s,
   // hidden operand region s): the MMA warp issues layer l of tile A, then of tile B, while the epilogue
   // warps turn A's accumulator into its next operand; both tiles use each weight stage before it is
   // released, so the weight ring moves half the bytes.  TF32X3 needs 256 columns per hidden operand
   // and keeps one tile in flight with ping-pong accumulators.
+  // 8-bit operands (INT8 / FP8): a hidden operand is 32 columns, so THREE tiles would fit (3 x (128 + 32) = 480 columns);
+  // the slot logic below is written for up to three and that was measured: FP8 edge network -2 %, edge encoder +13 %,
+  // INT8 embedding +10 % -- a third tile in flight does not help, because the eight epilogue warps process the tiles'
+  // jobs one after the other and are busy whatever the number of tiles waiting for them.  Two it stays.
   constexpr int NSLOT = (MODE == ETX_PREC_TF32X3) ? 1 : 2;
+  constexpr uint32_t COL_HID = (NSLOT == 3) ? 384 : 256;   // hidden operand regions behind the accumulators
   // MMA issuer warps.  2 (one per tile in flight, each walking its own tile's chain of waits) is implemented and correct,
   // and measured SLOWER (edge network 23.5 -> 25.4 ms per step, classifier 1.9 -> 2.4): issued concurrently, the two tiles'
   // MMAs interleave in the tensor pipe and both tiles finish their layer late and together, which destroys the stagger
@@ -307,7 +312,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   constexpr bool wide = (VAR == 1);             // (compile-time switches: the regular kernels carry none of it)
   constexpr bool feat = (VAR == 2 || VAR == 3);
   constexpr bool narrow = (VAR == 3);
-  static_assert(!wide || NSLOT == 2, "wide mode needs two accumulator slots");
+  static_assert(!wide || NSLOT >= 2, "wide mode needs two accumulator slots");
   const int n_pairs = wide ? my_tiles : (my_tiles + NSLOT - 1) / NSLOT;
   auto slots_of = [&](int pi) { return wide ? 2 : ((my_tiles - pi * NSLOT) < NSLOT ? (my_tiles - pi * NSLOT) : NSLOT); };
   auto tile_of = [&](int pi, int sl) { return (int)blockIdx.x + (wide ? pi : pi * NSLOT + sl) * (int)gridDim.x; };
@@ -352,8 +357,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   if (threadIdx.x == 0) {
     for (int i = 0; i < NSW; ++i) { mbar_init(smem_u32(&bars->w_full[i]), 1); mbar_init(smem_u32(&bars->w_empty[i]), NMW); }
     for (int i = 0; i < NSA; ++i) { mbar_init(smem_u32(&bars->a_full[i]), 1); mbar_init(smem_u32(&bars->a_empty[i]), wide ? 2 : 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(&bars->acc_full[i]), 1); mbar_init(smem_u32(&bars->acc_free[i]), kEpiThreads / 32); }
-    for (int i = 0; i < 8; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), op8 ? 8 : 4);   // 8-bit: ONE chunk per layer, written by all 8 warps
+    for (int i = 0; i < 3; ++i) { mbar_init(smem_u32(&bars->acc_full[i]), 1); mbar_init(smem_u32(&bars->acc_free[i]), kEpiThreads / 32); }
+    for (int i = 0; i < 12; ++i) mbar_init(smem_u32(&bars->hid_ready[i]), op8 ? 8 : 4);   // 8-bit: ONE chunk per layer, written by all 8 warps
     bars->w_issued = 0; bars->a_produced = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -636,15 +641,15 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
 #define EP_T0() if (edbg) tp = clock64()
 #define EP_ACC(i) if (edbg) { const long long tn = clock64(); ep[i] += tn - tp; tp = tn; }
     const long long e_start = edbg ? clock64() : 0;
-    uint32_t uacc[2] = {0, 0};                   // jobs seen per accumulator (mbarrier phase)
+    uint32_t uacc[3] = {0, 0, 0};                // jobs seen per accumulator (mbarrier phase)
     for (int pi = 0; pi < n_pairs; ++pi) {
       const int ns = slots_of(pi);
       for (int l = 0; l < n_gemm; ++l)
       for (int sl = 0; sl < ns; ++sl, ++g) {
-        const uint32_t b = (NSLOT == 2) ? (uint32_t)sl : (g & 1);
+        const uint32_t b = (NSLOT >= 2) ? (uint32_t)sl : (g & 1);
         const int tile = tile_of(pi, sl);
-        const uint32_t hid = lane_addr + COL_HID + (NSLOT == 2 ? sl * HIDW : 0);
-        uint64_t* hid_ready = bars->hid_ready + (NSLOT == 2 ? sl * 4 : 0);
+        const uint32_t hid = lane_addr + COL_HID + (NSLOT >= 2 ? sl * HIDW : 0);
+        uint64_t* hid_ready = bars->hid_ready + (NSLOT >= 2 ? sl * 4 : 0);
         long long te0 = edbg ? clock64() : 0;
         mbar_wait_warp(smem_u32(&bars->acc_full[b]), uacc[b] & 1, lane);
         ++uacc[b];
@@ -992,7 +997,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
     long long t_start = dbg ? clock64() : 0, t0 = 0;
 #define DBG_T0() if (dbg) t0 = clock64()
 #define DBG_ACC(i) if (dbg) dt[i] += clock64() - t0
-    uint32_t uacc[2] = {0, 0}, uhid[2] = {0, 0};  // jobs issued per accumulator / per hidden region (mbarrier phases)
+    uint32_t uacc[3] = {0, 0, 0}, uhid[3] = {0, 0, 0};  // jobs issued per accumulator / per hidden region (mbarrier phases)
     for (int pi = 0; pi < n_pairs; ++pi) {
       const int ns = slots_of(pi);
       for (int l = 0; l < n_gemm; ++l) {
@@ -1003,8 +1008,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
        const bool shared_w = (l > 0) || share1;
        for (int sl = 0; sl < ns; ++sl, ++g) {
         if (NMW == 2 && sl != mw) continue;         // the other issuer's tile
-        const uint32_t b = (NSLOT == 2) ? (uint32_t)sl : (g & 1);
-        const uint32_t hs = (NSLOT == 2) ? (uint32_t)sl : 0u;
+        const uint32_t b = (NSLOT >= 2) ? (uint32_t)sl : (g & 1);
+        const uint32_t hs = (NSLOT >= 2) ? (uint32_t)sl : 0u;
         uint32_t w_cnt = shared_w ? w_base : w_base + (uint32_t)(sl * nch);       // first weight stage this tile uses
         uint32_t a_cnt = a_base + (wide ? 0u : (uint32_t)(sl * ept));             // first operand entry of this tile
         // arrivals this issuer owes a weight stage: two complete it (one per issuer; both from the stage's only user)
