@@ -343,26 +343,44 @@ search_ballot_fill_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, co
     const int j0 = pp[p + 1];
     const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
     const int j1 = pp[top + 1];
-    unsigned long long n01 = 0, n23 = 0;
-    if (j1 - j0 > kBallotWords * 32) {
-      const float4 m = __ldg(reinterpret_cast<const float4*>(a.emb) + i);
-      n01 = pack2(-m.x, -m.y); n23 = pack2(-m.z, -m.w);
+    // Lane t owns vote word t: ONE coalesced load brings all of the source's words, a warp scan of their popcounts gives
+    // every word its first edge slot, and each lane walks its own set bits (1-3 per word) -- instead of the warp
+    // stepping through the words one after the other with 31 idle lanes per edge.
+    const int nw = (j1 - j0 + 31) >> 5;
+    const unsigned word = (lane < nw && lane < kBallotWords) ? __ldg(ballots + (size_t)i * kBallotWords + lane) : 0u;
+    int before = __popc(word);
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(kFull, before, o);
+      if (lane >= o) before += t;
     }
-    int cnt = 0;
-    for (int t = 0; cnt < deg; ++t) {
-      unsigned b;
-      if (t < kBallotWords) b = __ldg(ballots + (size_t)i * kBallotWords + t);
-      else {
+    const int kept = __shfl_sync(kFull, before, 31);       // edges described by the kept words
+    before -= __popc(word);
+    const int jw = j0 + lane * 32;
+    int k = 0;
+    for (unsigned w = word; w; w &= w - 1, ++k) {
+      const int j = jw + __ffs(w) - 1;
+      const int pos = base_out + before + k;
+      src[pos] = i;
+      dst[pos] = j;
+      in_perm[in_ptr[j] + atomicAdd(&cursor[j], 1)] = pos;
+    }
+    if (kept < deg) {
+      // a window longer than the kept words: the rest is re-tested, 32 candidates per step, as round 1's fill pass did
+      const float4 m = __ldg(reinterpret_cast<const float4*>(a.emb) + i);
+      const unsigned long long n01 = pack2(-m.x, -m.y), n23 = pack2(-m.z, -m.w);
+      int cnt = kept;
+      for (int t = kBallotWords; cnt < deg; ++t) {
         const int j = j0 + t * 32 + lane, jc = j < j1 ? j : j1 - 1;
-        b = __ballot_sync(kFull, (dist2_d4(n01, n23, __ldg(reinterpret_cast<const float4*>(a.emb) + jc)) < a.r2_max) & (j < j1));
+        const unsigned b = __ballot_sync(kFull, (dist2_d4(n01, n23, __ldg(reinterpret_cast<const float4*>(a.emb) + jc)) < a.r2_max) & (j < j1));
+        if ((b >> lane) & 1u) {
+          const int pos = base_out + cnt + __popc(b & lt);
+          src[pos] = i;
+          dst[pos] = j;
+          in_perm[in_ptr[j] + atomicAdd(&cursor[j], 1)] = pos;
+        }
+        cnt += __popc(b);
       }
-      if ((b >> lane) & 1u) {
-        const int pos = base_out + cnt + __popc(b & lt), j = j0 + t * 32 + lane;
-        src[pos] = i;
-        dst[pos] = j;
-        in_perm[in_ptr[j] + atomicAdd(&cursor[j], 1)] = pos;
-      }
-      cnt += __popc(b);
     }
   }
 }
