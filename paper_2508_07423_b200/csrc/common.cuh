@@ -40,6 +40,8 @@ struct Workspace {            // carved from the caller's buffer by carve_worksp
   int32_t* flags = nullptr;       // [8] validation flags / counters
   int32_t* sched = nullptr;       // [8] work counters of the dynamically scheduled kernels (scatter)
   uint32_t* ballots = nullptr;    // [n_hits][kBallotWords] vote words of the search's count pass (4-d embeddings)
+  uint16_t* prefix16 = nullptr;   // [n_hits][kBallotWords] votes of the source in the words before each word
+  int32_t* in_ptr3 = nullptr;     // [3 n_hits + 1] in-degree per (hit, plane gap 3/2/1), scanned into sub-list offsets
   float* h = nullptr;             // [n_hits, H]
   float* m = nullptr;             // [n_hits, 2H]
   float* p = nullptr;             // [n_hits, 2H] per-hit first-layer projections [A h | B h] (tensor-core modes)
@@ -115,15 +117,16 @@ struct GraphArgs {
 int launch_plane_index(const GraphArgs& a, int32_t* plane_ptr, int32_t* hit_event, int32_t* flags, cudaStream_t s);
 constexpr int kBallotWords = 32;   // vote words (32 candidates each) the count pass keeps per source for the fill pass
 int launch_search_count(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
-                        const int32_t* flags, int32_t* out_deg, int32_t* in_deg, uint32_t* ballots /*[n_hits][kBallotWords] or null*/,
-                        cudaStream_t s);
+                        int32_t* flags, int32_t* out_deg, int32_t* in_deg3, uint32_t* ballots /*[n_hits][kBallotWords] or null*/,
+                        uint16_t* prefix16, cudaStream_t s);
 int launch_search_kmax_cap(const GraphArgs& a, int k_max, const int32_t* plane_ptr, const int32_t* hit_event, int32_t* flags,
-                           int32_t* out_deg, int32_t* in_deg, uint32_t* ballots, cudaStream_t s);
+                           int32_t* out_deg, int32_t* in_deg3, uint32_t* ballots, uint16_t* prefix16, cudaStream_t s);
+int launch_in_ptr_from3(int n_hits, const int32_t* in_ptr3, int32_t* in_ptr, cudaStream_t s);
 int launch_exclusive_scan(int32_t* data /*[n+1], in place, data[n] = total*/, int n, int32_t* tmp, cudaStream_t s);
 int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
                        const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst,
                        const int32_t* in_ptr, int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/,
-                       const uint32_t* ballots, cudaStream_t s);
+                       const uint32_t* ballots, const uint16_t* prefix16, const int32_t* in_ptr3, cudaStream_t s);
 size_t scan_tmp_ints(int n);
 int launch_add_offset(const int32_t* in, int32_t* out, int64_t n, int32_t offset, cudaStream_t s);
 int launch_sort_in_lists(int n_hits, const int32_t* flags, const int32_t* in_ptr, int32_t* in_perm, cudaStream_t s);

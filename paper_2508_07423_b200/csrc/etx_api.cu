@@ -188,10 +188,14 @@ Workspace carve(const etx_ctx* c, int32_t n_events, int32_t n_hits, int64_t cap,
   w.plane_ptr = (int32_t*)take(sizeof(int32_t) * (size_t)n_events * (L + 1));
   w.hit_event = (int32_t*)take(sizeof(int32_t) * (size_t)n_hits);
   w.cursor = (int32_t*)take(sizeof(int32_t) * (size_t)n_hits);
-  w.scan_tmp = (int32_t*)take(sizeof(int32_t) * scan_tmp_ints(n_hits + 1));
+  w.scan_tmp = (int32_t*)take(sizeof(int32_t) * scan_tmp_ints(3 * n_hits + 1));
   w.flags = (int32_t*)take(sizeof(int32_t) * 8);
   w.sched = (int32_t*)take(sizeof(int32_t) * 8);
-  if (d == 4) w.ballots = (uint32_t*)take(sizeof(uint32_t) * (size_t)n_hits * kBallotWords);
+  if (d == 4) {
+    w.ballots = (uint32_t*)take(sizeof(uint32_t) * (size_t)n_hits * kBallotWords);
+    w.prefix16 = (uint16_t*)take(sizeof(uint16_t) * (size_t)n_hits * kBallotWords);
+    w.in_ptr3 = (int32_t*)take(sizeof(int32_t) * ((size_t)3 * n_hits + 1));
+  }
   w.h = (float*)take(sizeof(float) * (size_t)n_hits * H);
   w.m = (float*)take(sizeof(float) * (size_t)n_hits * 2 * H);
   if (c->desc.precision != ETX_PREC_FP32) w.p = (float*)take(sizeof(float) * (size_t)n_hits * 2 * H);
@@ -781,19 +785,25 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
   a.d = c->emb.dims[c->emb.n_layers]; a.gap = max_plane_gap; a.r2_max = r2_max;
   a.event_ptr = b->d_event_ptr; a.plane = b->d_plane; a.emb = d_emb;
 
-  // k_max > 0 on a 4-d embedding runs the tiled search too: a cap kernel clears the votes beyond the k_max nearest and
-  // the rest of the build is the hot path's (graph.cu); other dimensions, or a window with more candidates than kept vote
-  // words, use the one-warp-per-source kernels of graph_kmax.cu
-  bool kmax_tiled = k_max > 0 && a.d == 4 && w.ballots;
+  // A 4-d embedding runs the tiled search (graph.cu): count pass with kept vote words and per-(hit, plane gap) in-degrees,
+  // for k_max > 0 a cap kernel that clears the votes beyond the k_max nearest, scans, and one fill pass that writes src, dst
+  // and the by-destination lists at their final positions.  Other dimensions, or a window with more candidates than vote
+  // words are kept (flags[1]), use the one-warp-per-source kernels (graph.cu / graph_kmax.cu: cursor atomics + in-list sort).
+  bool tiled = a.d == 4 && w.ballots;
   int32_t host[3] = {0, 0, 0};
   for (int attempt = 0; attempt < 2; ++attempt) {
     {
       ProfScope ps(c, ETX_K_GRAPH, s);
       c->launches += launch_plane_index(a, w.plane_ptr, w.hit_event, w.flags, s);
-      if (k_max == 0 || kmax_tiled) {
-        c->launches += launch_search_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_in_ptr, w.ballots, s);
-        if (kmax_tiled)
-          c->launches += launch_search_kmax_cap(a, k_max, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_in_ptr, w.ballots, s);
+      if (tiled) {
+        c->launches += launch_search_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, w.in_ptr3, w.ballots, w.prefix16, s);
+        if (k_max > 0)
+          c->launches += launch_search_kmax_cap(a, k_max, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, w.in_ptr3, w.ballots, w.prefix16, s);
+        c->launches += launch_exclusive_scan(g->d_row_ptr, b->n_hits + 1, w.scan_tmp, s);
+        c->launches += launch_exclusive_scan(w.in_ptr3, 3 * b->n_hits + 1, w.scan_tmp, s);
+        c->launches += launch_in_ptr_from3(b->n_hits, w.in_ptr3, g->d_in_ptr, s);
+      } else if (k_max == 0) {
+        c->launches += launch_search_count(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_in_ptr, nullptr, nullptr, s);
         c->launches += launch_exclusive_scan(g->d_row_ptr, b->n_hits + 1, w.scan_tmp, s);
         c->launches += launch_exclusive_scan(g->d_in_ptr, b->n_hits + 1, w.scan_tmp, s);
       } else {                                       // next row: capped search (graph_kmax.cu)
@@ -805,17 +815,16 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
     cudaMemcpyAsync(&host[2], g->d_row_ptr + b->n_hits, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
     if (cudaStreamSynchronize(s) != cudaSuccess) return check_cuda(c, "etx_build_graph (count)");
     if (etx_status st = check_cuda(c, "etx_build_graph (count)")) return st;
-    if (kmax_tiled && host[1] != 0) { kmax_tiled = false; continue; }   // a window longer than the kept vote words: redo
+    if (tiled && host[1] != 0 && !(host[0] & 3)) { tiled = false; continue; }   // a window longer than the kept vote words: redo
     break;
   }
   if (host[0] & 1) return fail(c, ETX_ERR_INVALID, "malformed batch: event_ptr not monotone / plane id >= n_planes");
   if (host[0] & 2) return fail(c, ETX_ERR_UNSORTED, "hits of an event are not sorted by plane");
-  host[1] = host[2];
-  g->n_edges = host[1];
+  g->n_edges = host[2];
   if (g->n_edges > g->edge_capacity)
     return fail(c, ETX_ERR_CAPACITY, "graph needs " + std::to_string(g->n_edges) + " edges, capacity " +
                                          std::to_string(g->edge_capacity));
-  if (k_max > 0 && !kmax_tiled) {
+  if (k_max > 0 && !tiled) {
     // the by-destination lists depend on which edges survived the cap: forward fill first, then in-degrees,
     // scan, and the incoming side from the capped edge list
     ProfScope ps(c, ETX_K_GRAPH, s);
@@ -827,7 +836,7 @@ etx_status etx_build_graph(etx_ctx* c, const etx_batch* b, const float* d_emb, f
   } else if (g->n_edges > 0) {
     ProfScope ps(c, ETX_K_GRAPH, s);
     c->launches += launch_search_fill(a, w.plane_ptr, w.hit_event, w.flags, g->d_row_ptr, g->d_src, g->d_dst,
-                                      g->d_in_ptr, g->d_in_perm, w.cursor, w.ballots, s);
+                                      g->d_in_ptr, g->d_in_perm, w.cursor, tiled ? w.ballots : nullptr, w.prefix16, w.in_ptr3, s);
   }
   return check_cuda(c, "etx_build_graph (fill)");
 }

@@ -179,11 +179,13 @@ __device__ __forceinline__ unsigned sel4(unsigned b0, unsigned b1, unsigned b2, 
 }
 
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-search_tile_count_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t* __restrict__ flags,
-                         int32_t* __restrict__ out_deg /*zeroed*/, int32_t* __restrict__ in_deg /*zeroed*/,
-                         uint32_t* __restrict__ ballots /*[n_hits][kBallotWords]*/) {
+search_tile_count_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, int32_t* __restrict__ flags,
+                         int32_t* __restrict__ out_deg /*zeroed*/, int32_t* __restrict__ in_deg3 /*[n_hits][3], zeroed*/,
+                         uint32_t* __restrict__ ballots /*[n_hits][kBallotWords]*/,
+                         uint16_t* __restrict__ prefix16 /*[n_hits][kBallotWords]*/) {
   if (flags[0] != 0) return;
   __shared__ float4 cand[kTileCand];
+  __shared__ int s_in[kTileCand];                  // edges of THIS plane's sources into every candidate of the window
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int L = a.n_planes;
   const long long n_work = (long long)a.n_events * (L - 1);
@@ -196,39 +198,51 @@ search_tile_count_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, con
     const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
     const int j0 = s1, j1 = pp[top + 1];
     if (s1 <= s0 || j1 <= j0) continue;            // uniform over the CTA
-    for (int c0 = 0; c0 < j1 - j0; c0 += kTileCand) {
-      const int ncc = (j1 - j0 - c0) < kTileCand ? (j1 - j0 - c0) : kTileCand;
-      __syncthreads();                             // the previous chunk / window is no longer read
-      for (int t = threadIdx.x; t < ncc; t += blockDim.x) cand[t] = __ldg(emb4 + j0 + c0 + t);
-      __syncthreads();
-      const int nw = (ncc + 31) >> 5;
-      for (int i0 = s0 + 4 * warp; i0 < s1; i0 += 4 * kWarpsPerBlock) {
-        unsigned long long n01[4], n23[4];
+    const int ncc = j1 - j0;
+    if (ncc > kTileCand) {                         // more candidates than vote words are kept: the caller redoes the build
+      if (threadIdx.x == 0) atomicOr(&flags[1], 1);  // with the one-warp-per-source kernels
+      continue;
+    }
+    __syncthreads();                               // the previous window is no longer read
+    for (int t = threadIdx.x; t < ncc; t += blockDim.x) { cand[t] = __ldg(emb4 + j0 + t); s_in[t] = 0; }
+    __syncthreads();
+    const int nw = (ncc + 31) >> 5;
+    for (int i0 = s0 + 4 * warp; i0 < s1; i0 += 4 * kWarpsPerBlock) {
+      unsigned long long n01[4], n23[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const float4 m = __ldg(emb4 + (i0 + k < s1 ? i0 + k : s1 - 1));
-          n01[k] = pack2(-m.x, -m.y); n23[k] = pack2(-m.z, -m.w);
-        }
-        int cnt = 0;                               // lane k < 4 keeps source i0 + k's count
-        for (int t = 0; t < nw; ++t) {
-          const int idx = t * 32 + lane;
-          const bool vld = idx < ncc;
-          const float4 cq = cand[vld ? idx : ncc - 1];
-          const bool ok0 = (dist2_d4(n01[0], n23[0], cq) < r2) & vld, ok1 = (dist2_d4(n01[1], n23[1], cq) < r2) & vld;
-          const bool ok2 = (dist2_d4(n01[2], n23[2], cq) < r2) & vld, ok3 = (dist2_d4(n01[3], n23[3], cq) < r2) & vld;
-          const unsigned b0 = __ballot_sync(kFull, ok0), b1 = __ballot_sync(kFull, ok1);
-          const unsigned b2 = __ballot_sync(kFull, ok2), b3 = __ballot_sync(kFull, ok3);
-          const int tw = (c0 >> 5) + t;
-          const unsigned mine = sel4(b0, b1, b2, b3, lane & 3);
-          if (lane < 4 && i0 + lane < s1) {
-            if (tw < kBallotWords) ballots[(size_t)(i0 + lane) * kBallotWords + tw] = mine;
-            cnt += __popc(mine);
-          }
-          const int n_in = (int)ok0 + (int)(ok1 & (i0 + 1 < s1)) + (int)(ok2 & (i0 + 2 < s1)) + (int)(ok3 & (i0 + 3 < s1));
-          if (n_in) atomicAdd(&in_deg[j0 + c0 + idx], n_in);
-        }
-        if (lane < 4 && i0 + lane < s1) out_deg[i0 + lane] += cnt;      // one owner per source: plain add across chunks
+      for (int k = 0; k < 4; ++k) {
+        const float4 m = __ldg(emb4 + (i0 + k < s1 ? i0 + k : s1 - 1));
+        n01[k] = pack2(-m.x, -m.y); n23[k] = pack2(-m.z, -m.w);
       }
+      int cnt = 0;                                 // lane k < 4 keeps source i0 + k's count
+      for (int t = 0; t < nw; ++t) {
+        const int idx = t * 32 + lane;
+        const bool vld = idx < ncc;
+        const float4 cq = cand[vld ? idx : ncc - 1];
+        const bool ok0 = (dist2_d4(n01[0], n23[0], cq) < r2) & vld, ok1 = (dist2_d4(n01[1], n23[1], cq) < r2) & vld;
+        const bool ok2 = (dist2_d4(n01[2], n23[2], cq) < r2) & vld, ok3 = (dist2_d4(n01[3], n23[3], cq) < r2) & vld;
+        const unsigned b0 = __ballot_sync(kFull, ok0), b1 = __ballot_sync(kFull, ok1);
+        const unsigned b2 = __ballot_sync(kFull, ok2), b3 = __ballot_sync(kFull, ok3);
+        const unsigned mine = sel4(b0, b1, b2, b3, lane & 3);
+        if (lane < 4 && i0 + lane < s1) {
+          const size_t at = (size_t)(i0 + lane) * kBallotWords + t;
+          ballots[at] = mine;
+          prefix16[at] = (uint16_t)cnt;            // votes of this source in the words before this one (<= 1024)
+          cnt += __popc(mine);
+        }
+        const int n_in = (int)ok0 + (int)(ok1 & (i0 + 1 < s1)) + (int)(ok2 & (i0 + 2 < s1)) + (int)(ok3 & (i0 + 3 < s1));
+        if (n_in) atomicAdd(&s_in[idx], n_in);     // shared-memory counter: this CTA is the only writer of (candidate, plane gap)
+      }
+      if (lane < 4 && i0 + lane < s1) out_deg[i0 + lane] = cnt;
+    }
+    __syncthreads();
+    // The in-list of a hit is ordered by source index = by source plane first: three sub-lists (gap 3, 2, 1), each counted
+    // by exactly one CTA -- no global atomics, and the fill pass can place every edge id at its final position.
+    const int q2 = pp[(p + 2 < L) ? p + 2 : L], q3 = pp[(p + 3 < L) ? p + 3 : L];
+    for (int t = threadIdx.x; t < ncc; t += blockDim.x) {
+      const int j = j0 + t;
+      const int g = 1 + (int)(j >= q2) + (int)(j >= q3);
+      in_deg3[(size_t)3 * j + (3 - g)] = s_in[t];
     }
   }
 }
@@ -250,8 +264,8 @@ __device__ __forceinline__ unsigned long long cap_key(float d2, int j) {
 
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 search_kmax_cap_kernel(GraphArgs a, int k_max, const int32_t* __restrict__ plane_ptr, const int32_t* __restrict__ hit_event,
-                       int32_t* __restrict__ flags, int32_t* __restrict__ out_deg, int32_t* __restrict__ in_deg,
-                       uint32_t* __restrict__ ballots) {
+                       int32_t* __restrict__ flags, int32_t* __restrict__ out_deg, int32_t* __restrict__ in_deg3,
+                       uint32_t* __restrict__ ballots, uint16_t* __restrict__ prefix16) {
   if (flags[0] != 0) return;
   __shared__ unsigned long long s_keys[kWarpsPerBlock][kCapListMax];
   const int lane = threadIdx.x & 31;
@@ -268,10 +282,7 @@ search_kmax_cap_kernel(GraphArgs a, int k_max, const int32_t* __restrict__ plane
     const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
     const int j1 = pp[top + 1];
     const int nw = (j1 - j0 + 31) >> 5;
-    if (nw > kBallotWords) {                       // some votes were not kept: the caller redoes the build with graph_kmax.cu
-      if (lane == 0) atomicOr(&flags[1], 1);
-      continue;
-    }
+    if (nw > kBallotWords) continue;               // flagged by the count pass: the caller redoes the build with graph_kmax.cu
     const float4 m = __ldg(emb4 + i);
     const unsigned long long n01 = pack2(-m.x, -m.y), n23 = pack2(-m.z, -m.w);
     const unsigned word = lane < nw ? ballots[(size_t)i * kBallotWords + lane] : 0u;
@@ -317,72 +328,97 @@ search_kmax_cap_kernel(GraphArgs a, int k_max, const int32_t* __restrict__ plane
         if (cap_key(dist2_d4(n01, n23, __ldg(emb4 + jw + bit)), jw + bit) > thr) keep &= ~(1u << bit);
       }
     }
-    for (unsigned w = word & ~keep; w; w &= w - 1) atomicSub(&in_deg[jw + __ffs(w) - 1], 1);
-    if (lane < nw && keep != word) ballots[(size_t)i * kBallotWords + lane] = keep;
-    if (lane == 0) out_deg[i] = k_max;
-  }
-}
-
-// Fill pass for d = 4: one warp per source expands its vote words into edges (ascending candidate index, so the CSR is
-// the same unique array) and drops each edge id into its destination's list; words past kBallotWords are re-tested.
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
-search_ballot_fill_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t* __restrict__ hit_event,
-                          const int32_t* __restrict__ flags, const uint32_t* __restrict__ ballots,
-                          const int32_t* __restrict__ row_ptr, int32_t* __restrict__ src, int32_t* __restrict__ dst,
-                          const int32_t* __restrict__ in_ptr, int32_t* __restrict__ in_perm, int32_t* __restrict__ cursor) {
-  if (flags[0] != 0) return;
-  const int lane = threadIdx.x & 31;
-  const int n_warps = gridDim.x * kWarpsPerBlock;
-  const unsigned lt = (1u << lane) - 1u;
-  const int L = a.n_planes;
-  for (int i = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5); i < a.n_hits; i += n_warps) {
-    const int base_out = row_ptr[i], deg = row_ptr[i + 1] - base_out;
-    if (deg == 0) continue;
-    const int p = a.plane[i];
-    const int32_t* pp = plane_ptr + (size_t)hit_event[i] * (L + 1);
-    const int j0 = pp[p + 1];
-    const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
-    const int j1 = pp[top + 1];
-    // Lane t owns vote word t: ONE coalesced load brings all of the source's words, a warp scan of their popcounts gives
-    // every word its first edge slot, and each lane walks its own set bits (1-3 per word) -- instead of the warp
-    // stepping through the words one after the other with 31 idle lanes per edge.
-    const int nw = (j1 - j0 + 31) >> 5;
-    const unsigned word = (lane < nw && lane < kBallotWords) ? __ldg(ballots + (size_t)i * kBallotWords + lane) : 0u;
-    int before = __popc(word);
+    const int q2 = pp[(p + 2 < L) ? p + 2 : L], q3 = pp[(p + 3 < L) ? p + 3 : L];
+    for (unsigned w = word & ~keep; w; w &= w - 1) {
+      const int j = jw + __ffs(w) - 1;
+      const int g = 1 + (int)(j >= q2) + (int)(j >= q3);
+      atomicSub(&in_deg3[(size_t)3 * j + (3 - g)], 1);
+    }
+    int before = __popc(keep);                     // the surviving votes' prefix counts replace the count pass's
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       const int t = __shfl_up_sync(kFull, before, o);
       if (lane >= o) before += t;
     }
-    const int kept = __shfl_sync(kFull, before, 31);       // edges described by the kept words
-    before -= __popc(word);
-    const int jw = j0 + lane * 32;
-    int k = 0;
-    for (unsigned w = word; w; w &= w - 1, ++k) {
-      const int j = jw + __ffs(w) - 1;
-      const int pos = base_out + before + k;
-      src[pos] = i;
-      dst[pos] = j;
-      in_perm[in_ptr[j] + atomicAdd(&cursor[j], 1)] = pos;
+    before -= __popc(keep);
+    if (lane < nw) {
+      ballots[(size_t)i * kBallotWords + lane] = keep;
+      prefix16[(size_t)i * kBallotWords + lane] = (uint16_t)before;
     }
-    if (kept < deg) {
-      // a window longer than the kept words: the rest is re-tested, 32 candidates per step, as round 1's fill pass did
-      const float4 m = __ldg(reinterpret_cast<const float4*>(a.emb) + i);
-      const unsigned long long n01 = pack2(-m.x, -m.y), n23 = pack2(-m.z, -m.w);
-      int cnt = kept;
-      for (int t = kBallotWords; cnt < deg; ++t) {
-        const int j = j0 + t * 32 + lane, jc = j < j1 ? j : j1 - 1;
-        const unsigned b = __ballot_sync(kFull, (dist2_d4(n01, n23, __ldg(reinterpret_cast<const float4*>(a.emb) + jc)) < a.r2_max) & (j < j1));
-        if ((b >> lane) & 1u) {
-          const int pos = base_out + cnt + __popc(b & lt);
-          src[pos] = i;
-          dst[pos] = j;
-          in_perm[in_ptr[j] + atomicAdd(&cursor[j], 1)] = pos;
+    if (lane == 0) out_deg[i] = k_max;
+  }
+}
+
+// Fill pass for d = 4: the same (event, source plane) tiling as the count pass, candidate-major.  A warp takes one vote word of
+// the window -- 32 candidates, one per lane -- and walks the plane's sources in ascending order: a set bit is the edge
+// (i -> j); its id is row_ptr[i] + (votes of i before this word) + (votes of i below this bit), and because the sources come
+// in ascending order the lane's running count is the edge's rank inside the candidate's sub-list of this plane gap.  So src,
+// dst AND the by-destination lists are written at their final positions: no cursor atomics, no sort pass.
+constexpr int kFillSrc = 64;                       // sources whose vote words are staged per step
+
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+search_pair_fill_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t* __restrict__ flags,
+                        const uint32_t* __restrict__ ballots, const uint16_t* __restrict__ prefix16,
+                        const int32_t* __restrict__ row_ptr, const int32_t* __restrict__ in_ptr3,
+                        int32_t* __restrict__ src, int32_t* __restrict__ dst, int32_t* __restrict__ in_perm) {
+  if (flags[0] != 0) return;
+  // the sources' vote words, prefix counts and first edge ids are staged in shared memory by all threads at once (read
+  // one by one from global memory in the source loop they cost a DRAM latency each: 0.83 ms instead of 0.2)
+  __shared__ uint32_t s_w[kFillSrc * kBallotWords];
+  __shared__ uint16_t s_pre[kFillSrc * kBallotWords];
+  __shared__ int32_t s_row[kFillSrc];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
+  const int L = a.n_planes;
+  const long long n_work = (long long)a.n_events * (L - 1);
+  for (long long work = blockIdx.x; work < n_work; work += gridDim.x) {
+    const int ev = (int)(work / (L - 1)), p = (int)(work % (L - 1));
+    const int32_t* pp = plane_ptr + (size_t)ev * (L + 1);
+    const int s0 = pp[p], s1 = pp[p + 1];
+    const int top = (p + a.gap < L - 1) ? p + a.gap : L - 1;
+    const int j0 = s1, j1 = pp[top + 1];
+    if (s1 <= s0 || j1 <= j0 || j1 - j0 > kTileCand) continue;
+    const int q2 = pp[(p + 2 < L) ? p + 2 : L], q3 = pp[(p + 3 < L) ? p + 3 : L];
+    const int nw = (j1 - j0 + 31) >> 5;
+    int at[(kBallotWords + kWarpsPerBlock - 1) / kWarpsPerBlock];     // next free position of this lane's candidates' sub-lists
+#pragma unroll
+    for (int r = 0; r < (kBallotWords + kWarpsPerBlock - 1) / kWarpsPerBlock; ++r) {
+      const int j = j0 + (warp + r * kWarpsPerBlock) * 32 + lane;
+      const int g = 1 + (int)(j >= q2) + (int)(j >= q3);
+      at[r] = (warp + r * kWarpsPerBlock < nw && j < j1) ? in_ptr3[(size_t)3 * j + (3 - g)] : 0;
+    }
+    for (int c0 = s0; c0 < s1; c0 += kFillSrc) {
+      const int ns = (s1 - c0) < kFillSrc ? (s1 - c0) : kFillSrc;
+      __syncthreads();                             // the previous step's words are no longer read
+      for (int x = threadIdx.x; x < ns * nw; x += blockDim.x) {
+        const int ii = x / nw, t = x - ii * nw;
+        s_w[x] = __ldg(ballots + (size_t)(c0 + ii) * kBallotWords + t);
+        s_pre[x] = __ldg(prefix16 + (size_t)(c0 + ii) * kBallotWords + t);
+      }
+      for (int x = threadIdx.x; x < ns; x += blockDim.x) s_row[x] = row_ptr[c0 + x];
+      __syncthreads();
+#pragma unroll
+      for (int r = 0; r < (kBallotWords + kWarpsPerBlock - 1) / kWarpsPerBlock; ++r) {
+        const int t = warp + r * kWarpsPerBlock;
+        if (t >= nw) break;                        // uniform over the warp
+        const int j = j0 + t * 32 + lane;
+        for (int ii = 0; ii < ns; ++ii) {
+          const unsigned w = s_w[ii * nw + t];     // uniform over the warp
+          if ((w >> lane) & 1u) {
+            const int eid = s_row[ii] + (int)s_pre[ii * nw + t] + __popc(w & lt);
+            src[eid] = c0 + ii;
+            dst[eid] = j;
+            in_perm[at[r]++] = eid;
+          }
         }
-        cnt += __popc(b);
       }
     }
   }
+}
+
+// in_ptr[j] = start of hit j's in-list = start of its first sub-list; in_ptr[n_hits] = E
+__global__ void __launch_bounds__(256) in_ptr_from3_kernel(int n_hits, const int32_t* __restrict__ in_ptr3, int32_t* __restrict__ in_ptr) {
+  for (int j = blockIdx.x * blockDim.x + threadIdx.x; j <= n_hits; j += gridDim.x * blockDim.x) in_ptr[j] = in_ptr3[(size_t)3 * j];
 }
 
 // Orders every destination's list of edge ids ascending.  One warp per hit: a list of <= 32 ids (in-degrees are
@@ -536,26 +572,35 @@ static void launch_search(const GraphArgs& a, const int32_t* plane_ptr, const in
                                                                row_ptr, src, dst, in_ptr, in_perm, cursor);
 }
 
+// d = 4 with the tiled kernels (ballots != null): out_deg and in_deg3 [n_hits][3] (+1) are filled; otherwise the
+// one-warp-per-source count pass fills out_deg and in_deg [n_hits] (passed as in_deg3).
 int launch_search_count(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
-                        const int32_t* flags, int32_t* out_deg, int32_t* in_deg, uint32_t* ballots, cudaStream_t s) {
-  cudaMemsetAsync(in_deg, 0, sizeof(int32_t) * ((size_t)a.n_hits + 1), s);
+                        int32_t* flags, int32_t* out_deg, int32_t* in_deg3, uint32_t* ballots, uint16_t* prefix16, cudaStream_t s) {
   if (a.d == 4 && ballots) {                       // tiled count pass (shared-memory candidate windows, kept vote words)
+    cudaMemsetAsync(in_deg3, 0, sizeof(int32_t) * ((size_t)3 * a.n_hits + 1), s);
     cudaMemsetAsync(out_deg, 0, sizeof(int32_t) * ((size_t)a.n_hits + 1), s);
     const long long n_work = (long long)a.n_events * (a.n_planes - 1);
     const int cap = 148 * 8;
     search_tile_count_kernel<<<(int)(n_work < 1 ? 1 : (n_work < cap ? n_work : cap)), kWarpsPerBlock * 32, 0, s>>>(
-        a, plane_ptr, flags, out_deg, in_deg, ballots);
+        a, plane_ptr, flags, out_deg, in_deg3, ballots, prefix16);
     return 1;
   }
-  launch_search<0>(a, plane_ptr, hit_event, flags, out_deg, in_deg, nullptr, nullptr, nullptr, nullptr,
+  cudaMemsetAsync(in_deg3, 0, sizeof(int32_t) * ((size_t)a.n_hits + 1), s);
+  launch_search<0>(a, plane_ptr, hit_event, flags, out_deg, in_deg3, nullptr, nullptr, nullptr, nullptr,
                    nullptr, nullptr, s);
   return 1;
 }
 
 int launch_search_kmax_cap(const GraphArgs& a, int k_max, const int32_t* plane_ptr, const int32_t* hit_event, int32_t* flags,
-                           int32_t* out_deg, int32_t* in_deg, uint32_t* ballots, cudaStream_t s) {
+                           int32_t* out_deg, int32_t* in_deg3, uint32_t* ballots, uint16_t* prefix16, cudaStream_t s) {
   search_kmax_cap_kernel<<<search_grid(a.n_hits), kWarpsPerBlock * 32, 0, s>>>(a, k_max, plane_ptr, hit_event, flags, out_deg,
-                                                                               in_deg, ballots);
+                                                                               in_deg3, ballots, prefix16);
+  return 1;
+}
+
+int launch_in_ptr_from3(int n_hits, const int32_t* in_ptr3, int32_t* in_ptr, cudaStream_t s) {
+  const int need = (n_hits + 256) / 256;
+  in_ptr_from3_kernel<<<need < 148 * 8 ? need : 148 * 8, 256, 0, s>>>(n_hits, in_ptr3, in_ptr);
   return 1;
 }
 
@@ -567,16 +612,20 @@ int launch_exclusive_scan(int32_t* data, int n, int32_t* tmp, cudaStream_t s) {
   return 3;
 }
 
+// ballots != null: the tiled pair fill (in_ptr3 = scanned sub-list offsets, no cursor, no sort); else the one-warp-per-source
+// fill with cursor atomics and the in-list sort
 int launch_search_fill(const GraphArgs& a, const int32_t* plane_ptr, const int32_t* hit_event,
                        const int32_t* flags, const int32_t* row_ptr, int32_t* src, int32_t* dst,
                        const int32_t* in_ptr, int32_t* in_perm, int32_t* cursor /*[n_hits] scratch*/,
-                       const uint32_t* ballots, cudaStream_t s) {
-  cudaMemsetAsync(cursor, 0, sizeof(int32_t) * (size_t)a.n_hits, s);
+                       const uint32_t* ballots, const uint16_t* prefix16, const int32_t* in_ptr3, cudaStream_t s) {
   if (a.d == 4 && ballots) {
-    search_ballot_fill_kernel<<<search_grid(a.n_hits), kWarpsPerBlock * 32, 0, s>>>(a, plane_ptr, hit_event, flags, ballots,
-                                                                                    row_ptr, src, dst, in_ptr, in_perm, cursor);
-    return 1 + launch_sort_in_lists(a.n_hits, flags, in_ptr, in_perm, s);
+    const long long n_work = (long long)a.n_events * (a.n_planes - 1);
+    const int cap = 148 * 8;
+    search_pair_fill_kernel<<<(int)(n_work < 1 ? 1 : (n_work < cap ? n_work : cap)), kWarpsPerBlock * 32, 0, s>>>(
+        a, plane_ptr, flags, ballots, prefix16, row_ptr, in_ptr3, src, dst, in_perm);
+    return 1;
   }
+  cudaMemsetAsync(cursor, 0, sizeof(int32_t) * (size_t)a.n_hits, s);
   launch_search<1>(a, plane_ptr, hit_event, flags, nullptr, nullptr, row_ptr, src, dst, in_ptr, in_perm, cursor, s);
   return 1 + launch_sort_in_lists(a.n_hits, flags, in_ptr, in_perm, s);
 }
