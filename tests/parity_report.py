@@ -59,7 +59,7 @@ def main():
       "(0.40 / 0.25 were round 1's values, 0.50 / 0.30 the values before that).\n")
     plans = [("c2", [0.40, 0.45, 0.50, 0.55], [3, 1, 2])]
     if not args.quick:
-        plans.append(("c4", [0.25, 0.30, 0.35], [3]))
+        plans.append(("c4", [0.25, 0.30, 0.35], [3, 1]))
     else:
         plans = [("c2", [synth.CONFIGS["c2"].gain], [3, 2])]
     for name, gains, precs in plans:
