@@ -211,10 +211,14 @@ search_tile_count_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, int
       unsigned long long n01[4], n23[4];
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
-        const float4 m = __ldg(emb4 + (i0 + k < s1 ? i0 + k : s1 - 1));
+        // a source slot past the plane's last hit sits infinitely far away: its d^2 overflows to +inf and it never votes
+        const float4 m = (i0 + k < s1) ? __ldg(emb4 + i0 + k) : make_float4(1e30f, 1e30f, 1e30f, 1e30f);
         n01[k] = pack2(-m.x, -m.y); n23[k] = pack2(-m.z, -m.w);
       }
-      int cnt = 0;                                 // lane k < 4 keeps source i0 + k's count
+      const bool owner = lane < 4 && i0 + lane < s1;               // lane k < 4 keeps source i0 + k's words and count
+      uint32_t* const my_words = ballots + (size_t)(i0 + (lane & 3)) * kBallotWords;
+      uint16_t* const my_prefix = prefix16 + (size_t)(i0 + (lane & 3)) * kBallotWords;
+      int cnt = 0;
       for (int t = 0; t < nw; ++t) {
         const int idx = t * 32 + lane;
         const bool vld = idx < ncc;
@@ -223,17 +227,16 @@ search_tile_count_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, int
         const bool ok2 = (dist2_d4(n01[2], n23[2], cq) < r2) & vld, ok3 = (dist2_d4(n01[3], n23[3], cq) < r2) & vld;
         const unsigned b0 = __ballot_sync(kFull, ok0), b1 = __ballot_sync(kFull, ok1);
         const unsigned b2 = __ballot_sync(kFull, ok2), b3 = __ballot_sync(kFull, ok3);
-        const unsigned mine = sel4(b0, b1, b2, b3, lane & 3);
-        if (lane < 4 && i0 + lane < s1) {
-          const size_t at = (size_t)(i0 + lane) * kBallotWords + t;
-          ballots[at] = mine;
-          prefix16[at] = (uint16_t)cnt;            // votes of this source in the words before this one (<= 1024)
+        if (owner) {
+          const unsigned mine = sel4(b0, b1, b2, b3, lane);
+          my_words[t] = mine;
+          my_prefix[t] = (uint16_t)cnt;            // votes of this source in the words before this one (<= 1024)
           cnt += __popc(mine);
         }
-        const int n_in = (int)ok0 + (int)(ok1 & (i0 + 1 < s1)) + (int)(ok2 & (i0 + 2 < s1)) + (int)(ok3 & (i0 + 3 < s1));
+        const int n_in = (int)ok0 + (int)ok1 + (int)ok2 + (int)ok3;
         if (n_in) atomicAdd(&s_in[idx], n_in);     // shared-memory counter: this CTA is the only writer of (candidate, plane gap)
       }
-      if (lane < 4 && i0 + lane < s1) out_deg[i0 + lane] = cnt;
+      if (owner) out_deg[i0 + lane] = cnt;
     }
     __syncthreads();
     // The in-list of a hit is ordered by source index = by source plane first: three sub-lists (gap 3, 2, 1), each counted
@@ -404,6 +407,7 @@ search_pair_fill_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, cons
         const int j = j0 + t * 32 + lane;
         for (int ii = 0; ii < ns; ++ii) {
           const unsigned w = s_w[ii * nw + t];     // uniform over the warp
+          if (w == 0u) continue;
           if ((w >> lane) & 1u) {
             const int eid = s_row[ii] + (int)s_pre[ii * nw + t] + __popc(w & lt);
             src[eid] = c0 + ii;
