@@ -212,7 +212,7 @@ def oracle_events_per_s(cfg, event_ids, keep=None):
 CDF_AT = [1e-7, 1e-6, 1e-5, 1e-4, 1e-3, 1e-2, 2e-2, 5e-2]
 
 
-def compare_with_oracle(gpu, ora):
+def compare_with_oracle(gpu, ora, event_ptr=None):
     """End-to-end comparison of one GPU run with the oracle's on the same events (reading Q16): the edge sets
     (symmetric difference: the two embeddings decide pairs near the radius differently) and the score error on the common edges
     with its CDF and the oracle's score histogram (reading Q14)."""
@@ -222,7 +222,18 @@ def compare_with_oracle(gpu, ora):
     common, ig, io = np.intersect1d(kg, ko, assume_unique=True, return_indices=True)
     d = np.abs(gpu["scores"][ig].astype(np.float64) - np.asarray(ora["scores"], np.float64)[io])
     hist, _ = np.histogram(np.asarray(ora["scores"], np.float64), bins=10, range=(0.0, 1.0))
-    return {"edges_gpu": int(len(kg)), "edges_oracle": int(len(ko)), "common": int(len(common)),
+    same = {}
+    if event_ptr is not None:
+        # the tolerance is defined on identical graphs: the events in which both sides found exactly the same edges
+        ep = np.asarray(event_ptr, np.int64)
+        ev_of = lambda hits: np.searchsorted(ep, hits, side="right") - 1
+        only = np.concatenate([np.setdiff1d(kg, common), np.setdiff1d(ko, common)]) // n
+        bad = np.unique(ev_of(only)) if len(only) else np.zeros(0, np.int64)
+        keep = ~np.isin(ev_of(common // n), bad)
+        same = {"events_with_identical_graphs": int(len(ep) - 1 - len(bad)),
+                "score_err_on_identical_graphs": {"edges": int(keep.sum()), "max": float(d[keep].max(initial=0.0)),
+                                                  "p99": float(np.quantile(d[keep], 0.99)) if keep.any() else 0.0}}
+    return {**same, "edges_gpu": int(len(kg)), "edges_oracle": int(len(ko)), "common": int(len(common)),
             "only_gpu": int(len(kg) - len(common)), "only_oracle": int(len(ko) - len(common)),
             "score_err_on_common": {"max": float(d.max(initial=0.0)), "p99": float(np.quantile(d, 0.99)) if len(d) else 0.0,
                                     "median": float(np.median(d)) if len(d) else 0.0},
@@ -572,7 +583,7 @@ def run_ours(args):
                           "side has (pairs within 1e-5 of the radius) also move the scores of their neighbours, which is what the "
                           "maximum shows when only_gpu + only_oracle > 0",
                   "gate": {synth.PREC_BF16: 2e-2, synth.PREC_INT8: None, synth.PREC_FP8: None}.get(int(etx.desc.precision), 1e-4),
-                  **compare_with_oracle(gpu_s, kept["out"])}
+                  **compare_with_oracle(gpu_s, kept["out"], kept["batch"]["event_ptr"])}
         if H == 128 and int(etx.desc.precision) != synth.PREC_FP32:
             # reading Q16's report: the same events with a bf16 EMBEDDING (etx_embed_bf16) -- which edges change, and the
             # score error on the edges both graphs have
@@ -580,7 +591,7 @@ def run_ours(args):
                                      embed="etx_embed_bf16")
             next_rows["bf16_embedding_end_to_end"] = {
                 "note": "report only (reading Q16): the step with etx_embed_bf16 instead of the 3xTF32 embedding, same radius",
-                **compare_with_oracle(gpu_b, kept["out"])}
+                **compare_with_oracle(gpu_b, kept["out"], kept["batch"]["event_ptr"])}
         cpu = {"value": v, "unit": "events/s", "cores": orc.n_threads(), "kind": "oracle",
                "sample": f"first {n_s} events of {args.config} ({nh} hits, {ne} edges) in {dt:.1f} s",
                "note": "the oracle is deliberately unoptimised (per-neuron loops, double accumulators, no BLAS/SIMD, OpenMP "
