@@ -357,6 +357,19 @@ search_kmax_cap_kernel(GraphArgs a, int k_max, const int32_t* __restrict__ plane
 // (i -> j); its id is row_ptr[i] + (votes of i before this word) + (votes of i below this bit), and because the sources come
 // in ascending order the lane's running count is the edge's rank inside the candidate's sub-list of this plane gap.  So src,
 // dst AND the by-destination lists are written at their final positions: no cursor atomics, no sort pass.
+// Transposes a 32 x 32 bit matrix held one row per lane (bit c of lane l's word = element (l, c)); on return bit l of lane
+// c's word = element (l, c).  Five stages; stage j swaps the off-diagonal j x j blocks of every 2j x 2j block.
+__device__ __forceinline__ unsigned transpose_bits(unsigned x, int lane) {
+  unsigned lo_cols = 0x0000ffffu;                  // columns whose index has bit j clear
+#pragma unroll
+  for (int j = 16; j >= 1; j >>= 1) {
+    const unsigned other = __shfl_xor_sync(kFull, x, j);
+    x = (lane & j) ? ((x & ~lo_cols) | ((other >> j) & lo_cols)) : ((x & lo_cols) | ((other << j) & ~lo_cols));
+    lo_cols ^= lo_cols << (j >> 1);
+  }
+  return x;
+}
+
 constexpr int kFillSrc = 64;                       // sources whose vote words are staged per step
 
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
@@ -393,10 +406,11 @@ search_pair_fill_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, cons
     for (int c0 = s0; c0 < s1; c0 += kFillSrc) {
       const int ns = (s1 - c0) < kFillSrc ? (s1 - c0) : kFillSrc;
       __syncthreads();                             // the previous step's words are no longer read
+      // staged word-major, [t][source], so that the 32 sources of a block sit in 32 consecutive banks
       for (int x = threadIdx.x; x < ns * nw; x += blockDim.x) {
         const int ii = x / nw, t = x - ii * nw;
-        s_w[x] = __ldg(ballots + (size_t)(c0 + ii) * kBallotWords + t);
-        s_pre[x] = __ldg(prefix16 + (size_t)(c0 + ii) * kBallotWords + t);
+        s_w[t * kFillSrc + ii] = __ldg(ballots + (size_t)(c0 + ii) * kBallotWords + t);
+        s_pre[t * kFillSrc + ii] = __ldg(prefix16 + (size_t)(c0 + ii) * kBallotWords + t);
       }
       for (int x = threadIdx.x; x < ns; x += blockDim.x) s_row[x] = row_ptr[c0 + x];
       __syncthreads();
@@ -405,11 +419,17 @@ search_pair_fill_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, cons
         const int t = warp + r * kWarpsPerBlock;
         if (t >= nw) break;                        // uniform over the warp
         const int j = j0 + t * 32 + lane;
-        for (int ii = 0; ii < ns; ++ii) {
-          const unsigned w = s_w[ii * nw + t];     // uniform over the warp
-          if (w == 0u) continue;
-          if ((w >> lane) & 1u) {
-            const int eid = s_row[ii] + (int)s_pre[ii * nw + t] + __popc(w & lt);
+        for (int b0 = 0; b0 < ns; b0 += 32) {
+          // 32 sources x 32 candidates of votes: lane = source on the way in, lane = candidate after the transposition
+          // (five block-swap stages), so that every lane walks only ITS candidate's votes, sources ascending -- the order of
+          // the by-destination list -- instead of all lanes stepping through every (source, word) pair for one vote each.
+          unsigned v = (b0 + lane < ns) ? s_w[t * kFillSrc + b0 + lane] : 0u;
+          if (__ballot_sync(kFull, v != 0u) == 0u) continue;
+          v = transpose_bits(v, lane);
+          while (v != 0u) {
+            const int ii = b0 + __ffs((int)v) - 1;
+            v &= v - 1u;
+            const int eid = s_row[ii] + (int)s_pre[t * kFillSrc + ii] + __popc(s_w[t * kFillSrc + ii] & lt);
             src[eid] = c0 + ii;
             dst[eid] = j;
             in_perm[at[r]++] = eid;
