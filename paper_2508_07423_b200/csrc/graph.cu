@@ -174,8 +174,15 @@ search_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t*
 // longer than kBallotWords x 32 candidates re-tests only the words that did not fit.
 constexpr int kTileCand = 1024;                    // candidates staged per chunk (16 KB)
 
+// b[k & 3] as three selects (a chain of comparisons became a jump table in the inner loop)
 __device__ __forceinline__ unsigned sel4(unsigned b0, unsigned b1, unsigned b2, unsigned b3, int k) {
-  return k == 0 ? b0 : (k == 1 ? b1 : (k == 2 ? b2 : b3));
+  const unsigned lo = (k & 1) ? b1 : b0, hi = (k & 1) ? b3 : b2;
+  return (k & 2) ? hi : lo;
+}
+// shared-memory counter update on a 32-bit shared address (atomicAdd on the generic pointer re-derived the window base from
+// the CTA id in every iteration)
+__device__ __forceinline__ void red_shared_add(uint32_t addr, int v) {
+  asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
@@ -207,6 +214,7 @@ search_tile_count_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, int
     for (int t = threadIdx.x; t < ncc; t += blockDim.x) { cand[t] = __ldg(emb4 + j0 + t); s_in[t] = 0; }
     __syncthreads();
     const int nw = (ncc + 31) >> 5;
+    const uint32_t s_in_lane = (uint32_t)__cvta_generic_to_shared(s_in + lane);
     for (int i0 = s0 + 4 * warp; i0 < s1; i0 += 4 * kWarpsPerBlock) {
       unsigned long long n01[4], n23[4];
 #pragma unroll
@@ -234,7 +242,7 @@ search_tile_count_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, int
           cnt += __popc(mine);
         }
         const int n_in = (int)ok0 + (int)ok1 + (int)ok2 + (int)ok3;
-        if (n_in) atomicAdd(&s_in[idx], n_in);     // shared-memory counter: this CTA is the only writer of (candidate, plane gap)
+        if (n_in) red_shared_add(s_in_lane + (uint32_t)t * 128u, n_in);  // this CTA is the only writer of (candidate, plane gap)
       }
       if (owner) out_deg[i0 + lane] = cnt;
     }
