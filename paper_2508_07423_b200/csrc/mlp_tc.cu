@@ -74,7 +74,7 @@ constexpr uint32_t kBarEntry0 = 2;       // named barriers 2 .. 2 + NSTAGE_A - 1
 constexpr int kRegGather = 64, kRegEpi = 104, kRegCtl = 40;
 constexpr int HW = 128;                       // hidden width handled by this kernel
 constexpr int kAtomBytes = 128 * 128;         // one operand tile: 128 rows x 128 bytes (one swizzle atom wide)
-constexpr int kStageOutBytes = 8 * 4096;      // output staging: one 4 KB box [32 rows x 32 fp32 columns] per epilogue warp
+constexpr int kStageBoxBytes = 8 * 4096;      // output staging: 4 KB boxes [32 rows x 32 fp32 columns], Cfg::STAGE_BOXES per epilogue warp
 
 template <int MODE> struct Cfg;
 template <> struct Cfg<ETX_PREC_TF32X3> {
@@ -87,6 +87,7 @@ template <> struct Cfg<ETX_PREC_TF32X3> {
   static constexpr int NSTAGE_W = 2;          // weight ring stages (32 KB each)
   static constexpr int NSTAGE_A = 4;          // first-layer A operand ring stages (32 KB each)
   static constexpr int PREFETCH = 4;          // K-chunks a gather thread keeps in flight in registers
+  static constexpr int STAGE_BOXES = 1;
   static constexpr int HID_COLS = 128;        // TMEM columns per piece of a hidden operand
   static constexpr uint32_t IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);
 };
@@ -97,6 +98,7 @@ template <> struct Cfg<ETX_PREC_BF16> {
   static constexpr int NSTAGE_W = 4;          // 16 KB each
   static constexpr int NSTAGE_A = 8;          // 16 KB each
   static constexpr int PREFETCH = 2;
+  static constexpr int STAGE_BOXES = 1;
   static constexpr int HID_COLS = 64;         // 128 bf16 = 64 columns
   static constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);
 };
@@ -107,6 +109,7 @@ template <> struct Cfg<ETX_PREC_BF16X3> {
   static constexpr int NSTAGE_W = 2;          // 32 KB each
   static constexpr int NSTAGE_A = 4;          // 32 KB each
   static constexpr int PREFETCH = 2;
+  static constexpr int STAGE_BOXES = 1;
   static constexpr int HID_COLS = 64;
   static constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);
 };
@@ -122,6 +125,7 @@ template <> struct Cfg<ETX_PREC_INT8> {
   static constexpr int NSTAGE_W = 4;          // 16 KB each
   static constexpr int NSTAGE_A = 8;          // 16 KB each
   static constexpr int PREFETCH = 2;
+  static constexpr int STAGE_BOXES = 1;
   static constexpr int HID_COLS = 32;         // 128 codes = 32 columns
   static constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);   // D = s32, A = B = s8
 };
@@ -135,8 +139,19 @@ template <> struct Cfg<ETX_PREC_FP8> {
   static constexpr int NSTAGE_W = 4;          // 16 KB each
   static constexpr int NSTAGE_A = 8;          // 16 KB each
   static constexpr int PREFETCH = 2;
+  static constexpr int STAGE_BOXES = 1;
   static constexpr int HID_COLS = 32;         // 128 codes = 32 columns
   static constexpr uint32_t IDESC = (1u << 4) | (0u << 7) | (0u << 10) | ((HW >> 3) << 17) | ((TM >> 4) << 24);   // D = f32, A = B = e4m3
+};
+
+// Shared-memory split per launch variant.  The wide per-hit projection launches (VAR 1: one layer, 256 output columns,
+// output-bound) trade one operand-ring entry for a second staging slice per epilogue warp, so that a warp's two output
+// boxes never wait for each other's TMA read (projections 3.79 -> 3.38 ms per step at C2); the multi-layer launches keep
+// the deeper ring (edge network +2.5 % with 3 entries: its fp32 addend alone takes two).
+template <int MODE, int VAR> struct Split {
+  static constexpr bool kTwoBoxes = (MODE == ETX_PREC_BF16X3 && VAR == 1);
+  static constexpr int NSTAGE_A = Cfg<MODE>::NSTAGE_A - (kTwoBoxes ? 1 : 0);
+  static constexpr int STAGE_BOXES = kTwoBoxes ? 2 : Cfg<MODE>::STAGE_BOXES;
 };
 
 using namespace tcp;
@@ -255,7 +270,7 @@ __device__ __forceinline__ void tmem_cp_128x256b(uint32_t taddr, uint64_t desc) 
 template <int MODE, int VAR>
 __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap tmap) {
   using C = Cfg<MODE>;
-  constexpr int KA = C::KA, P = C::PIECES, NSW = C::NSTAGE_W, NSA = C::NSTAGE_A, HID_COLS = C::HID_COLS;
+  constexpr int KA = C::KA, P = C::PIECES, NSW = C::NSTAGE_W, NSA = Split<MODE, VAR>::NSTAGE_A, HID_COLS = C::HID_COLS;
   constexpr uint32_t kStageBytes = P * kAtomBytes;
   static_assert(NSW <= 8 && NSA <= 8, "Bars holds 8 mbarriers per ring");
   constexpr uint32_t COL_ACC = 0;
@@ -297,6 +312,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
   const uint32_t stage_out = aring + NSA * kStageBytes;                  // 32 KB: one swizzled 4 KB staging box per epilogue warp
   unsigned char* gen = smem_raw;
   float* wlast_s = reinterpret_cast<float*>(gen + (NSW + NSA) * kStageBytes);   // [128] / [128][8]: classifier and narrow-output launches stage no output, so this aliases the staging boxes
+  constexpr int kStageOutBytes = Split<MODE, VAR>::STAGE_BOXES * kStageBoxBytes;
   float* bias_s = reinterpret_cast<float*>(gen + (NSW + NSA) * kStageBytes + kStageOutBytes);   // [kTcLayers][128]
   Bars* bars = reinterpret_cast<Bars*>(bias_s + kTcLayers * HW);
   if (base & 1023u) __trap();
@@ -864,7 +880,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
           // warp starts the next tile's first layer while the boxes drain).  Two TMA operations per warp and tile:
           // in-kernel counters put the issue of one operation at ~420 cycles of the issuing warp with all eight
           // epilogue warps at it (16 boxes of 4 KB per tile instead of round 1's 32 of 2 KB).
-          const uint32_t stg = stage_out + ew * 4096;
+          constexpr int SB = Split<MODE, VAR>::STAGE_BOXES;
+          const uint32_t stg0 = stage_out + ew * (SB * 4096);
           const bool in_place_add = (a.out_mode == 1);
           const int row0 = tile * TM + q4 * 32;
           EP_T0();
@@ -881,7 +898,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
           for (int q = 0; q < (ETX_EXP(a, 16) ? 0 : 2); ++q) {       // (timing experiment 16, wrong results: no output at all)
             const int col0 = HH * 64 + q * 32;
             EP_T0();
-            if (lane == 0) bulk_wait_read0();      // the TMA unit has read the previous box out of the staging slice
+            const uint32_t stg = stg0 + (SB == 2 ? q * 4096 : 0);
+            if (lane == 0) {                       // the TMA unit has read the slice's previous box (with a slice per box that
+              if constexpr (SB == 2) bulk_wait_read1(); else bulk_wait_read0();   // is the LAST tile's: one newer group may be pending)
+            }
             __syncwarp();
             EP_ACC(6);
             // The box's 32 biases first, all eight 128-bit loads in flight together: st_shared_v4 is an asm volatile
@@ -1159,7 +1179,7 @@ int launch_mode(const TcArgs& a, int sm_count, cudaStream_t s) {
   if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return -1;
   // rings (192 KB) + output staging (32 KB; the classifier's / narrow output's last-layer weights alias it) + biases +
   // barriers: 226.8 of the 227 KB an SM offers
-  const size_t smem = (size_t)(C::NSTAGE_W + C::NSTAGE_A) * C::PIECES * kAtomBytes + kStageOutBytes +
+  const size_t smem = (size_t)(C::NSTAGE_W + Split<MODE, VAR>::NSTAGE_A) * C::PIECES * kAtomBytes + Split<MODE, VAR>::STAGE_BOXES * kStageBoxBytes +
                       kTcLayers * HW * sizeof(float) + sizeof(Bars) + 16;
   if (!configured[dev]) {
     if (cudaFuncSetAttribute(mlp_tc_kernel<MODE, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
