@@ -899,38 +899,39 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_tc_kernel(const TcArgs a, con
             const int col0 = HH * 64 + q * 32;
             EP_T0();
             const uint32_t stg = stg0 + (SB == 2 ? q * 4096 : 0);
-            // The box's 32 biases first, all eight 128-bit loads in flight together, and the whole box finished in
-            // registers BEFORE the wait for the staging slice: the previous box's TMA read (~400 cycles with one slice per
-            // warp) then overlaps this arithmetic, and the stores that follow the wait depend on nothing but registers
-            // (st_shared_v4 is an asm volatile with a memory clobber: a bias load written between two stores would be issued
-            // only after the store before it and the loop would pay one shared-memory latency per store).
-            float4 bq[8];
-#pragma unroll
-            for (int j = 0; j < 8; ++j) bq[j] = *reinterpret_cast<const float4*>(bias + col0 + 4 * j);
-            uint32_t* const vq = q == 0 ? va : vb;
-            if constexpr (!(q8 && wide)) {         // (8-bit per-hit projections: the raw int32 sums, added as integers later)
-#pragma unroll
-              for (int j = 0; j < 8; ++j) {
-                const float bj[4] = {bq[j].x, bq[j].y, bq[j].z, bq[j].w};
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                  const uint32_t v = vq[4 * j + c];
-                  float y;
-                  if constexpr (q8) y = dequant(v, a.q_sc[L], bj[c]);
-                  else if constexpr (f8 && !wide) y = __fadd_rn(__fmul_rn(__uint_as_float(v), a.q_sc[L]), bj[c]);  // y = acc * (S_a S_w) + b
-                  else y = __uint_as_float(v) + bj[c];
-                  vq[4 * j + c] = __float_as_uint(y);
-                }
-              }
-            }
             if (lane == 0) {                       // the TMA unit has read the slice's previous box (with a slice per box that
               if constexpr (SB == 2) bulk_wait_read1(); else bulk_wait_read0();   // is the LAST tile's: one newer group may be pending)
             }
             __syncwarp();
             EP_ACC(6);
+            // The box's 32 biases first, all eight 128-bit loads in flight together: st_shared_v4 is an asm volatile
+            // with a memory clobber, so a bias load written between two stores is issued only after the store before it
+            // and the loop pays one shared-memory latency per store (in-kernel counters: 2.2k cycles per tile for these
+            // 16 stores in the edge network, 3.7k for the 32 of the projection launches).
+            float4 bq[8];
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
-              st_shared_v4(stg + lane * 128 + ((j ^ (lane & 7)) << 4), vq[4 * j], vq[4 * j + 1], vq[4 * j + 2], vq[4 * j + 3]);
+            for (int j = 0; j < 8; ++j) bq[j] = *reinterpret_cast<const float4*>(bias + col0 + 4 * j);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const uint32_t v0 = q == 0 ? va[4 * j] : vb[4 * j], v1 = q == 0 ? va[4 * j + 1] : vb[4 * j + 1];
+              const uint32_t v2 = q == 0 ? va[4 * j + 2] : vb[4 * j + 2], v3 = q == 0 ? va[4 * j + 3] : vb[4 * j + 3];
+              const uint32_t dst = stg + lane * 128 + ((j ^ (lane & 7)) << 4);
+              if constexpr (q8 && wide)        // 8-bit per-hit projections: the raw int32 sums (they are added as integers)
+                st_shared_v4(dst, v0, v1, v2, v3);
+              else if constexpr (q8) {
+                const float sc = a.q_sc[L];
+                st_shared_v4(dst, __float_as_uint(dequant(v0, sc, bq[j].x)), __float_as_uint(dequant(v1, sc, bq[j].y)),
+                             __float_as_uint(dequant(v2, sc, bq[j].z)), __float_as_uint(dequant(v3, sc, bq[j].w)));
+              } else if constexpr (f8 && !wide) {   // fp32 sums of e4m3 products: y = acc * (S_a S_w) + b (the projections stay raw sums)
+                const float sc = a.q_sc[L];
+                st_shared_v4(dst, __float_as_uint(__fadd_rn(__fmul_rn(__uint_as_float(v0), sc), bq[j].x)),
+                             __float_as_uint(__fadd_rn(__fmul_rn(__uint_as_float(v1), sc), bq[j].y)),
+                             __float_as_uint(__fadd_rn(__fmul_rn(__uint_as_float(v2), sc), bq[j].z)),
+                             __float_as_uint(__fadd_rn(__fmul_rn(__uint_as_float(v3), sc), bq[j].w)));
+              } else
+              st_shared_v4(dst, __float_as_uint(__uint_as_float(v0) + bq[j].x), __float_as_uint(__uint_as_float(v1) + bq[j].y),
+                           __float_as_uint(__uint_as_float(v2) + bq[j].z), __float_as_uint(__uint_as_float(v3) + bq[j].w));
+            }
             EP_ACC(7);
             fence_async_smem();                    // generic-proxy writes -> async proxy (TMA)
             __syncwarp();
