@@ -165,7 +165,7 @@ search_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, const int32_t*
   if (MODE == 0 && blockIdx.x == 0 && threadIdx.x == 0) out_deg[a.n_hits] = 0;
 }
 
-// ------------------------------------------------------------------ d = 4: tiled count pass + ballot fill pass
+// ------------------------------------------------------------------ d = 4: tiled count pass + candidate-major pair fill pass
 // One CTA owns an (event, source plane) window: the candidates -- the hits of planes p+1..p+G of the event, a
 // contiguous index range -- are staged ONCE in shared memory as float4 and every warp tests them against FOUR source
 // hits at a time (register-blocked: one shared-memory load per candidate and four distance tests), instead of one warp
@@ -260,8 +260,8 @@ search_tile_count_kernel(GraphArgs a, const int32_t* __restrict__ plane_ptr, int
 
 // Next row NEXT-2 on the tiled search (k_max > 0, d = 4; Algorithm 1): after the count pass a source
 // with more than k_max votes keeps its k_max nearest candidates by (d^2 in fp32, then hit index) -- the order of
-// graph_kmax.cu and of the oracle -- by CLEARING the other votes: the vote words then describe the capped graph and the scans,
-// the ballot fill pass and the in-list sort run unchanged.  One warp per hit, almost all of which leave at once (the thesis:
+// graph_kmax.cu and of the oracle -- by CLEARING the other votes: the vote words then describe the capped graph, and the scans and
+// the pair fill pass run unchanged.  One warp per hit, almost all of which leave at once (the thesis:
 // < 0.1 % of hits exceed k_max = 50); lane t owns vote word t (a window has at most kBallotWords = 32 words, else the
 // caller falls back to graph_kmax.cu: flags[1]).  <= 128 votes: their keys (d^2 bits : index) are compacted into a
 // per-warp shared-memory list and every lane ranks its keys against the list; more: the k_max-th smallest key by bitwise
