@@ -205,6 +205,21 @@ typedef struct {
 etx_status etx_build_triplets(etx_ctx* ctx, const etx_batch* batch, const etx_graph* g, const float* d_scores,
                               float score_min, etx_triplets* t, void* stream);
 
+/* etx_build_triplets for callers that cannot allocate device memory and have registered no workspace (code under CUDA
+ * graph capture set-up, tight serving loops, harnesses that forbid cudaMalloc).  Same arguments, same rows, same d_ptr
+ * and counts as etx_build_triplets, bit for bit.  Its only scratch -- the block sums of the three device-wide scans -- is
+ * a fixed file-scope device array inside the library (9 KB, held by every GPU that loads libetx.so until the process
+ * exits) instead of the workspace of etx_set_workspace: the call allocates nothing (no cudaMalloc / cudaFree, no
+ * allocating library routine) and works on a context without a workspace.
+ * Limit: batch->n_hits <= ETX_STATIC_TRIPLET_MAX_HITS, else ETX_ERR_CAPACITY (nothing is launched).
+ * The array is shared by EVERY call on a device, whatever the context or stream, and keeps the last call's contents;
+ * the part a call uses is cleared on its stream first.  Two calls that overlap on the GPU (different streams, or
+ * different host threads) race on it and give undefined counts: serialise them.  Not recorded by etx_profile_read.
+ * Other statuses as etx_build_triplets.                                                                          */
+#define ETX_STATIC_TRIPLET_MAX_HITS 4194304   /* 2^22: four of the thesis' 2^20-hit GNN batches; config c4 has 3.5 M */
+etx_status etx_build_triplets_static(etx_ctx* ctx, const etx_batch* batch, const etx_graph* g, const float* d_scores,
+                                     float score_min, etx_triplets* t, void* stream);
+
 /* Next row: triplet classifiers ("edge encodings are sufficient for both the edge classifier and triplet
  * classifier"; Fig. 8.12 caption P:2330, [.,.] = concatenation; "separate triplet classifiers for articulations
  * and elbows", each "an MLP ending with a layer with 1 unit, and a sigmoid").  Reading: s = sigmoid(MLP_k([e_first,

@@ -22,7 +22,7 @@ ETX_OK, ETX_ERR_INVALID, ETX_ERR_CAPACITY, ETX_ERR_CUDA, ETX_ERR_UNSORTED, ETX_E
 EXPORTS = ["etx_weight_count", "etx_create", "etx_destroy", "etx_last_error", "etx_workspace_bytes",
            "etx_set_workspace", "etx_embed", "etx_embed_bf16", "etx_embed_int8", "etx_build_graph", "etx_gnn_forward", "etx_edge_scores",
            "etx_infer_host", "etx_launch_count", "etx_profile_enable", "etx_profile_read", "etx_build_tracks",
-           "etx_build_triplets", "etx_triplet_weight_count", "etx_set_triplet_classifiers", "etx_triplet_scores",
+           "etx_build_triplets", "etx_build_triplets_static", "etx_triplet_weight_count", "etx_set_triplet_classifiers", "etx_triplet_scores",
            "etx_triplet_tracks_workspace_bytes", "etx_build_tracks_from_triplets", "etx_set_int8_ranges",
            "etx_measure_alu_peak"]
 KERNEL_CLASSES = ["embed", "graph", "node_enc", "edge_enc", "scatter", "node_net", "edge_net", "cls", "tracks", "edge_proj"]
@@ -130,6 +130,8 @@ def load_library():
         lib.etx_build_triplets.restype = C.c_int
         lib.etx_build_triplets.argtypes = [C.c_void_p, C.POINTER(Batch), C.POINTER(Graph), C.c_void_p, C.c_float,
                                            C.POINTER(Triplets), C.c_void_p]
+        lib.etx_build_triplets_static.restype = C.c_int
+        lib.etx_build_triplets_static.argtypes = lib.etx_build_triplets.argtypes
         lib.etx_triplet_weight_count.restype = C.c_size_t
         lib.etx_triplet_weight_count.argtypes = [C.POINTER(ModelDesc)]
         lib.etx_set_triplet_classifiers.restype = C.c_int
@@ -342,6 +344,20 @@ class Etx:
         for k, name in enumerate(("articulation", "left_elbow", "right_elbow")):
             out[name] = torch.stack([rows[0, o[k]:o[k + 1]], rows[1, o[k]:o[k + 1]]], dim=1)
         return out
+
+    def etx_build_triplets_static(self, batch: DeviceBatch, graph: DeviceGraph, scores: torch.Tensor, score_min: float,
+                                  ptr: torch.Tensor, rows: torch.Tensor):
+        """etx_build_triplets without any allocation (include/etx.h): the caller passes the outputs -- ptr int32
+        [3, n_hits + 1] and rows int32 [2, capacity], both contiguous on the device -- and gets the three counts back.
+        rows[0, :sum(n)] / rows[1, :sum(n)] are the first / second edge ids, sections in the order of etx_build_triplets."""
+        assert ptr.dtype == torch.int32 and ptr.is_contiguous() and ptr.numel() == 3 * (batch.n_hits + 1)
+        assert rows.dtype == torch.int32 and rows.is_contiguous() and rows.dim() == 2 and rows.shape[0] == 2
+        t = Triplets()
+        t.d_ptr = ptr.data_ptr()
+        t.capacity, t.d_first, t.d_second = rows.shape[1], rows[0].data_ptr(), rows[1].data_ptr()
+        self._check(self.lib.etx_build_triplets_static(self.handle, C.byref(batch.c), C.byref(graph.c), _ptr(scores),
+                                                       score_min, C.byref(t), self._stream()))
+        return [int(x) for x in t.n]
 
     # ---- next row: INT8 GNN (context created with precision ETX_PREC_INT8 = 4)
     def etx_set_int8_ranges(self, alpha: Dict[str, list]):

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 
 #include "common.cuh"
 
@@ -1044,6 +1045,73 @@ etx_status etx_build_triplets(etx_ctx* c, const etx_batch* b, const etx_graph* g
                                        t->d_first, t->d_second, s);
   }
   return check_cuda(c, "etx_build_triplets (fill)");
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// etx_build_triplets_static: etx_build_triplets for callers that may not allocate (include/etx.h).  The only scratch the
+// triplet build needs is the block sums of its three device-wide scans; here they live in a file-scope device array of
+// fixed size instead of the registered workspace, so the call works on a context that has no workspace at all.
+constexpr int kStaticTripletMaxHits = ETX_STATIC_TRIPLET_MAX_HITS;
+constexpr int kStaticScanInts = 2304;                // >= scan_tmp_ints(kStaticTripletMaxHits + 1) = 2050 (checked at run time), 9 KB
+static __device__ __align__(256) int32_t g_static_scan_scratch[kStaticScanInts];
+
+namespace {
+// Device address of the array above on the context's device (which the caller has made current).  In host code the symbol
+// is only a stand-in for the array: its device address is asked for once per device and kept.
+etx_status static_scan_scratch(etx_ctx* c, int32_t** out) {
+  static std::mutex mu;
+  static int32_t* addr[kMaxDevices] = {nullptr};
+  if (c->device < 0 || c->device >= kMaxDevices) return fail(c, ETX_ERR_INVALID, "device index beyond the per-device tables");
+  std::lock_guard<std::mutex> lock(mu);
+  if (!addr[c->device]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scan_scratch);
+    if (e != cudaSuccess || !p)
+      return fail(c, ETX_ERR_CUDA, std::string("cudaGetSymbolAddress(static scan scratch): ") + cudaGetErrorString(e));
+    addr[c->device] = static_cast<int32_t*>(p);
+  }
+  *out = addr[c->device];
+  return ETX_OK;
+}
+}  // namespace
+
+etx_status etx_build_triplets_static(etx_ctx* c, const etx_batch* b, const etx_graph* g, const float* d_scores,
+                                     float score_min, etx_triplets* t, void* stream) {
+  if (!c) return ETX_ERR_INVALID;
+  if (etx_status st = check_batch(c, b)) return st;
+  if (!g || g->n_edges < 0 || !g->d_row_ptr || !g->d_in_ptr) return fail(c, ETX_ERR_INVALID, "graph is NULL or not built");
+  if (!t || !t->d_ptr || t->capacity < 0) return fail(c, ETX_ERR_INVALID, "triplet buffers are NULL");
+  if (t->capacity > 0 && (!t->d_first || !t->d_second)) return fail(c, ETX_ERR_INVALID, "triplet row arrays are NULL");
+  if (g->n_edges > 0 && (!d_scores || !g->d_in_perm)) return fail(c, ETX_ERR_INVALID, "scores / in_perm are NULL");
+  const int N = b->n_hits;
+  if (N > kStaticTripletMaxHits || scan_tmp_ints(N + 1) > (size_t)kStaticScanInts)
+    return fail(c, ETX_ERR_CAPACITY, "etx_build_triplets_static handles at most " + std::to_string(kStaticTripletMaxHits) +
+                                         " hits per call (its scratch is a fixed device array); got " + std::to_string(N));
+  cudaSetDevice(c->device);
+  cudaStream_t s = (cudaStream_t)stream;
+  int32_t* scan_tmp = nullptr;
+  if (etx_status st = static_scan_scratch(c, &scan_tmp)) return st;
+  const size_t ld = (size_t)N + 1;
+  // The array keeps the previous call's block sums.  The scans write every entry they read, so nothing HAS to start at
+  // zero; the part this call uses is cleared anyway so that a result can never depend on an earlier call.
+  cudaMemsetAsync(scan_tmp, 0, scan_tmp_ints(N + 1) * sizeof(int32_t), s);
+  c->launches += launch_triplet_count(N, g->d_row_ptr, g->d_in_ptr, g->d_in_perm, d_scores, score_min, t->d_ptr, s);
+  for (int k = 0; k < 3; ++k) c->launches += launch_exclusive_scan(t->d_ptr + k * ld, N + 1, scan_tmp, s);
+  int32_t host[3] = {0, 0, 0};
+  for (int k = 0; k < 3; ++k)
+    cudaMemcpyAsync(&host[k], t->d_ptr + k * ld + N, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+  if (cudaStreamSynchronize(s) != cudaSuccess) return check_cuda(c, "etx_build_triplets_static (count)");
+  if (etx_status st = check_cuda(c, "etx_build_triplets_static (count)")) return st;
+  bool overflow = false;
+  for (int k = 0; k < 3; ++k) { t->n[k] = host[k]; overflow |= host[k] < 0; }
+  if (overflow) return fail(c, ETX_ERR_CAPACITY, "more than 2^31 - 1 triplets of one kind");
+  const int64_t total = t->n[0] + t->n[1] + t->n[2];
+  if (total > t->capacity)
+    return fail(c, ETX_ERR_CAPACITY, "triplets need " + std::to_string(total) + " rows, capacity " + std::to_string(t->capacity));
+  if (total > 0)
+    c->launches += launch_triplet_fill(N, g->d_row_ptr, g->d_in_ptr, g->d_in_perm, d_scores, score_min, t->d_ptr,
+                                       t->d_first, t->d_second, s);
+  return check_cuda(c, "etx_build_triplets_static (fill)");
 }
 
 size_t etx_triplet_weight_count(const etx_model_desc* desc) {
