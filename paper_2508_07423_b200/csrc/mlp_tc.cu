@@ -147,10 +147,12 @@ template <> struct Cfg<ETX_PREC_FP8> {
 // Shared-memory split per launch variant.  The wide per-hit projection launches (VAR 1: one layer, 256 output columns,
 // output-bound) trade one operand-ring entry for a second staging slice per epilogue warp, so that a warp's two output
 // boxes never wait for each other's TMA read (projections 3.79 -> 3.38 ms per step at C2); the multi-layer launches keep
-// the deeper ring (edge network +2.5 % with 3 entries: its fp32 addend alone takes two).
+// the deeper ring (edge network +2.5 % with 3 entries: its fp32 addend alone takes two).  Same trade in the single-pass
+// bf16 mode (two of its eight 16 KB entries): projections 3.41 -> 3.26 ms at C3; on its multi-layer launches it nets zero
+// (edge encoder -0.11 ms, node network -0.06, edge network +0.18).
 template <int MODE, int VAR> struct Split {
-  static constexpr bool kTwoBoxes = (MODE == ETX_PREC_BF16X3 && VAR == 1);
-  static constexpr int NSTAGE_A = Cfg<MODE>::NSTAGE_A - (kTwoBoxes ? 1 : 0);
+  static constexpr bool kTwoBoxes = (MODE == ETX_PREC_BF16X3 || MODE == ETX_PREC_BF16) && VAR == 1;
+  static constexpr int NSTAGE_A = Cfg<MODE>::NSTAGE_A - (kTwoBoxes ? 2 / Cfg<MODE>::PIECES : 0);   // 32 KB of ring entries
   static constexpr int STAGE_BOXES = kTwoBoxes ? 2 : Cfg<MODE>::STAGE_BOXES;
 };
 
