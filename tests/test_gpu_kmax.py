@@ -116,3 +116,31 @@ def test_kmax_many_votes_and_windows_longer_than_the_kept_vote_words(B, c0, n_ca
         s = compare(B, etx, batch, emb, r2, 3, k_max)
         if r2 > 1e8:
             assert np.bincount(s, minlength=40)[:40].tolist() == [k_max] * 40
+
+
+def plane_sizes_event(sizes, seed):
+    """One event with sizes[p] hits on plane p and lattice embeddings (many exact ties with the radius)."""
+    rng = np.random.default_rng(seed)
+    n = int(sum(sizes))
+    batch = {"event_ptr": np.array([0, n], np.int32),
+             "plane": np.concatenate([np.full(s, p) for p, s in enumerate(sizes)]).astype(np.uint8)}
+    for k in ("r", "phi", "z", "x", "y"):
+        batch[k] = rng.normal(size=n).astype(np.float32)
+    emb = rng.integers(-2, 3, size=(n, 4)).astype(np.float32) * np.float32(0.5)
+    return batch, emb
+
+
+@pytest.mark.parametrize("sizes", [(1, 1, 1, 1), (31, 33, 32, 1), (32, 31, 65, 64), (33, 64, 0, 97), (64, 129, 200, 31),
+                                   (65, 512, 511, 1), (129, 1, 1022, 1), (200, 300, 400, 324), (5, 0, 0, 7, 3)])
+def test_tiled_build_block_boundaries(B, c0, sizes):
+    """The tiled d = 4 build at the edges of its blocking: sources in blocks of 4 (count pass), 32 (vote transposition) and
+    64 (staging step of the fill pass), candidate windows of 1..1024 hits in 32-candidate words with ragged last words,
+    empty planes, all three plane gaps feeding one in-list.  Uncapped and k_max = 3: arrays bit-equal to the oracle."""
+    cfg, _, blob = c0
+    etx = B.Etx(B.make_desc(cfg, precision=0), blob)
+    batch, emb = plane_sizes_event(sizes, sum(sizes))
+    for r2 in (0.6, 1.1, 1e9):
+        s = compare(B, etx, batch, emb, r2, 3, 0)
+        assert r2 < 1e8 or len(s) == sum(sizes[p] * sum(sizes[p + 1:p + 4]) for p in range(len(sizes)))
+    compare(B, etx, batch, emb, 1.1, 3, 3)
+    compare(B, etx, batch, emb, 1.1, 2, 0)
