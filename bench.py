@@ -606,7 +606,9 @@ def run_ours(args):
                    "n_events_per_gpu": n_ev, "n_hits": N, "n_edges": int(E),
                    "mean_out_degree": E / max(N, 1), "r2_max": r2, "hits_per_s": world * N / (ms_step * 1e-3),
                    "l2": "state larger than L2 (edge encodings %.1f GB), no flush needed" % (E * H * 4 / 1e9),
-                   "parallelism": "events sharded across GPUs, no collective" if world > 1 else "single GPU"},
+                   "parallelism": "events sharded across GPUs, no collective" if world > 1 else "single GPU",
+                   **({"precision_note": "per-edge MLP chains single-pass bf16; per-hit MLPs and the classifier run the bf16x3 split "
+                                         "(every edge of c3 then holds the 2e-2 gate, DESIGN.md section 6)"} if dtype == "bf16" else {})},
         "roofline": roof, "cpu_baseline": cpu, "parity": parity,
         "e2e": {"value": aggregate_events_per_s(world, n_ev, e2e_ms), "unit": "events/s", "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms},

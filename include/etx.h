@@ -50,7 +50,11 @@ typedef enum {
 typedef enum {
   ETX_PREC_FP32 = 0,    /* fp32 operands, FFMA on the CUDA cores, fp32 accumulate                 */
   ETX_PREC_TF32X3 = 1,  /* tcgen05 tensor cores, error-compensated 3xTF32 split (fp32-equivalent) */
-  ETX_PREC_BF16 = 2,    /* tcgen05 tensor cores, bf16 operands, fp32 accumulate, fp32 state       */
+  ETX_PREC_BF16 = 2,    /* tcgen05 tensor cores, bf16 operands, fp32 accumulate, fp32 state: the per-EDGE MLP chains
+                           (edge encoder, edge networks) run one kind::f16 MMA pass on bf16-rounded operands; the
+                           per-HIT MLPs (node encoder, node networks, per-hit projections of the edge MLPs' first
+                           layers) and the classifier run the BF16X3 split below -- they cost N rows instead of E (the
+                           classifier: one launch) and keep every edge of config c3 inside its 2e-2 gate             */
   ETX_PREC_BF16X3 = 3,  /* tcgen05, operands split x = hi + lo into two bf16 (16 significand bits),
                            three kind::f16 MMAs (lo.hi + hi.lo + hi.hi), fp32 accumulate and state:
                            meets the fp32 tolerance at half the tensor-core work of 3xTF32          */

@@ -67,6 +67,7 @@ struct etx_ctx {
   etx_model_desc desc;
   int device = 0;
   int sm_count = 148;
+  int hit_mode = -1;          // tensor-core mode of the per-hit MLPs (node encoder, node networks, projections) if not the context's
   float* d_weights = nullptr;      // transposed weights + biases, one allocation
   size_t d_weights_floats = 0;
   const float* d_zero_bias = nullptr;  // 128 zeros inside d_weights
@@ -157,6 +158,7 @@ struct MlpArgs {
   // 3 small-N sigmoid
   int out_mode = 0; float* out = nullptr; const float* res = nullptr; int out_ld = 0;
   int emb_mode = -1;          // out_mode 2 (embedding): tensor-core mode to run instead of the default 3xTF32 (etx_embed_bf16)
+  int tc_mode = -1;           // tensor-core mode of THIS launch if it differs from the context's (per-hit MLPs of ETX_PREC_BF16 run the split mode)
   float q_sa0 = 1.f; float q_sc[kMaxLayers] = {0}; float q_sn[kMaxLayers] = {0};   // ETX_PREC_INT8 scales (see TcArgs)
 };
 int launch_mlp_simt(const MlpArgs& a, cudaStream_t s);

@@ -307,7 +307,8 @@ int run_mlp_raw(etx_ctx* c, const MlpArgs& a, cudaStream_t s) {
   }
   // the embedding (narrow linear output, out_mode 2) always runs the 3xTF32 kernel, whatever the GNN's mode:
   // its result decides graph edges (DESIGN.md section 5 "Embedding on the tensor cores")
-  const int mode = (a.out_mode == 2) ? (a.emb_mode >= 0 ? a.emb_mode : (int)ETX_PREC_TF32X3) : (int)c->desc.precision;
+  const int mode = (a.out_mode == 2) ? (a.emb_mode >= 0 ? a.emb_mode : (int)ETX_PREC_TF32X3)
+                                     : (a.tc_mode >= 0 ? a.tc_mode : (int)c->desc.precision);
   t.w_last = a.mlp.Wt[a.mlp.n_layers - 1];         // [H][1] == [H]
   if (mode == ETX_PREC_INT8 || mode == ETX_PREC_FP8) {
     if (a.out_mode == 3) { if (!a.mlp.wq_last) return -1; t.w_last = a.mlp.wq_last; }
@@ -525,6 +526,11 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
     std::vector<unsigned char> img;
     std::vector<size_t> img_off(mlps.size(), (size_t)-1), img_a(mlps.size(), (size_t)-1), img_b(mlps.size(), (size_t)-1);
     const int H = desc->gnn_hidden, mode = desc->precision;
+    // ETX_PREC_BF16: the per-HIT MLPs (node encoder, node networks, the per-hit projections of the edge MLPs' first layers)
+    // run the fp32-equivalent split mode -- they cost N rows, not E, and h carries the largest values of the network --
+    // the per-EDGE chains stay single-pass bf16
+    const int hit_mode = (mode == ETX_PREC_BF16) ? (int)ETX_PREC_BF16X3 : mode;
+    c->hit_mode = (hit_mode != mode) ? hit_mode : -1;
     size_t wsrc = 0;
     for (size_t i = 0; i < mlps.size(); ++i) {
       const float* w = h_weights + wsrc;
@@ -540,20 +546,20 @@ etx_status etx_create(etx_ctx** out, const etx_model_desc* desc, const float* h_
       }
       if (i == 1 && mlps[i].n_layers >= 2) {             // node encoder: layers 2.. (layer 1 runs in the gather warps)
         img_off[i] = img.size();
-        append_wimg(img, mlps[i], w, 1, 0, mlps[i].n_layers, mode);
+        append_wimg(img, mlps[i], w, 1, 0, mlps[i].n_layers, hit_mode);
       }
       if (i >= 2) {
         const bool is_cls = (i + 1 == mlps.size());
         const bool is_node = !is_cls && i >= 3 && ((i - 3) % 2 == 0);
         if (is_cls || is_node) {
           img_off[i] = img.size();
-          append_wimg(img, mlps[i], w, 0, 0, is_cls ? mlps[i].n_layers - 1 : mlps[i].n_layers, mode);
+          append_wimg(img, mlps[i], w, 0, 0, is_cls ? mlps[i].n_layers - 1 : mlps[i].n_layers, hit_mode);
         } else {
           // edge encoder ([h_src | h_dst]) and edge networks ([h_src | h_dst | e]): first layer factorised
           // into the per-hit parts A (columns [0,H)), B ([H,2H)) and the per-edge part C ([2H,3H), networks only)
           const int fi = mlps[i].dims[0];
-          img_a[i] = img.size(); append_wimg_slab(img, w, fi, H, 0, H, mode);
-          img_b[i] = img.size(); append_wimg_slab(img, w, fi, H, H, 2 * H, mode);
+          img_a[i] = img.size(); append_wimg_slab(img, w, fi, H, 0, H, hit_mode);
+          img_b[i] = img.size(); append_wimg_slab(img, w, fi, H, H, 2 * H, hit_mode);
           img_off[i] = img.size();
           if (fi > 2 * H) append_wimg(img, mlps[i], w, 0, 2 * H, mlps[i].n_layers, mode);
           else append_wimg(img, mlps[i], w, 1, 0, mlps[i].n_layers, mode);
@@ -866,6 +872,7 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
     const int id[3] = {3, 4, 2};
     for (int i = 0; i < 3; ++i) { a.fc[i] = c->desc.norm_center[id[i]]; a.fs[i] = c->desc.norm_scale[id[i]]; }
     a.mlp = c->node_enc; a.out_mode = 0; a.out = w.h; a.out_ld = H;
+    a.tc_mode = c->hit_mode;
     ProfScope ps(c, ETX_K_NODE_ENC, s);
     if (q8) {
       // the 3-feature first layer stays fp32 (double accumulation: q8_aux.cu); its ReLU output, parked in m, is the
@@ -898,6 +905,7 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
       a.mlp.wimg = part == 0 ? mlp.wimg_a : mlp.wimg_b;
       a.mlp.b[0] = c->d_zero_bias; a.mlp.Wt[0] = c->d_zero_bias;
       a.wide = wide ? 1 : 0;
+      a.tc_mode = c->hit_mode;
       if (q8) a.q_sa0 = c->q_alpha[(size_t)mi * c->desc.gnn_n_layers] / (c->desc.precision == ETX_PREC_FP8 ? 448.0f : 127.0f);   // the edge MLP's layer-1 input scale; raw sums out
       a.out_mode = 0; a.out = w.p + part * H; a.out_ld = 2 * H;
       c->launches += run_mlp(c, a, s);
@@ -939,6 +947,7 @@ etx_status etx_gnn_forward(etx_ctx* c, const etx_batch* b, const etx_graph* g, f
       a.seg[0] = Segment{w.h, nullptr, H, H};
       a.seg[1] = Segment{w.m, nullptr, 2 * H, 2 * H};
       a.mlp = c->node_net[k]; a.out_mode = 1; a.out = w.h; a.res = w.h; a.out_ld = H;
+      a.tc_mode = c->hit_mode;
       if (q8) fill_q(c, a, 2 + 2 * k, c->node_net[k], 0, c->node_net[k].n_layers);
       ProfScope ps(c, ETX_K_NODE_NET, s);
       c->launches += run_mlp(c, a, s);
@@ -982,6 +991,7 @@ etx_status etx_edge_scores(etx_ctx* c, const etx_graph* g, const float* d_edge_e
   a.n_rows = (int)g->n_edges; a.n_seg = 1;
   a.seg[0] = Segment{d_edge_enc, nullptr, H, H};
   a.mlp = c->cls; a.out_mode = 3; a.out = d_scores; a.out_ld = 1;
+  a.tc_mode = c->hit_mode;
   if (c->desc.precision == ETX_PREC_INT8 || c->desc.precision == ETX_PREC_FP8) {
     if (c->q_alpha.empty()) return fail(c, ETX_ERR_INVALID, "ETX_PREC_INT8 / ETX_PREC_FP8 need calibrated ranges (etx_set_int8_ranges)");
     fill_q(c, a, 2 + 2 * c->desc.n_iter, c->cls, 0, c->cls.n_layers);

@@ -127,13 +127,14 @@ def test_full_batch_sampled_events(B, name, every, n_ext, precision):
 
 
 # Does BASELINE.json's gate hold on EVERY edge of the full batch at the oracle-calibrated gain?  Measured, round 2
-# (profiles/r02_parity.md): yes for the fp32-equivalent modes at C2 (max 4.0e-5 / 1.9e-5 of 9.6 M edges); NO for plain
-# bf16 at C3's scale (max 2.5e-2 against 2e-2: 2e-2 holds up to p99.99 = 8.3e-3 and on the oracle-sampled events) and NO
+# (profiles/r02_parity.md): yes for the fp32-equivalent modes at C2 (max 5.0e-5 / 1.9e-5 of 9.6 M edges); yes for the
+# bf16 mode at C3's scale since its per-hit MLPs and classifier run the split (max 1.47e-2 against 2e-2; with every MLP
+# in single-pass bf16 it was 2.5e-2: NOT met); NO
 # for the split modes at C4's scale (max 4.5e-4 against 1e-4), which is why C4 runs the exact FFMA mode.  The table is
 # asserted BOTH ways: a mode listed as failing must really exceed the gate (so this text cannot go stale), and stay
 # inside the looser bound given here.
 EVERY_EDGE = {("c2", synth.PREC_BF16X3): (True, 1e-4), ("c2", synth.PREC_TF32X3): (True, 1e-4),
-              ("c2", synth.PREC_BF16): (False, 4e-2), ("c4", synth.PREC_BF16X3): (False, 1e-3)}
+              ("c2", synth.PREC_BF16): (True, 2e-2), ("c4", synth.PREC_BF16X3): (False, 1e-3)}
 
 
 @pytest.mark.parametrize("name,precisions", [("c2", [synth.PREC_BF16X3, synth.PREC_TF32X3, synth.PREC_BF16]),
